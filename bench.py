@@ -1,0 +1,320 @@
+#!/usr/bin/env python
+"""bench.py -- GCUPS of one explicit Heun step of the AMR Euler hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+
+A "step" = compute_dt + advance = 2 x (ghost fill + fused stage kernel) over
+every block of the BASELINE.json config (default: config 3, 3D uniform 512^3
+in 16^3 blocks, fp64 -- the headline).  GCUPS = interior cells x 2 RK stages x
+steps / time / 1e9.  Rank 0 prints ONE JSON line.
+
+N > 1 (torchrun): the path does not shard in this build ("replicas only",
+DESIGN.md): every rank runs the same workload independently; value = units of
+all ranks / max-over-ranks time; no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2605_07612_b200 import workloads as W  # noqa: E402
+
+METRIC = "GCUPS (fp64, 3D, 1 B200) and achieved fraction of HBM roofline; ghost-fill GB/s"
+UNIT = "GCUPS"
+
+
+def workload_name(cfg):
+    d, n = cfg["dim"], cfg["block_n"]
+    ext = [cfg["brick"][a] * 2 ** cfg["base_level"] for a in range(d)]
+    return f"{cfg['name']}: {d}D {'x'.join(str(e * n) for e in ext)} cells, {n}^{d} blocks, " \
+           f"{'uniform' if cfg['max_level'] == cfg['base_level'] else 'adaptive'}, Ng=2, fp64, Heun, CFL {cfg['cfl']}"
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            with open(p) as f:
+                d = json.load(f)
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)", float(d.get("sm_max_mhz", 1965.0))
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)", 1965.0
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML during the timed region."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.stop_flag = index, [], set(), False
+        self.max_mhz = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {"hw_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8),
+                 "hw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40),
+                 "sw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20),
+                 "sw_power_cap": getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4)}
+        while not self.stop_flag:
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(0.01)
+
+    def result(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": 0}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def fill_initial_state(cfg, lev, co, out, chunk=1024):
+    """Seeded synthetic state written block-chunk by block-chunk into a (pinned) host array."""
+    for b0 in range(0, len(lev), chunk):
+        out[b0:b0 + chunk] = W.initial_state(cfg, lev[b0:b0 + chunk], co[b0:b0 + chunk])
+
+
+def oracle_sample(cfg, target_updates=1.2e7):
+    """The oracle, as it stands, on a bounded sample of the same workload: same generator and block
+    size, smaller uniform base level (or fewer extra levels); returns (GCUPS, cores, description)."""
+    from oracle import oracle as O
+    n, d = cfg["block_n"], cfg["dim"]
+    scfg = dict(cfg)
+    if cfg["max_level"] == cfg["base_level"]:
+        lvl = 0
+        while True:
+            cells = np.prod([cfg["brick"][a] * 2 ** (lvl + 1) * n for a in range(d)])
+            if cells * 2 * 4 > target_updates or lvl + 1 > cfg["base_level"]:
+                break
+            lvl += 1
+        scfg["base_level"] = scfg["max_level"] = lvl
+    else:
+        scfg["base_level"], scfg["max_level"] = 1, 1
+    om = O.OracleMesh.from_config(scfg)
+    lev, co = om.get_blocks()
+    om.set_state(0, W.initial_state(scfg, lev, co))
+    cells = len(lev) * n ** d
+    steps = max(2, int(round(target_updates / (2.0 * cells))))
+    om.advance(om.compute_dt(0, cfg["cfl"]))  # warm
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        om.advance(om.compute_dt(0, cfg["cfl"]))
+    el = time.perf_counter() - t0
+    ext = [scfg["brick"][a] * 2 ** scfg["base_level"] * n for a in range(d)]
+    desc = f"{'x'.join(map(str, ext))} cells ({len(lev)} blocks of {n}^{d}), {steps} Heun steps, same generator/seed"
+    return cells * 2.0 * steps / el / 1e9, 1, desc, el, steps
+
+
+def run_reference(args, cfg, rank):
+    """--impl reference: this tier's reference arm is the CPU oracle on the host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    from oracle import oracle as O
+    n, d = cfg["block_n"], cfg["dim"]
+    scfg = dict(cfg)
+    if cfg["max_level"] == cfg["base_level"]:
+        lvl = min(cfg["base_level"], 2 if n <= 16 else 1)
+        scfg["base_level"] = scfg["max_level"] = lvl
+    else:
+        scfg["base_level"], scfg["max_level"] = 1, 1
+    om = O.OracleMesh.from_config(scfg)
+    lev, co = om.get_blocks()
+    om.set_state(0, W.initial_state(scfg, lev, co))
+    cells = len(lev) * n ** d
+    for _ in range(args.warmup):
+        om.advance(om.compute_dt(0, cfg["cfl"]))
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        om.advance(om.compute_dt(0, cfg["cfl"]))
+    el = time.perf_counter() - t0
+    val = cells * 2.0 * args.steps / el / 1e9
+    ext = [scfg["brick"][a] * 2 ** scfg["base_level"] * n for a in range(d)]
+    sample = f"bounded sample of {cfg['name']}: {'x'.join(map(str, ext))} cells ({len(lev)} blocks of {n}^{d}) per step"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--scale", type=int, default=None, help="smaller base level (debug only; invalid as a bench number)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    cfg = W.config(args.config, scale=args.scale)
+
+    if args.impl == "reference":
+        run_reference(args, cfg, rank)
+        return
+
+    import torch
+    from paper_2605_07612_b200 import f4
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the f4 path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist_mod.init_process_group("nccl", device_id=torch.device(dev))
+        dist = dist_mod
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    mesh = f4.Mesh.from_config(cfg, max_blocks=None if cfg["max_level"] == cfg["base_level"] else 6000)
+    stream = torch.cuda.Stream(dev)
+    mesh.bind_torch(dev, stream)
+    lev, co = mesh.get_blocks()
+    nb, n, d = len(lev), cfg["block_n"], cfg["dim"]
+    cells = nb * n ** d
+    host = torch.empty(mesh._shape(False), dtype=torch.float64).pin_memory()
+    host_np = host.numpy()
+    fill_initial_state(cfg, lev, co, host_np)
+    mesh.set_state(0, host_np)
+
+    def step():
+        dt = mesh.compute_dt(0, cfg["cfl"])
+        mesh.advance(dt)
+
+    for _ in range(max(args.warmup, 0)):
+        step()
+    mesh.profile_get(reset=True)
+    mesh.profile_enable(True)
+    l0 = mesh.launch_count()
+    sampler = ClockSampler(local_rank)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler.start()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    barrier()
+    sampler.stop_flag = True
+    ms = ev0.elapsed_time(ev1)
+    launches = mesh.launch_count() - l0
+    prof = mesh.profile_get(reset=True)
+    mesh.profile_enable(False)
+    totals_after = mesh.conserved_totals(0)
+    if dist is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * cells * 2.0 * args.steps / (ms * 1e-3) / 1e9
+
+    # ---- end to end through the C-ABI with HOST buffers: H2D of the state, the step, D2H of the result metric
+    fill_initial_state(cfg, lev, co, host_np)
+    e2e_steps = max(1, args.e2e_steps)
+    mesh.set_state(0, host_np)
+    step()
+    barrier()
+    ev2, ev3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev2.record(stream)
+    for _ in range(e2e_steps):
+        mesh.set_state(0, host_np)          # pinned host -> device staging -> store
+        step()
+        tot = mesh.conserved_totals(0)      # device -> host: per-block sums + dt
+    ev3.record(stream)
+    barrier()
+    ms_e2e = ev2.elapsed_time(ev3)
+    if dist is not None:
+        t = torch.tensor([ms_e2e], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_e2e = float(t.item())
+    e2e = {"value": world * cells * 2.0 * e2e_steps / (ms_e2e * 1e-3) / 1e9, "unit": UNIT,
+           "h2d_bytes_per_step": int(host_np.nbytes), "d2h_bytes_per_step": int(nb * (d + 2) * 8 + 8),
+           "steps": e2e_steps, "ms_per_step": ms_e2e / e2e_steps}
+
+    if rank != 0:
+        return
+    # ---- roofline of the dominant kernel (fused stage kernel), algorithmic bytes
+    peak, peak_src, sm_max = peaks()
+    r = 1.0 + 2.0 * d * 2 / n
+    bpc = 8 * (d + 2)
+    stage_bytes = cells * (bpc * r + bpc + 0.5 * bpc)    # read s_deriv interior+halo, write s_out, avg extra s_prev read
+    ghost_bytes = cells * 2 * bpc * (r - 1.0)            # read + write of the face layers
+    st_ms, st_n = prof["stage"]
+    g_ms, g_n = prof["ghost_r1"][0] + prof["ghost_r2"][0], max(prof["ghost_r1"][1], 1)
+    stage_gbs = stage_bytes / (st_ms / max(st_n, 1) * 1e-3) / 1e9 if st_ms > 0 else None
+    ghost_gbs = ghost_bytes / (g_ms / g_n * 1e-3) / 1e9 if g_ms > 0 else None
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tp):
+        try:
+            traffic = json.load(open(tp)).get(f"config{args.config}_stage_dram_bytes_per_launch")
+        except Exception:
+            traffic = None
+    # fp64 issue bound of the stage kernel: 64 DFMA-class instr/clk/SM x 148 SM x clock
+    clocks = sampler.result()
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "blocks": nb, "cells": cells,
+                   "l2": "state (2 x %.1f GB) is larger than L2; no flush needed" % (mesh.storage_bytes() / 2e9),
+                   "parallelism": "replicas only" if world > 1 else "1 GPU"},
+        "roofline": {"bound": "hbm", "achieved": stage_gbs, "peak": peak, "unit": "GB/s",
+                     "frac": (stage_gbs / peak) if stage_gbs else None, "traffic": traffic,
+                     "kernel": "stage_kernel", "peak_source": peak_src,
+                     "algorithmic_bytes_per_launch": stage_bytes, "avg_launch_ms": st_ms / max(st_n, 1)},
+        "ghost_fill": {"GBps": ghost_gbs, "frac_of_hbm_peak": (ghost_gbs / peak) if ghost_gbs else None,
+                       "avg_fill_ms": g_ms / g_n, "algorithmic_bytes_per_fill": ghost_bytes},
+        "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()},
+        "step_algorithmic_GBps": (2 * (stage_bytes + ghost_bytes)) / (ms / args.steps * 1e-3) / 1e9,
+        "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        "totals": [float(x) for x in totals_after],
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        v, cores, desc, el, cs = oracle_sample(cfg)
+        out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+                               "seconds": el}
+    print(json.dumps(out))
+    mesh.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

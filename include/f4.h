@@ -1,0 +1,183 @@
+/* f4.h -- C-ABI of the B200-native hot path of foap4 (arxiv/paper_2605_07612).
+ *
+ * One explicit Heun step of Euler's equations over every block of a
+ * quadtree/octree AMR mesh: execution of a precomputed ghost-cell pattern
+ * (section 2.6) + the per-block finite-volume update
+ * (section 3.2), with mesh adapt / regrid transfer
+ * (section 2.2).  Citations are /root/reference/PAPER.md:<line>;
+ * "reading Ax" refers to DESIGN.md "Readings of the paper".
+ *
+ * General conventions
+ *  - Every function returns F4_OK (0) or a negative F4_E* code; nothing throws
+ *    across the ABI.  f4_last_error() gives the message of the last failure.
+ *  - Pointers are HOST pointers unless the argument says "device".  The block
+ *    store is DEVICE memory owned by the caller (e.g. a torch tensor) and lent
+ *    to the mesh with f4_bind_storage(); the library owns only small metadata
+ *    (block table, pattern records, staging buffers).
+ *  - All device work is enqueued on the stream given to f4_bind_storage().
+ *    Only f4_compute_dt, f4_get_state / f4_set_state with a host buffer,
+ *    f4_adapt, f4_conserved_totals and f4_profile_get synchronise that stream.
+ *  - There is no CPU fallback: a call that needs the device fails with
+ *    F4_EUNBOUND / F4_ECUDA when no storage is bound or CUDA reports an error.
+ *    Host-only calls (mesh_create, num_blocks, get_blocks, build_ghost_pattern,
+ *    pattern_size, get_pattern and adapt on an UNBOUND mesh = topology only)
+ *    work without a GPU.
+ *  - Variables per cell: Nvar = dim+2 = (rho, rho*u_1..dim, E)
+ *    eq. (14)-(15).  State arrays passed through this ABI are
+ *    [block][var][k][j][i], i fastest (eq. 3), block order =
+ *    the library's (Morton order over the brick; discover it with
+ *    f4_get_blocks).  "interior" arrays have N cells per axis, "padded" arrays
+ *    N+2*Ng per axis in natural order (index p = i+Ng for i in [-Ng, N+Ng)).
+ *    In 2D the k extent is 1.
+ *  - Device layout of the bound store: state-major,
+ *    then block, var, and a ghost-WRAPPED padded box: along every axis slot
+ *    s(i) = i for i >= 0 (interior, then high ghosts) and i + P for i < 0 (low
+ *    ghosts last), so that interior rows start on 32-byte sectors and both
+ *    x-ghost pairs of a row share one sector.
+ */
+#ifndef F4_H
+#define F4_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct f4_mesh f4_mesh; /* opaque: host mesh + pattern + device metadata */
+
+enum {
+  F4_OK = 0,
+  F4_EINVAL = -1,    /* bad argument (N odd, N < Ng, 2*Ng > N, dim not 2/3, ...) */
+  F4_ENOBLOCKS = -2, /* mesh would exceed max_blocks (store is statically sized) */
+  F4_ECUDA = -3,     /* a CUDA call failed; message in f4_last_error */
+  F4_EUNBOUND = -4,  /* device work requested but no storage bound */
+  F4_EUNBALANCED = -5, /* face connectivity found a >1 level jump */
+  F4_EUNSUPPORTED = -6 /* configuration outside the compiled kernel set (see f4_bind_storage) */
+};
+
+/* physical boundary kinds per face direction */
+enum {
+  F4_BC_PERIODIC = 0, /* via connectivity */
+  F4_BC_OUTFLOW = 1,  /* uniform Neumann, zero normal derivative: ghost = nearest interior layer (reading A10) */
+  F4_BC_KEEP = 2      /* ghosts on that face are left as the caller set them (linear-field test) */
+};
+
+enum { F4_LIM_VANLEER = 0, F4_LIM_MINMOD = 1, F4_LIM_MC = 2 }; /* PAPER.md:322-326; reading A1 */
+enum { F4_FLUX_HLL = 0, F4_FLUX_RUSANOV = 1 };                 /* PAPER.md:328; reading A2 */
+
+/* pattern record ops (data-flow naming) */
+enum {
+  F4_OP_SRL = 0, /* same-level copy, round R1 */
+  F4_OP_BC = 1,  /* physical boundary (outflow), round R1 */
+  F4_OP_F2C = 2, /* restriction of one fine neighbour into a quarter (3D) / half (2D) of a coarse ghost face, R1 */
+  F4_OP_C2F = 3  /* limited prolongation from the coarse neighbour into a fine ghost face, round R2 */
+};
+
+/* ---- mesh_create(dim, block_n, n_ghost, levels) ----------------------------
+ * Brick of brick[0] x brick[1] (x brick[2]) trees refined
+ * uniformly to base_level; leaves are blocks of block_n^dim cells with n_ghost
+ * ghost layers.  Domain: [0, brick[a]/max(brick)] along
+ * axis a, cubic cells of size dx_l = 1/(max(brick) * 2^l * block_n) (reading
+ * A13).  bc_kind[6]: per face direction -x,+x,-y,+y,-z,+z; an
+ * axis is periodic only if both its faces say so.  n_states >= 2 (Heun needs
+ * two); max_blocks sizes the store.  Host only.
+ * Errors: F4_EINVAL, F4_ENOBLOCKS (base mesh larger than max_blocks). */
+int f4_mesh_create(int dim, int block_n, int n_ghost, const int brick[3], int base_level, int max_level,
+                   const int bc_kind[6], double gamma, int n_states, int max_blocks, f4_mesh **out);
+int f4_mesh_destroy(f4_mesh *m);
+
+/* limiter / flux scheme / prolongation theta of eq. (1) (default van Leer, HLL, theta=1). */
+int f4_set_options(f4_mesh *m, int limiter, int flux_scheme, double theta);
+
+/* bytes of the block store: n_states*max_blocks*Nvar*P^dim*8. */
+size_t f4_storage_bytes(const f4_mesh *m);
+
+/* Lend the DEVICE store (>= f4_storage_bytes, 256-byte aligned) and a CUDA
+ * stream (cudaStream_t as void*, NULL = default stream).  Ownership stays with
+ * the caller, who must keep it alive until destroy/rebind.  Initialises every
+ * padded cell (unused edge/corner ghosts included) to a benign state
+ * (rho=1, u=0, p=1) and uploads the block table.  The CUDA kernels are
+ * compiled for n_ghost == 2 and (dim, block_n) in {(2,8), (2,16), (3,8), (3,16),
+ * (3,32)}: anything else gives F4_EUNSUPPORTED.  Errors: F4_EINVAL, F4_ECUDA. */
+int f4_bind_storage(f4_mesh *m, void *dev_ptr, size_t bytes, void *cuda_stream);
+
+int f4_num_blocks(const f4_mesh *m);
+/* Block metadata: refinement level, integer block coordinates
+ * on the level's grid [nb][3], spatial origin (low corner) [nb][3], cell size
+ * [nb].  Any output pointer may be NULL. */
+int f4_get_blocks(const f4_mesh *m, int *level, int *coords, double *origin, double *dx);
+
+/* ---- set_state / get_state -------------------------------------------------
+ * Copy a state between caller memory and the store.  with_ghosts = 0: interior
+ * array [nb][Nvar][N..]; 1: natural padded array [nb][Nvar][P..] (ghosts
+ * included).  *_is_device says where the caller's buffer lives; a host buffer
+ * is staged through pinned memory in chunks and the call returns after the
+ * last chunk (synchronises).  State s in [0, n_states). */
+int f4_set_state(f4_mesh *m, int state, const double *src, int src_is_device, int with_ghosts);
+int f4_get_state(f4_mesh *m, int state, double *dst, int dst_is_device, int with_ghosts);
+
+/* ---- build_ghost_pattern ---------------------------------------------------
+ * Host: face connectivity -> device-resident record lists for round R1
+ * {SRL, BC, F2C} and round R2 {C2F}, sorted by
+ * (destination block, face direction).  Uploaded when storage is bound.
+ * Called automatically by mesh_create, adapt.  Errors: F4_EUNBALANCED. */
+int f4_build_ghost_pattern(f4_mesh *m);
+int f4_pattern_size(const f4_mesh *m, int *n_r1, int *n_r2);
+/* records[n][6] = {op, face, dst_block, src_block, off_t1, off_t2}, R1 first.
+ * face: 0..5 = -x,+x,-y,+y,-z,+z of the DESTINATION block; off_*: hanging-face
+ * offset of the fine block within its group. */
+int f4_get_pattern(const f4_mesh *m, int *records);
+
+/* ---- fill_ghosts -----------------------------------------------------------
+ * Execute the pattern on one state: one batched kernel for R1, then one for R2
+ * iff the mesh has refinement boundaries.  Asynchronous. */
+int f4_fill_ghosts(f4_mesh *m, int state);
+
+/* ---- compute_dt ------------------------------------------------------------
+ * dt = cfl / max over interior cells of sum_dim (|u_dim| + c)/dx_l (PAPER.md:336,
+ * 339, eq. 16; readings A4-A6).  After f4_advance the maximum of the new
+ * state 0 is already on the device (fused into the last stage); otherwise a
+ * reduction kernel runs.  Synchronises to read one double back. */
+int f4_compute_dt(f4_mesh *m, int state, double cfl, double *dt_out);
+
+/* ---- advance(dt) -----------------------------------------------------------
+ * One step of Heun's method, eq. (6)-(7), as two sub-steps of
+ * eq. (5): fill_ghosts(0); u1 = dt F(ut) + ut -> state 1; fill_ghosts(1);
+ * u = dt/2 F(u1) + (ut + u1)/2 -> state 0 (in place).  F = limited primitive
+ * reconstruction + HLL/Einfeldt flux divergence.
+ * Asynchronous; result in state 0, whose ghosts are then stale. */
+int f4_advance(f4_mesh *m, double dt);
+
+/* ---- adapt(refine_flags) ---------------------------------------------------
+ * flags[nb]: >0 refine, <0 may coarsen, 0 keep.  refine, then
+ * coarsen complete families (one level per call, never below base_level or
+ * above max_level), then 2:1 balance with corner connectivity (
+ * reading A11).  If the mesh changed: state 0 is transferred (copy /
+ * prolongation / restriction; ghosts of state 0 are filled
+ * first), the pattern is rebuilt, *changed_out = 1.  On an unbound mesh only
+ * the topology changes.  Other states become undefined.  Synchronises.
+ * Errors: F4_ENOBLOCKS (nothing modified), F4_ECUDA. */
+int f4_adapt(f4_mesh *m, const int *refine_flags, int *changed_out);
+
+/* sum over interior cells of u * dx^dim, per variable [Nvar] (for conservation tests). */
+int f4_conserved_totals(f4_mesh *m, int state, double *totals);
+
+/* ---- measurement helpers ---------------------------------------------------
+ * f4_profile_enable(1): bracket every kernel class with CUDA events on the
+ * bound stream.  f4_profile_get: accumulated milliseconds and launch counts
+ * since the last reset, classes: 0 ghost R1, 1 ghost R2, 2 stage, 3 dt reduce,
+ * 4 regrid transfer, 5 layout (set/get/init).  f4_launch_count: kernels
+ * launched by this mesh since creation (always counted). */
+enum { F4_PROF_R1 = 0, F4_PROF_R2 = 1, F4_PROF_STAGE = 2, F4_PROF_DT = 3, F4_PROF_REGRID = 4, F4_PROF_LAYOUT = 5, F4_PROF_N = 6 };
+int f4_profile_enable(f4_mesh *m, int on);
+int f4_profile_get(f4_mesh *m, double ms[F4_PROF_N], long long launches[F4_PROF_N], int reset);
+long long f4_launch_count(const f4_mesh *m);
+
+const char *f4_last_error(const f4_mesh *m);
+const char *f4_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* F4_H */

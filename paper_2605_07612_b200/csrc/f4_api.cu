@@ -1,0 +1,493 @@
+// C-ABI of the f4 library (include/f4.h): argument checking, device metadata,
+// launch sequencing.  All arithmetic of the path lives in f4_ghost.cu / f4_stage.cu.
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/f4.h"
+#include "f4_dev.hpp"
+#include "f4_mesh.hpp"
+
+using namespace f4;
+
+struct f4_mesh {
+  HostMesh hm;
+  double gamma = 1.4, theta = 1.0;
+  int limiter = F4_LIM_VANLEER, flux = F4_FLUX_HLL;
+  int n_states = 2;
+  int nvar = 5;
+  size_t vs = 0, bs = 0, state_doubles = 0;  // doubles per (block,var), per block, per state
+  // device
+  bool bound = false;
+  double* store = nullptr;
+  cudaStream_t stream = nullptr;
+  std::vector<int> phys;  // logical state -> physical state slab
+  int* d_level = nullptr;
+  DevRecord* d_r1 = nullptr;
+  DevRecord* d_r2 = nullptr;
+  size_t cap_r1 = 0, cap_r2 = 0;
+  int n_r1 = 0, n_r2 = 0;
+  DevTransfer* d_plan = nullptr;
+  size_t cap_plan = 0;
+  unsigned long long* d_maxrate = nullptr;
+  double* d_sums = nullptr;
+  double* d_stage = nullptr;  // staging for host set/get
+  size_t stage_bytes = 0;
+  bool rate_valid = false;
+  // measurement
+  bool prof = false;
+  struct Ev { int cls; cudaEvent_t a, b; };
+  std::vector<Ev> evs;
+  double prof_ms[F4_PROF_N] = {0, 0, 0, 0, 0, 0};
+  long long prof_n[F4_PROF_N] = {0, 0, 0, 0, 0, 0};
+  long long launches = 0;
+  std::string err;
+
+  double* state_ptr(int s) { return store + (size_t)phys[s] * state_doubles; }
+};
+
+namespace {
+
+int fail(f4_mesh* m, int code, const std::string& msg) {
+  if (m) m->err = msg;
+  return code;
+}
+int cuda_fail(f4_mesh* m, cudaError_t e, const char* what) {
+  return fail(m, F4_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CU(call)                                          \
+  do {                                                    \
+    cudaError_t e_ = (call);                              \
+    if (e_ != cudaSuccess) return cuda_fail(m, e_, #call); \
+  } while (0)
+
+struct Scope {  // event bracket around one kernel launch
+  f4_mesh* m;
+  int cls;
+  f4_mesh::Ev ev{};
+  bool on;
+  Scope(f4_mesh* m_, int cls_) : m(m_), cls(cls_), on(m_->prof) {
+    m->launches++;
+    m->prof_n[cls]++;
+    if (on) {
+      ev.cls = cls;
+      cudaEventCreate(&ev.a);
+      cudaEventCreate(&ev.b);
+      cudaEventRecord(ev.a, m->stream);
+    }
+  }
+  ~Scope() {
+    if (on) {
+      cudaEventRecord(ev.b, m->stream);
+      m->evs.push_back(ev);
+    }
+  }
+};
+
+template <typename T>
+int ensure(f4_mesh* m, T*& ptr, size_t& cap, size_t need) {
+  if (need <= cap) return F4_OK;
+  if (ptr) cudaFree(ptr);
+  ptr = nullptr;
+  size_t ncap = need + need / 2 + 64;
+  CU(cudaMalloc((void**)&ptr, ncap * sizeof(T)));
+  cap = ncap;
+  return F4_OK;
+}
+
+int upload_meta(f4_mesh* m) {
+  if (!m->bound) return F4_OK;
+  const int nb = (int)m->hm.leaves.size();
+  std::vector<int> lev(nb);
+  for (int b = 0; b < nb; ++b) lev[b] = m->hm.leaves[b].level;
+  CU(cudaMemcpyAsync(m->d_level, lev.data(), nb * sizeof(int), cudaMemcpyHostToDevice, m->stream));
+  auto pack = [](const std::vector<Record>& r, std::vector<DevRecord>& out) {
+    out.resize(r.size());
+    for (size_t q = 0; q < r.size(); ++q)
+      out[q] = DevRecord{r[q].dst, r[q].src, r[q].op | r[q].face << 2 | r[q].o1 << 5 | r[q].o2 << 6, 0};
+  };
+  std::vector<DevRecord> a, b2;
+  pack(m->hm.r1, a);
+  pack(m->hm.r2, b2);
+  int rc;
+  if ((rc = ensure(m, m->d_r1, m->cap_r1, a.size()))) return rc;
+  if ((rc = ensure(m, m->d_r2, m->cap_r2, b2.size()))) return rc;
+  if (!a.empty()) CU(cudaMemcpyAsync(m->d_r1, a.data(), a.size() * sizeof(DevRecord), cudaMemcpyHostToDevice, m->stream));
+  if (!b2.empty()) CU(cudaMemcpyAsync(m->d_r2, b2.data(), b2.size() * sizeof(DevRecord), cudaMemcpyHostToDevice, m->stream));
+  m->n_r1 = (int)a.size();
+  m->n_r2 = (int)b2.size();
+  CU(cudaStreamSynchronize(m->stream));  // host vectors go out of scope
+  return F4_OK;
+}
+
+int fill_ghosts_impl(f4_mesh* m, int state) {
+  double* st = m->state_ptr(state);
+  if (m->n_r1) {
+    Scope sc(m, F4_PROF_R1);
+    CU(launch_ghost(m->hm.dim, m->hm.N, GhostParams{st, m->d_r1, m->n_r1, m->theta}, m->stream));
+  }
+  if (m->n_r2) {
+    Scope sc(m, F4_PROF_R2);
+    CU(launch_ghost(m->hm.dim, m->hm.N, GhostParams{st, m->d_r2, m->n_r2, m->theta}, m->stream));
+  }
+  return F4_OK;
+}
+
+int check_state(f4_mesh* m, int state) {
+  if (!m) return F4_EINVAL;
+  if (!m->bound) return fail(m, F4_EUNBOUND, "no device storage bound (f4_bind_storage); there is no CPU fallback");
+  if (state < 0 || state >= m->n_states) return fail(m, F4_EINVAL, "state index out of range");
+  return F4_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* f4_version(void) { return "f4 0.1 (sm_100a)"; }
+
+int f4_mesh_create(int dim, int block_n, int n_ghost, const int brick[3], int base_level, int max_level,
+                   const int bc_kind[6], double gamma, int n_states, int max_blocks, f4_mesh** out) {
+  if (!out || !brick || !bc_kind) return F4_EINVAL;
+  *out = nullptr;
+  if (n_states < 2 || max_blocks < 1 || !(gamma > 1.0)) return F4_EINVAL;
+  f4_mesh* m = new (std::nothrow) f4_mesh();
+  if (!m) return F4_EINVAL;
+  m->hm.dim = dim;
+  m->hm.N = block_n;
+  m->hm.Ng = n_ghost;
+  for (int a = 0; a < 3; ++a) m->hm.brick[a] = (a < dim) ? brick[a] : 1;
+  m->hm.base_level = base_level;
+  m->hm.max_level = max_level;
+  for (int f = 0; f < 6; ++f) m->hm.bc[f] = (f < 2 * dim) ? bc_kind[f] : F4_BC_PERIODIC;
+  m->hm.max_blocks = max_blocks;
+  m->gamma = gamma;
+  m->n_states = n_states;
+  std::string err;
+  int rc = m->hm.init(err);
+  if (rc != F4_OK) {
+    delete m;
+    return rc;
+  }
+  m->nvar = dim + 2;
+  const size_t P = block_n + 2 * n_ghost;
+  m->vs = P * P * (dim == 3 ? P : 1);
+  m->bs = m->vs * m->nvar;
+  m->state_doubles = m->bs * (size_t)max_blocks;
+  m->phys.resize(n_states);
+  for (int s = 0; s < n_states; ++s) m->phys[s] = s;
+  *out = m;
+  return F4_OK;
+}
+
+int f4_mesh_destroy(f4_mesh* m) {
+  if (!m) return F4_EINVAL;
+  if (m->bound) cudaStreamSynchronize(m->stream);
+  for (auto& e : m->evs) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+  if (m->d_level) cudaFree(m->d_level);
+  if (m->d_r1) cudaFree(m->d_r1);
+  if (m->d_r2) cudaFree(m->d_r2);
+  if (m->d_plan) cudaFree(m->d_plan);
+  if (m->d_maxrate) cudaFree(m->d_maxrate);
+  if (m->d_sums) cudaFree(m->d_sums);
+  if (m->d_stage) cudaFree(m->d_stage);
+  delete m;
+  return F4_OK;
+}
+
+int f4_set_options(f4_mesh* m, int limiter, int flux_scheme, double theta) {
+  if (!m) return F4_EINVAL;
+  if (limiter < 0 || limiter > F4_LIM_MC || flux_scheme < 0 || flux_scheme > F4_FLUX_RUSANOV || !(theta >= 1.0))
+    return fail(m, F4_EINVAL, "bad option");
+  m->limiter = limiter;
+  m->flux = flux_scheme;
+  m->theta = theta;
+  return F4_OK;
+}
+
+size_t f4_storage_bytes(const f4_mesh* m) { return m ? m->state_doubles * (size_t)m->n_states * sizeof(double) : 0; }
+
+int f4_bind_storage(f4_mesh* m, void* dev_ptr, size_t bytes, void* cuda_stream) {
+  if (!m) return F4_EINVAL;
+  if (!dev_ptr || bytes < f4_storage_bytes(m) || ((uintptr_t)dev_ptr & 255)) return fail(m, F4_EINVAL, "bad storage");
+  if (m->hm.Ng != NG || !stage_supported(m->hm.dim, m->hm.N))
+    return fail(m, F4_EUNSUPPORTED, "CUDA kernels exist for n_ghost=2 and (dim,N) in {(2,8),(2,16),(3,8),(3,16),(3,32)}");
+  int ndev = 0;
+  CU(cudaGetDeviceCount(&ndev));
+  if (ndev < 1) return fail(m, F4_ECUDA, "no CUDA device");
+  m->store = (double*)dev_ptr;
+  m->stream = (cudaStream_t)cuda_stream;
+  if (!m->d_level) {
+    CU(cudaMalloc((void**)&m->d_level, (size_t)m->hm.max_blocks * sizeof(int)));
+    CU(cudaMalloc((void**)&m->d_maxrate, sizeof(unsigned long long)));
+    CU(cudaMalloc((void**)&m->d_sums, (size_t)m->hm.max_blocks * m->nvar * sizeof(double)));
+    // staging: whole blocks of the natural padded layout, at most 128 MiB
+    size_t per_block = m->bs * sizeof(double);
+    size_t nblk = (128u << 20) / per_block;
+    if (nblk < 1) nblk = 1;
+    if (nblk > (size_t)m->hm.max_blocks) nblk = m->hm.max_blocks;
+    m->stage_bytes = nblk * per_block;
+    CU(cudaMalloc((void**)&m->d_stage, m->stage_bytes));
+  }
+  m->bound = true;
+  for (int s = 0; s < m->n_states; ++s) {
+    Scope sc(m, F4_PROF_LAYOUT);
+    CU(launch_init_benign(m->hm.dim, m->hm.N, m->state_ptr(s), m->hm.max_blocks, m->gamma, m->stream));
+  }
+  m->rate_valid = false;
+  return upload_meta(m);
+}
+
+int f4_num_blocks(const f4_mesh* m) { return m ? (int)m->hm.leaves.size() : F4_EINVAL; }
+
+int f4_get_blocks(const f4_mesh* m, int* level, int* coords, double* origin, double* dx) {
+  if (!m) return F4_EINVAL;
+  const int nb = (int)m->hm.leaves.size();
+  for (int b = 0; b < nb; ++b) {
+    const Leaf& l = m->hm.leaves[b];
+    const double h = m->hm.dx_of_level(l.level);
+    if (level) level[b] = l.level;
+    if (dx) dx[b] = h;
+    for (int a = 0; a < 3; ++a) {
+      if (coords) coords[3 * b + a] = l.c[a];
+      if (origin) origin[3 * b + a] = (a < m->hm.dim) ? (double)l.c[a] * m->hm.N * h : 0.0;
+    }
+  }
+  return F4_OK;
+}
+
+int f4_set_state(f4_mesh* m, int state, const double* src, int src_is_device, int with_ghosts) {
+  int rc = check_state(m, state);
+  if (rc) return rc;
+  if (!src) return fail(m, F4_EINVAL, "null source");
+  const int nb = (int)m->hm.leaves.size(), dim = m->hm.dim, N = m->hm.N;
+  const size_t E = with_ghosts ? N + 2 * m->hm.Ng : N;
+  const size_t per_block = (size_t)m->nvar * E * E * (dim == 3 ? E : 1);
+  if (state == 0) m->rate_valid = false;
+  if (src_is_device) {
+    Scope sc(m, F4_PROF_LAYOUT);
+    CU(launch_pack(dim, N, m->state_ptr(state), src, 0, nb, with_ghosts, m->stream));
+    return F4_OK;
+  }
+  const int chunk = (int)(m->stage_bytes / (per_block * sizeof(double)));
+  for (int b0 = 0; b0 < nb; b0 += chunk) {
+    const int n = (nb - b0 < chunk) ? nb - b0 : chunk;
+    CU(cudaMemcpyAsync(m->d_stage, src + (size_t)b0 * per_block, (size_t)n * per_block * sizeof(double),
+                       cudaMemcpyHostToDevice, m->stream));
+    Scope sc(m, F4_PROF_LAYOUT);
+    CU(launch_pack(dim, N, m->state_ptr(state), m->d_stage, b0, n, with_ghosts, m->stream));
+  }
+  CU(cudaStreamSynchronize(m->stream));
+  return F4_OK;
+}
+
+int f4_get_state(f4_mesh* m, int state, double* dst, int dst_is_device, int with_ghosts) {
+  int rc = check_state(m, state);
+  if (rc) return rc;
+  if (!dst) return fail(m, F4_EINVAL, "null destination");
+  const int nb = (int)m->hm.leaves.size(), dim = m->hm.dim, N = m->hm.N;
+  const size_t E = with_ghosts ? N + 2 * m->hm.Ng : N;
+  const size_t per_block = (size_t)m->nvar * E * E * (dim == 3 ? E : 1);
+  if (dst_is_device) {
+    Scope sc(m, F4_PROF_LAYOUT);
+    CU(launch_unpack(dim, N, m->state_ptr(state), dst, 0, nb, with_ghosts, m->stream));
+    return F4_OK;
+  }
+  const int chunk = (int)(m->stage_bytes / (per_block * sizeof(double)));
+  for (int b0 = 0; b0 < nb; b0 += chunk) {
+    const int n = (nb - b0 < chunk) ? nb - b0 : chunk;
+    {
+      Scope sc(m, F4_PROF_LAYOUT);
+      CU(launch_unpack(dim, N, m->state_ptr(state), m->d_stage, b0, n, with_ghosts, m->stream));
+    }
+    CU(cudaMemcpyAsync(dst + (size_t)b0 * per_block, m->d_stage, (size_t)n * per_block * sizeof(double),
+                       cudaMemcpyDeviceToHost, m->stream));
+  }
+  CU(cudaStreamSynchronize(m->stream));
+  return F4_OK;
+}
+
+int f4_build_ghost_pattern(f4_mesh* m) {
+  if (!m) return F4_EINVAL;
+  std::string err;
+  int rc = m->hm.build_pattern(err);
+  if (rc) return fail(m, rc, err);
+  return upload_meta(m);
+}
+
+int f4_pattern_size(const f4_mesh* m, int* n_r1, int* n_r2) {
+  if (!m) return F4_EINVAL;
+  if (n_r1) *n_r1 = (int)m->hm.r1.size();
+  if (n_r2) *n_r2 = (int)m->hm.r2.size();
+  return F4_OK;
+}
+
+int f4_get_pattern(const f4_mesh* m, int* records) {
+  if (!m || !records) return F4_EINVAL;
+  size_t q = 0;
+  for (const std::vector<Record>* r : {&m->hm.r1, &m->hm.r2})
+    for (const Record& x : *r) {
+      int* o = records + 6 * q++;
+      o[0] = x.op; o[1] = x.face; o[2] = x.dst; o[3] = x.src; o[4] = x.o1; o[5] = x.o2;
+    }
+  return F4_OK;
+}
+
+int f4_fill_ghosts(f4_mesh* m, int state) {
+  int rc = check_state(m, state);
+  if (rc) return rc;
+  return fill_ghosts_impl(m, state);
+}
+
+int f4_compute_dt(f4_mesh* m, int state, double cfl, double* dt_out) {
+  int rc = check_state(m, state);
+  if (rc) return rc;
+  if (!dt_out || !(cfl > 0.0)) return fail(m, F4_EINVAL, "bad cfl / null output");
+  if (!(state == 0 && m->rate_valid)) {
+    CU(cudaMemsetAsync(m->d_maxrate, 0, sizeof(unsigned long long), m->stream));
+    Scope sc(m, F4_PROF_DT);
+    CU(launch_maxrate(m->hm.dim, m->hm.N, m->state_ptr(state), m->d_level, (int)m->hm.leaves.size(), m->gamma,
+                      1.0 / m->hm.dx_of_level(0), m->d_maxrate, m->stream));
+  }
+  double rate = 0.0;
+  CU(cudaMemcpyAsync(&rate, m->d_maxrate, sizeof(double), cudaMemcpyDeviceToHost, m->stream));
+  CU(cudaStreamSynchronize(m->stream));
+  m->rate_valid = (state == 0);  // d_maxrate now describes this state
+  if (!(rate > 0.0) || rate != rate) return fail(m, F4_EINVAL, "compute_dt: wave speed is zero or not finite");
+  *dt_out = cfl / rate;
+  return F4_OK;
+}
+
+int f4_advance(f4_mesh* m, double dt) {
+  int rc = check_state(m, 0);
+  if (rc) return rc;
+  if (!(dt > 0.0)) return fail(m, F4_EINVAL, "dt must be positive");
+  const int dim = m->hm.dim, N = m->hm.N, nb = (int)m->hm.leaves.size();
+  StageParams p{};
+  p.gamma = m->gamma;
+  p.inv_dx0 = 1.0 / m->hm.dx_of_level(0);
+  p.level = m->d_level;
+  p.nblocks = nb;
+  p.limiter = m->limiter;
+  p.flux = m->flux;
+  // stage 1, eq. (6): u1 = dt F(ut) + ut
+  if ((rc = fill_ghosts_impl(m, 0))) return rc;
+  p.deriv = m->state_ptr(0);
+  p.prev0 = m->state_ptr(0);
+  p.prev1 = nullptr;
+  p.out = m->state_ptr(1);
+  p.w0 = 1.0;
+  p.w1 = 0.0;
+  p.dt_sub = dt;
+  p.maxrate = nullptr;
+  {
+    Scope sc(m, F4_PROF_STAGE);
+    CU(launch_stage(dim, N, p, m->stream));
+  }
+  // stage 2, eq. (7): u = dt/2 F(u1) + (ut + u1)/2, written over ut; CFL max of the new state fused in
+  if ((rc = fill_ghosts_impl(m, 1))) return rc;
+  CU(cudaMemsetAsync(m->d_maxrate, 0, sizeof(unsigned long long), m->stream));
+  p.deriv = m->state_ptr(1);
+  p.prev0 = m->state_ptr(0);
+  p.prev1 = m->state_ptr(1);
+  p.out = m->state_ptr(0);
+  p.w0 = 0.5;
+  p.w1 = 0.5;
+  p.dt_sub = 0.5 * dt;
+  p.maxrate = m->d_maxrate;
+  {
+    Scope sc(m, F4_PROF_STAGE);
+    CU(launch_stage(dim, N, p, m->stream));
+  }
+  m->rate_valid = true;
+  return F4_OK;
+}
+
+int f4_adapt(f4_mesh* m, const int* refine_flags, int* changed_out) {
+  if (!m || !refine_flags || !changed_out) return F4_EINVAL;
+  *changed_out = 0;
+  int rc;
+  if (m->bound && (rc = fill_ghosts_impl(m, 0))) return rc;  // prolongation reads the parents' face ghosts
+  std::vector<Transfer> plan;
+  bool changed = false;
+  std::string err;
+  rc = m->hm.adapt(refine_flags, plan, changed, err);
+  if (rc) return fail(m, rc, err);
+  if (!changed) return F4_OK;
+  *changed_out = 1;
+  if (!m->bound) return F4_OK;
+  std::vector<DevTransfer> dp(plan.size());
+  for (size_t q = 0; q < plan.size(); ++q) {
+    dp[q].kind = plan[q].kind;
+    dp[q].dst = plan[q].dst;
+    dp[q].oct = plan[q].oct;
+    dp[q].pad = 0;
+    for (int c = 0; c < 8; ++c) dp[q].src[c] = plan[q].src[c];
+  }
+  if ((rc = ensure(m, m->d_plan, m->cap_plan, dp.size()))) return rc;
+  CU(cudaMemcpyAsync(m->d_plan, dp.data(), dp.size() * sizeof(DevTransfer), cudaMemcpyHostToDevice, m->stream));
+  {
+    Scope sc(m, F4_PROF_REGRID);
+    CU(launch_transfer(m->hm.dim, m->hm.N, m->state_ptr(0), m->state_ptr(1), m->d_plan, (int)dp.size(), m->theta,
+                       m->stream));
+  }
+  CU(cudaStreamSynchronize(m->stream));
+  std::swap(m->phys[0], m->phys[1]);  // the new numbering lives in the slab that was state 1
+  m->rate_valid = false;
+  return upload_meta(m);
+}
+
+int f4_conserved_totals(f4_mesh* m, int state, double* totals) {
+  int rc = check_state(m, state);
+  if (rc) return rc;
+  if (!totals) return fail(m, F4_EINVAL, "null output");
+  const int nb = (int)m->hm.leaves.size();
+  {
+    Scope sc(m, F4_PROF_LAYOUT);
+    CU(launch_block_sums(m->hm.dim, m->hm.N, m->state_ptr(state), nb, m->d_sums, m->stream));
+  }
+  std::vector<double> sums((size_t)nb * m->nvar);
+  CU(cudaMemcpyAsync(sums.data(), m->d_sums, sums.size() * sizeof(double), cudaMemcpyDeviceToHost, m->stream));
+  CU(cudaStreamSynchronize(m->stream));
+  for (int v = 0; v < m->nvar; ++v) {
+    long double acc = 0.0L;
+    for (int b = 0; b < nb; ++b) {
+      long double h = m->hm.dx_of_level(m->hm.leaves[b].level);
+      acc += (long double)sums[(size_t)b * m->nvar + v] * (h * h * (m->hm.dim == 3 ? h : 1.0L));
+    }
+    totals[v] = (double)acc;
+  }
+  return F4_OK;
+}
+
+int f4_profile_enable(f4_mesh* m, int on) {
+  if (!m) return F4_EINVAL;
+  m->prof = on != 0;
+  return F4_OK;
+}
+
+int f4_profile_get(f4_mesh* m, double ms[F4_PROF_N], long long launches[F4_PROF_N], int reset) {
+  if (!m) return F4_EINVAL;
+  if (m->bound) CU(cudaStreamSynchronize(m->stream));
+  for (auto& e : m->evs) {
+    float t = 0.f;
+    if (cudaEventElapsedTime(&t, e.a, e.b) == cudaSuccess) m->prof_ms[e.cls] += t;
+    cudaEventDestroy(e.a);
+    cudaEventDestroy(e.b);
+  }
+  m->evs.clear();
+  for (int c = 0; c < F4_PROF_N; ++c) {
+    if (ms) ms[c] = m->prof_ms[c];
+    if (launches) launches[c] = m->prof_n[c];
+    if (reset) { m->prof_ms[c] = 0.0; m->prof_n[c] = 0; }
+  }
+  return F4_OK;
+}
+
+long long f4_launch_count(const f4_mesh* m) { return m ? m->launches : 0; }
+
+const char* f4_last_error(const f4_mesh* m) { return m ? m->err.c_str() : "null mesh"; }
+
+}  // extern "C"

@@ -1,0 +1,61 @@
+// Device-side interface between the C-ABI (f4_api.cu) and the kernels.
+// Store layout: [state][block][var][kslot][jslot][islot],
+// P = N + 2*NG slots per axis, slot(i) = i for i >= 0, i + P for i < 0.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstddef>
+#include <cstdint>
+
+namespace f4 {
+
+constexpr int NG = 2;  // ghost layers compiled into the kernels
+
+// meta = op | face << 2 | o1 << 5 | o2 << 6
+struct DevRecord {
+  int dst, src, meta, pad;
+};
+
+struct DevTransfer {
+  int kind, dst, oct, pad;
+  int src[8];
+};
+
+struct StageParams {
+  const double* deriv;  // state whose time derivative is taken (ghosts filled)
+  const double* prev0;  // eq. (5): out = dt_sub*F(deriv) + w0*prev0 + w1*prev1
+  const double* prev1;  // may be nullptr (w1 ignored)
+  double* out;
+  double w0, w1, dt_sub;
+  double gamma;
+  double inv_dx0;       // 1/dx at level 0
+  const int* level;     // per block
+  int nblocks;
+  int limiter, flux;
+  unsigned long long* maxrate;  // bits of a non-negative double, atomicMax; nullptr = no CFL reduction
+};
+
+struct GhostParams {
+  double* state;
+  const DevRecord* rec;
+  int nrec;
+  double theta;
+};
+
+// every launcher returns the cudaError_t of the launch
+cudaError_t launch_ghost(int dim, int n, const GhostParams& p, cudaStream_t s);
+cudaError_t launch_stage(int dim, int n, const StageParams& p, cudaStream_t s);
+cudaError_t launch_maxrate(int dim, int n, const double* state, const int* level, int nblocks, double gamma,
+                           double inv_dx0, unsigned long long* maxrate, cudaStream_t s);
+cudaError_t launch_transfer(int dim, int n, const double* old_state, double* new_state, const DevTransfer* plan,
+                            int nplan, double theta, cudaStream_t s);
+// layout kernels: natural (interior or padded) <-> wrapped padded store
+cudaError_t launch_pack(int dim, int n, double* store_state, const double* src, int b0, int nb, int with_ghosts,
+                        cudaStream_t s);
+cudaError_t launch_unpack(int dim, int n, const double* store_state, double* dst, int b0, int nb, int with_ghosts,
+                          cudaStream_t s);
+cudaError_t launch_init_benign(int dim, int n, double* store_state, int nb, double gamma, cudaStream_t s);
+cudaError_t launch_block_sums(int dim, int n, const double* state, int nb, double* sums /*[nb][nvar]*/, cudaStream_t s);
+bool stage_supported(int dim, int n);
+
+}  // namespace f4

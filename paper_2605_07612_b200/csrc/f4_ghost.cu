@@ -1,0 +1,404 @@
+// Ghost-pattern executor, regrid transfer and layout kernels (sm_100a).
+//
+// Ghost pattern (section 2.6): ONE batched kernel per round,
+// driven by a device-resident list of records (dst block, src block, face, op)
+// sorted by destination block, instead of one OpenACC loop per boundary type
+// and face direction.  A CTA takes 2*DIM consecutive
+// records (= all faces of one block on a uniform mesh), so that the -x and +x
+// ghost pairs of a row, which share one 32-byte sector in the wrapped layout,
+// are written back-to-back and merge in L2.  HBM-bound: 16-byte vector
+// accesses, all loads of a thread issued before its stores.
+#include "../../include/f4.h"
+#include "f4_dev.hpp"
+
+namespace f4 {
+namespace {
+
+template <int DIM, int N>
+struct Geo {
+  static constexpr int P = N + 2 * NG;
+  static constexpr int PZ = (DIM == 3) ? P : 1;
+  static constexpr int NZ = (DIM == 3) ? N : 1;
+  static constexpr int NVAR = DIM + 2;
+  static constexpr int H = N / 2;
+  static constexpr size_t VS = (size_t)P * P * PZ;   // doubles per (block, var)
+  static constexpr size_t BS = VS * NVAR;            // doubles per block
+  __host__ __device__ static constexpr int slot(int i) { return i < 0 ? i + P : i; }
+};
+
+__device__ __forceinline__ double2 ld2(const double* p) { return *reinterpret_cast<const double2*>(p); }
+__device__ __forceinline__ void st2(double* p, double2 v) { *reinterpret_cast<double2*>(p) = v; }
+
+// slot offset of cell (i,j,k) inside one (block,var) box
+template <int DIM, int N>
+__device__ __forceinline__ int cell_off(int i, int j, int k) {
+  using G = Geo<DIM, N>;
+  int o = G::slot(j) * G::P + G::slot(i);
+  if (DIM == 3) o += G::slot(k) * G::P * G::P;
+  return o;
+}
+
+// generalised minmod, eq. (1)
+__device__ __forceinline__ double minmod_g(double a, double b, double theta) {
+  double m = fmin(fmin(fabs(theta * a), fabs(theta * b)), fabs(a + b) * 0.5);
+  double r = (a > 0.0) ? m : -m;
+  return (a * b <= 0.0) ? 0.0 : r;
+}
+
+// mean of the 2^d fine cells with lowest member (i0,j0,k0); pairwise x -> y -> z, adds only
+// (reading A8): bit-exact by construction.  i0 is even, so each x pair is one 16-byte load.
+template <int DIM, int N>
+__device__ __forceinline__ double restrict_mean(const double* fv, int i0, int j0, int k0) {
+  using G = Geo<DIM, N>;
+  const double* p = fv + cell_off<DIM, N>(i0, j0, k0);
+  double2 a = ld2(p), b = ld2(p + G::P);
+  double s0 = __dadd_rn(__dadd_rn(a.x, a.y), __dadd_rn(b.x, b.y));
+  if (DIM == 2) return __dmul_rn(s0, 0.25);
+  double2 c = ld2(p + G::P * G::P), d = ld2(p + G::P * G::P + G::P);
+  double s1 = __dadd_rn(__dadd_rn(c.x, c.y), __dadd_rn(d.x, d.y));
+  return __dmul_rn(__dadd_rn(s0, s1), 0.125);
+}
+
+// limited slopes of coarse cell (ic,jc,kc): one-sided differences -> eq. (1)
+template <int DIM, int N>
+__device__ __forceinline__ void coarse_slopes(const double* cv, int ic, int jc, int kc, double theta, double& uc,
+                                              double& sx, double& sy, double& sz) {
+  uc = cv[cell_off<DIM, N>(ic, jc, kc)];
+  sx = minmod_g(uc - cv[cell_off<DIM, N>(ic - 1, jc, kc)], cv[cell_off<DIM, N>(ic + 1, jc, kc)] - uc, theta);
+  sy = minmod_g(uc - cv[cell_off<DIM, N>(ic, jc - 1, kc)], cv[cell_off<DIM, N>(ic, jc + 1, kc)] - uc, theta);
+  sz = 0.0;
+  if (DIM == 3)
+    sz = minmod_g(uc - cv[cell_off<DIM, N>(ic, jc, kc - 1)], cv[cell_off<DIM, N>(ic, jc, kc + 1)] - uc, theta);
+}
+// child value u_c + (+-1/4 dx +- 1/4 dy) +- 1/4 dz, evaluated in that order (reading A9)
+template <int DIM>
+__device__ __forceinline__ double child_value(double uc, double sx, double sy, double sz, int px, int py, int pz) {
+  double r = __dadd_rn(px ? 0.25 * sx : -0.25 * sx, py ? 0.25 * sy : -0.25 * sy);
+  if (DIM == 3) r = __dadd_rn(r, pz ? 0.25 * sz : -0.25 * sz);
+  return __dadd_rn(uc, r);
+}
+
+// ---------------------------------------------------------------------------
+// ghost executor
+// ---------------------------------------------------------------------------
+template <int DIM, int N>
+__device__ __forceinline__ void do_copy_face(double* __restrict__ st, int dst, int src, int face, bool outflow) {
+  using G = Geo<DIM, N>;
+  constexpr int P = G::P, NV = G::NVAR;
+  const int a = face >> 1, side = face & 1;
+  // destination ghost slots along the normal: low ghosts P-2,P-1 (cells -2,-1); high ghosts N,N+1
+  const int dn = side ? N : P - 2;
+  // source slots: SRL -x: neighbour's cells N-2,N-1; +x: cells 0,1.  Outflow: nearest own interior layer.
+  const int sn = outflow ? (side ? N - 1 : 0) : (side ? 0 : N - 2);
+  const int sq = outflow ? 0 : 1;  // source advances with the layer only for SRL
+  double* db = st + (size_t)dst * G::BS;
+  const double* sb = st + (size_t)src * G::BS;
+  constexpr int PER_VAR = (DIM == 3) ? N * N : N;  // 16-byte units per variable
+  constexpr int TOTAL = NV * PER_VAR;
+  constexpr int UNR = 5;
+  for (int e0 = threadIdx.x; e0 < TOTAL; e0 += UNR * blockDim.x) {
+    double2 val[UNR];
+    int doff[UNR];
+#pragma unroll
+    for (int u = 0; u < UNR; ++u) {
+      int e = e0 + u * blockDim.x;
+      doff[u] = -1;
+      if (e < TOTAL) {
+        int v = e / PER_VAR, r = e % PER_VAR;
+        int so, d_o;
+        if (a == 0) {  // one row = one 16-byte ghost pair
+          int j = r % N, k = (DIM == 3) ? r / N : 0;
+          int row = (DIM == 3 ? k * P * P : 0) + j * P;
+          d_o = row + dn;
+          so = row + sn;
+          if (outflow) {
+            double x = sb[(size_t)v * G::VS + so];
+            val[u] = make_double2(x, x);
+          } else {
+            val[u] = ld2(sb + (size_t)v * G::VS + so);
+          }
+        } else {
+          int h, q, t;
+          if (DIM == 3) {
+            if (a == 1) { t = r / N; q = (r % N) / G::H; h = r % G::H; }   // t = k
+            else        { q = r / (N * G::H); t = (r / G::H) % N; h = r % G::H; }  // t = j
+          } else { q = r / G::H; h = r % G::H; t = 0; }
+          int dl = dn + q, sl = sn + sq * q;
+          if (DIM == 3) {
+            if (a == 1) { d_o = t * P * P + dl * P + 2 * h; so = t * P * P + sl * P + 2 * h; }
+            else        { d_o = dl * P * P + t * P + 2 * h; so = sl * P * P + t * P + 2 * h; }
+          } else { d_o = dl * P + 2 * h; so = sl * P + 2 * h; }
+          val[u] = ld2(sb + (size_t)v * G::VS + so);
+        }
+        doff[u] = v * (int)G::VS + d_o;
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < UNR; ++u)
+      if (doff[u] >= 0) st2(db + doff[u], val[u]);
+  }
+}
+
+template <int DIM, int N>
+__device__ __forceinline__ void do_f2c(double* __restrict__ st, int dst, int src, int face, int o1, int o2) {
+  using G = Geo<DIM, N>;
+  constexpr int H = G::H, NV = G::NVAR;
+  const int a = face >> 1, side = face & 1;
+  constexpr int PER_VAR = NG * ((DIM == 3) ? H * H : H);
+  double* db = st + (size_t)dst * G::BS;
+  const double* sb = st + (size_t)src * G::BS;
+  for (int e = threadIdx.x; e < NV * PER_VAR; e += blockDim.x) {
+    int v = e / PER_VAR, r = e % PER_VAR;
+    int tt1 = r % H, tt2 = (DIM == 3) ? (r / H) % H : 0, q = r / ((DIM == 3) ? H * H : H);
+    // coarse ghost cell: normal index N+q (high) or -2+q (low); its fine children along the normal
+    int nc = side ? N + q : -2 + q;
+    int nf = side ? 2 * q : N - 4 + 2 * q;
+    int t1c = o1 * H + tt1, t2c = o2 * H + tt2;
+    int ci, cj, ck, fi, fj, fk;
+    if (a == 0) { ci = nc; cj = t1c; ck = t2c; fi = nf; fj = 2 * tt1; fk = 2 * tt2; }
+    else if (a == 1) { cj = nc; ci = t1c; ck = t2c; fj = nf; fi = 2 * tt1; fk = 2 * tt2; }
+    else { ck = nc; ci = t1c; cj = t2c; fk = nf; fi = 2 * tt1; fj = 2 * tt2; }
+    if (DIM == 2) { ck = 0; fk = 0; }
+    db[(size_t)v * G::VS + cell_off<DIM, N>(ci, cj, ck)] = restrict_mean<DIM, N>(sb + (size_t)v * G::VS, fi, fj, fk);
+  }
+}
+
+template <int DIM, int N>
+__device__ __forceinline__ void do_c2f(double* __restrict__ st, int dst, int src, int face, int o1, int o2,
+                                       double theta) {
+  using G = Geo<DIM, N>;
+  constexpr int H = G::H, NV = G::NVAR;
+  const int a = face >> 1, side = face & 1;
+  constexpr int PER_VAR = (DIM == 3) ? H * H : H;  // coarse cells of the one coarse layer (NG/2 = 1)
+  double* db = st + (size_t)dst * G::BS;
+  const double* sb = st + (size_t)src * G::BS;
+  const int ncoarse = side ? 0 : N - 1;   // F's high ghosts are covered by C's first cell, low ghosts by its last
+  const int nfine = side ? N : -2;        // lower of the two fine ghost cells (lower half of the coarse cell)
+  for (int e = threadIdx.x; e < NV * PER_VAR; e += blockDim.x) {
+    int v = e / PER_VAR, r = e % PER_VAR;
+    int tt1 = r % H, tt2 = (DIM == 3) ? r / H : 0;
+    int t1c = o1 * H + tt1, t2c = o2 * H + tt2;
+    int ic, jc, kc, fi, fj, fk;
+    if (a == 0) { ic = ncoarse; jc = t1c; kc = t2c; fi = nfine; fj = 2 * tt1; fk = 2 * tt2; }
+    else if (a == 1) { jc = ncoarse; ic = t1c; kc = t2c; fj = nfine; fi = 2 * tt1; fk = 2 * tt2; }
+    else { kc = ncoarse; ic = t1c; jc = t2c; fk = nfine; fi = 2 * tt1; fj = 2 * tt2; }
+    if (DIM == 2) { kc = 0; fk = 0; }
+    double uc, sx, sy, sz;
+    coarse_slopes<DIM, N>(sb + (size_t)v * G::VS, ic, jc, kc, theta, uc, sx, sy, sz);
+    double* dv = db + (size_t)v * G::VS;
+#pragma unroll
+    for (int pz = 0; pz < (DIM == 3 ? 2 : 1); ++pz)
+#pragma unroll
+      for (int py = 0; py < 2; ++py) {
+        double2 w;
+        w.x = child_value<DIM>(uc, sx, sy, sz, 0, py, pz);
+        w.y = child_value<DIM>(uc, sx, sy, sz, 1, py, pz);
+        st2(dv + cell_off<DIM, N>(fi, fj + py, fk + pz), w);   // fi even or -2: the x pair is 16-byte aligned
+      }
+  }
+}
+
+template <int DIM, int N>
+__global__ void __launch_bounds__(256) ghost_exec_kernel(GhostParams p) {
+  constexpr int CH = 2 * DIM;
+  int r0 = blockIdx.x * CH;
+#pragma unroll 1
+  for (int q = 0; q < CH; ++q) {
+    int r = r0 + q;
+    if (r >= p.nrec) break;
+    DevRecord rec = p.rec[r];
+    int op = rec.meta & 3, face = (rec.meta >> 2) & 7, o1 = (rec.meta >> 5) & 1, o2 = (rec.meta >> 6) & 1;
+    if (op == F4_OP_SRL) do_copy_face<DIM, N>(p.state, rec.dst, rec.src, face, false);
+    else if (op == F4_OP_BC) do_copy_face<DIM, N>(p.state, rec.dst, rec.src, face, true);
+    else if (op == F4_OP_F2C) do_f2c<DIM, N>(p.state, rec.dst, rec.src, face, o1, o2);
+    else do_c2f<DIM, N>(p.state, rec.dst, rec.src, face, o1, o2, p.theta);
+  }
+}
+
+// ---------------------------------------------------------------------------
+// regrid transfer: one CTA per new block
+// ---------------------------------------------------------------------------
+template <int DIM, int N>
+__global__ void __launch_bounds__(256) transfer_kernel(const double* __restrict__ old_st, double* __restrict__ new_st,
+                                                       const DevTransfer* __restrict__ plan, double theta) {
+  using G = Geo<DIM, N>;
+  constexpr int H = G::H, NV = G::NVAR, NZ = G::NZ;
+  const DevTransfer t = plan[blockIdx.x];
+  double* db = new_st + (size_t)t.dst * G::BS;
+  if (t.kind == 0) {  // unaltered: copy the interior
+    const double* sb = old_st + (size_t)t.src[0] * G::BS;
+    for (int e = threadIdx.x; e < NV * NZ * N * H; e += blockDim.x) {
+      int h = e % H, j = (e / H) % N, k = (e / (H * N)) % NZ, v = e / (H * N * NZ);
+      size_t o = (size_t)v * G::VS + cell_off<DIM, N>(2 * h, j, k);
+      st2(db + o, ld2(sb + o));
+    }
+  } else if (t.kind == 1) {  // refined: limited prolongation of the parent's octant (needs the parent's face ghosts)
+    const double* sb = old_st + (size_t)t.src[0] * G::BS;
+    const int ox = t.oct & 1, oy = (t.oct >> 1) & 1, oz = (t.oct >> 2) & 1;
+    constexpr int HZ = (DIM == 3) ? H : 1;
+    for (int e = threadIdx.x; e < NV * HZ * H * H; e += blockDim.x) {
+      int i = e % H, j = (e / H) % H, k = (e / (H * H)) % HZ, v = e / (H * H * HZ);
+      double uc, sx, sy, sz;
+      coarse_slopes<DIM, N>(sb + (size_t)v * G::VS, ox * H + i, oy * H + j, (DIM == 3) ? oz * H + k : 0, theta, uc, sx,
+                            sy, sz);
+      double* dv = db + (size_t)v * G::VS;
+#pragma unroll
+      for (int pz = 0; pz < (DIM == 3 ? 2 : 1); ++pz)
+#pragma unroll
+        for (int py = 0; py < 2; ++py) {
+          double2 w;
+          w.x = child_value<DIM>(uc, sx, sy, sz, 0, py, pz);
+          w.y = child_value<DIM>(uc, sx, sy, sz, 1, py, pz);
+          st2(dv + cell_off<DIM, N>(2 * i, 2 * j + py, 2 * k + pz), w);
+        }
+    }
+  } else {  // coarsened: restriction of the 2^d children
+    constexpr int HZ = (DIM == 3) ? H : 1;
+    constexpr int NCH = 1 << DIM;
+    for (int e = threadIdx.x; e < NCH * NV * HZ * H * H; e += blockDim.x) {
+      int i = e % H, j = (e / H) % H, k = (e / (H * H)) % HZ, v = (e / (H * H * HZ)) % NV, c = e / (H * H * HZ * NV);
+      const double* sb = old_st + (size_t)t.src[c] * G::BS + (size_t)v * G::VS;
+      int ox = c & 1, oy = (c >> 1) & 1, oz = (c >> 2) & 1;
+      db[(size_t)v * G::VS + cell_off<DIM, N>(ox * H + i, oy * H + j, (DIM == 3) ? oz * H + k : 0)] =
+          restrict_mean<DIM, N>(sb, 2 * i, 2 * j, 2 * k);
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------
+// layout kernels (not on the per-step path)
+// ---------------------------------------------------------------------------
+template <int DIM, int N, bool PACK>
+__global__ void __launch_bounds__(256) layout_kernel(double* __restrict__ store, double* __restrict__ user, int b0,
+                                                     int with_ghosts) {
+  using G = Geo<DIM, N>;
+  const int E = with_ghosts ? G::P : N, EZ = (DIM == 3) ? E : 1, lo = with_ghosts ? -NG : 0;
+  const int b = blockIdx.x, v = blockIdx.y;
+  const size_t ubase = ((size_t)b * G::NVAR + v) * (size_t)(E * E * EZ);
+  double* sv = store + ((size_t)(b0 + b) * G::NVAR + v) * G::VS;
+  for (int e = threadIdx.x; e < E * E * EZ; e += blockDim.x) {
+    int i = e % E + lo, j = (e / E) % E + lo, k = (DIM == 3) ? e / (E * E) + lo : 0;
+    int o = cell_off<DIM, N>(i, j, k);
+    if (PACK) sv[o] = user[ubase + e];
+    else user[ubase + e] = sv[o];
+  }
+}
+
+template <int DIM, int N>
+__global__ void __launch_bounds__(256) init_benign_kernel(double* __restrict__ store, double gamma) {
+  using G = Geo<DIM, N>;
+  const int b = blockIdx.x, v = blockIdx.y;
+  double val = (v == 0) ? 1.0 : (v == G::NVAR - 1 ? 1.0 / (gamma - 1.0) : 0.0);  // rho=1, u=0, p=1
+  double* sv = store + ((size_t)b * G::NVAR + v) * G::VS;
+  for (int e = threadIdx.x; e < (int)G::VS; e += blockDim.x) sv[e] = val;
+}
+
+// per-(block,var) interior sums, fixed order inside the CTA (for f4_conserved_totals)
+template <int DIM, int N>
+__global__ void __launch_bounds__(256) block_sums_kernel(const double* __restrict__ st, double* __restrict__ sums) {
+  using G = Geo<DIM, N>;
+  __shared__ double sh[256];
+  const int b = blockIdx.x, v = blockIdx.y;
+  const double* sv = st + ((size_t)b * G::NVAR + v) * G::VS;
+  double acc = 0.0;
+  for (int e = threadIdx.x; e < N * N * G::NZ; e += blockDim.x) {
+    int i = e % N, j = (e / N) % N, k = e / (N * N);
+    acc += sv[cell_off<DIM, N>(i, j, k)];
+  }
+  sh[threadIdx.x] = acc;
+  __syncthreads();
+  for (int s = 128; s > 0; s >>= 1) {
+    if ((int)threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) sums[(size_t)b * G::NVAR + v] = sh[0];
+}
+
+// CFL: max over interior cells of sum_dim (|u_d| + c)/dx (readings A4-A5).
+// Warp shuffle max, then one atomicMax per warp on the bit pattern (non-negative doubles order as integers).
+template <int DIM, int N>
+__global__ void __launch_bounds__(256) maxrate_kernel(const double* __restrict__ st, const int* __restrict__ level,
+                                                      double gamma, double inv_dx0, unsigned long long* maxrate) {
+  using G = Geo<DIM, N>;
+  const int b = blockIdx.x;
+  const double* sb = st + (size_t)b * G::BS;
+  const double inv_dx = inv_dx0 * (double)(1u << level[b]);
+  double mx = 0.0;
+  for (int e = threadIdx.x; e < N * N * G::NZ; e += blockDim.x) {
+    int i = e % N, j = (e / N) % N, k = e / (N * N);
+    int o = cell_off<DIM, N>(i, j, k);
+    double rho = sb[o], ir = 1.0 / rho, ke = 0.0, su = 0.0;
+#pragma unroll
+    for (int d = 0; d < DIM; ++d) {
+      double u = sb[(size_t)(1 + d) * G::VS + o] * ir;
+      ke += u * u;
+      su += fabs(u);
+    }
+    double p = (gamma - 1.0) * (sb[(size_t)(DIM + 1) * G::VS + o] - 0.5 * rho * ke);
+    double c = sqrt(gamma * p * ir);
+    mx = fmax(mx, (su + DIM * c) * inv_dx);
+  }
+  for (int s = 16; s > 0; s >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, s));
+  if ((threadIdx.x & 31) == 0) atomicMax(maxrate, (unsigned long long)__double_as_longlong(mx));
+}
+
+template <typename F>
+cudaError_t dispatch(int dim, int n, F&& f) {
+  if (dim == 2 && n == 8) return f(Geo<2, 8>{});
+  if (dim == 2 && n == 16) return f(Geo<2, 16>{});
+  if (dim == 3 && n == 8) return f(Geo<3, 8>{});
+  if (dim == 3 && n == 16) return f(Geo<3, 16>{});
+  if (dim == 3 && n == 32) return f(Geo<3, 32>{});
+  return cudaErrorInvalidValue;
+}
+template <int D, int N>
+constexpr int dim_of(Geo<D, N>) { return D; }
+template <int D, int N>
+constexpr int n_of(Geo<D, N>) { return N; }
+
+}  // namespace
+
+#define F4_DISPATCH(body)                                   \
+  return dispatch(dim, n, [&](auto g) -> cudaError_t {      \
+    constexpr int D = dim_of(decltype(g){});                \
+    constexpr int NN = n_of(decltype(g){});                 \
+    body;                                                   \
+    return cudaGetLastError();                              \
+  })
+
+cudaError_t launch_ghost(int dim, int n, const GhostParams& p, cudaStream_t s) {
+  if (p.nrec <= 0) return cudaSuccess;
+  F4_DISPATCH((ghost_exec_kernel<D, NN><<<(p.nrec + 2 * D - 1) / (2 * D), 256, 0, s>>>(p)));
+}
+cudaError_t launch_transfer(int dim, int n, const double* old_state, double* new_state, const DevTransfer* plan,
+                            int nplan, double theta, cudaStream_t s) {
+  if (nplan <= 0) return cudaSuccess;
+  F4_DISPATCH((transfer_kernel<D, NN><<<nplan, 256, 0, s>>>(old_state, new_state, plan, theta)));
+}
+cudaError_t launch_pack(int dim, int n, double* store_state, const double* src, int b0, int nb, int with_ghosts,
+                        cudaStream_t s) {
+  if (nb <= 0) return cudaSuccess;
+  F4_DISPATCH((layout_kernel<D, NN, true><<<dim3(nb, D + 2), 256, 0, s>>>(store_state, const_cast<double*>(src), b0,
+                                                                           with_ghosts)));
+}
+cudaError_t launch_unpack(int dim, int n, const double* store_state, double* dst, int b0, int nb, int with_ghosts,
+                          cudaStream_t s) {
+  if (nb <= 0) return cudaSuccess;
+  F4_DISPATCH((layout_kernel<D, NN, false><<<dim3(nb, D + 2), 256, 0, s>>>(const_cast<double*>(store_state), dst, b0,
+                                                                            with_ghosts)));
+}
+cudaError_t launch_init_benign(int dim, int n, double* store_state, int nb, double gamma, cudaStream_t s) {
+  if (nb <= 0) return cudaSuccess;
+  F4_DISPATCH((init_benign_kernel<D, NN><<<dim3(nb, D + 2), 256, 0, s>>>(store_state, gamma)));
+}
+cudaError_t launch_block_sums(int dim, int n, const double* state, int nb, double* sums, cudaStream_t s) {
+  if (nb <= 0) return cudaSuccess;
+  F4_DISPATCH((block_sums_kernel<D, NN><<<dim3(nb, D + 2), 256, 0, s>>>(state, sums)));
+}
+cudaError_t launch_maxrate(int dim, int n, const double* state, const int* level, int nblocks, double gamma,
+                           double inv_dx0, unsigned long long* maxrate, cudaStream_t s) {
+  if (nblocks <= 0) return cudaSuccess;
+  F4_DISPATCH((maxrate_kernel<D, NN><<<nblocks, 256, 0, s>>>(state, level, gamma, inv_dx0, maxrate)));
+}
+
+}  // namespace f4

@@ -1,0 +1,285 @@
+// Host-side mesh of the f4 library (see f4_mesh.hpp).  Written from the
+// paper's statement of what p4est provides: refine, coarsen,
+// balance with P4EST_CONNECT_FULL semantics, face connectivity with hanging
+// face offsets.  Linear octree: leaves sorted by the Morton key of their low
+// corner at max_level resolution; lookups are binary searches.
+#include "f4_mesh.hpp"
+
+#include <algorithm>
+#include <deque>
+#include <unordered_map>
+#include <unordered_set>
+
+#include "../../include/f4.h"
+
+namespace f4 {
+
+static inline uint64_t spread3(uint64_t v) {  // 21 bits -> every third bit
+  v &= 0x1fffffULL;
+  v = (v | v << 32) & 0x1f00000000ffffULL;
+  v = (v | v << 16) & 0x1f0000ff0000ffULL;
+  v = (v | v << 8) & 0x100f00f00f00f00fULL;
+  v = (v | v << 4) & 0x10c30c30c30c30c3ULL;
+  v = (v | v << 2) & 0x1249249249249249ULL;
+  return v;
+}
+uint64_t morton3(uint32_t x, uint32_t y, uint32_t z) { return spread3(x) | spread3(y) << 1 | spread3(z) << 2; }
+
+// (level, c) packed into one word for hashing: 5 + 3*19 bits
+static inline uint64_t pack(int level, int cx, int cy, int cz) {
+  return (uint64_t)level | (uint64_t)cx << 5 | (uint64_t)cy << 24 | (uint64_t)cz << 43;
+}
+static inline Leaf unpack(uint64_t k) {
+  Leaf l;
+  l.level = (int)(k & 31);
+  l.c[0] = (int)(k >> 5 & 0x7ffff);
+  l.c[1] = (int)(k >> 24 & 0x7ffff);
+  l.c[2] = (int)(k >> 43 & 0x7ffff);
+  return l;
+}
+
+double HostMesh::dx_of_level(int level) const {
+  int mb = std::max(brick[0], std::max(brick[1], dim == 3 ? brick[2] : 1));
+  return 1.0 / ((double)mb * (double)(1u << level) * (double)N);
+}
+
+int HostMesh::init(std::string& err) {
+  if (dim != 2 && dim != 3) { err = "dim must be 2 or 3"; return F4_EINVAL; }
+  if (N < 2 || N % 2 || N < Ng || 2 * Ng > N || Ng < 1) {  // PAPER.md:141; 2Ng <= N for restriction into ghosts
+    err = "block_n must be even, >= n_ghost and >= 2*n_ghost";
+    return F4_EINVAL;
+  }
+  if (base_level < 0 || max_level < base_level || max_level > 18) { err = "bad levels"; return F4_EINVAL; }
+  for (int a = 0; a < dim; ++a) {
+    if (brick[a] < 1 || ((int64_t)brick[a] << max_level) > (1 << 19)) { err = "bad brick"; return F4_EINVAL; }
+    if ((bc[2 * a] == F4_BC_PERIODIC) != (bc[2 * a + 1] == F4_BC_PERIODIC)) {
+      err = "an axis is periodic only if both of its faces are";
+      return F4_EINVAL;
+    }
+  }
+  for (int f = 0; f < 2 * dim; ++f)
+    if (bc[f] < 0 || bc[f] > F4_BC_KEEP) { err = "bad bc_kind"; return F4_EINVAL; }
+  if (dim == 2) brick[2] = 1;
+  int64_t nb = 1;
+  for (int a = 0; a < dim; ++a) nb *= extent(base_level, a);
+  if (nb > max_blocks) { err = "base mesh exceeds max_blocks"; return F4_ENOBLOCKS; }
+  leaves.clear();
+  int ez = (dim == 3) ? extent(base_level, 2) : 1;
+  for (int k = 0; k < ez; ++k)
+    for (int j = 0; j < extent(base_level, 1); ++j)
+      for (int i = 0; i < extent(base_level, 0); ++i) leaves.push_back(Leaf{base_level, {i, j, k}});
+  sort_leaves();
+  return build_pattern(err);
+}
+
+void HostMesh::sort_leaves() {
+  std::vector<std::pair<uint64_t, Leaf>> t(leaves.size());
+  for (size_t q = 0; q < leaves.size(); ++q) {
+    const Leaf& l = leaves[q];
+    int sh = max_level - l.level;
+    t[q] = {morton3((uint32_t)l.c[0] << sh, (uint32_t)l.c[1] << sh, (uint32_t)l.c[2] << sh), l};
+  }
+  std::sort(t.begin(), t.end(), [](const auto& a, const auto& b) { return a.first < b.first; });
+  mkeys.resize(t.size());
+  for (size_t q = 0; q < t.size(); ++q) { mkeys[q] = t[q].first; leaves[q] = t[q].second; }
+}
+
+int HostMesh::find_leaf(int level, const int c[3]) const {
+  int sh = max_level - level;
+  uint32_t ax = (uint32_t)c[0] << sh, ay = (uint32_t)c[1] << sh, az = (uint32_t)c[2] << sh;
+  uint64_t m = morton3(ax, ay, az);
+  auto it = std::upper_bound(mkeys.begin(), mkeys.end(), m);
+  if (it == mkeys.begin()) return -1;
+  int q = (int)(it - mkeys.begin()) - 1;
+  const Leaf& l = leaves[q];
+  int s2 = max_level - l.level;
+  if ((int)(ax >> s2) != l.c[0] || (int)(ay >> s2) != l.c[1] || (int)(az >> s2) != l.c[2]) return -1;
+  return q;
+}
+
+static inline void transverse(int a, int& ta, int& tb) {
+  if (a == 0) { ta = 1; tb = 2; } else if (a == 1) { ta = 0; tb = 2; } else { ta = 0; tb = 1; }
+}
+
+int HostMesh::build_pattern(std::string& err) {
+  r1.clear();
+  r2.clear();
+  const int nb = (int)leaves.size();
+  for (int b = 0; b < nb; ++b) {
+    const Leaf& L = leaves[b];
+    for (int f = 0; f < 2 * dim; ++f) {
+      const int a = f / 2, side = f % 2;
+      int n[3] = {L.c[0], L.c[1], L.c[2]};
+      n[a] += side ? 1 : -1;
+      const int ext = extent(L.level, a);
+      if (n[a] < 0 || n[a] >= ext) {
+        if (bc[f] == F4_BC_PERIODIC) n[a] = (n[a] + ext) % ext;
+        else {
+          if (bc[f] == F4_BC_OUTFLOW) r1.push_back(Record{F4_OP_BC, f, b, b, 0, 0});
+          continue;  // F4_BC_KEEP: no record
+        }
+      }
+      int q = find_leaf(L.level, n);
+      if (q < 0) { err = "face connectivity: no leaf covers a neighbour region"; return F4_EUNBALANCED; }
+      const int ql = leaves[q].level;
+      int ta, tb;
+      transverse(a, ta, tb);
+      if (ql == L.level) {
+        r1.push_back(Record{F4_OP_SRL, f, b, q, 0, 0});
+      } else if (ql == L.level - 1) {
+        // this block is fine, neighbour coarse: prolongation in R2; offset = position in the group
+        r2.push_back(Record{F4_OP_C2F, f, b, q, L.c[ta] & 1, dim == 3 ? (L.c[tb] & 1) : 0});
+      } else if (ql > L.level) {
+        // neighbour region is refined: the 2^(d-1) children touching the face restrict into my ghosts (R1)
+        for (int o2 = 0; o2 < (dim == 3 ? 2 : 1); ++o2)
+          for (int o1 = 0; o1 < 2; ++o1) {
+            int cc[3] = {2 * n[0], 2 * n[1], dim == 3 ? 2 * n[2] : 0};
+            cc[a] += side ? 0 : 1;
+            cc[ta] += o1;
+            if (dim == 3) cc[tb] += o2;
+            int qf = find_leaf(L.level + 1, cc);
+            if (qf < 0 || leaves[qf].level != L.level + 1) {
+              err = "face connectivity: neighbour more than one level finer (mesh not 2:1 balanced)";
+              return F4_EUNBALANCED;
+            }
+            r1.push_back(Record{F4_OP_F2C, f, b, qf, o1, o2});
+          }
+      } else {
+        err = "face connectivity: neighbour more than one level coarser (mesh not 2:1 balanced)";
+        return F4_EUNBALANCED;
+      }
+    }
+  }
+  return F4_OK;
+}
+
+int HostMesh::adapt(const int* flags, std::vector<Transfer>& plan, bool& changed, std::string& err) {
+  changed = false;
+  plan.clear();
+  const int nb_old = (int)leaves.size();
+  const int nch = 1 << dim;
+  std::unordered_map<uint64_t, int> old_index;
+  old_index.reserve(nb_old * 2);
+  std::unordered_set<uint64_t> S;
+  S.reserve(nb_old * 2);
+  for (int b = 0; b < nb_old; ++b) {
+    uint64_t k = pack(leaves[b].level, leaves[b].c[0], leaves[b].c[1], leaves[b].c[2]);
+    old_index[k] = b;
+    S.insert(k);
+  }
+  auto children = [&](const Leaf& l, uint64_t* out) {
+    int q = 0;
+    for (int dz = 0; dz < (dim == 3 ? 2 : 1); ++dz)
+      for (int dy = 0; dy < 2; ++dy)
+        for (int dx = 0; dx < 2; ++dx)
+          out[q++] = pack(l.level + 1, 2 * l.c[0] + dx, 2 * l.c[1] + dy, dim == 3 ? 2 * l.c[2] + dz : 0);
+  };
+  uint64_t ch[8];
+  // 1. refine
+  for (int b = 0; b < nb_old; ++b)
+    if (flags[b] > 0 && leaves[b].level < max_level) {
+      S.erase(pack(leaves[b].level, leaves[b].c[0], leaves[b].c[1], leaves[b].c[2]));
+      children(leaves[b], ch);
+      for (int q = 0; q < nch; ++q) S.insert(ch[q]);
+    }
+  // 2. coarsen complete families of old leaves, one level, never below base_level
+  {
+    std::unordered_map<uint64_t, int> fam;
+    for (int b = 0; b < nb_old; ++b) {
+      const Leaf& l = leaves[b];
+      if (flags[b] < 0 && l.level > base_level) fam[pack(l.level - 1, l.c[0] >> 1, l.c[1] >> 1, l.c[2] >> 1)]++;
+    }
+    for (auto& pr : fam)
+      if (pr.second == nch) {
+        Leaf par = unpack(pr.first);
+        children(par, ch);
+        for (int q = 0; q < nch; ++q) S.erase(ch[q]);
+        S.insert(pr.first);
+      }
+  }
+  // 3. balance, corner connectivity: ripple from a work queue
+  {
+    std::deque<uint64_t> Q(S.begin(), S.end());
+    while (!Q.empty()) {
+      uint64_t ka = Q.front();
+      Q.pop_front();
+      if (!S.count(ka)) continue;
+      Leaf A = unpack(ka);
+      bool again = false;
+      for (int dz = (dim == 3 ? -1 : 0); dz <= (dim == 3 ? 1 : 0) && !again; ++dz)
+        for (int dy = -1; dy <= 1 && !again; ++dy)
+          for (int dx = -1; dx <= 1 && !again; ++dx) {
+            if (!dx && !dy && !dz) continue;
+            int n[3] = {A.c[0] + dx, A.c[1] + dy, A.c[2] + dz};
+            bool outside = false;
+            for (int a = 0; a < dim; ++a) {
+              int ext = extent(A.level, a);
+              if (n[a] < 0 || n[a] >= ext) {
+                if (bc[2 * a] == F4_BC_PERIODIC) n[a] = (n[a] + ext) % ext; else outside = true;
+              }
+            }
+            if (outside) continue;
+            for (int l = A.level; l >= 0; --l) {
+              int sh = A.level - l;
+              uint64_t kq = pack(l, n[0] >> sh, n[1] >> sh, n[2] >> sh);
+              if (S.count(kq)) {
+                if (l < A.level - 1) {
+                  S.erase(kq);
+                  children(unpack(kq), ch);
+                  for (int q = 0; q < nch; ++q) { S.insert(ch[q]); Q.push_back(ch[q]); }
+                  Q.push_back(ka);  // look again: the new children may still be too coarse
+                  again = true;
+                }
+                break;
+              }
+            }
+          }
+    }
+  }
+  // 4. unchanged? (mesh revision)
+  if ((int)S.size() == nb_old) {
+    bool same = true;
+    for (auto& pr : old_index)
+      if (!S.count(pr.first)) { same = false; break; }
+    if (same) return F4_OK;
+  }
+  if ((int)S.size() > max_blocks) {
+    err = "adapt: mesh would need " + std::to_string(S.size()) + " blocks > max_blocks";
+    return F4_ENOBLOCKS;
+  }
+  // 5. new leaf array + transfer plan by comparing with the old leaves
+  std::vector<Leaf> old_leaves;
+  old_leaves.swap(leaves);
+  leaves.reserve(S.size());
+  for (uint64_t k : S) leaves.push_back(unpack(k));
+  sort_leaves();
+  plan.resize(leaves.size());
+  for (int b = 0; b < (int)leaves.size(); ++b) {
+    const Leaf& l = leaves[b];
+    Transfer t{};
+    t.dst = b;
+    auto it = old_index.find(pack(l.level, l.c[0], l.c[1], l.c[2]));
+    if (it != old_index.end()) {
+      t.kind = 0;
+      t.src[0] = it->second;
+    } else if (l.level > 0 &&
+               (it = old_index.find(pack(l.level - 1, l.c[0] >> 1, l.c[1] >> 1, l.c[2] >> 1))) != old_index.end()) {
+      t.kind = 1;
+      t.src[0] = it->second;
+      t.oct = (l.c[0] & 1) | (l.c[1] & 1) << 1 | (l.c[2] & 1) << 2;
+    } else {
+      t.kind = 2;
+      children(l, ch);
+      for (int q = 0; q < nch; ++q) {
+        auto jt = old_index.find(ch[q]);
+        if (jt == old_index.end()) { err = "adapt: block changed by more than one level"; leaves.swap(old_leaves); sort_leaves(); return F4_EINVAL; }
+        t.src[q] = jt->second;
+      }
+    }
+    plan[b] = t;
+  }
+  changed = true;
+  return build_pattern(err);
+}
+
+}  // namespace f4

@@ -1,0 +1,359 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C-ABI binding,
+against the CPU oracle on the same seeded inputs.  Bars (BASELINE.json
+north_star): ghost copies and restriction bit-exact; fp64 state within 1e-11
+relative L-inf (reading A16) after 10 steps; conserved totals within 1e-12
+relative; compute_dt within 1e-14 relative."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+import helpers as H
+from oracle import oracle as O
+from paper_2605_07612_b200 import f4
+from paper_2605_07612_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+PER, OUT, KEEP = W.PERIODIC, W.OUTFLOW, W.KEEP
+TOL_STATE, TOL_TOTALS, TOL_DT = 1e-11, 1e-12, 1e-14
+
+
+def make_pair(cfg, max_blocks=None):
+    lm = f4.Mesh.from_config(cfg, max_blocks=max_blocks)
+    lm.bind_torch()
+    om = O.OracleMesh.from_config(cfg)
+    return lm, om
+
+
+def perm_lib_to_ora(lm, om):
+    la, ca = lm.get_blocks()
+    lb, cb = om.get_blocks()
+    return H.match_blocks(la, ca, lb, cb)   # library block q = oracle block perm[q]
+
+
+def set_both(lm, om, cfg, noise=True):
+    la, ca = lm.get_blocks()
+    u = W.initial_state(cfg, la, ca, noise)
+    lm.set_state(0, u)
+    perm = perm_lib_to_ora(lm, om)
+    uo = np.empty_like(u)
+    uo[perm] = u
+    om.set_state(0, uo)
+    return u, perm
+
+
+def noncorner_mask(lm):
+    la, ca = lm.get_blocks()
+    _, nc, _ = H.padded_coords(lm.dim, lm.N, lm.Ng, (1, 1, 1), la, ca)
+    return nc
+
+
+def run_and_compare(cfg, nsteps, max_blocks=None, tol=TOL_STATE):
+    lm, om = make_pair(cfg, max_blocks)
+    u0, perm = set_both(lm, om, cfg)
+    t0 = om.totals(0)
+    for s in range(nsteps):
+        dt_o = om.compute_dt(0, cfg["cfl"])
+        dt_g = lm.compute_dt(0, cfg["cfl"])
+        assert abs(dt_g - dt_o) <= 1e-13 * dt_o, (s, dt_g, dt_o)   # state differs by ~1e-13 by now
+        om.advance(dt_o)
+        lm.advance(dt_o)                                            # same dt on both sides (reading A6)
+    ug = lm.get_state(0)
+    uo = om.get_state(0)[perm]
+    err = H.rel_linf(ug, uo)
+    assert np.all(err <= tol), err
+    tg, to = lm.conserved_totals(0), om.totals(0)
+    scale = np.abs(to).max()
+    assert np.all(np.abs(tg - to) <= TOL_TOTALS * scale), (tg - to) / scale
+    if all(b == PER for b in cfg["bc"][: 2 * cfg["dim"]]) and cfg["max_level"] == cfg["base_level"]:
+        assert np.all(np.abs(tg - t0) <= TOL_TOTALS * scale)        # conservation on periodic meshes
+    lm.close()
+    return err
+
+
+# ------------------------------------------------------------------ layout
+@pytest.mark.parametrize("dim,N", [(2, 8), (3, 8), (3, 16), (3, 32), (2, 16)])
+def test_layout_roundtrip(dim, N):
+    import torch
+    rng = np.random.default_rng(dim * 100 + N)
+    m = f4.Mesh(dim, N, 2, (3, 2, 1)[:dim] if dim == 2 else (3, 2, 1), 0, 0, [PER] * (2 * dim))
+    m.bind_torch()
+    for wg in (False, True):
+        a = rng.standard_normal(m._shape(wg))
+        m.set_state(1, a, with_ghosts=wg)
+        assert np.array_equal(m.get_state(1, with_ghosts=wg), a)
+        d = torch.from_numpy(a).cuda()
+        m.set_state(0, d, with_ghosts=wg)
+        out = torch.empty_like(d)
+        m.get_state(0, with_ghosts=wg, out=out)
+        torch.cuda.synchronize()
+        assert torch.equal(out, d)
+    # interior written through the padded view lands in the interior of the padded array
+    a = rng.standard_normal(m._shape(False))
+    m.set_state(0, a)
+    p = m.get_state(0, with_ghosts=True)
+    sl = (slice(None), slice(None), slice(2, 2 + N) if dim == 3 else slice(None), slice(2, 2 + N), slice(2, 2 + N))
+    assert np.array_equal(p[sl], a)
+    m.close()
+
+
+# ------------------------------------------------------------------ ghost fill, bit-exact
+@pytest.mark.parametrize("dim,N,brick,bc", [
+    (2, 8, (2, 2), [PER] * 4),
+    (2, 16, (3, 2), [OUT, OUT, PER, PER]),
+    (3, 8, (3, 2, 2), [PER, PER, OUT, OUT, PER, PER]),
+    (3, 16, (2, 2, 3), [OUT, OUT, PER, PER, OUT, OUT]),
+    (3, 32, (2, 1, 2), [PER, PER, PER, PER, OUT, OUT]),
+])
+def test_fill_ghosts_uniform_bit_exact(dim, N, brick, bc):
+    cfg = dict(dim=dim, block_n=N, n_ghost=2, brick=brick, base_level=0, max_level=0, bc=bc, gamma=1.4)
+    lm, om = make_pair(cfg)
+    rng = np.random.default_rng(N)
+    u = rng.uniform(0.5, 2.0, lm._shape(False))
+    perm = perm_lib_to_ora(lm, om)
+    uo = np.empty_like(u)
+    uo[perm] = u
+    lm.set_state(0, u)
+    om.set_state(0, uo)
+    lm.fill_ghosts(0)
+    om.fill_ghosts(0)
+    pg = lm.get_state(0, with_ghosts=True)
+    po = om.get_state(0, with_ghosts=True)[perm]
+    nc = noncorner_mask(lm)
+    for v in range(lm.nvar):
+        assert np.array_equal(pg[:, v][nc], po[:, v][nc])
+    lm.close()
+
+
+def _refined_pair(dim, N, bc, rounds=2, seed=3):
+    cfg = dict(dim=dim, block_n=N, n_ghost=2, brick=(2, 2, 2)[:dim], base_level=0, max_level=2, bc=bc, gamma=1.4)
+    lm, om = make_pair(cfg, max_blocks=600)
+    rng = np.random.default_rng(seed)
+    for _ in range(rounds):
+        la, ca = lm.get_blocks()
+        flags = (rng.uniform(size=len(la)) < 0.3).astype(np.int32)
+        flags[0] = 1
+        perm = perm_lib_to_ora(lm, om)
+        fo = np.empty_like(flags)
+        fo[perm] = flags
+        lm.adapt(flags)
+        om.adapt(fo)
+    return cfg, lm, om
+
+
+@pytest.mark.parametrize("dim,N,bc", [
+    (2, 8, [PER] * 4), (2, 16, [OUT] * 4), (3, 8, [PER] * 6), (3, 16, [OUT, OUT, PER, PER, OUT, OUT]), (3, 32, [PER] * 6)])
+def test_fill_ghosts_amr(dim, N, bc):
+    cfg, lm, om = _refined_pair(dim, N, bc, rounds=2 if N < 32 else 1)
+    rec, n1, n2 = lm.pattern()
+    assert n2 > 0 and (rec[:, 0] == f4.OP_F2C).any()
+    rng = np.random.default_rng(1)
+    u = rng.uniform(0.5, 2.0, lm._shape(False))
+    perm = perm_lib_to_ora(lm, om)
+    uo = np.empty_like(u)
+    uo[perm] = u
+    lm.set_state(0, u)
+    om.set_state(0, uo)
+    lm.fill_ghosts(0)
+    om.fill_ghosts(0)
+    pg = lm.get_state(0, with_ghosts=True)
+    po = om.get_state(0, with_ghosts=True)[perm]
+    nc = noncorner_mask(lm)
+    # which face ghosts are prolonged (C2F)?  everything else must be bit-exact
+    c2f = np.zeros(pg[:, 0].shape, dtype=bool)
+    P, ng = lm.P, 2
+    for op, face, dst, src, o1, o2 in rec[n1:]:
+        a, side = face // 2, face % 2
+        sl = [slice(ng, ng + N)] * 3
+        if dim == 2:
+            sl[0] = slice(0, 1)
+        sl[2 - a] = slice(ng + N, P) if side else slice(0, ng)
+        c2f[(dst,) + tuple(sl)] = True
+    for v in range(lm.nvar):
+        exact = nc & ~c2f
+        assert np.array_equal(pg[:, v][exact], po[:, v][exact]), "SRL/BC/F2C ghosts must be bit-exact"
+        d = np.abs(pg[:, v][c2f] - po[:, v][c2f])
+        assert d.max() <= 4 * np.spacing(2.0), d.max()    # prolongation: fp tolerance (same op order: usually 0)
+    lm.close()
+
+
+# ------------------------------------------------------------------ the step
+def test_config1_full_2d():
+    err = run_and_compare(W.config(1), 10)
+    print("config1 rel Linf", err)
+
+
+@pytest.mark.parametrize("n,scale,steps", [(2, 2, 10), (3, 1, 10), (3, 2, 3), (4, 1, 4)])
+def test_configs_3d_small(n, scale, steps):
+    err = run_and_compare(W.config(n, scale=scale), steps)
+    print(f"config{n} scale {scale} rel Linf", err)
+
+
+@pytest.mark.parametrize("dim,N,brick", [(3, 8, (3, 1, 2)), (3, 8, (1, 1, 1)), (2, 8, (3, 1)), (3, 16, (1, 2, 1)), (2, 16, (2, 3))])
+def test_ragged_and_nonpow2_bricks(dim, N, brick):
+    # block counts that are not a multiple of the groups per CTA; single-block periodic wrap onto itself
+    cfg = dict(W.config(2 if dim == 3 else 1), dim=dim, block_n=N, brick=tuple(brick) + (1,) * (3 - len(brick)),
+               base_level=0, max_level=0, bc=[PER] * (2 * dim), ic="kh" if dim == 3 else "sinewave")
+    run_and_compare(cfg, 5)
+
+
+@pytest.mark.parametrize("limiter,flux", [(f4.LIM_MINMOD, f4.FLUX_HLL), (f4.LIM_MC, f4.FLUX_RUSANOV)])
+def test_limiter_and_flux_variants(limiter, flux):
+    cfg = W.config(2, scale=1)
+    lm, om = make_pair(cfg)
+    lm.set_options(limiter, flux, 1.0)
+    om.set_options(limiter, flux, 1.0)
+    _, perm = set_both(lm, om, cfg)
+    for _ in range(5):
+        dt = om.compute_dt(0, 0.4)
+        om.advance(dt)
+        lm.advance(dt)
+    assert np.all(H.rel_linf(lm.get_state(0), om.get_state(0)[perm]) <= TOL_STATE)
+    lm.close()
+
+
+def test_compute_dt_parity_and_fused_value():
+    cfg = W.config(3, scale=1)
+    lm, om = make_pair(cfg)
+    set_both(lm, om, cfg)
+    dt_o = om.compute_dt(0, 0.4)
+    dt_g = lm.compute_dt(0, 0.4)           # reduction kernel
+    assert abs(dt_g - dt_o) <= TOL_DT * dt_o
+    lm.advance(dt_o)
+    om.advance(dt_o)
+    dt_f = lm.compute_dt(0, 0.4)           # fused into the last stage
+    lm.set_state(0, lm.get_state(0))       # invalidates the fused value -> reduction kernel on the same state
+    dt_k = lm.compute_dt(0, 0.4)
+    assert abs(dt_f - dt_k) <= TOL_DT * dt_k
+    assert abs(dt_f - om.compute_dt(0, 0.4)) <= 1e-13 * dt_k
+    lm.close()
+
+
+def test_uniform_state_bit_exact_on_gpu():
+    # P1 on the CUDA path: supersonic constant state, AMR + outflow + periodic
+    cfg, lm, om = _refined_pair(3, 8, [OUT, OUT, PER, PER, OUT, OUT])
+    la, ca = lm.get_blocks()
+    ucfg = dict(cfg, ic="uniform", rho0=1.7, vel0=(3.1, -0.4, 0.9), p0=0.6, seed=1)
+    u0 = W.initial_state(ucfg, la, ca)
+    lm.set_state(0, u0)
+    for _ in range(3):
+        lm.advance(lm.compute_dt(0, 0.4))
+    assert np.array_equal(lm.get_state(0), u0)
+    lm.close()
+
+
+# ------------------------------------------------------------------ AMR run (config 5 shape)
+def _flags_from_oracle(cfg, om):
+    om.fill_ghosts(0)
+    return W.pressure_jump_flags(cfg, om.get_state(0, with_ghosts=True))
+
+
+@pytest.mark.parametrize("base,extra,steps,every", [(1, 2, 12, 4)])
+def test_config5_small_adaptive(base, extra, steps, every):
+    cfg = dict(W.config(5), base_level=base, max_level=base + extra)
+    lm, om = make_pair(cfg, max_blocks=3000)
+    # initial mesh: {set analytic state, flag, adapt} (reading A15), one round fewer than the level budget so
+    # that the first regrid of the run is guaranteed to change the mesh; flags from the oracle state
+    for _ in range(extra - 1):
+        set_both(lm, om, cfg)
+        fo = _flags_from_oracle(cfg, om)
+        perm = perm_lib_to_ora(lm, om)
+        ch_o = om.adapt(fo)
+        ch_g = lm.adapt(fo[perm])
+        assert ch_o == ch_g
+        if not ch_o:
+            break
+    _, perm = set_both(lm, om, cfg)
+    assert lm.get_blocks()[0].max() == base + extra - 1
+    nregrid = 0
+    for s in range(steps):
+        if s and s % every == 0:
+            fo = _flags_from_oracle(cfg, om)
+            perm = perm_lib_to_ora(lm, om)
+            ch_o = om.adapt(fo)
+            ch_g = lm.adapt(fo[perm])
+            assert ch_o == ch_g
+            nregrid += ch_o
+            perm = perm_lib_to_ora(lm, om)
+            # regrid transfer: copies and restrictions bit-exact, prolongation to fp tolerance
+            d = np.abs(lm.get_state(0) - om.get_state(0)[perm])
+            assert np.all(H.rel_linf(lm.get_state(0), om.get_state(0)[perm]) <= TOL_STATE), d.max()
+        dt = om.compute_dt(0, cfg["cfl"])
+        assert abs(lm.compute_dt(0, cfg["cfl"]) - dt) <= 1e-12 * dt
+        om.advance(dt)
+        lm.advance(dt)
+    assert nregrid >= 1 and lm.get_blocks()[0].max() == base + extra
+    err = H.rel_linf(lm.get_state(0), om.get_state(0)[perm])
+    assert np.all(err <= TOL_STATE), err
+    tg, to = lm.conserved_totals(0), om.totals(0)
+    assert np.all(np.abs(tg - to) <= TOL_TOTALS * np.abs(to).max())
+    lm.close()
+
+
+def test_regrid_transfer_bit_exact():
+    # refine everything then coarsen everything: copy / prolong / restrict against the oracle
+    for dim, N in ((2, 8), (3, 8), (3, 16)):
+        cfg = dict(dim=dim, block_n=N, n_ghost=2, brick=(2, 1, 2)[:dim], base_level=0, max_level=1,
+                   bc=[PER] * (2 * dim), gamma=1.4)
+        lm, om = make_pair(cfg, max_blocks=64)
+        rng = np.random.default_rng(N + dim)
+        u = rng.uniform(0.5, 2.0, lm._shape(False))
+        perm = perm_lib_to_ora(lm, om)
+        uo = np.empty_like(u)
+        uo[perm] = u
+        lm.set_state(0, u)
+        om.set_state(0, uo)
+        nb = lm.num_blocks
+        for flags in (np.ones(nb, dtype=np.int32), None):
+            if flags is None:
+                flags = -np.ones(lm.num_blocks, dtype=np.int32)
+            assert lm.adapt(flags) and om.adapt(flags)
+            perm = perm_lib_to_ora(lm, om)
+            assert np.array_equal(lm.get_state(0), om.get_state(0)[perm])
+        lm.close()
+
+
+def test_linear_field_on_gpu():
+    # the paper's own ghost/prolong/restrict test through the CUDA path
+    tol = 4 * np.spacing(6.0)
+    for dim, N in ((2, 8), (3, 8), (3, 16)):
+        brick = (2, 2, 2)[:dim]
+        m = f4.Mesh(dim, N, 2, brick, 0, 2, [KEEP] * (2 * dim), max_blocks=400)
+        m.bind_torch()
+
+        def lin(X):
+            return X[0] + 2 * X[1] + (3 * X[2] if dim == 3 else 0.0)
+
+        def check():
+            lev, co = m.get_blocks()
+            X, noncorner, outside = H.padded_coords(dim, N, 2, brick, lev, co)
+            phi = lin(X)
+            u = m.get_state(0, with_ghosts=True)
+            for v in range(m.nvar):
+                u[:, v] = np.where(outside, phi, u[:, v])
+            m.set_state(0, u, with_ghosts=True)
+            m.fill_ghosts(0)
+            u = m.get_state(0, with_ghosts=True)
+            for v in range(m.nvar):
+                assert np.abs(u[:, v] - phi)[noncorner].max() <= tol
+
+        lev, co = m.get_blocks()
+        X, _, _ = H.padded_coords(dim, N, 2, brick, lev, co)
+        u = np.repeat(lin(X)[:, None], m.nvar, axis=1)
+        m.set_state(0, u, with_ghosts=True)
+        check()
+        for rref in ((0.01, 0.01, 0.99), (0.5, 0.99, 0.5)):
+            for _ in range(2):
+                lev, co = m.get_blocks()
+                size = 1.0 / (2 * 2.0 ** lev)
+                flags = np.ones(len(lev), dtype=np.int32)
+                for a in range(dim):
+                    lo = co[:, a] * size
+                    flags &= ((lo <= rref[a]) & (rref[a] < lo + size)).astype(np.int32)
+                m.adapt(flags)
+                check()
+            for _ in range(2):
+                lev, _ = m.get_blocks()
+                m.adapt(np.where(lev == lev.max(), -1, 0).astype(np.int32))
+                check()
+        m.close()
