@@ -123,7 +123,7 @@ __device__ __forceinline__ void riemann_flux(const double (&L)[5], const double 
   F[4] = fma(a, (EL + L[4]) * L[1], fma(b, (ER + R[4]) * R[1], c * (ER - EL)));
 }
 
-template <int DIM, int N, int TY, int G>
+template <int DIM, int N, int TY, int G, int EXBUF>
 struct Cfg {
   static constexpr int P = N + 2 * NG;
   static constexpr int PZ = (DIM == 3) ? P : 1;
@@ -136,25 +136,29 @@ struct Cfg {
   static constexpr int NSLOT = (DIM == 3) ? 3 : 1;
   static constexpr int EXV = (N + 1) * (TY + 1);  // exchange entries per variable
   static constexpr int EX = NVAR * EXV;
+  static constexpr int NH = TY + N;           // halo cells per side (x rows + y columns)
   static constexpr int TG = N * TY;           // threads per group
   static constexpr int NT = TG * G;
   static constexpr int YT = N / TY;           // y tiles per block
-  static constexpr int GROUP_DOUBLES = NSLOT * SLOT + 2 * EX;
+  // ring | exX[EXBUF] | exY[EXBUF] | right states of the high halo cells [NVAR][NH]
+  static constexpr int GROUP_DOUBLES = NSLOT * SLOT + 2 * EXBUF * EX + NVAR * NH;
   static constexpr size_t SMEM = (size_t)G * GROUP_DOUBLES * 8 + (size_t)G * NSLOT * 8;
   static constexpr int HALO = 4 * TY + 4 * N;  // halo cells of an interior plane
-  static_assert(HALO <= TG, "halo conversion needs one pass");
-  static_assert(TG % 32 == 0 && N % TY == 0, "tile shape");
+  static_assert(HALO <= TG && 2 * NH <= TG, "halo work needs one pass");
+  static_assert(TG % 32 == 0 && N % TY == 0 && GROUP_DOUBLES % 2 == 0, "tile shape");
 };
 
-template <int DIM, int N, int TY, int G>
-__global__ void __launch_bounds__(Cfg<DIM, N, TY, G>::NT, (Cfg<DIM, N, TY, G>::SMEM <= 100 * 1024) ? 2 : 1)
+template <int DIM, int N, int TY, int G, int EXBUF>
+__global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY, G, EXBUF>::SMEM <= 110 * 1024) ? 2 : 1)
     stage_kernel(StageParams p) {
-  using C = Cfg<DIM, N, TY, G>;
-  constexpr int P = C::P, NV = C::NVAR, PLANE = C::PLANE, TG = C::TG, EXV = C::EXV;
+  using C = Cfg<DIM, N, TY, G, EXBUF>;
+  constexpr int P = C::P, NV = C::NVAR, PLANE = C::PLANE, TG = C::TG, EXV = C::EXV, NH = C::NH;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int grp = threadIdx.x / TG, t = threadIdx.x % TG;
   double* ring = reinterpret_cast<double*>(smem_raw) + (size_t)grp * C::GROUP_DOUBLES;
-  double* exb = ring + C::NSLOT * C::SLOT;  // [2][NV][EXV]
+  double* exX = ring + C::NSLOT * C::SLOT;   // [EXBUF][NV][EXV]
+  double* exY = exX + EXBUF * C::EX;
+  double* sRh = exY + EXBUF * C::EX;         // [NV][NH]
   uint64_t* bars = reinterpret_cast<uint64_t*>(reinterpret_cast<double*>(smem_raw) + (size_t)G * C::GROUP_DOUBLES) +
                    grp * C::NSLOT;
   const int bar_id = 1 + grp;
@@ -171,6 +175,9 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G>::NT, (Cfg<DIM, N, TY, G>::S
   const double inv_dx = p.inv_dx0 * (double)(1u << p.level[blk]);
   const double* dbase = p.deriv + (size_t)blk * C::BS;
 
+  // register arrays are in "phys5" order (rho, u, v, w, p); smem plane of component q:
+  auto pl = [](int q) { return q < 4 ? q : NV - 1; };
+
   if (t == 0) {
     for (int s = 0; s < C::NSLOT; ++s) mbar_init(&bars[s], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -185,9 +192,9 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G>::NT, (Cfg<DIM, N, TY, G>::S
     const int kslot = (DIM == 3) ? (c < 0 ? c + P : c) : 0;
     double* dst = ring + s * C::SLOT;
     const double* src = dbase + (size_t)kslot * P * P;
-    // rows y in [ylo, yhi) -> smem rows y - (j0-2); low part wraps to slots y + P
+    // rows y in [ylo, yhi) -> smem rows y - (j0-2); rows with y < 0 live in slots y + P
     const int ylo = interior ? j0 - 2 : j0, yhi = interior ? j0 + TY + 2 : j0 + TY;
-    const int nlow = ylo < 0 ? -ylo : 0;  // rows with y < 0
+    const int nlow = ylo < 0 ? -ylo : 0;
     const uint32_t bytes_low = (uint32_t)nlow * P * 8, bytes_hi = (uint32_t)(yhi - ylo - nlow) * P * 8;
     mbar_expect_tx(&bars[s], (bytes_low + bytes_hi) * NV);
     for (int v = 0; v < NV; ++v) {
@@ -200,232 +207,248 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G>::NT, (Cfg<DIM, N, TY, G>::S
 
   // in-place conversion conservative -> primitive of one smem cell (to_primitive)
   auto convert = [&](double* W, int o, double (&w)[5]) {
-    double rho = W[o];
-    double ir = rcp_fast(rho);
+    const double rho = W[o];
+    const double ir = rcp_fast(rho);
     double ke = 0.0;
     w[0] = rho;
+    w[3] = 0.0;
 #pragma unroll
     for (int d = 0; d < DIM; ++d) {
       w[1 + d] = W[(1 + d) * PLANE + o] * ir;
       ke = fma(w[1 + d], w[1 + d], ke);
     }
-    if (DIM == 2) w[3] = 0.0;
     w[4] = gm1 * fma(-0.5 * rho, ke, W[(NV - 1) * PLANE + o]);
 #pragma unroll
     for (int d = 0; d < DIM; ++d) W[(1 + d) * PLANE + o] = w[1 + d];
     W[(NV - 1) * PLANE + o] = w[4];
   };
 
-  // x/y sweep on the converted plane in slot W: returns sum over x,y faces of (F_in - F_out) for the own cell
-  auto sweep_xy = [&](const double* W, int rot, double (&acc)[5]) {
+  // limited reconstruction of one cell from its two neighbours along a line (offsets o0, om, op)
+  auto slope_states = [&](const double* W, int o0, int om, int op, double (&L)[5], double (&R)[5]) {
 #pragma unroll
-    for (int v = 0; v < 5; ++v) acc[v] = 0.0;
-#pragma unroll 1
-    for (int dir = 0; dir < 2; ++dir) {
-      double* ex = exb + dir * C::EX;
-      const int cn = 1 + dir, ct = 2 - dir;                  // normal / tangential velocity planes
-      const int cnt = dir ? N : TY;                          // halo cells per side in this direction
-      // special roles, rotated over the warps from plane to plane
-      const int q = (t + 32 * ((rot + 2 * dir) % (TG / 32))) % TG;
-      const bool is_hi = q < cnt, is_lo = (q >= cnt) && (q < 2 * cnt);
-      const int qq = is_hi ? q : q - cnt;
-      double Rown[5], Rhi[5];
-      // ---- phase 1: slopes -> left/right states
-#pragma unroll 1
-      for (int pass = 0; pass < 2; ++pass) {
-        if (pass == 1 && !(is_hi || is_lo)) break;
-        // cell whose slope is taken: own cell, or halo cell -1 (lo) / N or TY (hi) of row/column qq
-        int ci = i, cj = j;
-        if (pass == 1) {
-          if (dir == 0) { cj = qq; ci = is_hi ? N : -1; } else { ci = qq; cj = is_hi ? TY : -1; }
+    for (int q = 0; q < 5; ++q) {
+      if (DIM == 2 && q == 3) { L[q] = 0.0; R[q] = 0.0; continue; }
+      const double* Wv = W + pl(q) * PLANE;
+      const double w0 = Wv[o0];
+      const double hs = half_slope(w0 - Wv[om], Wv[op] - w0, limiter);
+      L[q] = w0 + hs;
+      R[q] = w0 - hs;
+    }
+  };
+
+  // per-thread constants of the x/y sweep
+  const int own = (j + 2) * P + i;
+  const int own_xm = (j + 2) * P + (i == 0 ? P - 1 : i - 1);
+  const int fx = j * (N + 1) + i, fy = j * N + i;      // own low faces in the exchange arrays
+  // halo roles: threads [0,NH) take the high halo cells (slope + last face flux), [NH,2NH) the low ones (slope)
+  const bool is_hi = t < NH, is_lo = (t >= NH) && (t < 2 * NH);
+  const int hq = is_hi ? t : t - NH;
+  const bool h_isx = hq < TY;                          // x halo of row hq, else y halo of column hq-TY
+  int h_o0, h_om, h_op, h_f;
+  if (h_isx) {
+    const int row = (hq + 2) * P;
+    h_o0 = row + (is_hi ? N : P - 1);
+    h_om = row + (is_hi ? N - 1 : P - 2);
+    h_op = row + (is_hi ? N + 1 : 0);
+    h_f = hq * (N + 1) + (is_hi ? N : 0);
+  } else {
+    const int col = hq - TY;
+    h_o0 = (is_hi ? TY + 2 : 1) * P + col;
+    h_om = h_o0 - P;
+    h_op = h_o0 + P;
+    h_f = (is_hi ? TY : 0) * N + col;
+  }
+
+  // x/y sweep on the converted plane W: sum over the x,y faces of (F_in - F_out) of the own cell
+  auto sweep_xy = [&](const double* W, int par, double (&acc)[5]) {
+    double* eX = exX + (EXBUF == 2 ? par : 0) * C::EX;
+    double* eY = exY + (EXBUF == 2 ? par : 0) * C::EX;
+    double Rx[5], Ry[5];
+    {  // ---- phase 1: slopes -> left states to smem, right states stay in registers
+      double L[5];
+      slope_states(W, own, own_xm, own + 1, L, Rx);
+#pragma unroll
+      for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eX[pl(q) * EXV + fx + 1] = L[q];
+      slope_states(W, own, own - P, own + P, L, Ry);
+#pragma unroll
+      for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eY[pl(q) * EXV + fy + N] = L[q];
+      if (is_hi || is_lo) {
+        double R[5];
+        slope_states(W, h_o0, h_om, h_op, L, R);
+        double* e = h_isx ? eX : eY;
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+          if (DIM == 2 && q == 3) continue;
+          if (is_lo) e[pl(q) * EXV + h_f] = L[q];
+          else sRh[pl(q) * NH + hq] = R[q];
         }
-        int o0, om, op;
-        if (dir == 0) {
-          const int row = (cj + 2) * P;
-          o0 = row + (ci < 0 ? ci + P : ci);
-          om = row + (ci - 1 < 0 ? ci - 1 + P : ci - 1);
-          op = row + ci + 1;   // ci+1 <= N+1: natural slot
-        } else {
-          o0 = (cj + 2) * P + ci;
-          om = o0 - P;
-          op = o0 + P;
-        }
-        double Lst[5], Rst[5];
-        const int vmap[5] = {0, cn, ct, 3, NV - 1};
-#pragma unroll
-        for (int v = 0; v < 5; ++v) {
-          if (DIM == 2 && v == 3) { Lst[v] = 0.0; Rst[v] = 0.0; continue; }
-          const double* Wv = W + vmap[v] * PLANE;
-          double w0 = Wv[o0], wm = Wv[om], wp = Wv[op];
-          double hs = half_slope(w0 - wm, wp - w0, limiter);
-          Lst[v] = w0 + hs;
-          Rst[v] = w0 - hs;
-        }
-        // left state of face f is stored at ex[f]: x: f = ci+1 in row cj; y: f = cj+1 in column ci
-        const int fo = dir == 0 ? cj * (N + 1) + ci + 1 : (cj + 1) * N + ci;
-        if (pass == 0) {
-#pragma unroll
-          for (int v = 0; v < 5; ++v) { Rown[v] = Rst[v]; if (!(DIM == 2 && v == 3)) ex[(v < 4 ? v : NV - 1) * EXV + fo] = Lst[v]; }
-        } else if (is_lo) {
-#pragma unroll
-          for (int v = 0; v < 5; ++v) if (!(DIM == 2 && v == 3)) ex[(v < 4 ? v : NV - 1) * EXV + fo] = Lst[v];
-        } else {
-#pragma unroll
-          for (int v = 0; v < 5; ++v) Rhi[v] = Rst[v];
-        }
-      }
-      group_sync(bar_id, TG);
-      // ---- phase 2: fluxes at the low face of the own cell (+ the last face of the row/column)
-      double Fown[5];
-#pragma unroll 1
-      for (int pass = 0; pass < 2; ++pass) {
-        if (pass == 1 && !is_hi) break;
-        const int fo = pass == 0 ? (dir == 0 ? j * (N + 1) + i : j * N + i)
-                                 : (dir == 0 ? qq * (N + 1) + N : TY * N + qq);
-        double Lst[5], Rst[5], F[5];
-#pragma unroll
-        for (int v = 0; v < 5; ++v) {
-          Lst[v] = (DIM == 2 && v == 3) ? 0.0 : ex[(v < 4 ? v : NV - 1) * EXV + fo];
-          Rst[v] = pass == 0 ? Rown[v] : Rhi[v];
-        }
-        riemann_flux<DIM>(Lst, Rst, gamma, ig1, fluxs, F);
-#pragma unroll
-        for (int v = 0; v < 5; ++v) {
-          if (!(DIM == 2 && v == 3)) ex[(v < 4 ? v : NV - 1) * EXV + fo] = F[v];
-          if (pass == 0) Fown[v] = F[v];
-        }
-      }
-      group_sync(bar_id, TG);
-      // ---- phase 3: difference with the next face
-      {
-        const int fn = dir == 0 ? j * (N + 1) + i + 1 : (j + 1) * N + i;
-        const double d0 = Fown[0] - ex[0 * EXV + fn];
-        const double dn = Fown[1] - ex[1 * EXV + fn];
-        const double dt = Fown[2] - ex[2 * EXV + fn];
-        const double de = Fown[4] - ex[(NV - 1) * EXV + fn];
-        acc[0] += d0;
-        acc[1] += dir == 0 ? dn : dt;
-        acc[2] += dir == 0 ? dt : dn;
-        if (DIM == 3) acc[3] += Fown[3] - ex[3 * EXV + fn];
-        acc[4] += de;
       }
     }
+    group_sync(bar_id, TG);
+    double Fx[5], Fy[5];
+    {  // ---- phase 2: flux at the low x and y face of the own cell, and at the last face of each row/column
+      double L[5], F[5];
+#pragma unroll
+      for (int q = 0; q < 5; ++q) L[q] = (DIM == 2 && q == 3) ? 0.0 : eX[pl(q) * EXV + fx];
+      riemann_flux<DIM>(L, Rx, gamma, ig1, fluxs, Fx);
+#pragma unroll
+      for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eX[pl(q) * EXV + fx] = Fx[q];
+      // y: normal frame (rho, v, u, w, p)
+#pragma unroll
+      for (int q = 0; q < 5; ++q) L[q] = (DIM == 2 && q == 3) ? 0.0 : eY[pl(q) * EXV + fy];
+      {
+        const double Ln[5] = {L[0], L[2], L[1], L[3], L[4]}, Rn[5] = {Ry[0], Ry[2], Ry[1], Ry[3], Ry[4]};
+        riemann_flux<DIM>(Ln, Rn, gamma, ig1, fluxs, F);
+      }
+      Fy[0] = F[0]; Fy[1] = F[2]; Fy[2] = F[1]; Fy[3] = F[3]; Fy[4] = F[4];
+#pragma unroll
+      for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eY[pl(q) * EXV + fy] = Fy[q];
+      if (is_hi) {
+        double* e = h_isx ? eX : eY;
+        double Rr[5];
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+          L[q] = (DIM == 2 && q == 3) ? 0.0 : e[pl(q) * EXV + h_f];
+          Rr[q] = (DIM == 2 && q == 3) ? 0.0 : sRh[pl(q) * NH + hq];
+        }
+        const double Ln[5] = {L[0], h_isx ? L[1] : L[2], h_isx ? L[2] : L[1], L[3], L[4]};
+        const double Rn[5] = {Rr[0], h_isx ? Rr[1] : Rr[2], h_isx ? Rr[2] : Rr[1], Rr[3], Rr[4]};
+        riemann_flux<DIM>(Ln, Rn, gamma, ig1, fluxs, F);
+        const double Fp[5] = {F[0], h_isx ? F[1] : F[2], h_isx ? F[2] : F[1], F[3], F[4]};
+#pragma unroll
+        for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) e[pl(q) * EXV + h_f] = Fp[q];
+      }
+    }
+    group_sync(bar_id, TG);
+    // ---- phase 3: difference with the next faces
+#pragma unroll
+    for (int q = 0; q < 5; ++q) {
+      if (DIM == 2 && q == 3) { acc[q] = 0.0; continue; }
+      acc[q] = (Fx[q] - eX[pl(q) * EXV + fx + 1]) + (Fy[q] - eY[pl(q) * EXV + fy + N]);
+    }
+    if (EXBUF == 1) group_sync(bar_id, TG);
   };
 
   // Runge-Kutta combine eq. (5) + store + optional CFL rate of the new state
   double rate_max = 0.0;
-  auto finish = [&](int k, const double (&tot)[5]) {
+  const size_t cell0 = (size_t)blk * C::BS + (size_t)(j0 + j) * P + i;   // + k*P*P + v*VS
+  auto load_prev = [&](int k, double (&a)[5], double (&b)[5]) {
+    const size_t o = cell0 + (size_t)(DIM == 3 ? k : 0) * P * P;
+#pragma unroll
+    for (int q = 0; q < 5; ++q) {
+      if (DIM == 2 && q == 3) { a[q] = 0.0; b[q] = 0.0; continue; }
+      a[q] = p.prev0[o + pl(q) * C::VS];
+      b[q] = p.prev1 ? p.prev1[o + pl(q) * C::VS] : 0.0;
+    }
+  };
+  auto finish = [&](int k, const double (&tot)[5], const double (&a)[5], const double (&b)[5]) {
     if (!active) return;
-    const size_t o = (size_t)blk * C::BS + (size_t)(DIM == 3 ? k : 0) * P * P + (size_t)(j0 + j) * P + i;
+    const size_t o = cell0 + (size_t)(DIM == 3 ? k : 0) * P * P;
     double u[5];
     const double s = p.dt_sub * inv_dx;
 #pragma unroll
-    for (int v = 0; v < NV; ++v) {
-      const int tv = (v == NV - 1) ? 4 : v;
-      double base = p.w0 * p.prev0[o + v * C::VS];
-      if (p.prev1) base = fma(p.w1, p.prev1[o + v * C::VS], base);
-      u[tv] = fma(s, tot[tv], base);
-      p.out[o + v * C::VS] = u[tv];
+    for (int q = 0; q < 5; ++q) {
+      if (DIM == 2 && q == 3) { u[q] = 0.0; continue; }
+      u[q] = fma(s, tot[q], fma(p.w1, b[q], p.w0 * a[q]));
+      p.out[o + pl(q) * C::VS] = u[q];
     }
     if (p.maxrate) {
-      double ir = rcp_fast(u[0]);
+      const double ir = rcp_fast(u[0]);
       double ke = 0.0, su = 0.0;
 #pragma unroll
       for (int d = 0; d < DIM; ++d) {
-        double vel = u[1 + d] * ir;
+        const double vel = u[1 + d] * ir;
         ke = fma(vel, vel, ke);
         su += fabs(vel);
       }
-      double pr = gm1 * fma(-0.5 * u[0], ke, u[4]);
-      double c2 = gamma * pr * ir;
-      double c = c2 * rsqrt_fast(c2);
-      rate_max = fmax(rate_max, (su + DIM * c) * inv_dx);
+      const double pr = gm1 * fma(-0.5 * u[0], ke, u[4]);
+      const double c2 = gamma * pr * ir;
+      rate_max = fmax(rate_max, fma((double)DIM, c2 * rsqrt_fast(c2), su) * inv_dx);
+    }
+  };
+  auto convert_halo = [&](double* W) {
+    if (t < C::HALO) {
+      int row, col;
+      if (t < 4 * TY) { row = 2 + t / 4; col = N + (t % 4); }
+      else { const int tq = t - 4 * TY, r4 = tq / N; row = r4 < 2 ? r4 : TY + r4; col = tq % N; }
+      double tmp[5];
+      convert(W, row * P + col, tmp);
     }
   };
 
   if (DIM == 2) {
+    double a[5], b[5], w[5], acc[5];
     if (t == 0 && active) issue_plane(0);
-    if (active) mbar_wait(&bars[0], 0);
-    double w[5];
     if (active) {
-      convert(ring, (j + 2) * P + i, w);
-      if (t < C::HALO) {
-        int row, col;
-        if (t < 4 * TY) { row = 2 + t / 4; col = N + (t % 4); }
-        else { int tq = t - 4 * TY, r4 = tq / N; row = r4 < 2 ? r4 : TY + r4; col = tq % N; }
-        convert(ring, row * P + col, w);
-      }
+      load_prev(0, a, b);
+      mbar_wait(&bars[0], 0);
+      convert(ring, own, w);
+      convert_halo(ring);
     }
     group_sync(bar_id, TG);
-    double acc[5];
     sweep_xy(ring, 0, acc);
-    finish(0, acc);
+    finish(0, acc, a, b);
   } else {
     double dA[5], Lz[5], accp[5];
 #pragma unroll
-    for (int v = 0; v < 5; ++v) { dA[v] = 0.0; Lz[v] = 0.0; accp[v] = 0.0; }
-    if (t == 0 && active) issue_plane(-2);
+    for (int q = 0; q < 5; ++q) { dA[q] = 0.0; Lz[q] = 1.0; accp[q] = 0.0; }
+    if (t == 0 && active) { issue_plane(-2); issue_plane(-1); }
 #pragma unroll 1
     for (int c = -2; c <= N + 1; ++c) {
       const int idx = c + 2, s = idx % 3;
-      double* Wc = ring + s * C::SLOT;                    // plane c
+      double* Wc = ring + s * C::SLOT;                      // plane c
       const double* Wk = ring + ((idx + 2) % 3) * C::SLOT;  // plane c-1
-      if (t == 0 && active && c + 1 <= N + 1) issue_plane(c + 1);
+      double pa[5], pb[5];
+      if (c >= 2 && active) load_prev(c - 2, pa, pb);       // consumed after the z flux: latency hidden
       double wB[5];
       if (active) {
         mbar_wait(&bars[s], (idx / 3) & 1);
-        convert(Wc, (j + 2) * P + i, wB);
-        if (c >= 0 && c < N && t < C::HALO) {
-          int row, col;
-          if (t < 4 * TY) { row = 2 + t / 4; col = N + (t % 4); }
-          else { int tq = t - 4 * TY, r4 = tq / N; row = r4 < 2 ? r4 : TY + r4; col = tq % N; }
-          double tmp[5];
-          convert(Wc, row * P + col, tmp);
-        }
+        convert(Wc, own, wB);
+        if (c >= 0 && c < N) convert_halo(Wc);
+        fence_proxy_async();   // generic-proxy writes before the async-proxy refill of this slot
       } else {
 #pragma unroll
-        for (int v = 0; v < 5; ++v) wB[v] = 1.0;
+        for (int q = 0; q < 5; ++q) wB[q] = 1.0;
       }
-      // ---- z direction along the march (frame: normal = w, tangentials u, v):
-      //      slope of cell c-1 from w(c-2), w(c-1), w(c); flux at the face between cells c-2 and c-1
+      // ---- z direction along the march: slope of cell c-1 from w(c-2), w(c-1), w(c);
+      //      flux at the face between cells c-2 and c-1 (normal frame (rho, w, u, v, p))
       double Fz[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
       if (c >= -1) {
-        const int own = (j + 2) * P + i;
         double Rz[5], Ln[5];
 #pragma unroll
-        for (int v = 0; v < 5; ++v) {
-          const int pv = (v == 1) ? 3 : (v == 2 ? 1 : (v == 3 ? 2 : v));
-          const double wa = Wk[pv * PLANE + own];   // w(c-1), resident in its ring slot
-          const double dB = wB[pv] - wa;
-          const double hs = half_slope(dA[v], dB, limiter);  // c == -1: dA = 0 -> hs = 0, result unused
-          Rz[v] = wa - hs;
-          Ln[v] = wa + hs;
-          dA[v] = dB;
+        for (int q = 0; q < 5; ++q) {
+          const double wa = Wk[pl(q) * PLANE + own];   // w(c-1), resident in its ring slot
+          const double dB = wB[q] - wa;
+          const double hs = half_slope(dA[q], dB, limiter);  // c == -1: dA = 0 -> hs = 0, result unused
+          Rz[q] = wa - hs;
+          Ln[q] = wa + hs;
+          dA[q] = dB;
         }
-        if (c >= 1) riemann_flux<3>(Lz, Rz, gamma, ig1, fluxs, Fz);
+        if (c >= 1) {
+          const double Lf[5] = {Lz[0], Lz[3], Lz[1], Lz[2], Lz[4]}, Rf[5] = {Rz[0], Rz[3], Rz[1], Rz[2], Rz[4]};
+          double F[5];
+          riemann_flux<3>(Lf, Rf, gamma, ig1, fluxs, F);
+          Fz[0] = F[0]; Fz[3] = F[1]; Fz[1] = F[2]; Fz[2] = F[3]; Fz[4] = F[4];
+        }
 #pragma unroll
-        for (int v = 0; v < 5; ++v) Lz[v] = Ln[v];
+        for (int q = 0; q < 5; ++q) Lz[q] = Ln[q];
       }
       if (c >= 2) {
         double tot[5];
-        tot[0] = accp[0] - Fz[0];
-        tot[1] = accp[1] - Fz[2];   // Fz frame (mass, w, u, v, E) -> (rho, u, v, w, E)
-        tot[2] = accp[2] - Fz[3];
-        tot[3] = accp[3] - Fz[1];
-        tot[4] = accp[4] - Fz[4];
-        finish(c - 2, tot);
+#pragma unroll
+        for (int q = 0; q < 5; ++q) tot[q] = accp[q] - Fz[q];
+        finish(c - 2, tot, pa, pb);
       }
       if (c >= 1 && c <= N) {
         double acc[5];
-        sweep_xy(Wk, c, acc);
-        accp[0] = acc[0] + Fz[0];
-        accp[1] = acc[1] + Fz[2];
-        accp[2] = acc[2] + Fz[3];
-        accp[3] = acc[3] + Fz[1];
-        accp[4] = acc[4] + Fz[4];
+        sweep_xy(Wk, c & 1, acc);
+#pragma unroll
+        for (int q = 0; q < 5; ++q) accp[q] = acc[q] + Fz[q];
+      } else {
+        group_sync(bar_id, TG);
       }
-      fence_proxy_async();
-      group_sync(bar_id, TG);
+      // every thread is past its last read of plane c-1: refill that slot with plane c+2
+      if (t == 0 && active && c + 2 <= N + 1) issue_plane(c + 2);
     }
   }
 
@@ -436,19 +459,19 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G>::NT, (Cfg<DIM, N, TY, G>::S
   }
 }
 
-template <int DIM, int N, int TY, int G>
+template <int DIM, int N, int TY, int G, int EXBUF>
 cudaError_t launch_cfg(const StageParams& p, cudaStream_t s) {
-  using C = Cfg<DIM, N, TY, G>;
+  using C = Cfg<DIM, N, TY, G, EXBUF>;
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(stage_kernel<DIM, N, TY, G>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaError_t e = cudaFuncSetAttribute(stage_kernel<DIM, N, TY, G, EXBUF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)C::SMEM);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
   const int nitems = p.nblocks * C::YT;
   const int grid = (nitems + G - 1) / G;
-  stage_kernel<DIM, N, TY, G><<<grid, C::NT, C::SMEM, s>>>(p);
+  stage_kernel<DIM, N, TY, G, EXBUF><<<grid, C::NT, C::SMEM, s>>>(p);
   return cudaGetLastError();
 }
 
@@ -460,11 +483,11 @@ bool stage_supported(int dim, int n) {
 
 cudaError_t launch_stage(int dim, int n, const StageParams& p, cudaStream_t s) {
   if (p.nblocks <= 0) return cudaSuccess;
-  if (dim == 2 && n == 8) return launch_cfg<2, 8, 8, 4>(p, s);
-  if (dim == 2 && n == 16) return launch_cfg<2, 16, 16, 1>(p, s);
-  if (dim == 3 && n == 8) return launch_cfg<3, 8, 8, 4>(p, s);
-  if (dim == 3 && n == 16) return launch_cfg<3, 16, 16, 1>(p, s);
-  if (dim == 3 && n == 32) return launch_cfg<3, 32, 8, 1>(p, s);
+  if (dim == 2 && n == 8) return launch_cfg<2, 8, 8, 4, 1>(p, s);
+  if (dim == 2 && n == 16) return launch_cfg<2, 16, 16, 1, 1>(p, s);
+  if (dim == 3 && n == 8) return launch_cfg<3, 8, 8, 4, 1>(p, s);
+  if (dim == 3 && n == 16) return launch_cfg<3, 16, 16, 1, 2>(p, s);
+  if (dim == 3 && n == 32) return launch_cfg<3, 32, 8, 1, 2>(p, s);
   return cudaErrorInvalidValue;
 }
 
