@@ -17,6 +17,8 @@
 //    memory; the z direction lives in registers along the march;
 //  * fp64 division / sqrt are replaced by MUFU seeds + cubic Newton steps
 //    (the kernel is co-limited by the fp64 pipe).
+#include <type_traits>
+
 #include "../../include/f4.h"
 #include "f4_dev.hpp"
 
@@ -74,10 +76,11 @@ __device__ __forceinline__ void group_sync(int id, int nthreads) {
 }
 
 // limited HALF slope 1/2*phi(a,b) for the reconstruction w +- 1/2 phi (reading A1)
+template <bool FAST>
 __device__ __forceinline__ double half_slope(double a, double b, int limiter) {
   double ab = a * b;
   double r;
-  if (limiter == F4_LIM_VANLEER) {
+  if (FAST || limiter == F4_LIM_VANLEER) {
     r = ab * rcp_fast(a + b);                         // 1/2 * 2ab/(a+b)
   } else {
     double th = (limiter == F4_LIM_MC) ? 2.0 : 1.0;   // eq. (1)
@@ -89,7 +92,7 @@ __device__ __forceinline__ double half_slope(double a, double b, int limiter) {
 
 // HLL / Rusanov flux in the face-normal frame (readings A2-A3).
 // q = (rho, un, ut1, ut2, p); F = (mass, normal momentum, tangential momenta, energy).
-template <int DIM>
+template <int DIM, bool FAST>
 __device__ __forceinline__ void riemann_flux(const double (&L)[5], const double (&R)[5], double gamma, double ig1,
                                              int flux, double (&F)[5]) {
   const double yL = rsqrt_fast(L[0]), yR = rsqrt_fast(R[0]);  // 1/sqrt(rho)
@@ -101,7 +104,7 @@ __device__ __forceinline__ void riemann_flux(const double (&L)[5], const double 
   const double d2 = fma(gamma * (L[4] * yL + R[4] * yR), w, 0.5 * (rL * w) * (rR * w) * du * du);
   const double dhat = d2 * rsqrt_fast(d2);
   double sm = uhat - dhat, sp = uhat + dhat;
-  if (flux == F4_FLUX_RUSANOV) {
+  if (!FAST && flux == F4_FLUX_RUSANOV) {
     double s = fmax(fabs(sm), fabs(sp));
     sm = -s;
     sp = s;
@@ -124,7 +127,7 @@ __device__ __forceinline__ void riemann_flux(const double (&L)[5], const double 
 }
 
 template <int DIM, int N, int TY, int G, int EXBUF>
-struct Cfg {
+struct Cfg {  // FAST (van Leer + HLL fixed at compile time) does not change the geometry
   static constexpr int P = N + 2 * NG;
   static constexpr int PZ = (DIM == 3) ? P : 1;
   static constexpr int NVAR = DIM + 2;
@@ -148,7 +151,7 @@ struct Cfg {
   static_assert(TG % 32 == 0 && N % TY == 0 && GROUP_DOUBLES % 2 == 0, "tile shape");
 };
 
-template <int DIM, int N, int TY, int G, int EXBUF>
+template <int DIM, int N, int TY, int G, int EXBUF, bool FAST>
 __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY, G, EXBUF>::SMEM <= 110 * 1024) ? 2 : 1)
     stage_kernel(StageParams p) {
   using C = Cfg<DIM, N, TY, G, EXBUF>;
@@ -230,7 +233,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
       if (DIM == 2 && q == 3) { L[q] = 0.0; R[q] = 0.0; continue; }
       const double* Wv = W + pl(q) * PLANE;
       const double w0 = Wv[o0];
-      const double hs = half_slope(w0 - Wv[om], Wv[op] - w0, limiter);
+      const double hs = half_slope<FAST>(w0 - Wv[om], Wv[op] - w0, limiter);
       L[q] = w0 + hs;
       R[q] = w0 - hs;
     }
@@ -290,7 +293,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
       double L[5], F[5];
 #pragma unroll
       for (int q = 0; q < 5; ++q) L[q] = (DIM == 2 && q == 3) ? 0.0 : eX[pl(q) * EXV + fx];
-      riemann_flux<DIM>(L, Rx, gamma, ig1, fluxs, Fx);
+      riemann_flux<DIM, FAST>(L, Rx, gamma, ig1, fluxs, Fx);
 #pragma unroll
       for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eX[pl(q) * EXV + fx] = Fx[q];
       // y: normal frame (rho, v, u, w, p)
@@ -298,7 +301,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
       for (int q = 0; q < 5; ++q) L[q] = (DIM == 2 && q == 3) ? 0.0 : eY[pl(q) * EXV + fy];
       {
         const double Ln[5] = {L[0], L[2], L[1], L[3], L[4]}, Rn[5] = {Ry[0], Ry[2], Ry[1], Ry[3], Ry[4]};
-        riemann_flux<DIM>(Ln, Rn, gamma, ig1, fluxs, F);
+        riemann_flux<DIM, FAST>(Ln, Rn, gamma, ig1, fluxs, F);
       }
       Fy[0] = F[0]; Fy[1] = F[2]; Fy[2] = F[1]; Fy[3] = F[3]; Fy[4] = F[4];
 #pragma unroll
@@ -313,7 +316,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
         }
         const double Ln[5] = {L[0], h_isx ? L[1] : L[2], h_isx ? L[2] : L[1], L[3], L[4]};
         const double Rn[5] = {Rr[0], h_isx ? Rr[1] : Rr[2], h_isx ? Rr[2] : Rr[1], Rr[3], Rr[4]};
-        riemann_flux<DIM>(Ln, Rn, gamma, ig1, fluxs, F);
+        riemann_flux<DIM, FAST>(Ln, Rn, gamma, ig1, fluxs, F);
         const double Fp[5] = {F[0], h_isx ? F[1] : F[2], h_isx ? F[2] : F[1], F[3], F[4]};
 #pragma unroll
         for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) e[pl(q) * EXV + h_f] = Fp[q];
@@ -393,13 +396,15 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
 #pragma unroll
     for (int q = 0; q < 5; ++q) { dA[q] = 0.0; Lz[q] = 1.0; accp[q] = 0.0; }
     if (t == 0 && active) { issue_plane(-2); issue_plane(-1); }
-#pragma unroll 1
-    for (int c = -2; c <= N + 1; ++c) {
+    // one march iteration; the steady state (c in [2, N]) is the instance with every flag true
+    auto march = [&](int c, auto zslope_t, auto zflux_t, auto fin_t, auto sweep_t) {
+      constexpr bool ZSLOPE = decltype(zslope_t)::value, ZFLUX = decltype(zflux_t)::value;
+      constexpr bool FIN = decltype(fin_t)::value, SWEEP = decltype(sweep_t)::value;
       const int idx = c + 2, s = idx % 3;
       double* Wc = ring + s * C::SLOT;                      // plane c
       const double* Wk = ring + ((idx + 2) % 3) * C::SLOT;  // plane c-1
       double pa[5], pb[5];
-      if (c >= 2 && active) load_prev(c - 2, pa, pb);       // consumed after the z flux: latency hidden
+      if (FIN && active) load_prev(c - 2, pa, pb);          // consumed after the z flux: latency hidden
       double wB[5];
       if (active) {
         mbar_wait(&bars[s], (idx / 3) & 1);
@@ -413,33 +418,33 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
       // ---- z direction along the march: slope of cell c-1 from w(c-2), w(c-1), w(c);
       //      flux at the face between cells c-2 and c-1 (normal frame (rho, w, u, v, p))
       double Fz[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-      if (c >= -1) {
+      if (ZSLOPE) {
         double Rz[5], Ln[5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
           const double wa = Wk[pl(q) * PLANE + own];   // w(c-1), resident in its ring slot
           const double dB = wB[q] - wa;
-          const double hs = half_slope(dA[q], dB, limiter);  // c == -1: dA = 0 -> hs = 0, result unused
+          const double hs = half_slope<FAST>(dA[q], dB, limiter);  // c == -1: dA = 0 -> hs = 0, result unused
           Rz[q] = wa - hs;
           Ln[q] = wa + hs;
           dA[q] = dB;
         }
-        if (c >= 1) {
+        if (ZFLUX) {
           const double Lf[5] = {Lz[0], Lz[3], Lz[1], Lz[2], Lz[4]}, Rf[5] = {Rz[0], Rz[3], Rz[1], Rz[2], Rz[4]};
           double F[5];
-          riemann_flux<3>(Lf, Rf, gamma, ig1, fluxs, F);
+          riemann_flux<3, FAST>(Lf, Rf, gamma, ig1, fluxs, F);
           Fz[0] = F[0]; Fz[3] = F[1]; Fz[1] = F[2]; Fz[2] = F[3]; Fz[4] = F[4];
         }
 #pragma unroll
         for (int q = 0; q < 5; ++q) Lz[q] = Ln[q];
       }
-      if (c >= 2) {
+      if (FIN) {
         double tot[5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) tot[q] = accp[q] - Fz[q];
         finish(c - 2, tot, pa, pb);
       }
-      if (c >= 1 && c <= N) {
+      if (SWEEP) {
         double acc[5];
         sweep_xy(Wk, c & 1, acc);
 #pragma unroll
@@ -449,7 +454,16 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
       }
       // every thread is past its last read of plane c-1: refill that slot with plane c+2
       if (t == 0 && active && c + 2 <= N + 1) issue_plane(c + 2);
-    }
+    };
+    using T = std::true_type;
+    using F_ = std::false_type;
+    march(-2, F_{}, F_{}, F_{}, F_{});
+    march(-1, T{}, F_{}, F_{}, F_{});
+    march(0, T{}, F_{}, F_{}, F_{});
+    march(1, T{}, T{}, F_{}, T{});
+#pragma unroll 1
+    for (int c = 2; c <= N; ++c) march(c, T{}, T{}, T{}, T{});
+    march(N + 1, T{}, T{}, T{}, F_{});
   }
 
   if (p.maxrate) {
@@ -464,14 +478,20 @@ cudaError_t launch_cfg(const StageParams& p, cudaStream_t s) {
   using C = Cfg<DIM, N, TY, G, EXBUF>;
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(stage_kernel<DIM, N, TY, G, EXBUF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)C::SMEM);
+    cudaError_t e = cudaFuncSetAttribute(stage_kernel<DIM, N, TY, G, EXBUF, true>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(stage_kernel<DIM, N, TY, G, EXBUF, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)C::SMEM);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
   const int nitems = p.nblocks * C::YT;
   const int grid = (nitems + G - 1) / G;
-  stage_kernel<DIM, N, TY, G, EXBUF><<<grid, C::NT, C::SMEM, s>>>(p);
+  if (p.limiter == F4_LIM_VANLEER && p.flux == F4_FLUX_HLL)
+    stage_kernel<DIM, N, TY, G, EXBUF, true><<<grid, C::NT, C::SMEM, s>>>(p);
+  else
+    stage_kernel<DIM, N, TY, G, EXBUF, false><<<grid, C::NT, C::SMEM, s>>>(p);
   return cudaGetLastError();
 }
 
