@@ -32,8 +32,10 @@
  *  - Device layout of the bound store: state-major,
  *    then block, var, and a ghost-WRAPPED padded box: along every axis slot
  *    s(i) = i for i >= 0 (interior, then high ghosts) and i + P for i < 0 (low
- *    ghosts last), so that interior rows start on 32-byte sectors and both
- *    x-ghost pairs of a row share one sector.
+ *    ghosts last), so that interior rows start on 32-byte sectors; the four
+ *    x-ghost slots of each row pair (2m, 2m+1) are regrouped by side
+ *    ([hi(2m) hi(2m+1)] in row 2m, [lo(2m) lo(2m+1)] in row 2m+1) so that every
+ *    32-byte ghost sector has exactly one source block.
  */
 #ifndef F4_H
 #define F4_H
@@ -130,8 +132,11 @@ int f4_pattern_size(const f4_mesh *m, int *n_r1, int *n_r2);
 int f4_get_pattern(const f4_mesh *m, int *records);
 
 /* ---- fill_ghosts -----------------------------------------------------------
- * Execute the pattern on one state: one batched kernel for R1, then one for R2
- * iff the mesh has refinement boundaries.  Asynchronous. */
+ * Execute the whole pattern on one state: one batched kernel for R1, then one
+ * for R2 iff the mesh has refinement boundaries.
+ * Asynchronous.  (Inside f4_advance the same-level copies of the state a
+ * stage kernel produces are pushed by that kernel itself, and only the
+ * BC / F2C / C2F records are executed by the batched kernel.) */
 int f4_fill_ghosts(f4_mesh *m, int state);
 
 /* ---- compute_dt ------------------------------------------------------------

@@ -27,8 +27,11 @@ struct f4_mesh {
   int* d_level = nullptr;
   DevRecord* d_r1 = nullptr;
   DevRecord* d_r2 = nullptr;
-  size_t cap_r1 = 0, cap_r2 = 0;
-  int n_r1 = 0, n_r2 = 0;
+  DevRecord* d_r1n = nullptr;  // R1 without the same-level copies (those are pushed by the stage kernel)
+  int* d_nbr = nullptr;        // [max_blocks][6] same-level neighbour per face or -1
+  size_t cap_r1 = 0, cap_r2 = 0, cap_r1n = 0;
+  int n_r1 = 0, n_r2 = 0, n_r1n = 0;
+  std::vector<char> srl_valid;  // per logical state: same-level face ghosts are up to date (pushed or filled)
   DevTransfer* d_plan = nullptr;
   size_t cap_plan = 0;
   unsigned long long* d_maxrate = nullptr;
@@ -108,12 +111,22 @@ int upload_meta(f4_mesh* m) {
     for (size_t q = 0; q < r.size(); ++q)
       out[q] = DevRecord{r[q].dst, r[q].src, r[q].op | r[q].face << 2 | r[q].o1 << 5 | r[q].o2 << 6, 0};
   };
-  std::vector<DevRecord> a, b2;
+  std::vector<DevRecord> a, b2, an;
   pack(m->hm.r1, a);
   pack(m->hm.r2, b2);
+  std::vector<int> nbr((size_t)nb * 6, -1);
+  for (const Record& r : m->hm.r1) {
+    if (r.op == F4_OP_SRL) nbr[(size_t)r.dst * 6 + r.face] = r.src;
+    else an.push_back(DevRecord{r.dst, r.src, r.op | r.face << 2 | r.o1 << 5 | r.o2 << 6, 0});
+  }
   int rc;
   if ((rc = ensure(m, m->d_r1, m->cap_r1, a.size()))) return rc;
   if ((rc = ensure(m, m->d_r2, m->cap_r2, b2.size()))) return rc;
+  if ((rc = ensure(m, m->d_r1n, m->cap_r1n, an.size()))) return rc;
+  if (!an.empty()) CU(cudaMemcpyAsync(m->d_r1n, an.data(), an.size() * sizeof(DevRecord), cudaMemcpyHostToDevice, m->stream));
+  CU(cudaMemcpyAsync(m->d_nbr, nbr.data(), nbr.size() * sizeof(int), cudaMemcpyHostToDevice, m->stream));
+  m->n_r1n = (int)an.size();
+  std::fill(m->srl_valid.begin(), m->srl_valid.end(), 0);
   if (!a.empty()) CU(cudaMemcpyAsync(m->d_r1, a.data(), a.size() * sizeof(DevRecord), cudaMemcpyHostToDevice, m->stream));
   if (!b2.empty()) CU(cudaMemcpyAsync(m->d_r2, b2.data(), b2.size() * sizeof(DevRecord), cudaMemcpyHostToDevice, m->stream));
   m->n_r1 = (int)a.size();
@@ -122,12 +135,16 @@ int upload_meta(f4_mesh* m) {
   return F4_OK;
 }
 
-int fill_ghosts_impl(f4_mesh* m, int state) {
+// skip_srl: the same-level face ghosts of this state were already pushed by the stage kernel that produced it
+int fill_ghosts_impl(f4_mesh* m, int state, bool skip_srl) {
   double* st = m->state_ptr(state);
-  if (m->n_r1) {
+  const DevRecord* r1 = skip_srl ? m->d_r1n : m->d_r1;
+  const int n1 = skip_srl ? m->n_r1n : m->n_r1;
+  if (n1) {
     Scope sc(m, F4_PROF_R1);
-    CU(launch_ghost(m->hm.dim, m->hm.N, GhostParams{st, m->d_r1, m->n_r1, m->theta}, m->stream));
+    CU(launch_ghost(m->hm.dim, m->hm.N, GhostParams{st, r1, n1, m->theta}, m->stream));
   }
+  m->srl_valid[state] = 1;
   if (m->n_r2) {
     Scope sc(m, F4_PROF_R2);
     CU(launch_ghost(m->hm.dim, m->hm.N, GhostParams{st, m->d_r2, m->n_r2, m->theta}, m->stream));
@@ -177,6 +194,7 @@ int f4_mesh_create(int dim, int block_n, int n_ghost, const int brick[3], int ba
   m->bs = m->vs * m->nvar;
   m->state_doubles = m->bs * (size_t)max_blocks;
   m->phys.resize(n_states);
+  m->srl_valid.assign(n_states, 0);
   for (int s = 0; s < n_states; ++s) m->phys[s] = s;
   *out = m;
   return F4_OK;
@@ -189,6 +207,8 @@ int f4_mesh_destroy(f4_mesh* m) {
   if (m->d_level) cudaFree(m->d_level);
   if (m->d_r1) cudaFree(m->d_r1);
   if (m->d_r2) cudaFree(m->d_r2);
+  if (m->d_r1n) cudaFree(m->d_r1n);
+  if (m->d_nbr) cudaFree(m->d_nbr);
   if (m->d_plan) cudaFree(m->d_plan);
   if (m->d_maxrate) cudaFree(m->d_maxrate);
   if (m->d_sums) cudaFree(m->d_sums);
@@ -221,6 +241,7 @@ int f4_bind_storage(f4_mesh* m, void* dev_ptr, size_t bytes, void* cuda_stream) 
   m->stream = (cudaStream_t)cuda_stream;
   if (!m->d_level) {
     CU(cudaMalloc((void**)&m->d_level, (size_t)m->hm.max_blocks * sizeof(int)));
+    CU(cudaMalloc((void**)&m->d_nbr, (size_t)m->hm.max_blocks * 6 * sizeof(int)));
     CU(cudaMalloc((void**)&m->d_maxrate, sizeof(unsigned long long)));
     CU(cudaMalloc((void**)&m->d_sums, (size_t)m->hm.max_blocks * m->nvar * sizeof(double)));
     // staging: whole blocks of the natural padded layout, at most 128 MiB
@@ -266,6 +287,7 @@ int f4_set_state(f4_mesh* m, int state, const double* src, int src_is_device, in
   const size_t E = with_ghosts ? N + 2 * m->hm.Ng : N;
   const size_t per_block = (size_t)m->nvar * E * E * (dim == 3 ? E : 1);
   if (state == 0) m->rate_valid = false;
+  m->srl_valid[state] = 0;
   if (src_is_device) {
     Scope sc(m, F4_PROF_LAYOUT);
     CU(launch_pack(dim, N, m->state_ptr(state), src, 0, nb, with_ghosts, m->stream));
@@ -338,7 +360,7 @@ int f4_get_pattern(const f4_mesh* m, int* records) {
 int f4_fill_ghosts(f4_mesh* m, int state) {
   int rc = check_state(m, state);
   if (rc) return rc;
-  return fill_ghosts_impl(m, state);
+  return fill_ghosts_impl(m, state, false);
 }
 
 int f4_compute_dt(f4_mesh* m, int state, double cfl, double* dt_out) {
@@ -373,7 +395,8 @@ int f4_advance(f4_mesh* m, double dt) {
   p.limiter = m->limiter;
   p.flux = m->flux;
   // stage 1, eq. (6): u1 = dt F(ut) + ut
-  if ((rc = fill_ghosts_impl(m, 0))) return rc;
+  p.nbr = m->d_nbr;
+  if ((rc = fill_ghosts_impl(m, 0, m->srl_valid[0]))) return rc;
   p.deriv = m->state_ptr(0);
   p.prev0 = m->state_ptr(0);
   p.prev1 = nullptr;
@@ -387,7 +410,8 @@ int f4_advance(f4_mesh* m, double dt) {
     CU(launch_stage(dim, N, p, m->stream));
   }
   // stage 2, eq. (7): u = dt/2 F(u1) + (ut + u1)/2, written over ut; CFL max of the new state fused in
-  if ((rc = fill_ghosts_impl(m, 1))) return rc;
+  m->srl_valid[1] = 1;  // pushed by stage 1
+  if ((rc = fill_ghosts_impl(m, 1, true))) return rc;
   CU(cudaMemsetAsync(m->d_maxrate, 0, sizeof(unsigned long long), m->stream));
   p.deriv = m->state_ptr(1);
   p.prev0 = m->state_ptr(0);
@@ -402,6 +426,7 @@ int f4_advance(f4_mesh* m, double dt) {
     CU(launch_stage(dim, N, p, m->stream));
   }
   m->rate_valid = true;
+  m->srl_valid[0] = 1;  // pushed by stage 2; BC / F2C / C2F ghosts of state 0 are stale until the next fill
   return F4_OK;
 }
 
@@ -409,7 +434,7 @@ int f4_adapt(f4_mesh* m, const int* refine_flags, int* changed_out) {
   if (!m || !refine_flags || !changed_out) return F4_EINVAL;
   *changed_out = 0;
   int rc;
-  if (m->bound && (rc = fill_ghosts_impl(m, 0))) return rc;  // prolongation reads the parents' face ghosts
+  if (m->bound && (rc = fill_ghosts_impl(m, 0, m->srl_valid[0]))) return rc;  // prolongation reads the parents' face ghosts
   std::vector<Transfer> plan;
   bool changed = false;
   std::string err;
@@ -435,6 +460,7 @@ int f4_adapt(f4_mesh* m, const int* refine_flags, int* changed_out) {
   }
   CU(cudaStreamSynchronize(m->stream));
   std::swap(m->phys[0], m->phys[1]);  // the new numbering lives in the slab that was state 1
+  std::fill(m->srl_valid.begin(), m->srl_valid.end(), 0);
   m->rate_valid = false;
   return upload_meta(m);
 }

@@ -33,6 +33,7 @@ struct StageParams {
   int nblocks;
   int limiter, flux;
   unsigned long long* maxrate;  // bits of a non-negative double, atomicMax; nullptr = no CFL reduction
+  const int* nbr;               // [nblocks][6] same-level neighbour per face or -1: fused SRL ghost push; nullptr = off
 };
 
 struct GhostParams {

@@ -4,10 +4,11 @@
 // driven by a device-resident list of records (dst block, src block, face, op)
 // sorted by destination block, instead of one OpenACC loop per boundary type
 // and face direction.  A CTA takes 2*DIM consecutive
-// records (= all faces of one block on a uniform mesh), so that the -x and +x
-// ghost pairs of a row, which share one 32-byte sector in the wrapped layout,
-// are written back-to-back and merge in L2.  HBM-bound: 16-byte vector
-// accesses, all loads of a thread issued before its stores.
+// records (= all faces of one block on a uniform mesh).  HBM-bound: 16-byte
+// vector accesses, all loads of a thread issued before its stores; with the
+// pair-transposed x-ghost layout (cell_off) two adjacent lanes write one full
+// 32-byte ghost sector.  Inside f4_advance the SRL records are not executed
+// here: the stage kernel pushes those layers itself (f4_stage.cu).
 #include "../../include/f4.h"
 #include "f4_dev.hpp"
 
@@ -33,7 +34,13 @@ __device__ __forceinline__ void st2(double* p, double2 v) { *reinterpret_cast<do
 template <int DIM, int N>
 __device__ __forceinline__ int cell_off(int i, int j, int k) {
   using G = Geo<DIM, N>;
-  int o = G::slot(j) * G::P + G::slot(i);
+  // x ghosts are pair-transposed: the 4 ghost slots of rows (2m, 2m+1) hold [hi(2m) hi(2m+1)] in row 2m and
+  // [lo(2m) lo(2m+1)] in row 2m+1, so that each 32-byte ghost sector has a single source block
+  const int sj = G::slot(j);
+  int row = sj, col = i;
+  if (i >= N) { row = sj & ~1; col = N + 2 * (sj & 1) + (i - N); }
+  else if (i < 0) { row = sj | 1; col = N + 2 * (sj & 1) + (i + NG); }
+  int o = row * G::P + col;
   if (DIM == 3) o += G::slot(k) * G::P * G::P;
   return o;
 }
@@ -108,9 +115,9 @@ __device__ __forceinline__ void do_copy_face(double* __restrict__ st, int dst, i
         int so, d_o;
         if (a == 0) {  // one row = one 16-byte ghost pair
           int j = r % N, k = (DIM == 3) ? r / N : 0;
-          int row = (DIM == 3 ? k * P * P : 0) + j * P;
-          d_o = row + dn;
-          so = row + sn;
+          int pl0 = (DIM == 3 ? k * P * P : 0);
+          d_o = pl0 + (side ? (j & ~1) : (j | 1)) * P + N + 2 * (j & 1);   // pair-transposed x ghosts (cell_off)
+          so = pl0 + j * P + sn;
           if (outflow) {
             double x = sb[(size_t)v * G::VS + so];
             val[u] = make_double2(x, x);

@@ -241,7 +241,11 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
 
   // per-thread constants of the x/y sweep
   const int own = (j + 2) * P + i;
-  const int own_xm = (j + 2) * P + (i == 0 ? P - 1 : i - 1);
+  // x ghosts are pair-transposed (f4_ghost.cu cell_off): ghost (N+g, row r) sits in row r&~1, (g-2, row r) in row r|1,
+  // both at column N + 2*(r&1) + g
+  const int rr = j + 2;
+  const int own_xm = (i == 0) ? (rr | 1) * P + N + 2 * (rr & 1) + 1 : rr * P + i - 1;
+  const int own_xp = (i == N - 1) ? (rr & ~1) * P + N + 2 * (rr & 1) : own + 1;
   const int fx = j * (N + 1) + i, fy = j * N + i;      // own low faces in the exchange arrays
   // halo roles: threads [0,NH) take the high halo cells (slope + last face flux), [NH,2NH) the low ones (slope)
   const bool is_hi = t < NH, is_lo = (t >= NH) && (t < 2 * NH);
@@ -249,10 +253,10 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
   const bool h_isx = hq < TY;                          // x halo of row hq, else y halo of column hq-TY
   int h_o0, h_om, h_op, h_f;
   if (h_isx) {
-    const int row = (hq + 2) * P;
-    h_o0 = row + (is_hi ? N : P - 1);
-    h_om = row + (is_hi ? N - 1 : P - 2);
-    h_op = row + (is_hi ? N + 1 : 0);
+    const int r = hq + 2, gcol = N + 2 * (r & 1);
+    h_o0 = is_hi ? (r & ~1) * P + gcol : (r | 1) * P + gcol + 1;   // cell N / cell -1
+    h_om = is_hi ? r * P + N - 1 : h_o0 - 1;                       // cell N-1 / cell -2
+    h_op = is_hi ? h_o0 + 1 : r * P;                               // cell N+1 / cell 0
     h_f = hq * (N + 1) + (is_hi ? N : 0);
   } else {
     const int col = hq - TY;
@@ -269,7 +273,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
     double Rx[5], Ry[5];
     {  // ---- phase 1: slopes -> left states to smem, right states stay in registers
       double L[5];
-      slope_states(W, own, own_xm, own + 1, L, Rx);
+      slope_states(W, own, own_xm, own_xp, L, Rx);
 #pragma unroll
       for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eX[pl(q) * EXV + fx + 1] = L[q];
       slope_states(W, own, own - P, own + P, L, Ry);
@@ -335,6 +339,19 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
   // Runge-Kutta combine eq. (5) + store + optional CFL rate of the new state
   double rate_max = 0.0;
   const size_t cell0 = (size_t)blk * C::BS + (size_t)(j0 + j) * P + i;   // + k*P*P + v*VS
+  // fused same-level ghost fill: boundary layers are pushed from registers into the neighbours' ghost cells
+  // (a1 of the pattern).  nbr[f] = same-level neighbour across face f, or -1.
+  long long px_off = -1, py_off = -1;   // offsets (doubles, without k and var) of the x / y push targets
+  int nbz0 = -1, nbz1 = -1;
+  if (p.nbr && active) {
+    const int* nb = p.nbr + (size_t)blk * 6;
+    const int jg = j0 + j;
+    if (i < NG && nb[0] >= 0) px_off = (long long)nb[0] * C::BS + ((jg & ~1) * P + N + 2 * (jg & 1) + i);
+    if (i >= N - NG && nb[1] >= 0) px_off = (long long)nb[1] * C::BS + ((jg | 1) * P + N + 2 * (jg & 1) + (i - (N - NG)));
+    if (jg < NG && nb[2] >= 0) py_off = (long long)nb[2] * C::BS + ((N + jg) * P + i);
+    if (jg >= N - NG && nb[3] >= 0) py_off = (long long)nb[3] * C::BS + ((jg + 2 * NG) * P + i);
+    if (DIM == 3) { nbz0 = nb[4]; nbz1 = nb[5]; }
+  }
   auto load_prev = [&](int k, double (&a)[5], double (&b)[5]) {
     const size_t o = cell0 + (size_t)(DIM == 3 ? k : 0) * P * P;
 #pragma unroll
@@ -354,6 +371,23 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
       if (DIM == 2 && q == 3) { u[q] = 0.0; continue; }
       u[q] = fma(s, tot[q], fma(p.w1, b[q], p.w0 * a[q]));
       p.out[o + pl(q) * C::VS] = u[q];
+    }
+    const size_t kof = (size_t)(DIM == 3 ? k : 0) * P * P;
+    if (px_off >= 0) {
+#pragma unroll
+      for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) p.out[px_off + kof + pl(q) * C::VS] = u[q];
+    }
+    if (py_off >= 0) {
+#pragma unroll
+      for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) p.out[py_off + kof + pl(q) * C::VS] = u[q];
+    }
+    if (DIM == 3) {
+      const int nbz = (k < NG) ? nbz0 : (k >= N - NG ? nbz1 : -1);
+      if (nbz >= 0) {
+        const size_t zo = (size_t)nbz * C::BS + (size_t)(k < NG ? N + k : k + 2 * NG) * P * P + (size_t)(j0 + j) * P + i;
+#pragma unroll
+        for (int q = 0; q < 5; ++q) p.out[zo + pl(q) * C::VS] = u[q];
+      }
     }
     if (p.maxrate) {
       const double ir = rcp_fast(u[0]);

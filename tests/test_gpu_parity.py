@@ -357,3 +357,20 @@ def test_linear_field_on_gpu():
                 m.adapt(np.where(lev == lev.max(), -1, 0).astype(np.int32))
                 check()
         m.close()
+
+
+@pytest.mark.parametrize("n,scale", [(1, None), (2, 1), (3, 1), (4, 0)])
+def test_fused_srl_push_equals_pattern_fill(n, scale):
+    # advance() pushes the same-level ghost layers from the stage kernel; the batched executor must give the same bits
+    cfg = W.config(n, scale=scale)
+    lm, om = make_pair(cfg)
+    set_both(lm, om, cfg)
+    for _ in range(2):
+        lm.advance(lm.compute_dt(0, 0.4))
+    pushed = lm.get_state(0, with_ghosts=True)
+    lm.fill_ghosts(0)                       # full pattern: SRL records included
+    filled = lm.get_state(0, with_ghosts=True)
+    nc = noncorner_mask(lm)
+    for v in range(lm.nvar):
+        assert np.array_equal(pushed[:, v][nc], filled[:, v][nc])
+    lm.close()
