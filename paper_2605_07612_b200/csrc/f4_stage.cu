@@ -98,10 +98,11 @@ __device__ __forceinline__ void riemann_flux(const double (&L)[5], const double 
   const double yL = rsqrt_fast(L[0]), yR = rsqrt_fast(R[0]);  // 1/sqrt(rho)
   const double rL = L[0] * yL, rR = R[0] * yR;                // sqrt(rho)
   const double w = rcp_fast(rL + rR);
-  const double uhat = (rL * L[1] + rR * R[1]) * w;
+  const double wl = rL * w, wr = rR * w;                      // Roe weights
+  const double uhat = fma(wl, L[1], wr * R[1]);
   const double du = R[1] - L[1];
   // d^2 = (rL cL^2 + rR cR^2)/(rL+rR) + 1/2 rL rR/(rL+rR)^2 du^2,  r c^2 = gamma p / sqrt(rho)
-  const double d2 = fma(gamma * (L[4] * yL + R[4] * yR), w, 0.5 * (rL * w) * (rR * w) * du * du);
+  const double d2 = fma((0.5 * wl) * wr, du * du, fma(L[4], yL, R[4] * yR) * (gamma * w));
   const double dhat = d2 * rsqrt_fast(d2);
   double sm = uhat - dhat, sp = uhat + dhat;
   if (!FAST && flux == F4_FLUX_RUSANOV) {
@@ -112,18 +113,21 @@ __device__ __forceinline__ void riemann_flux(const double (&L)[5], const double 
     sm = fmin(sm, 0.0);
     sp = fmax(sp, 0.0);
   }
+  // F = a FL + b FR + c (UR - UL) with a = S+/(S+ - S-), b = -S-/(S+ - S-), c = S+ S-/(S+ - S-), regrouped per side:
+  //   beta_L = a uL - c, beta_R = b uR + c, alpha = rho beta;  mass = alpha_L + alpha_R, momentum = alpha u (+ a pL + b pR
+  //   for the normal component), energy = alpha h + p (beta/(gamma-1) + a u)  with h = |u|^2/2  (eq. 14-15)
   const double inv = rcp_fast(sp - sm);
-  const double a = sp * inv, b = -sm * inv, c = sp * sm * inv;  // F = a FL + b FR + c (UR - UL)
-  double keL = L[1] * L[1] + L[2] * L[2], keR = R[1] * R[1] + R[2] * R[2];
-  if (DIM == 3) { keL = fma(L[3], L[3], keL); keR = fma(R[3], R[3], keR); }
-  const double EL = fma(L[4], ig1, 0.5 * L[0] * keL), ER = fma(R[4], ig1, 0.5 * R[0] * keR);  // eq. (15)
-  const double mL = L[0] * L[1], mR = R[0] * R[1];
-  F[0] = fma(a, mL, fma(b, mR, c * (R[0] - L[0])));
-  F[1] = fma(a, fma(mL, L[1], L[4]), fma(b, fma(mR, R[1], R[4]), c * (mR - mL)));
-  F[2] = fma(a, mL * L[2], fma(b, mR * R[2], c * (R[0] * R[2] - L[0] * L[2])));
-  if (DIM == 3) F[3] = fma(a, mL * L[3], fma(b, mR * R[3], c * (R[0] * R[3] - L[0] * L[3])));
-  else F[3] = 0.0;
-  F[4] = fma(a, (EL + L[4]) * L[1], fma(b, (ER + R[4]) * R[1], c * (ER - EL)));
+  const double a = sp * inv, b = -sm * inv, c = a * sm;
+  const double auL = a * L[1], buR = b * R[1];
+  const double bL = auL - c, bR = buR + c;
+  const double aL = L[0] * bL, aR = R[0] * bR;
+  double hL = fma(L[1], L[1], L[2] * L[2]), hR = fma(R[1], R[1], R[2] * R[2]);
+  if (DIM == 3) { hL = fma(L[3], L[3], hL); hR = fma(R[3], R[3], hR); }
+  F[0] = aL + aR;
+  F[1] = fma(aL, L[1], fma(aR, R[1], fma(a, L[4], b * R[4])));
+  F[2] = fma(aL, L[2], aR * R[2]);
+  F[3] = (DIM == 3) ? fma(aL, L[3], aR * R[3]) : 0.0;
+  F[4] = fma(0.5 * aL, hL, fma(0.5 * aR, hR, fma(L[4], fma(bL, ig1, auL), R[4] * fma(bR, ig1, buR))));
 }
 
 template <int DIM, int N, int TY, int G, int EXBUF>
