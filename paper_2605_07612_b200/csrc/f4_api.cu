@@ -389,7 +389,14 @@ int f4_advance(f4_mesh* m, double dt) {
   const int dim = m->hm.dim, N = m->hm.N, nb = (int)m->hm.leaves.size();
   StageParams p{};
   p.gamma = m->gamma;
-  p.inv_dx0 = 1.0 / m->hm.dx_of_level(0);
+  const double inv_dx0 = 1.0 / m->hm.dx_of_level(0);
+  auto set_dt = [&](double dt_sub) {
+    p.dt_sub = dt_sub;
+    for (int l = 0; l < MAXL; ++l) {
+      p.inv_dx_l[l] = inv_dx0 * (double)(1u << l);
+      p.sdt_l[l] = dt_sub * p.inv_dx_l[l];
+    }
+  };
   p.level = m->d_level;
   p.nblocks = nb;
   p.limiter = m->limiter;
@@ -403,7 +410,7 @@ int f4_advance(f4_mesh* m, double dt) {
   p.out = m->state_ptr(1);
   p.w0 = 1.0;
   p.w1 = 0.0;
-  p.dt_sub = dt;
+  set_dt(dt);
   p.maxrate = nullptr;
   {
     Scope sc(m, F4_PROF_STAGE);
@@ -419,7 +426,7 @@ int f4_advance(f4_mesh* m, double dt) {
   p.out = m->state_ptr(0);
   p.w0 = 0.5;
   p.w1 = 0.5;
-  p.dt_sub = 0.5 * dt;
+  set_dt(0.5 * dt);
   p.maxrate = m->d_maxrate;
   {
     Scope sc(m, F4_PROF_STAGE);

@@ -10,6 +10,7 @@
 namespace f4 {
 
 constexpr int NG = 2;  // ghost layers compiled into the kernels
+constexpr int MAXL = 20;  // refinement levels (f4_mesh_create checks max_level <= 18)
 
 // meta = op | face << 2 | o1 << 5 | o2 << 6
 struct DevRecord {
@@ -28,7 +29,8 @@ struct StageParams {
   double* out;
   double w0, w1, dt_sub;
   double gamma;
-  double inv_dx0;       // 1/dx at level 0
+  double inv_dx_l[MAXL];  // 1/dx per refinement level (1/dx_0 * 2^l, exact)
+  double sdt_l[MAXL];     // dt_sub/dx per level: the factor of the flux difference in eq. (5)
   const int* level;     // per block
   int nblocks;
   int limiter, flux;

@@ -2,7 +2,8 @@
 //   u(s_out) = dt_sub * F(u(s_deriv)) + w0 u(s_prev0) + w1 u(s_prev1)
 // over every block, F = -div of HLL fluxes of
 // limited primitive reconstructions, optional
-// fused CFL max of the NEW state.
+// fused CFL max of the NEW state, fused same-level ghost copy
+// of the new state into the neighbours' ghost cells.
 //
 // Design (differs from the paper's gang-per-block / collapse(3) OpenACC loop,
 // PAPER.md:162-189, which converts the whole block to uu_prim in global
@@ -12,15 +13,23 @@
 //  * padded planes of the conservative state are fetched by bulk async copies
 //    (cp.async.bulk, the TMA engine, completion on an mbarrier) into a 3-slot
 //    shared-memory ring one plane ahead of use, and converted to primitives in
-//    place (to_primitive once per cell);
+//    place (to_primitive once per cell); when the tile is the
+//    whole block the smem plane keeps the store's wrapped row order, so one
+//    bulk copy per variable moves a plane;
 //  * x/y fluxes exchange reconstructed states and fluxes through shared
 //    memory; the z direction lives in registers along the march;
-//  * fp64 division / sqrt are replaced by MUFU seeds + cubic Newton steps
-//    (the kernel is co-limited by the fp64 pipe).
+//  * fp64 division / sqrt are replaced by MUFU seeds + cubic Newton steps, and
+//    1/(S+ - S-) of the HLL flux by 1/(2 d^) = rsqrt(d^2)/2 (already at hand)
+//    with the supersonic cases selected by sign bits: the kernel is co-limited
+//    by the fp64 pipe and by dependent-issue latency.
 #include <type_traits>
 
 #include "../../include/f4.h"
 #include "f4_dev.hpp"
+
+#ifndef F4_MINB
+#define F4_MINB(x) (x)
+#endif
 
 namespace f4 {
 namespace {
@@ -47,10 +56,10 @@ __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)_
 __device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
 }
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   asm volatile(
       "{\n"
       ".reg .pred p;\n"
@@ -59,15 +68,14 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
       "@p bra DONE_%=;\n"
       "bra WAIT_%=;\n"
       "DONE_%=:\n"
-      "}\n" ::"r"(smem_u32(bar)),
+      "}\n" ::"r"(bar),
       "r"(parity)
       : "memory");
 }
 // 1-D bulk async copy global -> shared (TMA engine; SASS UBLKCP), completion counted on the mbarrier
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                   smem_u32(dst)),
-               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+               "l"(src), "r"(bytes), "r"(bar)
                : "memory");
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
@@ -79,9 +87,15 @@ __device__ __forceinline__ void group_sync(int id, int nthreads) {
 template <bool FAST>
 __device__ __forceinline__ double half_slope(double a, double b, int limiter) {
   double ab = a * b;
+  if (FAST) {
+    // van Leer: 1/2 * 2ab/(a+b) where ab > 0.  The sign test is taken on the high word of ab (an integer compare
+    // instead of a DSETP on the fp64 pipe); it differs from ab > 0 only for 0 < ab < 2^-1042, where the slope is < 1e-150.
+    double r = ab * rcp_fast(a + b);
+    return (__double2hiint(ab) > 0) ? r : 0.0;
+  }
   double r;
-  if (FAST || limiter == F4_LIM_VANLEER) {
-    r = ab * rcp_fast(a + b);                         // 1/2 * 2ab/(a+b)
+  if (limiter == F4_LIM_VANLEER) {
+    r = ab * rcp_fast(a + b);
   } else {
     double th = (limiter == F4_LIM_MC) ? 2.0 : 1.0;   // eq. (1)
     double m = fmin(fmin(fabs(th * a), fabs(th * b)), fabs(a + b) * 0.5);
@@ -103,21 +117,40 @@ __device__ __forceinline__ void riemann_flux(const double (&L)[5], const double 
   const double du = R[1] - L[1];
   // d^2 = (rL cL^2 + rR cR^2)/(rL+rR) + 1/2 rL rR/(rL+rR)^2 du^2,  r c^2 = gamma p / sqrt(rho)
   const double d2 = fma((0.5 * wl) * wr, du * du, fma(L[4], yL, R[4] * yR) * (gamma * w));
-  const double dhat = d2 * rsqrt_fast(d2);
+  const double y2 = rsqrt_fast(d2);
+  const double dhat = d2 * y2;
   double sm = uhat - dhat, sp = uhat + dhat;
-  if (!FAST && flux == F4_FLUX_RUSANOV) {
-    double s = fmax(fabs(sm), fabs(sp));
-    sm = -s;
-    sp = s;
+  // F = a FL + b FR + c (UR - UL) with a = S+/(S+ - S-), b = -S-/(S+ - S-), c = S+ S-/(S+ - S-)
+  double a, b, c;
+  if (FAST) {
+    // HLL: S- = min(sm,0), S+ = max(sp,0).  Subsonic: S+ - S- = 2 d^, so 1/(S+ - S-) = y2/2 (no second reciprocal);
+    // supersonic: (a,b,c) = (1,0,0) or (0,1,0) exactly.  Sign bits instead of fp64 compares.
+    const double inv = 0.5 * y2;
+    const bool right = __double2hiint(sm) >= 0, left = __double2hiint(sp) < 0;
+    sm = right ? 0.0 : sm;
+    sp = left ? 0.0 : sp;
+    a = sp * inv;
+    b = -sm * inv;
+    a = right ? 1.0 : a;
+    b = left ? 1.0 : b;
+    c = a * sm;
   } else {
-    sm = fmin(sm, 0.0);
-    sp = fmax(sp, 0.0);
+    if (flux == F4_FLUX_RUSANOV) {
+      double s = fmax(fabs(sm), fabs(sp));
+      sm = -s;
+      sp = s;
+    } else {
+      sm = fmin(sm, 0.0);
+      sp = fmax(sp, 0.0);
+    }
+    const double inv = rcp_fast(sp - sm);
+    a = sp * inv;
+    b = -sm * inv;
+    c = a * sm;
   }
-  // F = a FL + b FR + c (UR - UL) with a = S+/(S+ - S-), b = -S-/(S+ - S-), c = S+ S-/(S+ - S-), regrouped per side:
-  //   beta_L = a uL - c, beta_R = b uR + c, alpha = rho beta;  mass = alpha_L + alpha_R, momentum = alpha u (+ a pL + b pR
-  //   for the normal component), energy = alpha h + p (beta/(gamma-1) + a u)  with h = |u|^2/2  (eq. 14-15)
-  const double inv = rcp_fast(sp - sm);
-  const double a = sp * inv, b = -sm * inv, c = a * sm;
+  // regrouped per side: beta_L = a uL - c, beta_R = b uR + c, alpha = rho beta;  mass = alpha_L + alpha_R,
+  //   momentum = alpha u (+ a pL + b pR for the normal component), energy = alpha h + p (beta/(gamma-1) + a u)
+  //   with h = |u|^2/2  (eq. 14-15)
   const double auL = a * L[1], buR = b * R[1];
   const double bL = auL - c, bR = buR + c;
   const double aL = L[0] * bL, aR = R[0] * bR;
@@ -137,6 +170,7 @@ struct Cfg {  // FAST (van Leer + HLL fixed at compile time) does not change the
   static constexpr int NVAR = DIM + 2;
   static constexpr size_t VS = (size_t)P * P * PZ;
   static constexpr size_t BS = VS * NVAR;
+  static constexpr bool WHOLE = (TY == N);    // the tile is the whole block plane: smem rows keep the wrapped slot order
   static constexpr int ROWS = TY + 4;
   static constexpr int PLANE = ROWS * P;      // doubles per variable in one ring slot
   static constexpr int SLOT = NVAR * PLANE;
@@ -156,34 +190,41 @@ struct Cfg {  // FAST (van Leer + HLL fixed at compile time) does not change the
 };
 
 template <int DIM, int N, int TY, int G, int EXBUF, bool FAST>
-__global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY, G, EXBUF>::SMEM <= 110 * 1024) ? 2 : 1)
-    stage_kernel(StageParams p) {
+__global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT,
+                                  F4_MINB((Cfg<DIM, N, TY, G, EXBUF>::SMEM <= 110 * 1024) ? 2 : 1))
+    stage_kernel(const __grid_constant__ StageParams p) {
   using C = Cfg<DIM, N, TY, G, EXBUF>;
-  constexpr int P = C::P, NV = C::NVAR, PLANE = C::PLANE, TG = C::TG, EXV = C::EXV, NH = C::NH;
+  constexpr int P = C::P, PP = C::P * C::P, NV = C::NVAR, PLANE = C::PLANE, TG = C::TG, EXV = C::EXV, NH = C::NH;
+  constexpr bool WHOLE = C::WHOLE;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  const int grp = threadIdx.x / TG, t = threadIdx.x % TG;
+  const int grp = (G == 1) ? 0 : (int)threadIdx.x / TG;
+  const int t = (G == 1) ? (int)threadIdx.x : (int)threadIdx.x % TG;
+  const int item = blockIdx.x * G + grp;
+  // a whole group leaves together: its named barrier and mbarriers are private to the group
+  if (item >= p.nblocks * C::YT) return;
+  const int blk = WHOLE ? item : item / C::YT;
+  const int j0 = WHOLE ? 0 : (item % C::YT) * TY;
+  const int i = t % N, j = t / N;
+
   double* ring = reinterpret_cast<double*>(smem_raw) + (size_t)grp * C::GROUP_DOUBLES;
   double* exX = ring + C::NSLOT * C::SLOT;   // [EXBUF][NV][EXV]
   double* exY = exX + EXBUF * C::EX;
   double* sRh = exY + EXBUF * C::EX;         // [NV][NH]
   uint64_t* bars = reinterpret_cast<uint64_t*>(reinterpret_cast<double*>(smem_raw) + (size_t)G * C::GROUP_DOUBLES) +
                    grp * C::NSLOT;
+  const uint32_t ring_u32 = smem_u32(ring), bars_u32 = smem_u32(bars);
   const int bar_id = 1 + grp;
-
-  const int item = blockIdx.x * G + grp;
-  const int nitems = p.nblocks * C::YT;
-  const bool active = item < nitems;
-  const int blk = active ? item / C::YT : 0;
-  const int j0 = active ? (item % C::YT) * TY : 0;
-  const int i = t % N, j = t / N;
 
   const double gamma = p.gamma, gm1 = gamma - 1.0, ig1 = 1.0 / gm1;
   const int limiter = p.limiter, fluxs = p.flux;
-  const double inv_dx = p.inv_dx0 * (double)(1u << p.level[blk]);
-  const double* dbase = p.deriv + (size_t)blk * C::BS;
+  const int lvl = p.level[blk];
+  const size_t boff = (size_t)blk * C::BS;
+  const double* dbase = p.deriv + boff;
 
   // register arrays are in "phys5" order (rho, u, v, w, p); smem plane of component q:
   auto pl = [](int q) { return q < 4 ? q : NV - 1; };
+  // smem row of block row y (y in [j0-2, j0+TY+2)): the store's wrapped slot when the tile is the whole plane
+  auto rown = [&](int y) { return WHOLE ? (y < 0 ? y + P : y) : y - j0 + 2; };
 
   if (t == 0) {
     for (int s = 0; s < C::NSLOT; ++s) mbar_init(&bars[s], 1);
@@ -191,24 +232,30 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
   }
   group_sync(bar_id, TG);
 
-  // issue the bulk copies of z plane c (c in [-2, N+2); 2D: c = 0) into its ring slot
-  auto issue_plane = [&](int c) {
-    const int idx = (DIM == 3) ? c + 2 : 0;
-    const int s = idx % C::NSLOT;
+  // issue the bulk copies of z plane c (c in [-2, N+2); 2D: c = 0) into ring slot s
+  auto issue_plane = [&](int c, int s) {
     const bool interior = (DIM == 2) || (c >= 0 && c < N);
     const int kslot = (DIM == 3) ? (c < 0 ? c + P : c) : 0;
-    double* dst = ring + s * C::SLOT;
-    const double* src = dbase + (size_t)kslot * P * P;
-    // rows y in [ylo, yhi) -> smem rows y - (j0-2); rows with y < 0 live in slots y + P
-    const int ylo = interior ? j0 - 2 : j0, yhi = interior ? j0 + TY + 2 : j0 + TY;
-    const int nlow = ylo < 0 ? -ylo : 0;
-    const uint32_t bytes_low = (uint32_t)nlow * P * 8, bytes_hi = (uint32_t)(yhi - ylo - nlow) * P * 8;
-    mbar_expect_tx(&bars[s], (bytes_low + bytes_hi) * NV);
-    for (int v = 0; v < NV; ++v) {
-      const double* sv = src + (size_t)v * C::VS;
-      double* dv = dst + v * PLANE;
-      if (nlow) bulk_g2s(dv + (ylo - (j0 - 2)) * P, sv + (size_t)(ylo + P) * P, bytes_low, &bars[s]);
-      bulk_g2s(dv + (ylo + nlow - (j0 - 2)) * P, sv + (size_t)(ylo + nlow) * P, bytes_hi, &bars[s]);
+    const uint32_t dst = ring_u32 + (uint32_t)(s * C::SLOT) * 8u, bar = bars_u32 + 8u * s;
+    const double* src = dbase + (size_t)kslot * PP;
+    if (WHOLE) {
+      // interior plane: all P slot rows (N interior, 2 high, 2 low ghost rows); z-ghost plane: the N interior rows
+      const uint32_t bytes = (uint32_t)(interior ? P : N) * P * 8;
+      mbar_expect_tx(bar, bytes * NV);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) bulk_g2s(dst + (uint32_t)(v * PLANE) * 8u, src + (size_t)v * C::VS, bytes, bar);
+    } else {
+      // rows y in [ylo, yhi) -> smem rows y - (j0-2); rows with y < 0 live in slots y + P
+      const int ylo = interior ? j0 - 2 : j0, yhi = interior ? j0 + TY + 2 : j0 + TY;
+      const int nlow = ylo < 0 ? -ylo : 0;
+      const uint32_t bytes_low = (uint32_t)nlow * P * 8, bytes_hi = (uint32_t)(yhi - ylo - nlow) * P * 8;
+      mbar_expect_tx(bar, (bytes_low + bytes_hi) * NV);
+      for (int v = 0; v < NV; ++v) {
+        const double* sv = src + (size_t)v * C::VS;
+        const uint32_t dv = dst + (uint32_t)(v * PLANE) * 8u;
+        if (nlow) bulk_g2s(dv + (uint32_t)((ylo - (j0 - 2)) * P) * 8u, sv + (size_t)(ylo + P) * P, bytes_low, bar);
+        bulk_g2s(dv + (uint32_t)((ylo + nlow - (j0 - 2)) * P) * 8u, sv + (size_t)(ylo + nlow) * P, bytes_hi, bar);
+      }
     }
   };
 
@@ -244,11 +291,12 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
   };
 
   // per-thread constants of the x/y sweep
-  const int own = (j + 2) * P + i;
+  const int rr = rown(j0 + j);
+  const int own = rr * P + i;
+  const int own_ym = rown(j0 + j - 1) * P + i, own_yp = rown(j0 + j + 1) * P + i;
   // x ghosts are pair-transposed (f4_ghost.cu cell_off): ghost (N+g, row r) sits in row r&~1, (g-2, row r) in row r|1,
-  // both at column N + 2*(r&1) + g
-  const int rr = j + 2;
-  const int own_xm = (i == 0) ? (rr | 1) * P + N + 2 * (rr & 1) + 1 : rr * P + i - 1;
+  // both at column N + 2*(r&1) + g  (smem rows have the parity of the store's slot rows)
+  const int own_xm = (i == 0) ? (rr | 1) * P + N + 2 * (rr & 1) + 1 : own - 1;
   const int own_xp = (i == N - 1) ? (rr & ~1) * P + N + 2 * (rr & 1) : own + 1;
   const int fx = j * (N + 1) + i, fy = j * N + i;      // own low faces in the exchange arrays
   // halo roles: threads [0,NH) take the high halo cells (slope + last face flux), [NH,2NH) the low ones (slope)
@@ -257,17 +305,27 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
   const bool h_isx = hq < TY;                          // x halo of row hq, else y halo of column hq-TY
   int h_o0, h_om, h_op, h_f;
   if (h_isx) {
-    const int r = hq + 2, gcol = N + 2 * (r & 1);
+    const int r = rown(j0 + hq), gcol = N + 2 * (r & 1);
     h_o0 = is_hi ? (r & ~1) * P + gcol : (r | 1) * P + gcol + 1;   // cell N / cell -1
     h_om = is_hi ? r * P + N - 1 : h_o0 - 1;                       // cell N-1 / cell -2
     h_op = is_hi ? h_o0 + 1 : r * P;                               // cell N+1 / cell 0
     h_f = hq * (N + 1) + (is_hi ? N : 0);
   } else {
     const int col = hq - TY;
-    h_o0 = (is_hi ? TY + 2 : 1) * P + col;
-    h_om = h_o0 - P;
-    h_op = h_o0 + P;
+    const int y = is_hi ? j0 + TY : j0 - 1;                        // row TY / row -1 of the tile
+    h_o0 = rown(y) * P + col;
+    h_om = rown(y - 1) * P + col;
+    h_op = rown(y + 1) * P + col;
     h_f = (is_hi ? TY : 0) * N + col;
+  }
+  // halo cell converted by this thread on interior planes
+  int hc_o = -1;
+  if (t < C::HALO) {
+    if (t < 4 * TY) hc_o = rown(j0 + t / 4) * P + N + (t % 4);
+    else {
+      const int tq = t - 4 * TY, r4 = tq / N;
+      hc_o = rown(r4 < 2 ? j0 - 2 + r4 : j0 + TY + r4 - 2) * P + tq % N;
+    }
   }
 
   // x/y sweep on the converted plane W: sum over the x,y faces of (F_in - F_out) of the own cell
@@ -280,7 +338,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
       slope_states(W, own, own_xm, own_xp, L, Rx);
 #pragma unroll
       for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eX[pl(q) * EXV + fx + 1] = L[q];
-      slope_states(W, own, own - P, own + P, L, Ry);
+      slope_states(W, own, own_ym, own_yp, L, Ry);
 #pragma unroll
       for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eY[pl(q) * EXV + fy + N] = L[q];
       if (is_hi || is_lo) {
@@ -342,55 +400,57 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
 
   // Runge-Kutta combine eq. (5) + store + optional CFL rate of the new state
   double rate_max = 0.0;
-  const size_t cell0 = (size_t)blk * C::BS + (size_t)(j0 + j) * P + i;   // + k*P*P + v*VS
+  const double sdt = p.sdt_l[lvl];                          // dt_sub / dx of this block's level
+  const int co = (j0 + j) * P + i;                          // own cell inside a (block, var) box, + k*PP + v*VS
+  const double* pa = p.prev0 + boff + co;
+  const double* pb = p.prev1 ? p.prev1 + boff + co : nullptr;
+  double* po = p.out + boff + co;
   // fused same-level ghost fill: boundary layers are pushed from registers into the neighbours' ghost cells
   // (a1 of the pattern).  nbr[f] = same-level neighbour across face f, or -1.
-  long long px_off = -1, py_off = -1;   // offsets (doubles, without k and var) of the x / y push targets
+  double* ppx = nullptr;   // x / y push targets of this thread (k = 0, var 0)
+  double* ppy = nullptr;
   int nbz0 = -1, nbz1 = -1;
-  if (p.nbr && active) {
+  if (p.nbr) {
     const int* nb = p.nbr + (size_t)blk * 6;
     const int jg = j0 + j;
-    if (i < NG && nb[0] >= 0) px_off = (long long)nb[0] * C::BS + ((jg & ~1) * P + N + 2 * (jg & 1) + i);
-    if (i >= N - NG && nb[1] >= 0) px_off = (long long)nb[1] * C::BS + ((jg | 1) * P + N + 2 * (jg & 1) + (i - (N - NG)));
-    if (jg < NG && nb[2] >= 0) py_off = (long long)nb[2] * C::BS + ((N + jg) * P + i);
-    if (jg >= N - NG && nb[3] >= 0) py_off = (long long)nb[3] * C::BS + ((jg + 2 * NG) * P + i);
+    if (i < NG && nb[0] >= 0) ppx = p.out + (size_t)nb[0] * C::BS + ((jg & ~1) * P + N + 2 * (jg & 1) + i);
+    if (i >= N - NG && nb[1] >= 0) ppx = p.out + (size_t)nb[1] * C::BS + ((jg | 1) * P + N + 2 * (jg & 1) + (i - (N - NG)));
+    if (jg < NG && nb[2] >= 0) ppy = p.out + (size_t)nb[2] * C::BS + ((N + jg) * P + i);
+    if (jg >= N - NG && nb[3] >= 0) ppy = p.out + (size_t)nb[3] * C::BS + ((jg + 2 * NG) * P + i);
     if (DIM == 3) { nbz0 = nb[4]; nbz1 = nb[5]; }
   }
   auto load_prev = [&](int k, double (&a)[5], double (&b)[5]) {
-    const size_t o = cell0 + (size_t)(DIM == 3 ? k : 0) * P * P;
+    const int ko = (DIM == 3 ? k : 0) * PP;
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
       if (DIM == 2 && q == 3) { a[q] = 0.0; b[q] = 0.0; continue; }
-      a[q] = p.prev0[o + pl(q) * C::VS];
-      b[q] = p.prev1 ? p.prev1[o + pl(q) * C::VS] : 0.0;
+      a[q] = pa[ko + pl(q) * (int)C::VS];
+      b[q] = pb ? pb[ko + pl(q) * (int)C::VS] : 0.0;
     }
   };
   auto finish = [&](int k, const double (&tot)[5], const double (&a)[5], const double (&b)[5]) {
-    if (!active) return;
-    const size_t o = cell0 + (size_t)(DIM == 3 ? k : 0) * P * P;
+    const int ko = (DIM == 3 ? k : 0) * PP;
     double u[5];
-    const double s = p.dt_sub * inv_dx;
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
       if (DIM == 2 && q == 3) { u[q] = 0.0; continue; }
-      u[q] = fma(s, tot[q], fma(p.w1, b[q], p.w0 * a[q]));
-      p.out[o + pl(q) * C::VS] = u[q];
+      u[q] = fma(sdt, tot[q], fma(p.w1, b[q], p.w0 * a[q]));
+      po[ko + pl(q) * (int)C::VS] = u[q];
     }
-    const size_t kof = (size_t)(DIM == 3 ? k : 0) * P * P;
-    if (px_off >= 0) {
+    if (ppx) {
 #pragma unroll
-      for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) p.out[px_off + kof + pl(q) * C::VS] = u[q];
+      for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) ppx[ko + pl(q) * (int)C::VS] = u[q];
     }
-    if (py_off >= 0) {
+    if (ppy) {
 #pragma unroll
-      for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) p.out[py_off + kof + pl(q) * C::VS] = u[q];
+      for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) ppy[ko + pl(q) * (int)C::VS] = u[q];
     }
-    if (DIM == 3) {
-      const int nbz = (k < NG) ? nbz0 : (k >= N - NG ? nbz1 : -1);
+    if (DIM == 3 && (k < NG || k >= N - NG)) {
+      const int nbz = (k < NG) ? nbz0 : nbz1;
       if (nbz >= 0) {
-        const size_t zo = (size_t)nbz * C::BS + (size_t)(k < NG ? N + k : k + 2 * NG) * P * P + (size_t)(j0 + j) * P + i;
+        double* pz = p.out + (size_t)nbz * C::BS + (size_t)(k < NG ? N + k : k + 2 * NG) * PP + co;
 #pragma unroll
-        for (int q = 0; q < 5; ++q) p.out[zo + pl(q) * C::VS] = u[q];
+        for (int q = 0; q < 5; ++q) pz[pl(q) * (int)C::VS] = u[q];
       }
     }
     if (p.maxrate) {
@@ -404,28 +464,23 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
       }
       const double pr = gm1 * fma(-0.5 * u[0], ke, u[4]);
       const double c2 = gamma * pr * ir;
-      rate_max = fmax(rate_max, fma((double)DIM, c2 * rsqrt_fast(c2), su) * inv_dx);
+      rate_max = fmax(rate_max, fma((double)DIM, c2 * rsqrt_fast(c2), su));
     }
   };
   auto convert_halo = [&](double* W) {
-    if (t < C::HALO) {
-      int row, col;
-      if (t < 4 * TY) { row = 2 + t / 4; col = N + (t % 4); }
-      else { const int tq = t - 4 * TY, r4 = tq / N; row = r4 < 2 ? r4 : TY + r4; col = tq % N; }
+    if (hc_o >= 0) {
       double tmp[5];
-      convert(W, row * P + col, tmp);
+      convert(W, hc_o, tmp);
     }
   };
 
   if (DIM == 2) {
     double a[5], b[5], w[5], acc[5];
-    if (t == 0 && active) issue_plane(0);
-    if (active) {
-      load_prev(0, a, b);
-      mbar_wait(&bars[0], 0);
-      convert(ring, own, w);
-      convert_halo(ring);
-    }
+    if (t == 0) issue_plane(0, 0);
+    load_prev(0, a, b);
+    mbar_wait(bars_u32, 0);
+    convert(ring, own, w);
+    convert_halo(ring);
     group_sync(bar_id, TG);
     sweep_xy(ring, 0, acc);
     finish(0, acc, a, b);
@@ -433,26 +488,24 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
     double dA[5], Lz[5], accp[5];
 #pragma unroll
     for (int q = 0; q < 5; ++q) { dA[q] = 0.0; Lz[q] = 1.0; accp[q] = 0.0; }
-    if (t == 0 && active) { issue_plane(-2); issue_plane(-1); }
+    if (t == 0) { issue_plane(-2, 0); issue_plane(-1, 1); }
+    int sc = 0;            // ring slot of plane c (planes take the slots 0,1,2,0,...)
+    uint32_t ph = 0;       // phase parity of each slot's mbarrier
     // one march iteration; the steady state (c in [2, N]) is the instance with every flag true
     auto march = [&](int c, auto zslope_t, auto zflux_t, auto fin_t, auto sweep_t) {
       constexpr bool ZSLOPE = decltype(zslope_t)::value, ZFLUX = decltype(zflux_t)::value;
       constexpr bool FIN = decltype(fin_t)::value, SWEEP = decltype(sweep_t)::value;
-      const int idx = c + 2, s = idx % 3;
-      double* Wc = ring + s * C::SLOT;                      // plane c
-      const double* Wk = ring + ((idx + 2) % 3) * C::SLOT;  // plane c-1
-      double pa[5], pb[5];
-      if (FIN && active) load_prev(c - 2, pa, pb);          // consumed after the z flux: latency hidden
+      const int sk = (sc == 0) ? 2 : sc - 1;                // slot of plane c-1
+      double* Wc = ring + sc * C::SLOT;
+      const double* Wk = ring + sk * C::SLOT;
+      double pa5[5], pb5[5];
+      if (FIN) load_prev(c - 2, pa5, pb5);                  // consumed after the z flux: latency hidden
       double wB[5];
-      if (active) {
-        mbar_wait(&bars[s], (idx / 3) & 1);
-        convert(Wc, own, wB);
-        if (c >= 0 && c < N) convert_halo(Wc);
-        fence_proxy_async();   // generic-proxy writes before the async-proxy refill of this slot
-      } else {
-#pragma unroll
-        for (int q = 0; q < 5; ++q) wB[q] = 1.0;
-      }
+      mbar_wait(bars_u32 + 8u * sc, (ph >> sc) & 1u);
+      ph ^= 1u << sc;
+      convert(Wc, own, wB);
+      if (c >= 0 && c < N) convert_halo(Wc);
+      fence_proxy_async();   // generic-proxy writes before the async-proxy refill of this slot
       // ---- z direction along the march: slope of cell c-1 from w(c-2), w(c-1), w(c);
       //      flux at the face between cells c-2 and c-1 (normal frame (rho, w, u, v, p))
       double Fz[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
@@ -480,7 +533,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
         double tot[5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) tot[q] = accp[q] - Fz[q];
-        finish(c - 2, tot, pa, pb);
+        finish(c - 2, tot, pa5, pb5);
       }
       if (SWEEP) {
         double acc[5];
@@ -491,7 +544,8 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
         group_sync(bar_id, TG);
       }
       // every thread is past its last read of plane c-1: refill that slot with plane c+2
-      if (t == 0 && active && c + 2 <= N + 1) issue_plane(c + 2);
+      if (t == 0 && c + 2 <= N + 1) issue_plane(c + 2, sk);
+      sc = (sc == 2) ? 0 : sc + 1;
     };
     using T = std::true_type;
     using F_ = std::false_type;
@@ -505,6 +559,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
   }
 
   if (p.maxrate) {
+    rate_max *= p.inv_dx_l[lvl];   // max over cells of sum_d (|u_d| + c), scaled by 1/dx (> 0) once
     for (int sft = 16; sft > 0; sft >>= 1) rate_max = fmax(rate_max, __shfl_xor_sync(0xffffffffu, rate_max, sft));
     if ((threadIdx.x & 31) == 0 && rate_max > 0.0)
       atomicMax(p.maxrate, (unsigned long long)__double_as_longlong(rate_max));

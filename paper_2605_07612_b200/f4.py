@@ -45,8 +45,10 @@ def lib():
     global _lib
     if _lib is not None:
         return _lib
-    path = _build.LIB
+    path = os.environ.get("F4_LIB") or _build.LIB   # F4_LIB: load another build of the same library
     if not os.path.exists(path):
+        if path != _build.LIB:
+            raise FileNotFoundError(path)
         path = _build.build()
     L = C.CDLL(path)
     vp, ip, dp = C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_double)
