@@ -131,6 +131,40 @@ def oracle_sample(cfg, target_updates=1.2e7):
     return cells * 2.0 * steps / el / 1e9, 1, desc, el, steps
 
 
+def pattern_bytes(mesh, n, d):
+    """Algorithmic bytes (read, written) of one full execution of the ghost pattern, from its records
+    (SURVEY.md 8(a) rows a1-a4): SRL/BC copy Ng*N^(d-1)*Nvar doubles; an F2C record writes a
+    1/2^(d-1) share of a coarse face and reads 2^d fine cells per ghost; a C2F record writes a fine face and
+    reads the (Ng/2+2) x (N/2+2)^(d-1) coarse cells of its slope stencils."""
+    rec, n1, n2 = mesh.pattern()
+    nvar, ng = d + 2, 2
+    face = ng * n ** (d - 1) * nvar * 8
+    ops = rec[:, 0]
+    n_copy = int(np.sum((ops == 0) | (ops == 1)))
+    n_f2c = int(np.sum(ops == 2))
+    n_c2f = int(np.sum(ops == 3))
+    rd = n_copy * face + n_f2c * face * 2 + n_c2f * (ng // 2 + 2) * (n // 2 + 2) ** (d - 1) * nvar * 8
+    wr = n_copy * face + n_f2c * face // 2 ** (d - 1) + n_c2f * face
+    return rd, wr, {"srl_bc": n_copy, "f2c": n_f2c, "c2f": n_c2f}
+
+
+def adaptive_flags(cfg, mesh):
+    """Reading A15 (harness side): pressure-jump flags from the ghost-filled state 0."""
+    mesh.fill_ghosts(0)
+    return W.pressure_jump_flags(cfg, mesh.get_state(0, with_ghosts=True))
+
+
+def adaptive_initial_mesh(cfg, mesh):
+    """{set analytic state, fill ghosts, flag, adapt} up to (max_level - base_level) times, then the analytic state."""
+    for _ in range(cfg["max_level"] - cfg["base_level"]):
+        lev, co = mesh.get_blocks()
+        mesh.set_state(0, W.initial_state(cfg, lev, co))
+        if not mesh.adapt(adaptive_flags(cfg, mesh)):
+            break
+    lev, co = mesh.get_blocks()
+    mesh.set_state(0, W.initial_state(cfg, lev, co))
+
+
 def run_reference(args, cfg, rank):
     """--impl reference: this tier's reference arm is the CPU oracle on the host cores (rank 0 only)."""
     if rank != 0:
@@ -203,26 +237,41 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    mesh = f4.Mesh.from_config(cfg, max_blocks=None if cfg["max_level"] == cfg["base_level"] else 6000)
+    adaptive = cfg["max_level"] > cfg["base_level"]
+    mesh = f4.Mesh.from_config(cfg, max_blocks=None if not adaptive else 12000)
     stream = torch.cuda.Stream(dev)
     mesh.bind_torch(dev, stream)
-    lev, co = mesh.get_blocks()
-    nb, n, d = len(lev), cfg["block_n"], cfg["dim"]
-    cells = nb * n ** d
-    host = torch.empty(mesh._shape(False), dtype=torch.float64).pin_memory()
-    host_np = host.numpy()
-    fill_initial_state(cfg, lev, co, host_np)
-    mesh.set_state(0, host_np)
+    n, d = cfg["block_n"], cfg["dim"]
+    if adaptive:
+        adaptive_initial_mesh(cfg, mesh)
+        host = host_np = None
+    else:
+        lev, co = mesh.get_blocks()
+        host = torch.empty(mesh._shape(False), dtype=torch.float64).pin_memory()
+        host_np = host.numpy()
+        fill_initial_state(cfg, lev, co, host_np)
+        mesh.set_state(0, host_np)
+
+    counters = {"step": 0, "updates": 0.0, "adapt_s": 0.0, "regrids": 0, "changed": 0}
 
     def step():
+        # config 5: regrid on the host every cfg["regrid_every"] steps (rule A15), inside the timed region
+        if adaptive and counters["step"] and counters["step"] % cfg["regrid_every"] == 0:
+            t0 = time.perf_counter()
+            counters["changed"] += int(mesh.adapt(adaptive_flags(cfg, mesh)))
+            counters["regrids"] += 1
+            counters["adapt_s"] += time.perf_counter() - t0
         dt = mesh.compute_dt(0, cfg["cfl"])
         mesh.advance(dt)
+        counters["step"] += 1
+        counters["updates"] += 2.0 * mesh.num_blocks * n ** d
 
     for _ in range(max(args.warmup, 0)):
         step()
     mesh.profile_get(reset=True)
     mesh.profile_enable(True)
     l0 = mesh.launch_count()
+    counters.update(updates=0.0, adapt_s=0.0, regrids=0, changed=0)
     sampler = ClockSampler(local_rank)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
@@ -237,15 +286,37 @@ def main():
     launches = mesh.launch_count() - l0
     prof = mesh.profile_get(reset=True)
     mesh.profile_enable(False)
+    updates = counters["updates"]
+    adapt_info = dict(counters)
     totals_after = mesh.conserved_totals(0)
     if dist is not None:
         t = torch.tensor([ms], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t.item())
-    value = world * cells * 2.0 * args.steps / (ms * 1e-3) / 1e9
+    value = world * updates / (ms * 1e-3) / 1e9
+    nb = mesh.num_blocks
+    cells = nb * n ** d
+
+    # ---- ghost-fill GB/s: the whole pattern (SRL included) executed standalone by f4_fill_ghosts, outside the step
+    rd_b, wr_b, rec_counts = pattern_bytes(mesh, n, d)
+    mesh.fill_ghosts(0)
+    mesh.profile_get(reset=True)
+    mesh.profile_enable(True)
+    NFILL = 5
+    for _ in range(NFILL):
+        mesh.fill_ghosts(0)
+    gprof = mesh.profile_get(reset=True)
+    mesh.profile_enable(False)
+    fill_ms = (gprof["ghost_r1"][0] + gprof["ghost_r2"][0]) / NFILL
 
     # ---- end to end through the C-ABI with HOST buffers: H2D of the state, the step, D2H of the result metric
-    fill_initial_state(cfg, lev, co, host_np)
+    if adaptive:
+        host = torch.empty(mesh._shape(False), dtype=torch.float64).pin_memory()
+        host_np = host.numpy()
+        mesh.get_state(0, out=host_np)
+        counters["step"] = 1                 # no regrid inside the end-to-end loop
+    else:
+        fill_initial_state(cfg, lev, co, host_np)
     e2e_steps = max(1, args.e2e_steps)
     mesh.set_state(0, host_np)
     step()
@@ -254,6 +325,8 @@ def main():
     ev2.record(stream)
     for _ in range(e2e_steps):
         mesh.set_state(0, host_np)          # pinned host -> device staging -> store
+        if adaptive:
+            counters["step"] = 1
         step()
         tot = mesh.conserved_totals(0)      # device -> host: per-block sums + dt
     ev3.record(stream)
@@ -276,13 +349,13 @@ def main():
     # stage kernel, so on a uniform mesh there is no separate ghost-fill traffic.
     r = 1.0 + 2.0 * d * 2 / n
     bpc = 8 * (d + 2)
-    stage_bytes = cells * (2.0 * bpc * r + 0.5 * bpc)
-    ghost_bytes = cells * 2 * bpc * (r - 1.0)            # what a separate fill pass would move (read + write)
     st_ms, st_n = prof["stage"]
+    cells_per_launch = updates / max(st_n, 1)            # = cells on a static mesh; the average on an adaptive one
+    stage_bytes = cells_per_launch * (2.0 * bpc * r + 0.5 * bpc)
     g_n = prof["ghost_r1"][1] + prof["ghost_r2"][1]
     g_ms = prof["ghost_r1"][0] + prof["ghost_r2"][0]
     stage_gbs = stage_bytes / (st_ms / max(st_n, 1) * 1e-3) / 1e9 if st_ms > 0 else None
-    ghost_gbs = (ghost_bytes / (g_ms / max(prof["ghost_r1"][1], 1) * 1e-3) / 1e9) if g_ms > 0 else None
+    ghost_gbs = ((rd_b + wr_b) / (fill_ms * 1e-3) / 1e9) if fill_ms > 0 else None
     traffic = None
     tp = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tp):
@@ -304,11 +377,18 @@ def main():
                      "kernel": "stage_kernel", "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": stage_bytes, "avg_launch_ms": st_ms / max(st_n, 1)},
         "ghost_fill": {"GBps": ghost_gbs, "frac_of_hbm_peak": (ghost_gbs / peak) if ghost_gbs else None,
-                       "executor_launches": int(g_n), "executor_ms_per_step": g_ms / args.steps,
-                       "note": "same-level copies are pushed by the stage kernel; the executor runs only BC/F2C/C2F "
-                               "records inside advance (none on a uniform periodic mesh)"},
+                       "ms_per_fill": fill_ms, "bytes_read": int(rd_b), "bytes_written": int(wr_b),
+                       "records": rec_counts, "launches_per_fill": (gprof["ghost_r1"][1] + gprof["ghost_r2"][1]) // NFILL,
+                       "in_step_executor_launches": int(g_n), "in_step_executor_ms_per_step": g_ms / args.steps,
+                       "note": "GBps: f4_fill_ghosts (whole pattern, SRL included) timed standalone after the step "
+                               "loop; inside advance the same-level copies are pushed by the stage kernel and the "
+                               "executor runs only BC/F2C/C2F records (none on a uniform periodic mesh)"},
         "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()},
         "step_algorithmic_GBps": (2 * stage_bytes) / (ms / args.steps * 1e-3) / 1e9,
+        "adaptive": ({"regrids": adapt_info["regrids"], "mesh_changed": adapt_info["changed"],
+                      "adapt_ms_total": 1e3 * adapt_info["adapt_s"], "blocks_at_end": nb,
+                      "value_excluding_adapt": world * updates / max(ms * 1e-3 - adapt_info["adapt_s"], 1e-9) / 1e9}
+                     if adaptive else None),
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         "totals": [float(x) for x in totals_after],
     }

@@ -185,7 +185,7 @@ struct Cfg {  // FAST (van Leer + HLL fixed at compile time) does not change the
   static constexpr int GROUP_DOUBLES = NSLOT * SLOT + 2 * EXBUF * EX + NVAR * NH;
   static constexpr size_t SMEM = (size_t)G * GROUP_DOUBLES * 8 + (size_t)G * NSLOT * 8;
   static constexpr int HALO = 4 * TY + 4 * N;  // halo cells of an interior plane
-  static_assert(HALO <= TG && 2 * NH <= TG, "halo work needs one pass");
+  static_assert(HALO <= TG && 3 * NH <= TG, "halo work needs one pass");
   static_assert(TG % 32 == 0 && N % TY == 0 && GROUP_DOUBLES % 2 == 0, "tile shape");
 };
 
@@ -318,6 +318,12 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT,
     h_op = rown(y + 1) * P + col;
     h_f = (is_hi ? TY : 0) * N + col;
   }
+  // the flux at the last face of each row / column is taken by a third set of threads [2NH,3NH) (another warp than
+  // the halo slopes: the passes between two barriers stay balanced across warps)
+  const bool is_hf = (t >= 2 * NH) && (t < 3 * NH);
+  const int fq = t - 2 * NH;
+  const bool f_isx = fq < TY;
+  const int f_f = f_isx ? fq * (N + 1) + N : TY * N + (fq - TY);
   // halo cell converted by this thread on interior planes
   int hc_o = -1;
   if (t < C::HALO) {
@@ -372,20 +378,20 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT,
       Fy[0] = F[0]; Fy[1] = F[2]; Fy[2] = F[1]; Fy[3] = F[3]; Fy[4] = F[4];
 #pragma unroll
       for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eY[pl(q) * EXV + fy] = Fy[q];
-      if (is_hi) {
-        double* e = h_isx ? eX : eY;
+      if (is_hf) {
+        double* e = f_isx ? eX : eY;
         double Rr[5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
-          L[q] = (DIM == 2 && q == 3) ? 0.0 : e[pl(q) * EXV + h_f];
-          Rr[q] = (DIM == 2 && q == 3) ? 0.0 : sRh[pl(q) * NH + hq];
+          L[q] = (DIM == 2 && q == 3) ? 0.0 : e[pl(q) * EXV + f_f];
+          Rr[q] = (DIM == 2 && q == 3) ? 0.0 : sRh[pl(q) * NH + fq];
         }
-        const double Ln[5] = {L[0], h_isx ? L[1] : L[2], h_isx ? L[2] : L[1], L[3], L[4]};
-        const double Rn[5] = {Rr[0], h_isx ? Rr[1] : Rr[2], h_isx ? Rr[2] : Rr[1], Rr[3], Rr[4]};
+        const double Ln[5] = {L[0], f_isx ? L[1] : L[2], f_isx ? L[2] : L[1], L[3], L[4]};
+        const double Rn[5] = {Rr[0], f_isx ? Rr[1] : Rr[2], f_isx ? Rr[2] : Rr[1], Rr[3], Rr[4]};
         riemann_flux<DIM, FAST>(Ln, Rn, gamma, ig1, fluxs, F);
-        const double Fp[5] = {F[0], h_isx ? F[1] : F[2], h_isx ? F[2] : F[1], F[3], F[4]};
+        const double Fp[5] = {F[0], f_isx ? F[1] : F[2], f_isx ? F[2] : F[1], F[3], F[4]};
 #pragma unroll
-        for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) e[pl(q) * EXV + h_f] = Fp[q];
+        for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) e[pl(q) * EXV + f_f] = Fp[q];
       }
     }
     group_sync(bar_id, TG);
