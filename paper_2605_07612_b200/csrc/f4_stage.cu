@@ -90,8 +90,14 @@ __device__ __forceinline__ double half_slope(double a, double b, int limiter) {
   if (FAST) {
     // van Leer: 1/2 * 2ab/(a+b) where ab > 0.  The sign test is taken on the high word of ab (an integer compare
     // instead of a DSETP on the fp64 pipe); it differs from ab > 0 only for 0 < ab < 2^-1042, where the slope is < 1e-150.
-    double r = ab * rcp_fast(a + b);
-    return (__double2hiint(ab) > 0) ? r : 0.0;
+    // the select is taken on the MUFU seed (one 32-bit select: the seed's low word is zero): seed 0 -> rcp 0 -> slope 0
+    const double x = a + b;
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    y = __hiloint2double((__double2hiint(ab) > 0) ? __double2hiint(y) : 0, 0);
+    const double e = fma(-x, y, 1.0);
+    const double e2 = fma(e, e, e);
+    return ab * fma(y, e2, y);
   }
   double r;
   if (limiter == F4_LIM_VANLEER) {
@@ -118,23 +124,21 @@ __device__ __forceinline__ void riemann_flux(const double (&L)[5], const double 
   // d^2 = (rL cL^2 + rR cR^2)/(rL+rR) + 1/2 rL rR/(rL+rR)^2 du^2,  r c^2 = gamma p / sqrt(rho)
   const double d2 = fma((0.5 * wl) * wr, du * du, fma(L[4], yL, R[4] * yR) * (gamma * w));
   const double y2 = rsqrt_fast(d2);
-  const double dhat = d2 * y2;
-  double sm = uhat - dhat, sp = uhat + dhat;
   // F = a FL + b FR + c (UR - UL) with a = S+/(S+ - S-), b = -S-/(S+ - S-), c = S+ S-/(S+ - S-)
   double a, b, c;
   if (FAST) {
-    // HLL: S- = min(sm,0), S+ = max(sp,0).  Subsonic: S+ - S- = 2 d^, so 1/(S+ - S-) = y2/2 (no second reciprocal);
-    // supersonic: (a,b,c) = (1,0,0) or (0,1,0) exactly.  Sign bits instead of fp64 compares.
-    const double inv = 0.5 * y2;
-    const bool right = __double2hiint(sm) >= 0, left = __double2hiint(sp) < 0;
-    sm = right ? 0.0 : sm;
-    sp = left ? 0.0 : sp;
-    a = sp * inv;
-    b = -sm * inv;
-    a = right ? 1.0 : a;
-    b = left ? 1.0 : b;
-    c = a * sm;
+    // HLL: S- = min(u^ - d^, 0), S+ = max(u^ + d^, 0).  Subsonic: S+ - S- = 2 d^ and 1/(2 d^) = y2/2 (no second
+    // reciprocal), so a = 1/2 + u^/(2 d^); supersonic: (a,b,c) = (1,0,0) or (0,1,0).  Both cases:
+    //   a = clamp(1/2 + u^ y2/2, 0, 1), b = 1 - a, c = -a b (2 d^);  the clamp is taken on the high word (no fp64 compare)
+    const double a0 = fma(uhat, 0.5 * y2, 0.5);
+    const int ah = __double2hiint(a0);
+    const bool neg = ah < 0, big = ah >= 0x3FF00000;
+    a = __hiloint2double(neg ? 0 : (big ? 0x3FF00000 : ah), (neg || big) ? 0 : __double2loint(a0));
+    b = 1.0 - a;
+    c = (a * b) * (d2 * (-2.0 * y2));
   } else {
+    const double dhat = d2 * y2;
+    double sm = uhat - dhat, sp = uhat + dhat;
     if (flux == F4_FLUX_RUSANOV) {
       double s = fmax(fabs(sm), fabs(sp));
       sm = -s;
@@ -326,10 +330,11 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT,
   const int f_f = f_isx ? fq * (N + 1) + N : TY * N + (fq - TY);
   // halo cell converted by this thread on interior planes
   int hc_o = -1;
-  if (t < C::HALO) {
-    if (t < 4 * TY) hc_o = rown(j0 + t / 4) * P + N + (t % 4);
+  const int th = t - (TG - C::HALO);   // the last HALO threads: other warps than the halo slopes / fluxes
+  if (th >= 0 && th < C::HALO) {
+    if (th < 4 * TY) hc_o = rown(j0 + th / 4) * P + N + (th % 4);
     else {
-      const int tq = t - 4 * TY, r4 = tq / N;
+      const int tq = th - 4 * TY, r4 = tq / N;
       hc_o = rown(r4 < 2 ? j0 - 2 + r4 : j0 + TY + r4 - 2) * P + tq % N;
     }
   }
@@ -506,6 +511,11 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT,
       const double* Wk = ring + sk * C::SLOT;
       double pa5[5], pb5[5];
       if (FIN) load_prev(c - 2, pa5, pb5);                  // consumed after the z flux: latency hidden
+      if (FIN && pb && c - 1 < N && (i & 3) == 0) {         // stage 2: u_t of the next plane comes from DRAM: pull it into L2 now
+#pragma unroll
+        for (int q = 0; q < 5; ++q)
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(pa + (c - 1) * PP + pl(q) * (int)C::VS));
+      }
       double wB[5];
       mbar_wait(bars_u32 + 8u * sc, (ph >> sc) & 1u);
       ph ^= 1u << sc;
