@@ -88,62 +88,34 @@ __device__ __forceinline__ double child_value(double uc, double sx, double sy, d
 // ---------------------------------------------------------------------------
 // ghost executor
 // ---------------------------------------------------------------------------
+// Offsets, inside one (block, var) box, of the r-th 16-byte unit of a same-level / outflow face copy:
+// so = source doubles (a pair, or one double replicated for an outflow x face), d_o = destination pair.
 template <int DIM, int N>
-__device__ __forceinline__ void do_copy_face(double* __restrict__ st, int dst, int src, int face, bool outflow) {
+__device__ __forceinline__ void copy_unit(int face, bool outflow, int r, int& so, int& d_o) {
   using G = Geo<DIM, N>;
-  constexpr int P = G::P, NV = G::NVAR;
+  constexpr int P = G::P;
   const int a = face >> 1, side = face & 1;
   // destination ghost slots along the normal: low ghosts P-2,P-1 (cells -2,-1); high ghosts N,N+1
   const int dn = side ? N : P - 2;
   // source slots: SRL -x: neighbour's cells N-2,N-1; +x: cells 0,1.  Outflow: nearest own interior layer.
   const int sn = outflow ? (side ? N - 1 : 0) : (side ? 0 : N - 2);
-  const int sq = outflow ? 0 : 1;  // source advances with the layer only for SRL
-  double* db = st + (size_t)dst * G::BS;
-  const double* sb = st + (size_t)src * G::BS;
-  constexpr int PER_VAR = (DIM == 3) ? N * N : N;  // 16-byte units per variable
-  constexpr int TOTAL = NV * PER_VAR;
-  constexpr int UNR = 5;
-  for (int e0 = threadIdx.x; e0 < TOTAL; e0 += UNR * blockDim.x) {
-    double2 val[UNR];
-    int doff[UNR];
-#pragma unroll
-    for (int u = 0; u < UNR; ++u) {
-      int e = e0 + u * blockDim.x;
-      doff[u] = -1;
-      if (e < TOTAL) {
-        int v = e / PER_VAR, r = e % PER_VAR;
-        int so, d_o;
-        if (a == 0) {  // one row = one 16-byte ghost pair
-          int j = r % N, k = (DIM == 3) ? r / N : 0;
-          int pl0 = (DIM == 3 ? k * P * P : 0);
-          d_o = pl0 + (side ? (j & ~1) : (j | 1)) * P + N + 2 * (j & 1);   // pair-transposed x ghosts (cell_off)
-          so = pl0 + j * P + sn;
-          if (outflow) {
-            double x = sb[(size_t)v * G::VS + so];
-            val[u] = make_double2(x, x);
-          } else {
-            val[u] = ld2(sb + (size_t)v * G::VS + so);
-          }
-        } else {
-          int h, q, t;
-          if (DIM == 3) {
-            if (a == 1) { t = r / N; q = (r % N) / G::H; h = r % G::H; }   // t = k
-            else        { q = r / (N * G::H); t = (r / G::H) % N; h = r % G::H; }  // t = j
-          } else { q = r / G::H; h = r % G::H; t = 0; }
-          int dl = dn + q, sl = sn + sq * q;
-          if (DIM == 3) {
-            if (a == 1) { d_o = t * P * P + dl * P + 2 * h; so = t * P * P + sl * P + 2 * h; }
-            else        { d_o = dl * P * P + t * P + 2 * h; so = sl * P * P + t * P + 2 * h; }
-          } else { d_o = dl * P + 2 * h; so = sl * P + 2 * h; }
-          val[u] = ld2(sb + (size_t)v * G::VS + so);
-        }
-        doff[u] = v * (int)G::VS + d_o;
-      }
-    }
-#pragma unroll
-    for (int u = 0; u < UNR; ++u)
-      if (doff[u] >= 0) st2(db + doff[u], val[u]);
+  if (a == 0) {  // one row = one 16-byte ghost pair
+    const int j = r % N, k = (DIM == 3) ? r / N : 0;
+    const int pl0 = (DIM == 3 ? k * P * P : 0);
+    d_o = pl0 + (side ? (j & ~1) : (j | 1)) * P + N + 2 * (j & 1);   // pair-transposed x ghosts (cell_off)
+    so = pl0 + j * P + sn;
+    return;
   }
+  int h, q, t;
+  if (DIM == 3) {
+    if (a == 1) { t = r / N; q = (r % N) / G::H; h = r % G::H; }               // t = k
+    else        { q = r / (N * G::H); t = (r / G::H) % N; h = r % G::H; }      // t = j
+  } else { q = r / G::H; h = r % G::H; t = 0; }
+  const int dl = dn + q, sl = outflow ? sn : sn + q;   // the source advances with the layer only for SRL
+  if (DIM == 3) {
+    if (a == 1) { d_o = t * P * P + dl * P + 2 * h; so = t * P * P + sl * P + 2 * h; }
+    else        { d_o = dl * P * P + t * P + 2 * h; so = sl * P * P + t * P + 2 * h; }
+  } else { d_o = dl * P + 2 * h; so = sl * P + 2 * h; }
 }
 
 template <int DIM, int N>
@@ -206,19 +178,56 @@ __device__ __forceinline__ void do_c2f(double* __restrict__ st, int dst, int src
 }
 
 template <int DIM, int N>
-__global__ void __launch_bounds__(256) ghost_exec_kernel(GhostParams p) {
-  constexpr int CH = 2 * DIM;
-  int r0 = blockIdx.x * CH;
+__global__ void __launch_bounds__(256, 4) ghost_exec_kernel(GhostParams p) {
+  using G = Geo<DIM, N>;
+  constexpr int CH = 2 * DIM, NV = G::NVAR;
+  constexpr int PER_VAR = (DIM == 3) ? N * N : N;   // 16-byte units per variable of one face copy
+  __shared__ DevRecord recs[CH];
+  const int r0 = blockIdx.x * CH;
+  const int n = (p.nrec - r0 < CH) ? p.nrec - r0 : CH;
+  if ((int)threadIdx.x < n) recs[threadIdx.x] = p.rec[r0 + threadIdx.x];
+  __syncthreads();
+  // ---- same-level and outflow copies of all records of this CTA, flattened over (record, unit); every thread
+  //      has the loads of two units (2 x NV x 16 bytes) in flight before it stores
+  constexpr int UNR = 2;
+  for (int e0 = threadIdx.x; e0 < n * PER_VAR; e0 += UNR * blockDim.x) {
+    double2 val[UNR][NV];
+    double* dptr[UNR];
+#pragma unroll
+    for (int u = 0; u < UNR; ++u) {
+      const int e = e0 + u * blockDim.x;
+      dptr[u] = nullptr;
+      if (e >= n * PER_VAR) continue;
+      const DevRecord rec = recs[e / PER_VAR];
+      const int op = rec.meta & 3, face = (rec.meta >> 2) & 7;
+      if (op > F4_OP_BC) continue;
+      const bool outflow = (op == F4_OP_BC);
+      int so, d_o;
+      copy_unit<DIM, N>(face, outflow, e % PER_VAR, so, d_o);
+      const double* sp = p.state + (size_t)rec.src * G::BS + so;
+      dptr[u] = p.state + (size_t)rec.dst * G::BS + d_o;
+      if (outflow && face < 2) {
+#pragma unroll
+        for (int v = 0; v < NV; ++v) { const double x = sp[(size_t)v * G::VS]; val[u][v] = make_double2(x, x); }
+      } else {
+#pragma unroll
+        for (int v = 0; v < NV; ++v) val[u][v] = ld2(sp + (size_t)v * G::VS);
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < UNR; ++u)
+      if (dptr[u]) {
+#pragma unroll
+        for (int v = 0; v < NV; ++v) st2(dptr[u] + (size_t)v * G::VS, val[u][v]);
+      }
+  }
+  // ---- restriction / prolongation records
 #pragma unroll 1
-  for (int q = 0; q < CH; ++q) {
-    int r = r0 + q;
-    if (r >= p.nrec) break;
-    DevRecord rec = p.rec[r];
-    int op = rec.meta & 3, face = (rec.meta >> 2) & 7, o1 = (rec.meta >> 5) & 1, o2 = (rec.meta >> 6) & 1;
-    if (op == F4_OP_SRL) do_copy_face<DIM, N>(p.state, rec.dst, rec.src, face, false);
-    else if (op == F4_OP_BC) do_copy_face<DIM, N>(p.state, rec.dst, rec.src, face, true);
-    else if (op == F4_OP_F2C) do_f2c<DIM, N>(p.state, rec.dst, rec.src, face, o1, o2);
-    else do_c2f<DIM, N>(p.state, rec.dst, rec.src, face, o1, o2, p.theta);
+  for (int q = 0; q < n; ++q) {
+    const DevRecord rec = recs[q];
+    const int op = rec.meta & 3, face = (rec.meta >> 2) & 7, o1 = (rec.meta >> 5) & 1, o2 = (rec.meta >> 6) & 1;
+    if (op == F4_OP_F2C) do_f2c<DIM, N>(p.state, rec.dst, rec.src, face, o1, o2);
+    else if (op == F4_OP_C2F) do_c2f<DIM, N>(p.state, rec.dst, rec.src, face, o1, o2, p.theta);
   }
 }
 
