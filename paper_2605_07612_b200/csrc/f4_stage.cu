@@ -167,7 +167,74 @@ __device__ __forceinline__ void riemann_flux(const double (&L)[5], const double 
   F[4] = fma(0.5 * aL, hL, fma(0.5 * aR, hR, fma(L[4], fma(bL, ig1, auL), R[4] * fma(bR, ig1, buR))));
 }
 
-template <int DIM, int N, int TY, int G, int EXBUF>
+// Two independent HLL fluxes (van Leer/HLL fast path) written step by step across both faces, so that the
+// rsqrt -> rcp -> rsqrt dependency chains of the two Riemann problems overlap (the kernel is bound by
+// dependent-issue latency, not by instruction count).  Same arithmetic as riemann_flux<DIM, true>.
+template <int DIM>
+__device__ __forceinline__ void riemann_flux2(const double (&L)[2][5], const double (&R)[2][5], double gamma,
+                                              double ig1, double (&F)[2][5]) {
+  double x[4] = {L[0][0], R[0][0], L[1][0], R[1][0]}, y[4];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y[q]) : "d"(x[q]));
+  {
+    double e[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) e[q] = fma(-(x[q] * y[q]), y[q], 1.0);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) y[q] = fma(y[q], fma(0.375, e[q], 0.5) * e[q], y[q]);   // 1/sqrt(rho)
+  }
+  double rL[2], rR[2], w[2], sum[2];
+#pragma unroll
+  for (int f = 0; f < 2; ++f) { rL[f] = x[2 * f] * y[2 * f]; rR[f] = x[2 * f + 1] * y[2 * f + 1]; sum[f] = rL[f] + rR[f]; }
+#pragma unroll
+  for (int f = 0; f < 2; ++f) asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(w[f]) : "d"(sum[f]));
+  {
+    double e[2];
+#pragma unroll
+    for (int f = 0; f < 2; ++f) e[f] = fma(-sum[f], w[f], 1.0);
+#pragma unroll
+    for (int f = 0; f < 2; ++f) w[f] = fma(w[f], fma(e[f], e[f], e[f]), w[f]);
+  }
+  double wl[2], wr[2], uhat[2], d2[2], y2[2];
+#pragma unroll
+  for (int f = 0; f < 2; ++f) {
+    wl[f] = rL[f] * w[f];
+    wr[f] = rR[f] * w[f];
+    uhat[f] = fma(wl[f], L[f][1], wr[f] * R[f][1]);
+    const double du = R[f][1] - L[f][1];
+    d2[f] = fma((0.5 * wl[f]) * wr[f], du * du, fma(L[f][4], y[2 * f], R[f][4] * y[2 * f + 1]) * (gamma * w[f]));
+  }
+#pragma unroll
+  for (int f = 0; f < 2; ++f) asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y2[f]) : "d"(d2[f]));
+  {
+    double e[2];
+#pragma unroll
+    for (int f = 0; f < 2; ++f) e[f] = fma(-(d2[f] * y2[f]), y2[f], 1.0);
+#pragma unroll
+    for (int f = 0; f < 2; ++f) y2[f] = fma(y2[f], fma(0.375, e[f], 0.5) * e[f], y2[f]);
+  }
+#pragma unroll
+  for (int f = 0; f < 2; ++f) {
+    const double a0 = fma(uhat[f], 0.5 * y2[f], 0.5);
+    const int ah = __double2hiint(a0);
+    const bool neg = ah < 0, big = ah >= 0x3FF00000;
+    const double a = __hiloint2double(neg ? 0 : (big ? 0x3FF00000 : ah), (neg || big) ? 0 : __double2loint(a0));
+    const double b = 1.0 - a;
+    const double c = (a * b) * (d2[f] * (-2.0 * y2[f]));
+    const double auL = a * L[f][1], buR = b * R[f][1];
+    const double bL = auL - c, bR = buR + c;
+    const double aL = L[f][0] * bL, aR = R[f][0] * bR;
+    double hL = fma(L[f][1], L[f][1], L[f][2] * L[f][2]), hR = fma(R[f][1], R[f][1], R[f][2] * R[f][2]);
+    if (DIM == 3) { hL = fma(L[f][3], L[f][3], hL); hR = fma(R[f][3], R[f][3], hR); }
+    F[f][0] = aL + aR;
+    F[f][1] = fma(aL, L[f][1], fma(aR, R[f][1], fma(a, L[f][4], b * R[f][4])));
+    F[f][2] = fma(aL, L[f][2], aR * R[f][2]);
+    F[f][3] = (DIM == 3) ? fma(aL, L[f][3], aR * R[f][3]) : 0.0;
+    F[f][4] = fma(0.5 * aL, hL, fma(0.5 * aR, hR, fma(L[f][4], fma(bL, ig1, auL), R[f][4] * fma(bR, ig1, buR))));
+  }
+}
+
+template <int DIM, int N, int TY, int G, int EXBUF, int HW = 0>
 struct Cfg {  // FAST (van Leer + HLL fixed at compile time) does not change the geometry
   static constexpr int P = N + 2 * NG;
   static constexpr int PZ = (DIM == 3) ? P : 1;
@@ -182,27 +249,30 @@ struct Cfg {  // FAST (van Leer + HLL fixed at compile time) does not change the
   static constexpr int EXV = (N + 1) * (TY + 1);  // exchange entries per variable
   static constexpr int EX = NVAR * EXV;
   static constexpr int NH = TY + N;           // halo cells per side (x rows + y columns)
-  static constexpr int TG = N * TY;           // threads per group
-  static constexpr int NT = TG * G;
+  static constexpr int TG = N * TY;           // cell threads per group
+  static constexpr int TGA = TG + 32 * HW;    // + HW helper warps (halo conversion, halo slopes, last-face fluxes, TMA issue)
+  static constexpr int NT = TGA * G;
   static constexpr int YT = N / TY;           // y tiles per block
   // ring | exX[EXBUF] | exY[EXBUF] | right states of the high halo cells [NVAR][NH]
   static constexpr int GROUP_DOUBLES = NSLOT * SLOT + 2 * EXBUF * EX + NVAR * NH;
   static constexpr size_t SMEM = (size_t)G * GROUP_DOUBLES * 8 + (size_t)G * NSLOT * 8;
   static constexpr int HALO = 4 * TY + 4 * N;  // halo cells of an interior plane
-  static_assert(HALO <= TG && 3 * NH <= TG, "halo work needs one pass");
+  static_assert(HW == 1 || (HALO <= TG && 3 * NH <= TG), "halo work needs one pass");
+  static_assert(HW == 0 || (HW == 1 && DIM == 3), "helper warp: 3D only");
   static_assert(TG % 32 == 0 && N % TY == 0 && GROUP_DOUBLES % 2 == 0, "tile shape");
 };
 
-template <int DIM, int N, int TY, int G, int EXBUF, bool FAST>
-__global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT,
-                                  F4_MINB((Cfg<DIM, N, TY, G, EXBUF>::SMEM <= 110 * 1024) ? 2 : 1))
+template <int DIM, int N, int TY, int G, int EXBUF, int HW, bool FAST>
+__global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
+                                  F4_MINB((Cfg<DIM, N, TY, G, EXBUF, HW>::SMEM <= 110 * 1024) ? 2 : 1))
     stage_kernel(const __grid_constant__ StageParams p) {
-  using C = Cfg<DIM, N, TY, G, EXBUF>;
+  using C = Cfg<DIM, N, TY, G, EXBUF, HW>;
   constexpr int P = C::P, PP = C::P * C::P, NV = C::NVAR, PLANE = C::PLANE, TG = C::TG, EXV = C::EXV, NH = C::NH;
+  constexpr int TGA = C::TGA;
   constexpr bool WHOLE = C::WHOLE;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  const int grp = (G == 1) ? 0 : (int)threadIdx.x / TG;
-  const int t = (G == 1) ? (int)threadIdx.x : (int)threadIdx.x % TG;
+  const int grp = (G == 1) ? 0 : (int)threadIdx.x / TGA;
+  const int t = (G == 1) ? (int)threadIdx.x : (int)threadIdx.x % TGA;
   const int item = blockIdx.x * G + grp;
   // a whole group leaves together: its named barrier and mbarriers are private to the group
   if (item >= p.nblocks * C::YT) return;
@@ -234,7 +304,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT,
     for (int s = 0; s < C::NSLOT; ++s) mbar_init(&bars[s], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  group_sync(bar_id, TG);
+  group_sync(bar_id, TGA);
 
   // issue the bulk copies of z plane c (c in [-2, N+2); 2D: c = 0) into ring slot s
   auto issue_plane = [&](int c, int s) {
@@ -303,41 +373,73 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT,
   const int own_xm = (i == 0) ? (rr | 1) * P + N + 2 * (rr & 1) + 1 : own - 1;
   const int own_xp = (i == N - 1) ? (rr & ~1) * P + N + 2 * (rr & 1) : own + 1;
   const int fx = j * (N + 1) + i, fy = j * N + i;      // own low faces in the exchange arrays
-  // halo roles: threads [0,NH) take the high halo cells (slope + last face flux), [NH,2NH) the low ones (slope)
-  const bool is_hi = t < NH, is_lo = (t >= NH) && (t < 2 * NH);
-  const int hq = is_hi ? t : t - NH;
-  const bool h_isx = hq < TY;                          // x halo of row hq, else y halo of column hq-TY
-  int h_o0, h_om, h_op, h_f;
-  if (h_isx) {
-    const int r = rown(j0 + hq), gcol = N + 2 * (r & 1);
-    h_o0 = is_hi ? (r & ~1) * P + gcol : (r | 1) * P + gcol + 1;   // cell N / cell -1
-    h_om = is_hi ? r * P + N - 1 : h_o0 - 1;                       // cell N-1 / cell -2
-    h_op = is_hi ? h_o0 + 1 : r * P;                               // cell N+1 / cell 0
-    h_f = hq * (N + 1) + (is_hi ? N : 0);
-  } else {
-    const int col = hq - TY;
-    const int y = is_hi ? j0 + TY : j0 - 1;                        // row TY / row -1 of the tile
-    h_o0 = rown(y) * P + col;
-    h_om = rown(y - 1) * P + col;
-    h_op = rown(y + 1) * P + col;
-    h_f = (is_hi ? TY : 0) * N + col;
-  }
-  // the flux at the last face of each row / column is taken by a third set of threads [2NH,3NH) (another warp than
-  // the halo slopes: the passes between two barriers stay balanced across warps)
-  const bool is_hf = (t >= 2 * NH) && (t < 3 * NH);
-  const int fq = t - 2 * NH;
-  const bool f_isx = fq < TY;
-  const int f_f = f_isx ? fq * (N + 1) + N : TY * N + (fq - TY);
-  // halo cell converted by this thread on interior planes
-  int hc_o = -1;
-  const int th = t - (TG - C::HALO);   // the last HALO threads: other warps than the halo slopes / fluxes
-  if (th >= 0 && th < C::HALO) {
-    if (th < 4 * TY) hc_o = rown(j0 + th / 4) * P + N + (th % 4);
+  // ---- halo tasks (cells and faces outside the tile's own N x TY cells).  Without a helper warp they are roles of
+  //      the cell threads: [0,NH) high halo slopes, [NH,2NH) low halo slopes, [2NH,3NH) last-face fluxes, the last
+  //      HALO threads convert the halo cells.  With HW = 1 the helper warp loops over all of them, so that the cell
+  //      warps (whose dependent-issue latency is the critical path of a plane) all carry the same work.
+  // slope task h in [0, 2NH): high halo cell of row/column h (right state -> sRh), low halo cell h-NH (left state -> e)
+  auto halo_slope_task = [&](const double* W, double* eX, double* eY, int h) {
+    const bool hi = h < NH;
+    const int hq = hi ? h : h - NH;
+    const bool isx = hq < TY;                          // x halo of row hq, else y halo of column hq-TY
+    int o0, om, op, f;
+    if (isx) {
+      const int r = rown(j0 + hq), gcol = N + 2 * (r & 1);
+      o0 = hi ? (r & ~1) * P + gcol : (r | 1) * P + gcol + 1;   // cell N / cell -1
+      om = hi ? r * P + N - 1 : o0 - 1;                         // cell N-1 / cell -2
+      op = hi ? o0 + 1 : r * P;                                 // cell N+1 / cell 0
+      f = hq * (N + 1);
+    } else {
+      const int col = hq - TY;
+      const int y = hi ? j0 + TY : j0 - 1;                      // row TY / row -1 of the tile
+      o0 = rown(y) * P + col;
+      om = rown(y - 1) * P + col;
+      op = rown(y + 1) * P + col;
+      f = col;
+    }
+    double L[5], R[5];
+    slope_states(W, o0, om, op, L, R);
+    double* e = isx ? eX : eY;
+#pragma unroll
+    for (int q = 0; q < 5; ++q) {
+      if (DIM == 2 && q == 3) continue;
+      if (!hi) e[pl(q) * EXV + f] = L[q];
+      else sRh[pl(q) * NH + hq] = R[q];
+    }
+  };
+  // flux task fq in [0, NH): the last face of row fq (x) or of column fq-TY (y)
+  auto halo_flux_task = [&](double* eX, double* eY, int fq) {
+    const bool f_isx = fq < TY;
+    const int f_f = f_isx ? fq * (N + 1) + N : TY * N + (fq - TY);
+    double* e = f_isx ? eX : eY;
+    double L[5], Rr[5], F[5];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) {
+      L[q] = (DIM == 2 && q == 3) ? 0.0 : e[pl(q) * EXV + f_f];
+      Rr[q] = (DIM == 2 && q == 3) ? 0.0 : sRh[pl(q) * NH + fq];
+    }
+    const double Ln[5] = {L[0], f_isx ? L[1] : L[2], f_isx ? L[2] : L[1], L[3], L[4]};
+    const double Rn[5] = {Rr[0], f_isx ? Rr[1] : Rr[2], f_isx ? Rr[2] : Rr[1], Rr[3], Rr[4]};
+    riemann_flux<DIM, FAST>(Ln, Rn, gamma, ig1, fluxs, F);
+    const double Fp[5] = {F[0], f_isx ? F[1] : F[2], f_isx ? F[2] : F[1], F[3], F[4]};
+#pragma unroll
+    for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) e[pl(q) * EXV + f_f] = Fp[q];
+  };
+  // conversion task th in [0, HALO): x halo cells (4 per row), then the two rows below and above the tile
+  auto halo_convert_task = [&](double* W, int th) {
+    int o;
+    if (th < 4 * TY) o = rown(j0 + th / 4) * P + N + (th % 4);
     else {
       const int tq = th - 4 * TY, r4 = tq / N;
-      hc_o = rown(r4 < 2 ? j0 - 2 + r4 : j0 + TY + r4 - 2) * P + tq % N;
+      o = rown(r4 < 2 ? j0 - 2 + r4 : j0 + TY + r4 - 2) * P + tq % N;
     }
-  }
+    double tmp[5];
+    convert(W, o, tmp);
+  };
+  const bool is_hs = (HW == 0) && t < 2 * NH;
+  const bool is_hf = (HW == 0) && (t >= 2 * NH) && (t < 3 * NH);
+  const int th = t - (TG - C::HALO);
+  const bool is_hc = (HW == 0) && th >= 0 && th < C::HALO;
 
   // x/y sweep on the converted plane W: sum over the x,y faces of (F_in - F_out) of the own cell
   auto sweep_xy = [&](const double* W, int par, double (&acc)[5]) {
@@ -352,61 +454,54 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT,
       slope_states(W, own, own_ym, own_yp, L, Ry);
 #pragma unroll
       for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eY[pl(q) * EXV + fy + N] = L[q];
-      if (is_hi || is_lo) {
-        double R[5];
-        slope_states(W, h_o0, h_om, h_op, L, R);
-        double* e = h_isx ? eX : eY;
-#pragma unroll
-        for (int q = 0; q < 5; ++q) {
-          if (DIM == 2 && q == 3) continue;
-          if (is_lo) e[pl(q) * EXV + h_f] = L[q];
-          else sRh[pl(q) * NH + hq] = R[q];
-        }
-      }
+      if (is_hs) halo_slope_task(W, eX, eY, t);
     }
-    group_sync(bar_id, TG);
+    group_sync(bar_id, TGA);
     double Fx[5], Fy[5];
     {  // ---- phase 2: flux at the low x and y face of the own cell, and at the last face of each row/column
       double L[5], F[5];
-#pragma unroll
-      for (int q = 0; q < 5; ++q) L[q] = (DIM == 2 && q == 3) ? 0.0 : eX[pl(q) * EXV + fx];
-      riemann_flux<DIM, FAST>(L, Rx, gamma, ig1, fluxs, Fx);
-#pragma unroll
-      for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eX[pl(q) * EXV + fx] = Fx[q];
-      // y: normal frame (rho, v, u, w, p)
-#pragma unroll
-      for (int q = 0; q < 5; ++q) L[q] = (DIM == 2 && q == 3) ? 0.0 : eY[pl(q) * EXV + fy];
-      {
-        const double Ln[5] = {L[0], L[2], L[1], L[3], L[4]}, Rn[5] = {Ry[0], Ry[2], Ry[1], Ry[3], Ry[4]};
-        riemann_flux<DIM, FAST>(Ln, Rn, gamma, ig1, fluxs, F);
-      }
-      Fy[0] = F[0]; Fy[1] = F[2]; Fy[2] = F[1]; Fy[3] = F[3]; Fy[4] = F[4];
-#pragma unroll
-      for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eY[pl(q) * EXV + fy] = Fy[q];
-      if (is_hf) {
-        double* e = f_isx ? eX : eY;
-        double Rr[5];
+      if (FAST) {
+        // x and y faces together (riemann_flux2); y in its normal frame (rho, v, u, w, p)
+        double L2[2][5], R2[2][5], F2[2][5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
-          L[q] = (DIM == 2 && q == 3) ? 0.0 : e[pl(q) * EXV + f_f];
-          Rr[q] = (DIM == 2 && q == 3) ? 0.0 : sRh[pl(q) * NH + fq];
+          L2[0][q] = (DIM == 2 && q == 3) ? 0.0 : eX[pl(q) * EXV + fx];
+          L[q] = (DIM == 2 && q == 3) ? 0.0 : eY[pl(q) * EXV + fy];
+          R2[0][q] = Rx[q];
         }
-        const double Ln[5] = {L[0], f_isx ? L[1] : L[2], f_isx ? L[2] : L[1], L[3], L[4]};
-        const double Rn[5] = {Rr[0], f_isx ? Rr[1] : Rr[2], f_isx ? Rr[2] : Rr[1], Rr[3], Rr[4]};
-        riemann_flux<DIM, FAST>(Ln, Rn, gamma, ig1, fluxs, F);
-        const double Fp[5] = {F[0], f_isx ? F[1] : F[2], f_isx ? F[2] : F[1], F[3], F[4]};
+        L2[1][0] = L[0]; L2[1][1] = L[2]; L2[1][2] = L[1]; L2[1][3] = L[3]; L2[1][4] = L[4];
+        R2[1][0] = Ry[0]; R2[1][1] = Ry[2]; R2[1][2] = Ry[1]; R2[1][3] = Ry[3]; R2[1][4] = Ry[4];
+        riemann_flux2<DIM>(L2, R2, gamma, ig1, F2);
 #pragma unroll
-        for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) e[pl(q) * EXV + f_f] = Fp[q];
+        for (int q = 0; q < 5; ++q) Fx[q] = F2[0][q];
+        Fy[0] = F2[1][0]; Fy[1] = F2[1][2]; Fy[2] = F2[1][1]; Fy[3] = F2[1][3]; Fy[4] = F2[1][4];
+      } else {
+#pragma unroll
+        for (int q = 0; q < 5; ++q) L[q] = (DIM == 2 && q == 3) ? 0.0 : eX[pl(q) * EXV + fx];
+        riemann_flux<DIM, FAST>(L, Rx, gamma, ig1, fluxs, Fx);
+        // y: normal frame (rho, v, u, w, p)
+#pragma unroll
+        for (int q = 0; q < 5; ++q) L[q] = (DIM == 2 && q == 3) ? 0.0 : eY[pl(q) * EXV + fy];
+        {
+          const double Ln[5] = {L[0], L[2], L[1], L[3], L[4]}, Rn[5] = {Ry[0], Ry[2], Ry[1], Ry[3], Ry[4]};
+          riemann_flux<DIM, FAST>(Ln, Rn, gamma, ig1, fluxs, F);
+        }
+        Fy[0] = F[0]; Fy[1] = F[2]; Fy[2] = F[1]; Fy[3] = F[3]; Fy[4] = F[4];
       }
+#pragma unroll
+      for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eX[pl(q) * EXV + fx] = Fx[q];
+#pragma unroll
+      for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eY[pl(q) * EXV + fy] = Fy[q];
+      if (is_hf) halo_flux_task(eX, eY, t - 2 * NH);
     }
-    group_sync(bar_id, TG);
+    group_sync(bar_id, TGA);
     // ---- phase 3: difference with the next faces
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
       if (DIM == 2 && q == 3) { acc[q] = 0.0; continue; }
       acc[q] = (Fx[q] - eX[pl(q) * EXV + fx + 1]) + (Fy[q] - eY[pl(q) * EXV + fy + N]);
     }
-    if (EXBUF == 1) group_sync(bar_id, TG);
+    if (EXBUF == 1) group_sync(bar_id, TGA);
   };
 
   // Runge-Kutta combine eq. (5) + store + optional CFL rate of the new state
@@ -479,11 +574,49 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT,
     }
   };
   auto convert_halo = [&](double* W) {
-    if (hc_o >= 0) {
-      double tmp[5];
-      convert(W, hc_o, tmp);
-    }
+    if (is_hc) halo_convert_task(W, th);
   };
+
+  if (DIM == 3 && t == 0) { issue_plane(-2, 0); issue_plane(-1, 1); }
+  if (HW == 1 && t >= TG) {
+    // ---- helper warp (3D): mirrors the barrier sequence of the march below.  Per plane: convert the halo cells of
+    //      plane c, halo slopes of plane c-1 | barrier | last-face fluxes | barrier | refill the freed ring slot.
+    const int lane = t - TG;
+    int sc = 0;
+    uint32_t ph = 0;
+#pragma unroll 1
+    for (int c = -2; c <= N + 1; ++c) {
+      const int sk = (sc == 0) ? 2 : sc - 1;
+      double* Wc = ring + sc * C::SLOT;
+      const double* Wk = ring + sk * C::SLOT;
+      mbar_wait(bars_u32 + 8u * sc, (ph >> sc) & 1u);
+      ph ^= 1u << sc;
+      if (c >= 0 && c < N) {
+#pragma unroll
+        for (int h = 0; h < (C::HALO + 31) / 32; ++h)
+          if (h * 32 + lane < C::HALO) halo_convert_task(Wc, h * 32 + lane);
+      }
+      fence_proxy_async();
+      if (c >= 1 && c <= N) {
+        double* eX = exX + (EXBUF == 2 ? (c & 1) : 0) * C::EX;
+        double* eY = exY + (EXBUF == 2 ? (c & 1) : 0) * C::EX;
+#pragma unroll
+        for (int h = 0; h < (2 * NH + 31) / 32; ++h)
+          if (h * 32 + lane < 2 * NH) halo_slope_task(Wk, eX, eY, h * 32 + lane);
+        group_sync(bar_id, TGA);
+#pragma unroll
+        for (int h = 0; h < (NH + 31) / 32; ++h)
+          if (h * 32 + lane < NH) halo_flux_task(eX, eY, h * 32 + lane);
+        group_sync(bar_id, TGA);
+        if (EXBUF == 1) group_sync(bar_id, TGA);
+      } else {
+        group_sync(bar_id, TGA);
+      }
+      if (lane == 0 && c + 2 <= N + 1) issue_plane(c + 2, sk);
+      sc = (sc == 2) ? 0 : sc + 1;
+    }
+    return;
+  }
 
   if (DIM == 2) {
     double a[5], b[5], w[5], acc[5];
@@ -492,14 +625,13 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT,
     mbar_wait(bars_u32, 0);
     convert(ring, own, w);
     convert_halo(ring);
-    group_sync(bar_id, TG);
+    group_sync(bar_id, TGA);
     sweep_xy(ring, 0, acc);
     finish(0, acc, a, b);
   } else {
     double dA[5], Lz[5], accp[5];
 #pragma unroll
     for (int q = 0; q < 5; ++q) { dA[q] = 0.0; Lz[q] = 1.0; accp[q] = 0.0; }
-    if (t == 0) { issue_plane(-2, 0); issue_plane(-1, 1); }
     int sc = 0;            // ring slot of plane c (planes take the slots 0,1,2,0,...)
     uint32_t ph = 0;       // phase parity of each slot's mbarrier
     // one march iteration; the steady state (c in [2, N]) is the instance with every flag true
@@ -557,10 +689,10 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT,
 #pragma unroll
         for (int q = 0; q < 5; ++q) accp[q] = acc[q] + Fz[q];
       } else {
-        group_sync(bar_id, TG);
+        group_sync(bar_id, TGA);
       }
       // every thread is past its last read of plane c-1: refill that slot with plane c+2
-      if (t == 0 && c + 2 <= N + 1) issue_plane(c + 2, sk);
+      if (HW == 0 && t == 0 && c + 2 <= N + 1) issue_plane(c + 2, sk);
       sc = (sc == 2) ? 0 : sc + 1;
     };
     using T = std::true_type;
@@ -582,15 +714,15 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT,
   }
 }
 
-template <int DIM, int N, int TY, int G, int EXBUF>
+template <int DIM, int N, int TY, int G, int EXBUF, int HW = 0>
 cudaError_t launch_cfg(const StageParams& p, cudaStream_t s) {
-  using C = Cfg<DIM, N, TY, G, EXBUF>;
+  using C = Cfg<DIM, N, TY, G, EXBUF, HW>;
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(stage_kernel<DIM, N, TY, G, EXBUF, true>,
+    cudaError_t e = cudaFuncSetAttribute(stage_kernel<DIM, N, TY, G, EXBUF, HW, true>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
     if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(stage_kernel<DIM, N, TY, G, EXBUF, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    e = cudaFuncSetAttribute(stage_kernel<DIM, N, TY, G, EXBUF, HW, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)C::SMEM);
     if (e != cudaSuccess) return e;
     attr_set = true;
@@ -598,9 +730,9 @@ cudaError_t launch_cfg(const StageParams& p, cudaStream_t s) {
   const int nitems = p.nblocks * C::YT;
   const int grid = (nitems + G - 1) / G;
   if (p.limiter == F4_LIM_VANLEER && p.flux == F4_FLUX_HLL)
-    stage_kernel<DIM, N, TY, G, EXBUF, true><<<grid, C::NT, C::SMEM, s>>>(p);
+    stage_kernel<DIM, N, TY, G, EXBUF, HW, true><<<grid, C::NT, C::SMEM, s>>>(p);
   else
-    stage_kernel<DIM, N, TY, G, EXBUF, false><<<grid, C::NT, C::SMEM, s>>>(p);
+    stage_kernel<DIM, N, TY, G, EXBUF, HW, false><<<grid, C::NT, C::SMEM, s>>>(p);
   return cudaGetLastError();
 }
 
@@ -614,8 +746,17 @@ cudaError_t launch_stage(int dim, int n, const StageParams& p, cudaStream_t s) {
   if (p.nblocks <= 0) return cudaSuccess;
   if (dim == 2 && n == 8) return launch_cfg<2, 8, 8, 4, 1>(p, s);
   if (dim == 2 && n == 16) return launch_cfg<2, 16, 16, 1, 1>(p, s);
-  if (dim == 3 && n == 8) return launch_cfg<3, 8, 8, 4, 1>(p, s);
-  if (dim == 3 && n == 16) return launch_cfg<3, 16, 16, 1, 2>(p, s);
+  // HW = 1 (a ninth warp per block for all halo work) is correct and halves the barrier stalls, but a CTA of 288
+  // threads is allocated registers as 10 warps, which caps the cell threads at 96 registers (spills, late u_t loads):
+  // measured 19.7 vs 20.8 GCUPS on config 3, so the default keeps the halo roles on cell threads.
+#ifndef F4_HW16
+#define F4_HW16 0
+#endif
+#ifndef F4_HW8
+#define F4_HW8 0
+#endif
+  if (dim == 3 && n == 8) return launch_cfg<3, 8, 8, 4, 1, F4_HW8>(p, s);
+  if (dim == 3 && n == 16) return launch_cfg<3, 16, 16, 1, 2, F4_HW16>(p, s);
   if (dim == 3 && n == 32) return launch_cfg<3, 32, 8, 1, 2>(p, s);
   return cudaErrorInvalidValue;
 }
