@@ -72,6 +72,8 @@ struct Mesh {
   int nstates;
   bool test_rhs = false;  // P9 pin: F(u) = lambda*u
   double test_lambda = 0.0;
+  bool flux_fix = false;  // PAPER.md:253-261 section 2.7: conservative correction at refinement boundaries
+  std::map<std::pair<int, int>, std::vector<double>> bflux;  // (block, face) -> fluxes [var][t2][t1] at that face
   std::vector<Key> blocks;
   std::map<Key, int> index;
   std::vector<std::vector<double>> uu;  // [state][block][var][k][j][i] padded, i fastest (eq. 3)
@@ -443,6 +445,27 @@ int forward_euler(Mesh& m, int s_out, int s_deriv, double dt_sub, int n_prev, co
             result[(size_t)v * vs + m.off(i, j, k)] = dt_sub * Lu[v] + acc;
           }
         }
+    // flux fixing, step 0: "during the flux computation, fluxes at refinement boundaries are
+    // stored in a pre-allocated array bflux" -- the face-normal flux at every cell face of a block face whose
+    // neighbour is coarser or finer, from the same face_flux as the update.
+    if (m.flux_fix && !m.test_rhs) {
+      for (int f = 0; f < 2 * dim; ++f) {
+        Neighbor nb = find_neighbor(m, b, f);
+        if (nb.kind != NB_FINE && nb.kind != NB_COARSE) continue;
+        const int a = f / 2, side = f % 2;
+        std::vector<double>& bf = m.bflux[{b, f}];
+        bf.assign((size_t)nvar * N * kmax, 0.0);
+        for (int t2 = 1; t2 <= kmax; ++t2)
+          for (int t1 = 1; t1 <= N; ++t1) {
+            int i, j, k;
+            compose(a, side ? N : 0, t1, (dim == 3) ? t2 : 1, i, j, k);   // face between cells n and n+1 along a
+            if (dim == 2) k = 1;
+            double F[5];
+            face_flux(i, j, k, a, F);
+            for (int v = 0; v < nvar; ++v) bf[((size_t)v * kmax + (t2 - 1)) * N + (t1 - 1)] = F[v];
+          }
+      }
+    }
     for (int k = 1; k <= kmax; ++k)
       for (int j = 1; j <= N; ++j)
         for (int i = 1; i <= N; ++i)
@@ -466,6 +489,44 @@ int forward_euler(Mesh& m, int s_out, int s_deriv, double dt_sub, int n_prev, co
           }
         }
     (void)P;
+  }
+  // flux fixing, step 3: "a loop over all coarse sides of refinement boundaries is performed, and
+  // the solution in the cells adjacent to the boundary is corrected based on the difference in the coarse-side
+  // flux and the average fine-side flux".  The update above used the coarse flux Fc through that face; with the
+  // mean Ff of the 2^(d-1) fine fluxes instead, u changes by -+ dt_sub/dx_c (Ff - Fc) (+ on the low side, where
+  // the face flux enters the cell; - on the high side, where it leaves).
+  if (m.flux_fix && !m.test_rhs) {
+    const int h = N / 2;
+    for (int C = 0; C < (int)m.blocks.size(); ++C) {
+      const double dxc = m.dx_of_level(m.blocks[C].level);
+      for (int f = 0; f < 2 * dim; ++f) {
+        Neighbor nb = find_neighbor(m, C, f);
+        if (nb.kind != NB_FINE) continue;
+        const int a = f / 2, side = f % 2;
+        const std::vector<double>& bc = m.bflux[{C, f}];
+        for (int v = 0; v < nvar; ++v)
+          for (int t2 = 1; t2 <= kmax; ++t2)
+            for (int t1 = 1; t1 <= N; ++t1) {
+              int o1 = (t1 - 1) / h, tt1 = (t1 - 1) % h;
+              int o2 = (dim == 3) ? (t2 - 1) / h : 0, tt2 = (dim == 3) ? (t2 - 1) % h : 0;
+              const std::vector<double>& bf = m.bflux[{nb.blk[o1 + 2 * o2], f ^ 1}];
+              double sum = 0.0;
+              int cnt = 0;
+              for (int q2 = 0; q2 < (dim == 3 ? 2 : 1); ++q2)
+                for (int q1 = 0; q1 < 2; ++q1) {
+                  sum += bf[((size_t)v * kmax + (2 * tt2 + q2)) * N + (2 * tt1 + q1)];
+                  ++cnt;
+                }
+              double Ff = sum / cnt;
+              double Fc = bc[((size_t)v * kmax + (t2 - 1)) * N + (t1 - 1)];
+              int i, j, k;
+              compose(a, side ? N : 1, t1, (dim == 3) ? t2 : 1, i, j, k);
+              if (dim == 2) k = 1;
+              double corr = dt_sub / dxc * (Ff - Fc);
+              m.at(s_out, C, v, i, j, k) += side ? -corr : corr;
+            }
+      }
+    }
   }
   return 0;
 }
@@ -662,6 +723,7 @@ void ora_destroy(void* h) { delete (Mesh*)h; }
 void ora_set_options(void* h, int limiter, int flux_scheme, double theta) {
   Mesh* m = (Mesh*)h; m->limiter = limiter; m->flux_scheme = flux_scheme; m->theta = theta;
 }
+void ora_set_flux_fix(void* h, int on) { ((Mesh*)h)->flux_fix = on != 0; }
 void ora_set_test_rhs(void* h, int on, double lambda) { Mesh* m = (Mesh*)h; m->test_rhs = on; m->test_lambda = lambda; }
 int ora_num_blocks(void* h) { return (int)((Mesh*)h)->blocks.size(); }
 void ora_get_blocks(void* h, int* level, int* coords) {

@@ -44,6 +44,7 @@ def lib():
         L.ora_destroy.argtypes = [C.c_void_p]
         L.ora_set_options.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double]
         L.ora_set_test_rhs.argtypes = [C.c_void_p, C.c_int, C.c_double]
+        L.ora_set_flux_fix.argtypes = [C.c_void_p, C.c_int]
         L.ora_num_blocks.argtypes = [C.c_void_p]
         L.ora_get_blocks.argtypes = [C.c_void_p, ip, ip]
         L.ora_dx.restype = C.c_double
@@ -116,6 +117,10 @@ class OracleMesh:
 
     def set_options(self, limiter=LIM_VANLEER, flux=FLUX_HLL, theta=1.0):
         self.L.ora_set_options(self.h, limiter, flux, theta)
+
+    def set_flux_fix(self, on=True):
+        """Conservative flux correction at refinement boundaries."""
+        self.L.ora_set_flux_fix(self.h, int(on))
 
     def set_test_rhs(self, on, lam):
         self.L.ora_set_test_rhs(self.h, int(on), lam)
