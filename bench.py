@@ -357,10 +357,13 @@ def main():
     stage_gbs = stage_bytes / (st_ms / max(st_n, 1) * 1e-3) / 1e9 if st_ms > 0 else None
     ghost_gbs = ((rd_b + wr_b) / (fill_ms * 1e-3) / 1e9) if fill_ms > 0 else None
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    tp = os.path.join(ROOT, "profiles", "traffic.csv")     # from the committed ncu --set full summary
     if os.path.exists(tp):
         try:
-            traffic = json.load(open(tp)).get(f"config{args.config}_stage_dram_bytes_per_launch")
+            import csv
+            for row in csv.DictReader(open(tp)):
+                if row["key"] == f"config{args.config}_stage_dram_bytes_per_launch":
+                    traffic = float(row["dram_bytes_per_launch"])
         except Exception:
             traffic = None
     # fp64 issue bound of the stage kernel: 64 DFMA-class instr/clk/SM x 148 SM x clock
