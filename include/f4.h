@@ -92,6 +92,14 @@ int f4_mesh_destroy(f4_mesh *m);
 /* limiter / flux scheme / prolongation theta of eq. (1) (default van Leer, HLL, theta=1). */
 int f4_set_options(f4_mesh *m, int limiter, int flux_scheme, double theta);
 
+/* Flux fixing at refinement boundaries (section 2.7; the paper's f4_fix_c2f_flux), default off.
+ * When on, every stage of f4_advance stores the face-normal fluxes of block faces whose neighbour is coarser or
+ * finer ("bflux"; device memory owned by the library, sized by f4_build_ghost_pattern / f4_adapt) and
+ * then corrects the coarse cells next to such a face by -+ dt_sub/dx_c * (mean of the 2^(dim-1) fine fluxes - coarse
+ * flux), which makes the update conservative across levels.  A mesh without refinement boundaries
+ * takes exactly the same path as with the switch off.  Host only; takes effect at the next f4_advance. */
+int f4_set_flux_fix(f4_mesh *m, int on);
+
 /* bytes of the block store: n_states*max_blocks*Nvar*P^dim*8. */
 size_t f4_storage_bytes(const f4_mesh *m);
 

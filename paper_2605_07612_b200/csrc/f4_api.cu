@@ -34,6 +34,13 @@ struct f4_mesh {
   std::vector<char> srl_valid;  // per logical state: same-level face ghosts are up to date (pushed or filled)
   DevTransfer* d_plan = nullptr;
   size_t cap_plan = 0;
+  // flux fixing at refinement boundaries
+  bool flux_fix = false;
+  int* d_bfslot = nullptr;       // [max_blocks][6] bflux slot of a block face at a refinement boundary, or -1
+  DevFixBlock* d_fix = nullptr;  // coarse blocks with a finer face neighbour
+  double* d_bflux = nullptr;     // [n_bfslots][nvar][N^(d-1)]
+  size_t cap_fix = 0, cap_bflux = 0;
+  int n_fix = 0, n_bfslots = 0;
   unsigned long long* d_maxrate = nullptr;
   double* d_sums = nullptr;
   double* d_stage = nullptr;  // staging for host set/get
@@ -131,6 +138,47 @@ int upload_meta(f4_mesh* m) {
   if (!b2.empty()) CU(cudaMemcpyAsync(m->d_r2, b2.data(), b2.size() * sizeof(DevRecord), cudaMemcpyHostToDevice, m->stream));
   m->n_r1 = (int)a.size();
   m->n_r2 = (int)b2.size();
+  // flux fixing: a bflux slot for every block face whose neighbour is finer (F2C records end there) or coarser
+  // (a C2F record ends there); one DevFixBlock per coarse block with a finer face neighbour
+  std::vector<int> bfslot((size_t)nb * 6, -1);
+  std::vector<DevFixBlock> fix;
+  {
+    int nslots = 0;
+    for (const Record& r : m->hm.r1)
+      if (r.op == F4_OP_F2C && bfslot[(size_t)r.dst * 6 + r.face] < 0) bfslot[(size_t)r.dst * 6 + r.face] = nslots++;
+    for (const Record& r : m->hm.r2)
+      if (r.op == F4_OP_C2F) bfslot[(size_t)r.dst * 6 + r.face] = nslots++;
+    std::vector<int> fix_of(nb, -1);
+    for (const Record& r : m->hm.r1) {
+      if (r.op != F4_OP_F2C) continue;
+      if (fix_of[r.dst] < 0) {
+        fix_of[r.dst] = (int)fix.size();
+        DevFixBlock fb;
+        fb.blk = r.dst;
+        fb.level = m->hm.leaves[r.dst].level;
+        for (int f = 0; f < 6; ++f) {
+          fb.slot_c[f] = -1;
+          for (int o = 0; o < 4; ++o) fb.slot_f[f][o] = -1;
+        }
+        fix.push_back(fb);
+      }
+      DevFixBlock& fb = fix[fix_of[r.dst]];
+      fb.slot_c[r.face] = bfslot[(size_t)r.dst * 6 + r.face];
+      fb.slot_f[r.face][r.o1 + 2 * r.o2] = bfslot[(size_t)r.src * 6 + (r.face ^ 1)];   // the fine block's face towards us
+    }
+    for (const DevFixBlock& fb : fix)
+      for (int f = 0; f < 2 * m->hm.dim; ++f)
+        if (fb.slot_c[f] >= 0)
+          for (int o = 0; o < (m->hm.dim == 3 ? 4 : 2); ++o)
+            if (fb.slot_f[f][o] < 0) return fail(m, F4_EUNBALANCED, "flux fixing: a fine face has no coarse-to-fine record");
+    m->n_bfslots = nslots;
+    m->n_fix = (int)fix.size();
+    size_t face_doubles = (size_t)m->nvar * m->hm.N * (m->hm.dim == 3 ? m->hm.N : 1);
+    if ((rc = ensure(m, m->d_fix, m->cap_fix, fix.size()))) return rc;
+    if ((rc = ensure(m, m->d_bflux, m->cap_bflux, (size_t)nslots * face_doubles))) return rc;
+    CU(cudaMemcpyAsync(m->d_bfslot, bfslot.data(), bfslot.size() * sizeof(int), cudaMemcpyHostToDevice, m->stream));
+    if (!fix.empty()) CU(cudaMemcpyAsync(m->d_fix, fix.data(), fix.size() * sizeof(DevFixBlock), cudaMemcpyHostToDevice, m->stream));
+  }
   CU(cudaStreamSynchronize(m->stream));  // host vectors go out of scope
   return F4_OK;
 }
@@ -209,6 +257,9 @@ int f4_mesh_destroy(f4_mesh* m) {
   if (m->d_r2) cudaFree(m->d_r2);
   if (m->d_r1n) cudaFree(m->d_r1n);
   if (m->d_nbr) cudaFree(m->d_nbr);
+  if (m->d_bfslot) cudaFree(m->d_bfslot);
+  if (m->d_fix) cudaFree(m->d_fix);
+  if (m->d_bflux) cudaFree(m->d_bflux);
   if (m->d_plan) cudaFree(m->d_plan);
   if (m->d_maxrate) cudaFree(m->d_maxrate);
   if (m->d_sums) cudaFree(m->d_sums);
@@ -227,6 +278,12 @@ int f4_set_options(f4_mesh* m, int limiter, int flux_scheme, double theta) {
   return F4_OK;
 }
 
+int f4_set_flux_fix(f4_mesh* m, int on) {
+  if (!m) return F4_EINVAL;
+  m->flux_fix = on != 0;
+  return F4_OK;
+}
+
 size_t f4_storage_bytes(const f4_mesh* m) { return m ? m->state_doubles * (size_t)m->n_states * sizeof(double) : 0; }
 
 int f4_bind_storage(f4_mesh* m, void* dev_ptr, size_t bytes, void* cuda_stream) {
@@ -242,6 +299,7 @@ int f4_bind_storage(f4_mesh* m, void* dev_ptr, size_t bytes, void* cuda_stream) 
   if (!m->d_level) {
     CU(cudaMalloc((void**)&m->d_level, (size_t)m->hm.max_blocks * sizeof(int)));
     CU(cudaMalloc((void**)&m->d_nbr, (size_t)m->hm.max_blocks * 6 * sizeof(int)));
+    CU(cudaMalloc((void**)&m->d_bfslot, (size_t)m->hm.max_blocks * 6 * sizeof(int)));
     CU(cudaMalloc((void**)&m->d_maxrate, sizeof(unsigned long long)));
     CU(cudaMalloc((void**)&m->d_sums, (size_t)m->hm.max_blocks * m->nvar * sizeof(double)));
     // staging: whole blocks of the natural padded layout, at most 128 MiB
@@ -401,8 +459,18 @@ int f4_advance(f4_mesh* m, double dt) {
   p.nblocks = nb;
   p.limiter = m->limiter;
   p.flux = m->flux;
+  // flux fixing acts only where the mesh has refinement boundaries.  The corrected cells must be
+  // what the neighbours see, so the same-level copy is then left to the pattern executor (no fused push) and the
+  // CFL maximum to the standalone reduction (the stage kernel would take it before the correction).
+  const bool ff = m->flux_fix && m->n_fix > 0;
+  FixParams fp{};
+  fp.fix = m->d_fix;
+  fp.nfix = m->n_fix;
+  fp.bflux = m->d_bflux;
+  p.bfslot = ff ? m->d_bfslot : nullptr;
+  p.bflux = m->d_bflux;
   // stage 1, eq. (6): u1 = dt F(ut) + ut
-  p.nbr = m->d_nbr;
+  p.nbr = ff ? nullptr : m->d_nbr;
   if ((rc = fill_ghosts_impl(m, 0, m->srl_valid[0]))) return rc;
   p.deriv = m->state_ptr(0);
   p.prev0 = m->state_ptr(0);
@@ -412,13 +480,22 @@ int f4_advance(f4_mesh* m, double dt) {
   p.w1 = 0.0;
   set_dt(dt);
   p.maxrate = nullptr;
+  auto fix_after_stage = [&]() -> int {
+    if (!ff) return F4_OK;
+    fp.out = p.out;
+    for (int l = 0; l < MAXL; ++l) fp.sdt_l[l] = p.sdt_l[l];
+    Scope sc(m, F4_PROF_STAGE);
+    CU(launch_fluxfix(dim, N, fp, m->stream));
+    return F4_OK;
+  };
   {
     Scope sc(m, F4_PROF_STAGE);
     CU(launch_stage(dim, N, p, m->stream));
   }
+  if ((rc = fix_after_stage())) return rc;
   // stage 2, eq. (7): u = dt/2 F(u1) + (ut + u1)/2, written over ut; CFL max of the new state fused in
-  m->srl_valid[1] = 1;  // pushed by stage 1
-  if ((rc = fill_ghosts_impl(m, 1, true))) return rc;
+  m->srl_valid[1] = ff ? 0 : 1;  // pushed by stage 1
+  if ((rc = fill_ghosts_impl(m, 1, m->srl_valid[1]))) return rc;
   CU(cudaMemsetAsync(m->d_maxrate, 0, sizeof(unsigned long long), m->stream));
   p.deriv = m->state_ptr(1);
   p.prev0 = m->state_ptr(0);
@@ -427,13 +504,14 @@ int f4_advance(f4_mesh* m, double dt) {
   p.w0 = 0.5;
   p.w1 = 0.5;
   set_dt(0.5 * dt);
-  p.maxrate = m->d_maxrate;
+  p.maxrate = ff ? nullptr : m->d_maxrate;
   {
     Scope sc(m, F4_PROF_STAGE);
     CU(launch_stage(dim, N, p, m->stream));
   }
-  m->rate_valid = true;
-  m->srl_valid[0] = 1;  // pushed by stage 2; BC / F2C / C2F ghosts of state 0 are stale until the next fill
+  if ((rc = fix_after_stage())) return rc;
+  m->rate_valid = !ff;
+  m->srl_valid[0] = ff ? 0 : 1;  // pushed by stage 2; BC / F2C / C2F ghosts of state 0 are stale until the next fill
   return F4_OK;
 }
 

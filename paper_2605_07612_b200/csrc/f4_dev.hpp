@@ -36,6 +36,17 @@ struct StageParams {
   int limiter, flux;
   unsigned long long* maxrate;  // bits of a non-negative double, atomicMax; nullptr = no CFL reduction
   const int* nbr;               // [nblocks][6] same-level neighbour per face or -1: fused SRL ghost push; nullptr = off
+  // flux fixing: face-normal fluxes at refinement boundaries are stored "during the flux
+  // computation" into bflux[slot][var][t2][t1]; bfslot[blk][6] = slot of that block face or -1; nullptr = off
+  const int* bfslot;
+  double* bflux;
+};
+
+// one coarse block with at least one finer face neighbour (flux fixing)
+struct DevFixBlock {
+  int blk, level;
+  int slot_c[6];     // bflux slot of the coarse side of face f, or -1 when the neighbour across f is not finer
+  int slot_f[6][4];  // bflux slots of the fine sides, index o1 + 2*o2 (hanging-face offsets)
 };
 
 struct GhostParams {
@@ -59,6 +70,15 @@ cudaError_t launch_unpack(int dim, int n, const double* store_state, double* dst
                           cudaStream_t s);
 cudaError_t launch_init_benign(int dim, int n, double* store_state, int nb, double gamma, cudaStream_t s);
 cudaError_t launch_block_sums(int dim, int n, const double* state, int nb, double* sums /*[nb][nvar]*/, cudaStream_t s);
+// coarse-side correction u -= -+ dt_sub/dx_c (mean fine flux - coarse flux) in the cells next to refinement boundaries
+struct FixParams {
+  double* out;              // the state the stage kernel just wrote
+  const DevFixBlock* fix;
+  int nfix;
+  const double* bflux;
+  double sdt_l[MAXL];       // dt_sub/dx per level
+};
+cudaError_t launch_fluxfix(int dim, int n, const FixParams& p, cudaStream_t s);
 bool stage_supported(int dim, int n);
 
 }  // namespace f4

@@ -262,7 +262,7 @@ struct Cfg {  // FAST (van Leer + HLL fixed at compile time) does not change the
   static_assert(TG % 32 == 0 && N % TY == 0 && GROUP_DOUBLES % 2 == 0, "tile shape");
 };
 
-template <int DIM, int N, int TY, int G, int EXBUF, int HW, bool FAST>
+template <int DIM, int N, int TY, int G, int EXBUF, int HW, bool FAST, bool BF>
 __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
                                   F4_MINB((Cfg<DIM, N, TY, G, EXBUF, HW>::SMEM <= 110 * 1024) ? 2 : 1))
     stage_kernel(const __grid_constant__ StageParams p) {
@@ -441,8 +441,20 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
   const int th = t - (TG - C::HALO);
   const bool is_hc = (HW == 0) && th >= 0 && th < C::HALO;
 
-  // x/y sweep on the converted plane W: sum over the x,y faces of (F_in - F_out) of the own cell
-  auto sweep_xy = [&](const double* W, int par, double (&acc)[5]) {
+  // flux fixing: slots of this block's faces at refinement boundaries (BF instances only)
+  int bfs[6] = {-1, -1, -1, -1, -1, -1};
+  if (BF) {
+#pragma unroll
+    for (int f = 0; f < 2 * DIM; ++f) bfs[f] = p.bfslot[(size_t)blk * 6 + f];
+  }
+  constexpr int BFS = N * ((DIM == 3) ? N : 1);   // cell faces of one block face
+  auto bf_store = [&](int slot, const double (&F)[5], int t1, int t2) {
+    double* d = p.bflux + (size_t)slot * NV * BFS + t2 * N + t1;
+#pragma unroll
+    for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) d[pl(q) * BFS] = F[q];
+  };
+  // x/y sweep on the converted plane W (z index kk): sum over the x,y faces of (F_in - F_out) of the own cell
+  auto sweep_xy = [&](const double* W, int par, int kk, double (&acc)[5]) {
     double* eX = exX + (EXBUF == 2 ? par : 0) * C::EX;
     double* eY = exY + (EXBUF == 2 ? par : 0) * C::EX;
     double Rx[5], Ry[5];
@@ -493,6 +505,10 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
 #pragma unroll
       for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eY[pl(q) * EXV + fy] = Fy[q];
       if (is_hf) halo_flux_task(eX, eY, t - 2 * NH);
+      if (BF) {
+        if (i == 0 && bfs[0] >= 0) bf_store(bfs[0], Fx, j0 + j, kk);
+        if (j0 + j == 0 && bfs[2] >= 0) bf_store(bfs[2], Fy, i, kk);
+      }
     }
     group_sync(bar_id, TGA);
     // ---- phase 3: difference with the next faces
@@ -500,6 +516,20 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
     for (int q = 0; q < 5; ++q) {
       if (DIM == 2 && q == 3) { acc[q] = 0.0; continue; }
       acc[q] = (Fx[q] - eX[pl(q) * EXV + fx + 1]) + (Fy[q] - eY[pl(q) * EXV + fy + N]);
+    }
+    if (BF) {
+      if (i == N - 1 && bfs[1] >= 0) {
+        double Fh[5];
+#pragma unroll
+        for (int q = 0; q < 5; ++q) Fh[q] = (DIM == 2 && q == 3) ? 0.0 : eX[pl(q) * EXV + fx + 1];
+        bf_store(bfs[1], Fh, j0 + j, kk);
+      }
+      if (j0 + j == N - 1 && bfs[3] >= 0) {
+        double Fh[5];
+#pragma unroll
+        for (int q = 0; q < 5; ++q) Fh[q] = (DIM == 2 && q == 3) ? 0.0 : eY[pl(q) * EXV + fy + N];
+        bf_store(bfs[3], Fh, i, kk);
+      }
     }
     if (EXBUF == 1) group_sync(bar_id, TGA);
   };
@@ -626,7 +656,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
     convert(ring, own, w);
     convert_halo(ring);
     group_sync(bar_id, TGA);
-    sweep_xy(ring, 0, acc);
+    sweep_xy(ring, 0, 0, acc);
     finish(0, acc, a, b);
   } else {
     double dA[5], Lz[5], accp[5];
@@ -673,6 +703,10 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
           double F[5];
           riemann_flux<3, FAST>(Lf, Rf, gamma, ig1, fluxs, F);
           Fz[0] = F[0]; Fz[3] = F[1]; Fz[1] = F[2]; Fz[2] = F[3]; Fz[4] = F[4];
+          if (BF) {   // the face between cells c-2 and c-1 is the block's low (c = 1) / high (c = N+1) z face
+            if (c == 1 && bfs[4] >= 0) bf_store(bfs[4], Fz, i, j0 + j);
+            if (c == N + 1 && bfs[5] >= 0) bf_store(bfs[5], Fz, i, j0 + j);
+          }
         }
 #pragma unroll
         for (int q = 0; q < 5; ++q) Lz[q] = Ln[q];
@@ -685,7 +719,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
       }
       if (SWEEP) {
         double acc[5];
-        sweep_xy(Wk, c & 1, acc);
+        sweep_xy(Wk, c & 1, c - 1, acc);
 #pragma unroll
         for (int q = 0; q < 5; ++q) accp[q] = acc[q] + Fz[q];
       } else {
@@ -719,20 +753,29 @@ cudaError_t launch_cfg(const StageParams& p, cudaStream_t s) {
   using C = Cfg<DIM, N, TY, G, EXBUF, HW>;
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(stage_kernel<DIM, N, TY, G, EXBUF, HW, true>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(stage_kernel<DIM, N, TY, G, EXBUF, HW, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)C::SMEM);
+    cudaError_t e = cudaSuccess;
+    auto set = [&](auto* k) {
+      if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+    };
+    set(stage_kernel<DIM, N, TY, G, EXBUF, HW, true, false>);
+    set(stage_kernel<DIM, N, TY, G, EXBUF, HW, false, false>);
+    set(stage_kernel<DIM, N, TY, G, EXBUF, HW, true, true>);
+    set(stage_kernel<DIM, N, TY, G, EXBUF, HW, false, true>);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
   const int nitems = p.nblocks * C::YT;
   const int grid = (nitems + G - 1) / G;
-  if (p.limiter == F4_LIM_VANLEER && p.flux == F4_FLUX_HLL)
-    stage_kernel<DIM, N, TY, G, EXBUF, HW, true><<<grid, C::NT, C::SMEM, s>>>(p);
-  else
-    stage_kernel<DIM, N, TY, G, EXBUF, HW, false><<<grid, C::NT, C::SMEM, s>>>(p);
+  const bool fast = p.limiter == F4_LIM_VANLEER && p.flux == F4_FLUX_HLL;
+  if (p.bfslot) {   // flux fixing on: the instances that store boundary fluxes
+    if (HW != 0) return cudaErrorInvalidValue;   // the helper-warp variant has no flux store
+    if (fast) stage_kernel<DIM, N, TY, G, EXBUF, HW, true, true><<<grid, C::NT, C::SMEM, s>>>(p);
+    else stage_kernel<DIM, N, TY, G, EXBUF, HW, false, true><<<grid, C::NT, C::SMEM, s>>>(p);
+  } else if (fast) {
+    stage_kernel<DIM, N, TY, G, EXBUF, HW, true, false><<<grid, C::NT, C::SMEM, s>>>(p);
+  } else {
+    stage_kernel<DIM, N, TY, G, EXBUF, HW, false, false><<<grid, C::NT, C::SMEM, s>>>(p);
+  }
   return cudaGetLastError();
 }
 
@@ -756,7 +799,16 @@ cudaError_t launch_stage(int dim, int n, const StageParams& p, cudaStream_t s) {
 #define F4_HW8 0
 #endif
   if (dim == 3 && n == 8) return launch_cfg<3, 8, 8, 4, 1, F4_HW8>(p, s);
-  if (dim == 3 && n == 16) return launch_cfg<3, 16, 16, 1, 2, F4_HW16>(p, s);
+#ifndef F4_TY16
+#define F4_TY16 16
+#endif
+#ifndef F4_G16
+#define F4_G16 1
+#endif
+#ifndef F4_EX16
+#define F4_EX16 2
+#endif
+  if (dim == 3 && n == 16) return launch_cfg<3, 16, F4_TY16, F4_G16, F4_EX16, F4_HW16>(p, s);
   if (dim == 3 && n == 32) return launch_cfg<3, 32, 8, 1, 2>(p, s);
   return cudaErrorInvalidValue;
 }
