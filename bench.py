@@ -149,9 +149,10 @@ def pattern_bytes(mesh, n, d):
 
 
 def adaptive_flags(cfg, mesh):
-    """Reading A15 (harness side): pressure-jump flags from the ghost-filled state 0."""
-    mesh.fill_ghosts(0)
-    return W.pressure_jump_flags(cfg, mesh.get_state(0, with_ghosts=True))
+    """Reading A15: config 5's pressure-jump flags, computed on the device from state 0 (f4_refine_flags fills the
+    ghosts and returns one int per block)."""
+    from paper_2605_07612_b200 import f4
+    return mesh.refine_flags(0, f4.CRIT_PJUMP, (0.1, 0.025))[0]
 
 
 def adaptive_initial_mesh(cfg, mesh):
@@ -163,6 +164,23 @@ def adaptive_initial_mesh(cfg, mesh):
             break
     lev, co = mesh.get_blocks()
     mesh.set_state(0, W.initial_state(cfg, lev, co))
+
+
+def max_over_ranks(ms, dist, device):
+    """Timing rule for N > 1: the step time of the job is the MAX over ranks of the device-timed region.
+    `dist` is torch.distributed (or None for one process); works on any backend (nccl on GPUs, gloo in the CPU tests)."""
+    if dist is None:
+        return float(ms)
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world, updates_per_rank, ms):
+    """Replicas only: every rank advances the same workload independently; value = cell
+    updates of ALL ranks / max-over-ranks time, in GCUPS."""
+    return world * updates_per_rank / (ms * 1e-3) / 1e9
 
 
 def run_reference(args, cfg, rank):
@@ -289,11 +307,8 @@ def main():
     updates = counters["updates"]
     adapt_info = dict(counters)
     totals_after = mesh.conserved_totals(0)
-    if dist is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * updates / (ms * 1e-3) / 1e9
+    ms = max_over_ranks(ms, dist, dev)
+    value = whole_job_value(world, updates, ms)
     nb = mesh.num_blocks
     cells = nb * n ** d
 
@@ -332,11 +347,8 @@ def main():
     ev3.record(stream)
     barrier()
     ms_e2e = ev2.elapsed_time(ev3)
-    if dist is not None:
-        t = torch.tensor([ms_e2e], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e2e = float(t.item())
-    e2e = {"value": world * cells * 2.0 * e2e_steps / (ms_e2e * 1e-3) / 1e9, "unit": UNIT,
+    ms_e2e = max_over_ranks(ms_e2e, dist, dev)
+    e2e = {"value": whole_job_value(world, cells * 2.0 * e2e_steps, ms_e2e), "unit": UNIT,
            "h2d_bytes_per_step": int(host_np.nbytes), "d2h_bytes_per_step": int(nb * (d + 2) * 8 + 8),
            "steps": e2e_steps, "ms_per_step": ms_e2e / e2e_steps}
 

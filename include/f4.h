@@ -67,6 +67,7 @@ enum {
 
 enum { F4_LIM_VANLEER = 0, F4_LIM_MINMOD = 1, F4_LIM_MC = 2 }; /* PAPER.md:322-326; reading A1 */
 enum { F4_FLUX_HLL = 0, F4_FLUX_RUSANOV = 1 };                 /* PAPER.md:328; reading A2 */
+enum { F4_CRIT_LOHNER = 0, F4_CRIT_PJUMP = 1 };                 /* PAPER.md:349-362 eq. (12); reading A15 */
 
 /* pattern record ops (data-flow naming) */
 enum {
@@ -161,6 +162,21 @@ int f4_compute_dt(f4_mesh *m, int state, double cfl, double *dt_out);
  * reconstruction + HLL/Einfeldt flux divergence.
  * Asynchronous; result in state 0, whose ghosts are then stale. */
 int f4_advance(f4_mesh *m, double dt);
+
+/* ---- refinement flags on the device ----------------------------------------
+ * Per-block flags for f4_adapt from state `state` (its ghosts are filled first: the criteria read the first layer
+ * of face ghosts, never edge / corner ghosts).
+ *   F4_CRIT_LOHNER  PAPER.md:349-362 eq. (12) on stored variable `var` (0 = density, the paper's choice,
+ *                   PAPER.md:560): per cell and direction E_n = |u_{n-1} - 2u_n + u_{n+1}| /
+ *                   (eps_abs + |u_n - u_{n-1}| + |u_{n+1} - u_n| + eps (|u_{n-1}| + 2|u_n| + |u_{n+1}|)),
+ *                   |E| = sqrt(sum_n E_n^2); params = {c_refine, c_derefine, eps, eps_abs}.
+ *   F4_CRIT_PJUMP   BASELINE config 5 (reading A15): J = max over face-adjacent cell pairs (interior-interior,
+ *                   interior-first ghost layer) of |p_a - p_b| / min(p_a, p_b); params = {hi, lo, -, -}.
+ * flag = +1 if the block maximum exceeds params[0] ("in one cell"), -1 if it is below params[1] ("in all cells"),
+ * else 0; strict comparisons.  flags_out[nb] (host, required) and indicator_out[nb] (host, may be NULL: the block
+ * maxima) are filled; synchronises.  Errors: F4_EINVAL, F4_EUNBOUND, F4_ECUDA. */
+int f4_refine_flags(f4_mesh *m, int state, int criterion, int var, const double params[4], int *flags_out,
+                    double *indicator_out);
 
 /* ---- adapt(refine_flags) ---------------------------------------------------
  * flags[nb]: >0 refine, <0 may coarsen, 0 keep.  refine, then

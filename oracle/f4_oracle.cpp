@@ -8,7 +8,8 @@
 // restriction, C2F prolongation in two rounds) + per-block finite-volume
 // update (primitive reconstruction, HLL flux with Einfeldt speeds,
 // conservative update, Runge-Kutta combine, CFL reduction) + mesh adapt with
-// regrid data transfer.
+// regrid data transfer; also flux fixing at refinement boundaries
+// and the refinement criteria (eq. (12); config 5's pressure jump).
 //
 // Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
 // --impl reference legs may build, load or call this file.  It shares no code
@@ -691,6 +692,70 @@ int adapt(Mesh& m, const int* flags, int* changed_out) {
   return 0;
 }
 
+// ----------------------------------------------------------------------------
+// Refinement criteria: per-block flags {+1 refine, 0 keep, -1 derefine} from a ghost-filled state.
+// ----------------------------------------------------------------------------
+// CRIT_LOHNER -- PAPER.md:349-362 section 3.3 eq. (12), on stored variable `var` (the paper uses the gas density,
+//   PAPER.md:560).  Per interior cell and per direction n = i, j, k:
+//     E_n = |u_{n-1} - 2 u_n + u_{n+1}| / (eps_abs + |u_n - u_{n-1}| + |u_{n+1} - u_n| + eps u*),
+//     u* = |u_{n-1}| + 2 |u_n| + |u_{n+1}|,   |E| = sqrt(E_i^2 + E_j^2 + E_k^2);
+//   "If in one cell in a block |E| > c_refine, mark the block for refinement; if in all cells in a block
+//   |E| < c_derefine, mark the block for derefinement; otherwise keep".  No cross-derivative terms, so only face
+//   ghosts are read.  params = {c_refine, c_derefine, eps, eps_abs}.
+// CRIT_PJUMP -- BASELINE.json config 5 / DESIGN.md reading A15: J = max over face-adjacent cell pairs
+//   (interior-interior and interior-first ghost layer) of |p_a - p_b| / min(p_a, p_b), p from eq. (15);
+//   +1 if J > hi, -1 if J < lo, else 0.  params = {hi, lo}.
+// indicator[b] = max over the block's cells of |E| (or J).  Strict comparisons: ties keep (reading A19).
+enum { CRIT_LOHNER = 0, CRIT_PJUMP = 1 };
+
+int refine_flags(Mesh& m, int s, int criterion, int var, const double* params, int* flags, double* indicator) {
+  const int N = m.N, dim = m.dim, kmax = (dim == 3) ? N : 1;
+  if (criterion == CRIT_LOHNER && (var < 0 || var >= m.nvar)) { m.err = "refine_flags: bad variable"; return -1; }
+  auto pressure = [&](int b, int i, int j, int k) {
+    double rho = m.at(s, b, 0, i, j, k), ke = 0.0;
+    for (int a = 0; a < dim; ++a) { double mom = m.at(s, b, 1 + a, i, j, k); ke = ke + mom * mom; }
+    return (m.gamma - 1.0) * (m.at(s, b, m.nvar - 1, i, j, k) - 0.5 * ke / rho);   // eq. (15) inverted
+  };
+  for (int b = 0; b < (int)m.blocks.size(); ++b) {
+    double ind = 0.0;
+    for (int k = 1; k <= kmax; ++k)
+      for (int j = 1; j <= N; ++j)
+        for (int i = 1; i <= N; ++i) {
+          double cell = 0.0;
+          if (criterion == CRIT_LOHNER) {
+            const double c_eps = params[2], c_abs = params[3];
+            double sumsq = 0.0;
+            for (int a = 0; a < dim; ++a) {
+              int e[3] = {0, 0, 0}; e[a] = 1;
+              double um = m.at(s, b, var, i - e[0], j - e[1], k - e[2]);
+              double u0 = m.at(s, b, var, i, j, k);
+              double up = m.at(s, b, var, i + e[0], j + e[1], k + e[2]);
+              double num = std::fabs((um - 2.0 * u0) + up);
+              double ustar = (std::fabs(um) + 2.0 * std::fabs(u0)) + std::fabs(up);
+              double den = ((c_abs + std::fabs(u0 - um)) + std::fabs(up - u0)) + c_eps * ustar;
+              double En = num / den;
+              sumsq = sumsq + En * En;
+            }
+            cell = std::sqrt(sumsq);
+          } else {
+            double p0 = pressure(b, i, j, k);
+            for (int a = 0; a < dim; ++a) {
+              int e[3] = {0, 0, 0}; e[a] = 1;
+              for (int sgn = -1; sgn <= 1; sgn += 2) {
+                double p1 = pressure(b, i + sgn * e[0], j + sgn * e[1], k + sgn * e[2]);
+                double jump = std::fabs(p0 - p1) / std::min(p0, p1);
+                if (jump > cell) cell = jump;
+              }
+            }
+          }
+          if (cell > ind) ind = cell;
+        }
+    if (indicator) indicator[b] = ind;
+    flags[b] = (ind > params[0]) ? 1 : ((ind < params[1]) ? -1 : 0);
+  }
+  return 0;
+}
+
 }  // namespace
 
 // =============================================================================
@@ -766,6 +831,10 @@ int ora_forward_euler(void* h, int s_out, int s_deriv, double dt_sub, int n_prev
   return forward_euler(*(Mesh*)h, s_out, s_deriv, dt_sub, n_prev, w, s_prev);
 }
 int ora_adapt(void* h, const int* flags, int* changed) { return adapt(*(Mesh*)h, flags, changed); }
+// ghosts of state s must be filled (ora_fill_ghosts); criterion 0 = eq. (12), 1 = pressure jump (see refine_flags)
+int ora_refine_flags(void* h, int s, int criterion, int var, const double* params, int* flags, double* indicator) {
+  return refine_flags(*(Mesh*)h, s, criterion, var, params, flags, indicator);
+}
 
 // sum u * dx^d per variable, fixed block order, long double accumulation (P2)
 void ora_totals(void* h, int s, double* out) {

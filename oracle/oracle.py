@@ -61,6 +61,7 @@ def lib():
         L.ora_advance.argtypes = [C.c_void_p, C.c_double]
         L.ora_forward_euler.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_int, dp, ip]
         L.ora_adapt.argtypes = [C.c_void_p, ip, ip]
+        L.ora_refine_flags.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, dp, ip, dp]
         L.ora_totals.argtypes = [C.c_void_p, C.c_int, dp]
         L.ora_permute.argtypes = [C.c_void_p, ip]
         L.ora_face_table.argtypes = [C.c_void_p, ip, ip, ip]
@@ -177,6 +178,19 @@ class OracleMesh:
         ch = C.c_int(0)
         self._chk(self.L.ora_adapt(self.h, _ip(f), C.byref(ch)))
         return bool(ch.value)
+
+    CRIT_LOHNER, CRIT_PJUMP = 0, 1
+
+    def refine_flags(self, state, criterion, params, var=0):
+        """Per-block flags and indicator of a GHOST-FILLED state: criterion 0 = eq. (12) with
+        params (c_refine, c_derefine, eps, eps_abs) on stored variable var; 1 = pressure jump (reading A15) with
+        params (hi, lo)."""
+        pr = np.zeros(4, dtype=np.float64)
+        pr[:len(params)] = params
+        flags = np.zeros(self.num_blocks, dtype=np.int32)
+        ind = np.zeros(self.num_blocks, dtype=np.float64)
+        self._chk(self.L.ora_refine_flags(self.h, state, criterion, var, _dp(pr), _ip(flags), _dp(ind)))
+        return flags, ind
 
     def totals(self, state):
         out = np.zeros(self.nvar, dtype=np.float64)

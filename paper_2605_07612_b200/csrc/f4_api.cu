@@ -43,6 +43,8 @@ struct f4_mesh {
   int n_fix = 0, n_bfslots = 0;
   unsigned long long* d_maxrate = nullptr;
   double* d_sums = nullptr;
+  int* d_flags = nullptr;        // [max_blocks] refinement flags
+  double* d_indicator = nullptr; // [max_blocks] block maxima of the refinement indicator
   double* d_stage = nullptr;  // staging for host set/get
   size_t stage_bytes = 0;
   bool rate_valid = false;
@@ -263,6 +265,8 @@ int f4_mesh_destroy(f4_mesh* m) {
   if (m->d_plan) cudaFree(m->d_plan);
   if (m->d_maxrate) cudaFree(m->d_maxrate);
   if (m->d_sums) cudaFree(m->d_sums);
+  if (m->d_flags) cudaFree(m->d_flags);
+  if (m->d_indicator) cudaFree(m->d_indicator);
   if (m->d_stage) cudaFree(m->d_stage);
   delete m;
   return F4_OK;
@@ -302,6 +306,8 @@ int f4_bind_storage(f4_mesh* m, void* dev_ptr, size_t bytes, void* cuda_stream) 
     CU(cudaMalloc((void**)&m->d_bfslot, (size_t)m->hm.max_blocks * 6 * sizeof(int)));
     CU(cudaMalloc((void**)&m->d_maxrate, sizeof(unsigned long long)));
     CU(cudaMalloc((void**)&m->d_sums, (size_t)m->hm.max_blocks * m->nvar * sizeof(double)));
+    CU(cudaMalloc((void**)&m->d_flags, (size_t)m->hm.max_blocks * sizeof(int)));
+    CU(cudaMalloc((void**)&m->d_indicator, (size_t)m->hm.max_blocks * sizeof(double)));
     // staging: whole blocks of the natural padded layout, at most 128 MiB
     size_t per_block = m->bs * sizeof(double);
     size_t nblk = (128u << 20) / per_block;
@@ -512,6 +518,27 @@ int f4_advance(f4_mesh* m, double dt) {
   if ((rc = fix_after_stage())) return rc;
   m->rate_valid = !ff;
   m->srl_valid[0] = ff ? 0 : 1;  // pushed by stage 2; BC / F2C / C2F ghosts of state 0 are stale until the next fill
+  return F4_OK;
+}
+
+int f4_refine_flags(f4_mesh* m, int state, int criterion, int var, const double params[4], int* flags_out,
+                    double* indicator_out) {
+  int rc = check_state(m, state);
+  if (rc) return rc;
+  if (!params || !flags_out) return fail(m, F4_EINVAL, "null params / flags");
+  if (criterion != F4_CRIT_LOHNER && criterion != F4_CRIT_PJUMP) return fail(m, F4_EINVAL, "unknown criterion");
+  if (criterion == F4_CRIT_LOHNER && (var < 0 || var >= m->nvar)) return fail(m, F4_EINVAL, "variable out of range");
+  const int nb = (int)m->hm.leaves.size();
+  if ((rc = fill_ghosts_impl(m, state, m->srl_valid[state]))) return rc;
+  {
+    Scope sc(m, F4_PROF_REGRID);
+    CU(launch_flags(m->hm.dim, m->hm.N, m->state_ptr(state), nb, criterion, var, m->gamma, params, m->d_flags,
+                    m->d_indicator, m->stream));
+  }
+  CU(cudaMemcpyAsync(flags_out, m->d_flags, (size_t)nb * sizeof(int), cudaMemcpyDeviceToHost, m->stream));
+  if (indicator_out)
+    CU(cudaMemcpyAsync(indicator_out, m->d_indicator, (size_t)nb * sizeof(double), cudaMemcpyDeviceToHost, m->stream));
+  CU(cudaStreamSynchronize(m->stream));
   return F4_OK;
 }
 

@@ -79,6 +79,9 @@ struct FixParams {
   double sdt_l[MAXL];       // dt_sub/dx per level
 };
 cudaError_t launch_fluxfix(int dim, int n, const FixParams& p, cudaStream_t s);
+// per-block refinement flags and indicator (device arrays) from a ghost-filled state
+cudaError_t launch_flags(int dim, int n, const double* state, int nblocks, int criterion, int var, double gamma,
+                         const double params[4], int* flags, double* indicator, cudaStream_t s);
 bool stage_supported(int dim, int n);
 
 }  // namespace f4

@@ -330,6 +330,74 @@ __global__ void __launch_bounds__(256) block_sums_kernel(const double* __restric
   if (threadIdx.x == 0) sums[(size_t)b * G::NVAR + v] = sh[0];
 }
 
+// Refinement criteria (section 3.3 eq. (12); BASELINE config 5's pressure-jump rule, reading A15):
+// one CTA per block reduces the per-cell indicator to its maximum over the block's interior cells and writes the
+// flag (+1 if max > params[0]; -1 if max < params[1], i.e. ALL cells below; else 0).  Face ghosts of the first layer
+// are read, so the state must be ghost-filled.  The flag is a discrete decision taken from floating point: every
+// operation is an explicitly rounded IEEE add / mul / div / sqrt in the order the paper writes the formula, no
+// contraction, so that the indicator does not depend on compiler choices.
+template <int DIM, int N>
+__global__ void __launch_bounds__(256) flags_kernel(const double* __restrict__ st, int criterion, int var, double gamma,
+                                                    double p0, double p1, double p2, double p3,
+                                                    int* __restrict__ flags, double* __restrict__ indicator) {
+  using G = Geo<DIM, N>;
+  __shared__ double sh[8];
+  const int b = blockIdx.x;
+  const double* sb = st + (size_t)b * G::BS;
+  auto pressure = [&](int i, int j, int k) {   // eq. (15) inverted: p = (gamma-1)(E - 1/2 |m|^2 / rho)
+    const int o = cell_off<DIM, N>(i, j, k);
+    const double rho = sb[o];
+    double ke = 0.0;
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) { const double mom = sb[(size_t)(1 + a) * G::VS + o]; ke = __dadd_rn(ke, __dmul_rn(mom, mom)); }
+    return __dmul_rn(gamma - 1.0, __dsub_rn(sb[(size_t)(G::NVAR - 1) * G::VS + o], __ddiv_rn(__dmul_rn(0.5, ke), rho)));
+  };
+  double mx = 0.0;
+  for (int e = threadIdx.x; e < N * N * G::NZ; e += blockDim.x) {
+    const int i = e % N, j = (e / N) % N, k = e / (N * N);
+    double cell = 0.0;
+    if (criterion == F4_CRIT_LOHNER) {
+      const double* sv = sb + (size_t)var * G::VS;
+      const double u0 = sv[cell_off<DIM, N>(i, j, k)];
+      double sumsq = 0.0;
+#pragma unroll
+      for (int a = 0; a < DIM; ++a) {
+        const int di = (a == 0), dj = (a == 1), dk = (a == 2);
+        const double um = sv[cell_off<DIM, N>(i - di, j - dj, k - dk)];
+        const double up = sv[cell_off<DIM, N>(i + di, j + dj, k + dk)];
+        const double num = fabs(__dadd_rn(__dsub_rn(um, __dmul_rn(2.0, u0)), up));
+        const double ustar = __dadd_rn(__dadd_rn(fabs(um), __dmul_rn(2.0, fabs(u0))), fabs(up));
+        const double den = __dadd_rn(__dadd_rn(__dadd_rn(p3, fabs(__dsub_rn(u0, um))), fabs(__dsub_rn(up, u0))),
+                                     __dmul_rn(p2, ustar));
+        const double En = __ddiv_rn(num, den);
+        sumsq = __dadd_rn(sumsq, __dmul_rn(En, En));
+      }
+      cell = __dsqrt_rn(sumsq);
+    } else {
+      const double pc = pressure(i, j, k);
+#pragma unroll
+      for (int a = 0; a < DIM; ++a) {
+        const int di = (a == 0), dj = (a == 1), dk = (a == 2);
+#pragma unroll
+        for (int sg = -1; sg <= 1; sg += 2) {
+          const double pn = pressure(i + sg * di, j + sg * dj, k + sg * dk);
+          const double jump = __ddiv_rn(fabs(__dsub_rn(pc, pn)), fmin(pc, pn));
+          if (jump > cell) cell = jump;
+        }
+      }
+    }
+    if (cell > mx) mx = cell;
+  }
+  for (int sft = 16; sft > 0; sft >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, sft));
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = mx;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < 8; ++w) mx = fmax(mx, sh[w]);
+    if (indicator) indicator[b] = mx;
+    flags[b] = (mx > p0) ? 1 : ((mx < p1) ? -1 : 0);
+  }
+}
+
 // CFL: max over interior cells of sum_dim (|u_d| + c)/dx (readings A4-A5).
 // Warp shuffle max, then one atomicMax per warp on the bit pattern (non-negative doubles order as integers).
 template <int DIM, int N>
@@ -410,6 +478,12 @@ cudaError_t launch_init_benign(int dim, int n, double* store_state, int nb, doub
 cudaError_t launch_block_sums(int dim, int n, const double* state, int nb, double* sums, cudaStream_t s) {
   if (nb <= 0) return cudaSuccess;
   F4_DISPATCH((block_sums_kernel<D, NN><<<dim3(nb, D + 2), 256, 0, s>>>(state, sums)));
+}
+cudaError_t launch_flags(int dim, int n, const double* state, int nblocks, int criterion, int var, double gamma,
+                         const double params[4], int* flags, double* indicator, cudaStream_t s) {
+  if (nblocks <= 0) return cudaSuccess;
+  F4_DISPATCH((flags_kernel<D, NN><<<nblocks, 256, 0, s>>>(state, criterion, var, gamma, params[0], params[1],
+                                                           params[2], params[3], flags, indicator)));
 }
 cudaError_t launch_maxrate(int dim, int n, const double* state, const int* level, int nblocks, double gamma,
                            double inv_dx0, unsigned long long* maxrate, cudaStream_t s) {

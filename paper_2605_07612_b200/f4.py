@@ -20,13 +20,14 @@ ERRORS = {-1: "F4_EINVAL", -2: "F4_ENOBLOCKS", -3: "F4_ECUDA", -4: "F4_EUNBOUND"
 BC_PERIODIC, BC_OUTFLOW, BC_KEEP = 0, 1, 2
 LIM_VANLEER, LIM_MINMOD, LIM_MC = 0, 1, 2
 FLUX_HLL, FLUX_RUSANOV = 0, 1
+CRIT_LOHNER, CRIT_PJUMP = 0, 1
 OP_SRL, OP_BC, OP_F2C, OP_C2F = 0, 1, 2, 3
 PROF_NAMES = ("ghost_r1", "ghost_r2", "stage", "dt_reduce", "regrid", "layout")
 
 # every symbol include/f4.h declares
 SYMBOLS = ("f4_mesh_create", "f4_mesh_destroy", "f4_set_options", "f4_set_flux_fix", "f4_storage_bytes", "f4_bind_storage",
            "f4_num_blocks", "f4_get_blocks", "f4_set_state", "f4_get_state", "f4_build_ghost_pattern",
-           "f4_pattern_size", "f4_get_pattern", "f4_fill_ghosts", "f4_compute_dt", "f4_advance", "f4_adapt",
+           "f4_pattern_size", "f4_get_pattern", "f4_fill_ghosts", "f4_compute_dt", "f4_advance", "f4_refine_flags", "f4_adapt",
            "f4_conserved_totals", "f4_profile_enable", "f4_profile_get", "f4_launch_count", "f4_last_error",
            "f4_version")
 
@@ -57,6 +58,7 @@ def lib():
     L.f4_mesh_destroy.argtypes = [vp]
     L.f4_set_options.argtypes = [vp, C.c_int, C.c_int, C.c_double]
     L.f4_set_flux_fix.argtypes = [vp, C.c_int]
+    L.f4_refine_flags.argtypes = [vp, C.c_int, C.c_int, C.c_int, dp, ip, dp]
     L.f4_storage_bytes.restype = C.c_size_t
     L.f4_storage_bytes.argtypes = [vp]
     L.f4_bind_storage.argtypes = [vp, vp, C.c_size_t, vp]
@@ -187,6 +189,15 @@ class Mesh:
         if rec.size:
             self._chk(self.L.f4_get_pattern(self.h, _ip(rec)))
         return rec, n1.value, n2.value
+
+    def refine_flags(self, state, criterion, params, var=0):
+        """(flags, indicator) per block, computed on the device (f4_refine_flags)."""
+        pr = np.zeros(4, dtype=np.float64)
+        pr[:len(params)] = params
+        flags = np.zeros(self.num_blocks, dtype=np.int32)
+        ind = np.zeros(self.num_blocks, dtype=np.float64)
+        self._chk(self.L.f4_refine_flags(self.h, state, criterion, var, _dp(pr), _ip(flags), _dp(ind)))
+        return flags, ind
 
     def adapt(self, flags):
         f = np.ascontiguousarray(flags, dtype=np.int32)

@@ -239,41 +239,3 @@ def uniform_blocks(cfg: dict):
     kk, jj, ii = np.meshgrid(np.arange(ext[2]), np.arange(ext[1]), np.arange(ext[0]), indexing="ij")
     coords = np.stack([ii.ravel(), jj.ravel(), kk.ravel()], axis=1).astype(np.int32)
     return np.full(coords.shape[0], l, dtype=np.int32), coords
-
-
-# --------------------------------------------------------------------------
-# config-5 refinement rule (harness-side, reading A15)
-# --------------------------------------------------------------------------
-def pressure_jump_flags(cfg: dict, padded: np.ndarray, hi: float = 0.1, lo: float = 0.025) -> np.ndarray:
-    """Flags from a ghost-filled conservative state in natural padded layout
-    [nb, nvar, Pz, Py, Px].  J = max over face-adjacent cell pairs
-    (interior-interior and interior-first ghost layer) of |pa-pb|/min(pa,pb);
-    +1 if J>hi, -1 if J<lo, else 0."""
-    dim, n, ng, gamma = cfg["dim"], cfg["block_n"], cfg["n_ghost"], cfg["gamma"]
-    nvar = dim + 2
-    rho = padded[:, 0]
-    ke = np.zeros_like(rho)
-    with np.errstate(all="ignore"):
-        for a in range(dim):
-            ke = ke + padded[:, 1 + a] ** 2
-        p = (gamma - 1.0) * (padded[:, nvar - 1] - 0.5 * ke / rho)
-    nb = padded.shape[0]
-    J = np.zeros(nb)
-    lo_i, hi_i = ng, ng + n  # interior slice
-    ints = [slice(lo_i, hi_i)] * 3
-    if dim == 2:
-        ints[0] = slice(0, 1)
-    for a in range(dim):
-        ax = 3 - a  # array axis in [nb, z, y, x]
-        sl_a = [slice(None)] + list(ints)
-        sl_b = [slice(None)] + list(ints)
-        sl_a[ax] = slice(lo_i - 1, hi_i)      # cells -1 .. N-1
-        sl_b[ax] = slice(lo_i, hi_i + 1)      # cells  0 .. N
-        pa, pb = p[tuple(sl_a)], p[tuple(sl_b)]
-        with np.errstate(all="ignore"):
-            jump = np.abs(pa - pb) / np.minimum(pa, pb)
-        J = np.maximum(J, jump.reshape(nb, -1).max(axis=1))
-    flags = np.zeros(nb, dtype=np.int32)
-    flags[J > hi] = 1
-    flags[J < lo] = -1
-    return flags

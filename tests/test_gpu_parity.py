@@ -243,9 +243,22 @@ def test_uniform_state_bit_exact_on_gpu():
 
 
 # ------------------------------------------------------------------ AMR run (config 5 shape)
-def _flags_from_oracle(cfg, om):
+PJUMP = (0.1, 0.025)      # reading A15
+
+
+def _flags_from_oracle(cfg, om, lm=None, perm=None):
+    """Config 5's rule from the ORACLE state (the array fed to both adapt calls, reading A15).  With lm: the flags
+    the device computes from ITS state must agree, except where the oracle's indicator sits on a threshold within
+    the state tolerance (a 1e-13 state difference may legitimately flip a discrete flag there)."""
     om.fill_ghosts(0)
-    return W.pressure_jump_flags(cfg, om.get_state(0, with_ghosts=True))
+    fo, io = om.refine_flags(0, om.CRIT_PJUMP, PJUMP)
+    if lm is not None:
+        fg, ig = lm.refine_flags(0, f4.CRIT_PJUMP, PJUMP)
+        assert np.all(np.abs(ig - io[perm]) <= 1e-9 * np.maximum(io[perm], 1e-3)), np.abs(ig - io[perm]).max()
+        diff = fg != fo[perm]
+        near = np.minimum(np.abs(io[perm] - PJUMP[0]), np.abs(io[perm] - PJUMP[1])) <= 1e-9
+        assert not np.any(diff & ~near), np.argwhere(diff & ~near)
+    return fo
 
 
 @pytest.mark.parametrize("base,extra,steps,every", [(1, 2, 12, 4)])
@@ -268,8 +281,8 @@ def test_config5_small_adaptive(base, extra, steps, every):
     nregrid = 0
     for s in range(steps):
         if s and s % every == 0:
-            fo = _flags_from_oracle(cfg, om)
             perm = perm_lib_to_ora(lm, om)
+            fo = _flags_from_oracle(cfg, om, lm, perm)
             ch_o = om.adapt(fo)
             ch_g = lm.adapt(fo[perm])
             assert ch_o == ch_g
@@ -446,3 +459,33 @@ def test_flux_fixing_is_a_no_op_on_a_uniform_mesh_on_gpu():
         out.append((lm.get_state(0), lm.launch_count() - n0))
         lm.close()
     assert np.array_equal(out[0][0], out[1][0]) and out[0][1] == out[1][1]
+
+
+# ------------------------------------------------------------------ refinement flags on the device
+@pytest.mark.parametrize("dim,N,bc", [(2, 8, [PER] * 4), (2, 16, [OUT] * 4), (3, 8, [OUT] * 6), (3, 16, [PER] * 6),
+                                      (3, 32, [PER] * 6)])
+def test_refine_flags_bit_exact(dim, N, bc):
+    # same ghost-filled input on both sides: the indicator is a sequence of individually rounded IEEE operations
+    # in the paper's order, so flags AND indicators are equal bit for bit (eq. 12; reading A15)
+    cfg, lm, om = _refined_pair(dim, N, bc, rounds=2 if N < 32 else 1, seed=5)
+    perm = perm_lib_to_ora(lm, om)
+    rng = np.random.default_rng(2)
+    u = rng.uniform(0.5, 2.0, lm._shape(False))
+    u[:, -1] += 3.0                                   # energy large enough for p > 0
+    smooth = 1.0 + 1e-3 * rng.uniform(size=lm._shape(False))
+    smooth[:, 1:-1] *= 0.1
+    smooth[:, -1] += 2.0
+    for state_in in (u, smooth):
+        uo = np.empty_like(state_in)
+        uo[perm] = state_in
+        lm.set_state(0, state_in)
+        om.set_state(0, uo)
+        om.fill_ghosts(0)
+        for crit, params, var in [(f4.CRIT_LOHNER, (5e-2, 6.25e-3, 1e-2, 1e-10), 0),
+                                  (f4.CRIT_LOHNER, (0.3, 0.05, 1e-2, 1e-10), dim + 1),
+                                  (f4.CRIT_PJUMP, PJUMP, 0)]:
+            fg, ig = lm.refine_flags(0, crit, params, var)
+            fo, io = om.refine_flags(0, crit, params, var)
+            assert np.array_equal(ig, io[perm]), (crit, np.abs(ig - io[perm]).max())
+            assert np.array_equal(fg, fo[perm])
+    lm.close()

@@ -659,3 +659,122 @@ def test_flux_fixing_is_a_no_op_on_uniform_meshes_and_keeps_uniform_states():
     m.set_state(0, u)
     run_steps(m, 3)
     assert np.array_equal(m.get_state(0), u)
+
+
+# ---------------------------------------------------------------- refinement criteria (eq. 12; A15)
+LOHNER = (5e-2, 6.25e-3, 1e-2, 1e-10)     # c_refine, c_derefine, eps, eps_abs of PAPER.md:560
+
+
+def _one_block(dim, N=8, bc=KEEP):
+    return mesh(dim, N, (1,) * dim, 0, 0, [bc] * (2 * dim))
+
+
+def _padded_from_profile(dim, N, prof_x, var=0, base=0.0):
+    """Natural padded state [1, nvar, Pz, P, P] whose variable `var` depends on x only: prof_x[P] (ghosts included)."""
+    P = N + 4
+    u = np.full((1, dim + 2, P if dim == 3 else 1, P, P), base)
+    u[0, var] = np.asarray(prof_x)[None, None, :]
+    return u
+
+
+@pytest.mark.parametrize("dim", [2, 3])
+def test_lohner_indicator_hand_values(dim):
+    # one triple at cells (3,4,5) of an otherwise constant row: the block indicator is the largest E of the cells
+    # whose stencil sees the triple; the golden file holds numerator and denominator worked by hand
+    N, P = 8, 12
+    for um, u0, up, num, den in _golden("lohner_eq12.txt"):
+        m = _one_block(dim, N)
+        prof = np.empty(P)
+        prof[:5] = um            # padded index p = i + 1 (1-based interior i): cells <= 3 hold um
+        prof[5] = u0             # cell 4
+        prof[6:] = up            # cells >= 5
+        m.set_state(0, _padded_from_profile(dim, N, prof), with_ghosts=True)
+        flags, ind = m.refine_flags(0, m.CRIT_LOHNER, LOHNER)
+        # stencils centred on cells 3 and 5 see (um,um,u0) and (u0,up,up): include them in the expectation
+        def E(a, b, c):
+            return abs(a - 2 * b + c) / (1e-10 + abs(b - a) + abs(c - b) + 1e-2 * (abs(a) + 2 * abs(b) + abs(c)))
+        centre = num / (den + 1e-10)
+        assert abs(E(um, u0, up) - centre) <= 1e-15            # the hand-worked row is what the formula gives
+        expect = max(centre, E(um, um, u0), E(u0, up, up))
+        assert abs(ind[0] - expect) <= 2e-16 * max(expect, 1.0), (um, u0, up, ind[0], expect)
+        assert flags[0] == (1 if expect > LOHNER[0] else (-1 if expect < LOHNER[1] else 0))
+
+
+def test_lohner_linear_field_is_never_refined_and_norm_is_euclidean():
+    # a linear field has zero second differences: |E| = 0 in every cell -> derefine (the paper's linear-field
+    # test input, PAPER.md:437 eq. 21); a step in x, y and z at the same cell gives |E| = sqrt(3) E_1
+    dim, N, P = 3, 8, 12
+    m = _one_block(dim, N)
+    idx = np.arange(P, dtype=np.float64)
+    u = np.zeros((1, 5, P, P, P))
+    u[0, 0] = 1.0 * idx[None, None, :] + 2.0 * idx[None, :, None] + 3.0 * idx[:, None, None]
+    m.set_state(0, u, with_ghosts=True)
+    flags, ind = m.refine_flags(0, m.CRIT_LOHNER, LOHNER)
+    assert ind[0] == 0.0 and flags[0] == -1
+    step = (idx >= 6).astype(np.float64)                       # cells <= 4 are 0, cells >= 5 are 1
+    u[0, 0] = step[None, None, :] + step[None, :, None] + step[:, None, None]
+    m.set_state(0, u, with_ghosts=True)
+    _, ind3 = m.refine_flags(0, m.CRIT_LOHNER, (5e-2, 6.25e-3, 0.0, 0.0))
+    # eps = eps_abs = 0: at cell (4,4,4) every direction sees (0,0,1) -> E_n = 1, |E| = sqrt(3); no cell exceeds it
+    assert abs(ind3[0] - np.sqrt(3.0)) <= 4e-16
+
+
+def test_lohner_scale_invariance_thresholds_and_ghost_use():
+    dim, N, P = 2, 8, 12
+    rng = np.random.default_rng(5)
+    base = rng.uniform(0.5, 2.0, (1, 4, 1, P, P))
+    m = _one_block(dim, N)
+    m.set_state(0, base, with_ghosts=True)
+    _, i1 = m.refine_flags(0, m.CRIT_LOHNER, (5e-2, 6.25e-3, 1e-2, 0.0), var=2)
+    m.set_state(0, 1024.0 * base, with_ghosts=True)            # eps_abs = 0: E is homogeneous of degree 0
+    _, i2 = m.refine_flags(0, m.CRIT_LOHNER, (5e-2, 6.25e-3, 1e-2, 0.0), var=2)
+    assert i1[0] == i2[0] and i1[0] > 0
+    # strict comparisons (reading A19): thresholds equal to the indicator keep the block
+    for cr, cd, want in [(i1[0], 0.0, 0), (np.nextafter(i1[0], 0), 0.0, 1), (9.0, i1[0], 0), (9.0, np.nextafter(i1[0], 9), -1)]:
+        f, _ = m.refine_flags(0, m.CRIT_LOHNER, (cr, cd, 1e-2, 0.0), var=2)
+        assert f[0] == want
+    # only face ghosts of the first layer are read: a spike in the first ghost layer is seen, one in the second
+    # layer or in a corner ghost is not ("we do not consider cross-derivative terms", PAPER.md:362)
+    flat = np.ones((1, 4, 1, P, P))
+    for (jj, ii), seen in [((5, 1), True), ((5, 0), False), ((1, 1), False), ((10, 6), True), ((11, 6), False)]:
+        u = flat.copy()
+        u[0, 0, 0, jj, ii] = 2.0
+        m.set_state(0, u, with_ghosts=True)
+        _, ind = m.refine_flags(0, m.CRIT_LOHNER, LOHNER)
+        assert (ind[0] > 0) == seen, (jj, ii)
+
+
+def test_pressure_jump_rule_hand_values_and_harness_definition():
+    # reading A15: J = max |pa - pb| / min(pa, pb) over face-adjacent pairs, interior + first ghost layer
+    cfg = dict(dim=3, block_n=8, n_ghost=2, brick=(2, 1, 1), base_level=0, max_level=0, bc=[PER] * 6, gamma=1.4)
+    m = O.OracleMesh.from_config(cfg)
+    lev, co = m.get_blocks()
+    w = np.zeros((2, 5, 8, 8, 8))
+    w[:, 0] = 1.0
+    w[:, 4] = 0.7
+    b0 = int(np.argmax(co[:, 0] == 0))
+    def flags_for(cell, factor):
+        ww = w.copy()
+        ww[(b0, 4) + cell] = 0.7 * factor
+        m.set_state(0, np.ascontiguousarray(W.prim_to_cons(ww, 1.4)))
+        m.fill_ghosts(0)
+        return m.refine_flags(0, m.CRIT_PJUMP, (0.1, 0.025))
+    f, J = flags_for((3, 3, 3), 1.0)
+    assert np.all(J == 0.0) and np.all(f == -1)                # uniform pressure
+    f, J = flags_for((3, 3, 3), 2.0)                           # interior cell: only its own block sees it
+    assert abs(J[b0] - 1.0) <= 1e-15 and f[b0] == 1 and J[1 - b0] == 0.0 and f[1 - b0] == -1
+    f, J = flags_for((3, 3, 7), 0.5)                           # cell at the +x face: the neighbour sees it in its ghost
+    assert abs(J[b0] - 1.0) <= 1e-15 and abs(J[1 - b0] - 1.0) <= 1e-15 and np.all(f == 1)
+    f, J = flags_for((3, 3, 3), 1.05)                          # 0.025 < 0.05 < 0.1: keep
+    assert abs(J[b0] - 0.05) <= 1e-14 and f[b0] == 0
+    # the harness's numpy statement of the same rule (tests/helpers.py), on a config-5 blast with refinement
+    cfg5 = W.config(5, scale=1)
+    m5 = O.OracleMesh.from_config(cfg5)
+    for _ in range(2):
+        l5, c5 = m5.get_blocks()
+        m5.set_state(0, W.initial_state(cfg5, l5, c5))
+        m5.fill_ghosts(0)
+        f5, _ = m5.refine_flags(0, m5.CRIT_PJUMP, (0.1, 0.025))
+        assert np.array_equal(f5, H.pressure_jump_flags_numpy(cfg5, m5.get_state(0, with_ghosts=True)))
+        assert (f5 == 1).any() and (f5 == -1).any()
+        m5.adapt(f5)
