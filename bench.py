@@ -228,6 +228,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--rk", default="heun", choices=["heun", "euler", "ssp33", "ssp43", "rk4"],
+                    help="Runge-Kutta scheme of eq. (5) (default: Heun, the configs' scheme); GCUPS counts one cell "
+                         "update per sub-step (PAPER.md:453)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -256,7 +259,10 @@ def main():
         torch.cuda.synchronize()
 
     adaptive = cfg["max_level"] > cfg["base_level"]
-    mesh = f4.Mesh.from_config(cfg, max_blocks=None if not adaptive else 12000)
+    rk = {"heun": f4.RK_HEUN, "euler": f4.RK_EULER, "ssp33": f4.RK_SSP33, "ssp43": f4.RK_SSP43, "rk4": f4.RK_RK4}[args.rk]
+    nstages = f4.RK_STAGES[rk]
+    mesh = f4.Mesh.from_config(cfg, n_states=f4.RK_STATES[rk], max_blocks=None if not adaptive else 12000)
+    mesh.set_rk_scheme(rk)
     stream = torch.cuda.Stream(dev)
     mesh.bind_torch(dev, stream)
     n, d = cfg["block_n"], cfg["dim"]
@@ -282,7 +288,7 @@ def main():
         dt = mesh.compute_dt(0, cfg["cfl"])
         mesh.advance(dt)
         counters["step"] += 1
-        counters["updates"] += 2.0 * mesh.num_blocks * n ** d
+        counters["updates"] += float(nstages) * mesh.num_blocks * n ** d
 
     for _ in range(max(args.warmup, 0)):
         step()
@@ -348,7 +354,7 @@ def main():
     barrier()
     ms_e2e = ev2.elapsed_time(ev3)
     ms_e2e = max_over_ranks(ms_e2e, dist, dev)
-    e2e = {"value": whole_job_value(world, cells * 2.0 * e2e_steps, ms_e2e), "unit": UNIT,
+    e2e = {"value": whole_job_value(world, cells * float(nstages) * e2e_steps, ms_e2e), "unit": UNIT,
            "h2d_bytes_per_step": int(host_np.nbytes), "d2h_bytes_per_step": int(nb * (d + 2) * 8 + 8),
            "steps": e2e_steps, "ms_per_step": ms_e2e / e2e_steps}
 
@@ -363,7 +369,9 @@ def main():
     bpc = 8 * (d + 2)
     st_ms, st_n = prof["stage"]
     cells_per_launch = updates / max(st_n, 1)            # = cells on a static mesh; the average on an adaptive one
-    stage_bytes = cells_per_launch * (2.0 * bpc * r + 0.5 * bpc)
+    # previous states other than s_deriv read per sub-step, averaged over the scheme's sub-steps (Heun: 0 and 1)
+    extra_prev = {"heun": 0.5, "euler": 0.0, "ssp33": 2.0 / 3.0, "ssp43": 0.25, "rk4": 1.25}[args.rk]
+    stage_bytes = cells_per_launch * (2.0 * bpc * r + extra_prev * bpc)
     g_n = prof["ghost_r1"][1] + prof["ghost_r2"][1]
     g_ms = prof["ghost_r1"][0] + prof["ghost_r2"][0]
     stage_gbs = stage_bytes / (st_ms / max(st_n, 1) * 1e-3) / 1e9 if st_ms > 0 else None
@@ -386,7 +394,7 @@ def main():
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(cfg), "blocks": nb, "cells": cells,
                    "l2": "state (2 x %.1f GB) is larger than L2; no flush needed" % (mesh.storage_bytes() / 2e9),
-                   "parallelism": "replicas only" if world > 1 else "1 GPU"},
+                   "parallelism": "replicas only" if world > 1 else "1 GPU", "rk": args.rk},
         "roofline": {"bound": "hbm", "achieved": stage_gbs, "peak": peak, "unit": "GB/s",
                      "frac": (stage_gbs / peak) if stage_gbs else None, "traffic": traffic,
                      "kernel": "stage_kernel", "peak_source": peak_src,
@@ -399,7 +407,7 @@ def main():
                                "loop; inside advance the same-level copies are pushed by the stage kernel and the "
                                "executor runs only BC/F2C/C2F records (none on a uniform periodic mesh)"},
         "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()},
-        "step_algorithmic_GBps": (2 * stage_bytes) / (ms / args.steps * 1e-3) / 1e9,
+        "step_algorithmic_GBps": (nstages * stage_bytes) / (ms / args.steps * 1e-3) / 1e9,
         "adaptive": ({"regrids": adapt_info["regrids"], "mesh_changed": adapt_info["changed"],
                       "adapt_ms_total": 1e3 * adapt_info["adapt_s"], "blocks_at_end": nb,
                       "value_excluding_adapt": world * updates / max(ms * 1e-3 - adapt_info["adapt_s"], 1e-9) / 1e9}

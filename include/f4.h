@@ -67,6 +67,10 @@ enum {
 
 enum { F4_LIM_VANLEER = 0, F4_LIM_MINMOD = 1, F4_LIM_MC = 2 }; /* PAPER.md:322-326; reading A1 */
 enum { F4_FLUX_HLL = 0, F4_FLUX_RUSANOV = 1 };                 /* PAPER.md:328; reading A2 */
+/* Runge-Kutta schemes of the restricted class eq. (5): Heun = SSPRK(2,2) eq. (6)-(7) (default),
+ * forward Euler, SSPRK(3,3), SSPRK(4,3) ("optimal SSP schemes with two, three and four stages"),
+ * classical RK4 eq. (8)-(11).  Temporal states needed (n_states of f4_mesh_create): 2, 2, 3, 3, 4. */
+enum { F4_RK_HEUN = 0, F4_RK_EULER = 1, F4_RK_SSP33 = 2, F4_RK_SSP43 = 3, F4_RK_RK4 = 4, F4_RK_N = 5 };
 enum { F4_CRIT_LOHNER = 0, F4_CRIT_PJUMP = 1 };                 /* PAPER.md:349-362 eq. (12); reading A15 */
 
 /* pattern record ops (data-flow naming) */
@@ -155,8 +159,15 @@ int f4_fill_ghosts(f4_mesh *m, int state);
  * reduction kernel runs.  Synchronises to read one double back. */
 int f4_compute_dt(f4_mesh *m, int state, double cfl, double *dt_out);
 
+/* Select the time integrator used by f4_advance (F4_RK_*).  Every sub-step is one launch of the fused stage kernel
+ * in the form of eq. (5), u(s_out) = dt_sub F(u(s_deriv)) + sum_i w_i u(s_prev,i), n_prev <= 4, preceded by the ghost
+ * fill of s_deriv; the CFL maximum of the new state is fused into the last sub-step.  GCUPS counts one
+ * cell update per sub-step.  Errors: F4_EINVAL (unknown scheme, or n_states too small). */
+int f4_set_rk_scheme(f4_mesh *m, int scheme);
+
 /* ---- advance(dt) -----------------------------------------------------------
- * One step of Heun's method, eq. (6)-(7), as two sub-steps of
+ * One step of the selected Runge-Kutta scheme (f4_set_rk_scheme); default:
+ * one step of Heun's method, eq. (6)-(7), as two sub-steps of
  * eq. (5): fill_ghosts(0); u1 = dt F(ut) + ut -> state 1; fill_ghosts(1);
  * u = dt/2 F(u1) + (ut + u1)/2 -> state 0 (in place).  F = limited primitive
  * reconstruction + HLL/Einfeldt flux divergence.

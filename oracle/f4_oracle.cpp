@@ -565,6 +565,43 @@ int advance_heun(Mesh& m, double dt) {
   return 0;
 }
 
+// The other members of the restricted Runge-Kutta class eq. (5) that foap4 includes: every
+// sub-step is one forward_euler call preceded by the ghost fill of the state it differentiates.
+// States: 0 = u_t (and the result), 1.. = intermediate u_1, u_2, u_3.
+enum { RK_HEUN = 0, RK_EULER = 1, RK_SSP33 = 2, RK_SSP43 = 3, RK_RK4 = 4 };
+
+int advance_rk(Mesh& m, int scheme, double dt) {
+  int rc;
+  auto sub = [&](int s_out, int s_deriv, double dt_sub, std::vector<double> w, std::vector<int> sp) -> int {
+    if ((rc = fill_ghosts(m, s_deriv))) return rc;
+    return forward_euler(m, s_out, s_deriv, dt_sub, (int)w.size(), w.data(), sp.data());
+  };
+  switch (scheme) {
+    case RK_HEUN:
+      return advance_heun(m, dt);
+    case RK_EULER:   // u_{t+1} = dt F(u_t) + u_t
+      if ((rc = sub(1, 0, dt, {1.0}, {0}))) return rc;
+      m.uu[0] = m.uu[1];
+      return 0;
+    case RK_SSP33:   // optimal 3-stage SSP scheme [20]: Shu-Osher form with one F per sub-step
+      if ((rc = sub(1, 0, dt, {1.0}, {0}))) return rc;                                  // u1 = ut + dt F(ut)
+      if ((rc = sub(2, 1, 0.25 * dt, {0.75, 0.25}, {0, 1}))) return rc;                 // u2 = 3/4 ut + 1/4 (u1 + dt F(u1))
+      return sub(0, 2, 2.0 / 3.0 * dt, {1.0 / 3.0, 2.0 / 3.0}, {0, 2});                 // u  = 1/3 ut + 2/3 (u2 + dt F(u2))
+    case RK_SSP43:   // optimal 4-stage, third-order SSP scheme [20]
+      if ((rc = sub(1, 0, 0.5 * dt, {1.0}, {0}))) return rc;                            // u1 = ut + dt/2 F(ut)
+      if ((rc = sub(2, 1, 0.5 * dt, {1.0}, {1}))) return rc;                            // u2 = u1 + dt/2 F(u1)
+      if ((rc = sub(1, 2, dt / 6.0, {2.0 / 3.0, 1.0 / 3.0}, {0, 2}))) return rc;        // u3 = 2/3 ut + 1/3 (u2 + dt/2 F(u2))
+      return sub(0, 1, 0.5 * dt, {1.0}, {1});                                           // u  = u3 + dt/2 F(u3)
+    case RK_RK4:     // eq. (8)-(11)
+      if ((rc = sub(1, 0, 0.5 * dt, {1.0}, {0}))) return rc;                            // (8)
+      if ((rc = sub(2, 1, 0.5 * dt, {1.0}, {0}))) return rc;                            // (9)
+      if ((rc = sub(3, 2, dt, {1.0}, {0}))) return rc;                                  // (10)
+      return sub(0, 3, dt / 6.0, {-1.0 / 3.0, 1.0 / 3.0, 2.0 / 3.0, 1.0 / 3.0}, {0, 1, 2, 3});   // (11)
+  }
+  m.err = "unknown Runge-Kutta scheme";
+  return -1;
+}
+
 // ----------------------------------------------------------------------------
 // Mesh adapt + regrid transfer, PAPER.md:111-117 (readings A11, A12)
 // ----------------------------------------------------------------------------
@@ -827,6 +864,7 @@ int ora_fill_ghosts(void* h, int s) { return fill_ghosts(*(Mesh*)h, s); }
 double ora_max_wave_rate(void* h, int s) { return max_wave_rate(*(Mesh*)h, s); }
 double ora_compute_dt(void* h, int s, double cfl) { return cfl / max_wave_rate(*(Mesh*)h, s); }
 int ora_advance(void* h, double dt) { return advance_heun(*(Mesh*)h, dt); }
+int ora_advance_rk(void* h, int scheme, double dt) { return advance_rk(*(Mesh*)h, scheme, dt); }
 int ora_forward_euler(void* h, int s_out, int s_deriv, double dt_sub, int n_prev, const double* w, const int* s_prev) {
   return forward_euler(*(Mesh*)h, s_out, s_deriv, dt_sub, n_prev, w, s_prev);
 }

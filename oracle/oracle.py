@@ -59,6 +59,7 @@ def lib():
         L.ora_compute_dt.restype = C.c_double
         L.ora_compute_dt.argtypes = [C.c_void_p, C.c_int, C.c_double]
         L.ora_advance.argtypes = [C.c_void_p, C.c_double]
+        L.ora_advance_rk.argtypes = [C.c_void_p, C.c_int, C.c_double]
         L.ora_forward_euler.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_int, dp, ip]
         L.ora_adapt.argtypes = [C.c_void_p, ip, ip]
         L.ora_refine_flags.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, dp, ip, dp]
@@ -164,8 +165,14 @@ class OracleMesh:
     def compute_dt(self, state, cfl):
         return self.L.ora_compute_dt(self.h, state, cfl)
 
-    def advance(self, dt):
-        self._chk(self.L.ora_advance(self.h, dt))
+    RK_HEUN, RK_EULER, RK_SSP33, RK_SSP43, RK_RK4 = 0, 1, 2, 3, 4
+
+    def advance(self, dt, scheme=None):
+        """One step: Heun (eq. 6-7) by default, else the scheme of PAPER.md:296-314 (needs 3 / 4 states)."""
+        if scheme is None:
+            self._chk(self.L.ora_advance(self.h, dt))
+        else:
+            self._chk(self.L.ora_advance_rk(self.h, int(scheme), dt))
 
     def forward_euler(self, s_out, s_deriv, dt_sub, w, s_prev):
         w = np.asarray(w, dtype=np.float64)

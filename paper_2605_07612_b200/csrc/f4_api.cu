@@ -16,6 +16,7 @@ struct f4_mesh {
   HostMesh hm;
   double gamma = 1.4, theta = 1.0;
   int limiter = F4_LIM_VANLEER, flux = F4_FLUX_HLL;
+  int rk = F4_RK_HEUN;
   int n_states = 2;
   int nvar = 5;
   size_t vs = 0, bs = 0, state_doubles = 0;  // doubles per (block,var), per block, per state
@@ -446,21 +447,68 @@ int f4_compute_dt(f4_mesh* m, int state, double cfl, double* dt_out) {
   return F4_OK;
 }
 
+namespace {
+
+// One sub-step of eq. (5): u(out) = dtf*dt F(u(deriv)) + sum_i w[i] u(prev[i]); logical states.
+struct SubStep {
+  int out, deriv;
+  double dtf;
+  int np;
+  double w[4];
+  int prev[4];
+};
+struct Scheme {
+  int n_sub, n_states, result;   // result: logical state that holds u(t+dt) after the last sub-step
+  SubStep sub[4];
+};
+
+// The schemes foap4 includes ("optimal SSP schemes with two, three and four stages", eq. (6)-(11)).
+// out != deriv always (the stage kernel pushes ghost layers of `out` into neighbour blocks that may still be
+// reading `deriv`); out == prev[i] is allowed (a cell of prev is read only by the thread that writes it).
+const Scheme& scheme_table(int rk) {
+  static const Scheme tab[F4_RK_N] = {
+      // Heun = SSPRK(2,2), eq. (6)-(7)
+      {2, 2, 0, {{1, 0, 1.0, 1, {1.0}, {0}}, {0, 1, 0.5, 2, {0.5, 0.5}, {0, 1}}}},
+      // forward Euler: one sub-step of eq. (5) with n_prev = 1
+      {1, 2, 1, {{1, 0, 1.0, 1, {1.0}, {0}}}},
+      // SSPRK(3,3) (Shu-Osher): u1 = ut + dt F(ut); u2 = 3/4 ut + 1/4 (u1 + dt F(u1)); u = 1/3 ut + 2/3 (u2 + dt F(u2))
+      {3, 3, 0, {{1, 0, 1.0, 1, {1.0}, {0}},
+                 {2, 1, 0.25, 2, {0.75, 0.25}, {0, 1}},
+                 {0, 2, 2.0 / 3.0, 2, {1.0 / 3.0, 2.0 / 3.0}, {0, 2}}}},
+      // SSPRK(4,3): u1 = ut + dt/2 F(ut); u2 = u1 + dt/2 F(u1); u3 = 2/3 ut + 1/3 (u2 + dt/2 F(u2)); u = u3 + dt/2 F(u3)
+      {4, 3, 0, {{1, 0, 0.5, 1, {1.0}, {0}},
+                 {2, 1, 0.5, 1, {1.0}, {1}},
+                 {1, 2, 1.0 / 6.0, 2, {2.0 / 3.0, 1.0 / 3.0}, {0, 2}},
+                 {0, 1, 0.5, 1, {1.0}, {1}}}},
+      // classical RK4, eq. (8)-(11)
+      {4, 4, 0, {{1, 0, 0.5, 1, {1.0}, {0}},
+                 {2, 1, 0.5, 1, {1.0}, {0}},
+                 {3, 2, 1.0, 1, {1.0}, {0}},
+                 {0, 3, 1.0 / 6.0, 4, {-1.0 / 3.0, 1.0 / 3.0, 2.0 / 3.0, 1.0 / 3.0}, {0, 1, 2, 3}}}},
+  };
+  return tab[rk];
+}
+
+}  // namespace
+
+int f4_set_rk_scheme(f4_mesh* m, int scheme) {
+  if (!m) return F4_EINVAL;
+  if (scheme < 0 || scheme >= F4_RK_N) return fail(m, F4_EINVAL, "unknown Runge-Kutta scheme");
+  if (scheme_table(scheme).n_states > m->n_states)
+    return fail(m, F4_EINVAL, "this scheme needs more temporal states than f4_mesh_create allocated (PAPER.md:318)");
+  m->rk = scheme;
+  return F4_OK;
+}
+
 int f4_advance(f4_mesh* m, double dt) {
   int rc = check_state(m, 0);
   if (rc) return rc;
   if (!(dt > 0.0)) return fail(m, F4_EINVAL, "dt must be positive");
   const int dim = m->hm.dim, N = m->hm.N, nb = (int)m->hm.leaves.size();
+  const Scheme& sch = scheme_table(m->rk);
   StageParams p{};
   p.gamma = m->gamma;
   const double inv_dx0 = 1.0 / m->hm.dx_of_level(0);
-  auto set_dt = [&](double dt_sub) {
-    p.dt_sub = dt_sub;
-    for (int l = 0; l < MAXL; ++l) {
-      p.inv_dx_l[l] = inv_dx0 * (double)(1u << l);
-      p.sdt_l[l] = dt_sub * p.inv_dx_l[l];
-    }
-  };
   p.level = m->d_level;
   p.nblocks = nb;
   p.limiter = m->limiter;
@@ -475,49 +523,41 @@ int f4_advance(f4_mesh* m, double dt) {
   fp.bflux = m->d_bflux;
   p.bfslot = ff ? m->d_bfslot : nullptr;
   p.bflux = m->d_bflux;
-  // stage 1, eq. (6): u1 = dt F(ut) + ut
   p.nbr = ff ? nullptr : m->d_nbr;
-  if ((rc = fill_ghosts_impl(m, 0, m->srl_valid[0]))) return rc;
-  p.deriv = m->state_ptr(0);
-  p.prev0 = m->state_ptr(0);
-  p.prev1 = nullptr;
-  p.out = m->state_ptr(1);
-  p.w0 = 1.0;
-  p.w1 = 0.0;
-  set_dt(dt);
-  p.maxrate = nullptr;
-  auto fix_after_stage = [&]() -> int {
-    if (!ff) return F4_OK;
-    fp.out = p.out;
-    for (int l = 0; l < MAXL; ++l) fp.sdt_l[l] = p.sdt_l[l];
-    Scope sc(m, F4_PROF_STAGE);
-    CU(launch_fluxfix(dim, N, fp, m->stream));
-    return F4_OK;
-  };
-  {
-    Scope sc(m, F4_PROF_STAGE);
-    CU(launch_stage(dim, N, p, m->stream));
+  for (int q = 0; q < sch.n_sub; ++q) {
+    const SubStep& ss = sch.sub[q];
+    const bool last = (q == sch.n_sub - 1);
+    // ghost fill precedes each F evaluation; same-level ghosts of a state a stage produced were pushed
+    if ((rc = fill_ghosts_impl(m, ss.deriv, m->srl_valid[ss.deriv]))) return rc;
+    p.deriv = m->state_ptr(ss.deriv);
+    p.out = m->state_ptr(ss.out);
+    const double* pv[4] = {nullptr, nullptr, nullptr, nullptr};
+    double w[4] = {0.0, 0.0, 0.0, 0.0};
+    for (int r = 0; r < ss.np; ++r) { pv[r] = m->state_ptr(ss.prev[r]); w[r] = ss.w[r]; }
+    p.prev0 = pv[0]; p.prev1 = pv[1]; p.prev2 = pv[2]; p.prev3 = pv[3];
+    p.w0 = w[0]; p.w1 = w[1]; p.w2 = w[2]; p.w3 = w[3];
+    p.dt_sub = ss.dtf * dt;
+    for (int l = 0; l < MAXL; ++l) {
+      p.inv_dx_l[l] = inv_dx0 * (double)(1u << l);
+      p.sdt_l[l] = p.dt_sub * p.inv_dx_l[l];
+    }
+    // CFL max of the new state fused into the last sub-step ("a limit for the next time step")
+    p.maxrate = (last && !ff) ? m->d_maxrate : nullptr;
+    if (p.maxrate) CU(cudaMemsetAsync(m->d_maxrate, 0, sizeof(unsigned long long), m->stream));
+    {
+      Scope sc(m, F4_PROF_STAGE);
+      CU(launch_stage(dim, N, p, m->stream));
+    }
+    if (ff) {
+      fp.out = p.out;
+      for (int l = 0; l < MAXL; ++l) fp.sdt_l[l] = p.sdt_l[l];
+      Scope sc(m, F4_PROF_STAGE);
+      CU(launch_fluxfix(dim, N, fp, m->stream));
+    }
+    m->srl_valid[ss.out] = ff ? 0 : 1;   // pushed by the stage; BC / F2C / C2F ghosts of `out` are stale until the next fill
   }
-  if ((rc = fix_after_stage())) return rc;
-  // stage 2, eq. (7): u = dt/2 F(u1) + (ut + u1)/2, written over ut; CFL max of the new state fused in
-  m->srl_valid[1] = ff ? 0 : 1;  // pushed by stage 1
-  if ((rc = fill_ghosts_impl(m, 1, m->srl_valid[1]))) return rc;
-  CU(cudaMemsetAsync(m->d_maxrate, 0, sizeof(unsigned long long), m->stream));
-  p.deriv = m->state_ptr(1);
-  p.prev0 = m->state_ptr(0);
-  p.prev1 = m->state_ptr(1);
-  p.out = m->state_ptr(0);
-  p.w0 = 0.5;
-  p.w1 = 0.5;
-  set_dt(0.5 * dt);
-  p.maxrate = ff ? nullptr : m->d_maxrate;
-  {
-    Scope sc(m, F4_PROF_STAGE);
-    CU(launch_stage(dim, N, p, m->stream));
-  }
-  if ((rc = fix_after_stage())) return rc;
+  if (sch.result != 0) std::swap(m->phys[0], m->phys[sch.result]), std::swap(m->srl_valid[0], m->srl_valid[sch.result]);
   m->rate_valid = !ff;
-  m->srl_valid[0] = ff ? 0 : 1;  // pushed by stage 2; BC / F2C / C2F ghosts of state 0 are stale until the next fill
   return F4_OK;
 }
 

@@ -26,8 +26,10 @@ struct StageParams {
   const double* deriv;  // state whose time derivative is taken (ghosts filled)
   const double* prev0;  // eq. (5): out = dt_sub*F(deriv) + w0*prev0 + w1*prev1
   const double* prev1;  // may be nullptr (w1 ignored)
+  const double* prev2;  // third / fourth previous state (classical RK4 eq. (11)); nullptr = none; prev3 needs prev2
+  const double* prev3;
   double* out;
-  double w0, w1, dt_sub;
+  double w0, w1, w2, w3, dt_sub;
   double gamma;
   double inv_dx_l[MAXL];  // 1/dx per refinement level (1/dx_0 * 2^l, exact)
   double sdt_l[MAXL];     // dt_sub/dx per level: the factor of the flux difference in eq. (5)

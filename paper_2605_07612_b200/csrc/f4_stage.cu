@@ -79,8 +79,15 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
                : "memory");
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+#ifndef F4_ABL
+#define F4_ABL 0   // timing ablations (wrong results): 1 no sweep barriers, 2 no halo tasks, 4 no ghost push
+#endif
 __device__ __forceinline__ void group_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+__device__ __forceinline__ void sweep_sync(int id, int nthreads) {
+  if (F4_ABL & 1) { __syncwarp(); return; }
+  group_sync(id, nthreads);
 }
 
 // limited HALF slope 1/2*phi(a,b) for the reconstruction w +- 1/2 phi (reading A1)
@@ -436,14 +443,14 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
     double tmp[5];
     convert(W, o, tmp);
   };
-  const bool is_hs = (HW == 0) && t < 2 * NH;
-  const bool is_hf = (HW == 0) && (t >= 2 * NH) && (t < 3 * NH);
+  const bool is_hs = (HW == 0) && !(F4_ABL & 2) && t < 2 * NH;
+  const bool is_hf = (HW == 0) && !(F4_ABL & 2) && (t >= 2 * NH) && (t < 3 * NH);
   const int th = t - (TG - C::HALO);
-  const bool is_hc = (HW == 0) && th >= 0 && th < C::HALO;
+  const bool is_hc = (HW == 0) && !(F4_ABL & 2) && th >= 0 && th < C::HALO;
 
   // flux fixing: slots of this block's faces at refinement boundaries (BF instances only)
   int bfs[6] = {-1, -1, -1, -1, -1, -1};
-  if (BF) {
+  if (BF && p.bfslot) {
 #pragma unroll
     for (int f = 0; f < 2 * DIM; ++f) bfs[f] = p.bfslot[(size_t)blk * 6 + f];
   }
@@ -468,7 +475,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
       for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eY[pl(q) * EXV + fy + N] = L[q];
       if (is_hs) halo_slope_task(W, eX, eY, t);
     }
-    group_sync(bar_id, TGA);
+    sweep_sync(bar_id, TGA);
     double Fx[5], Fy[5];
     {  // ---- phase 2: flux at the low x and y face of the own cell, and at the last face of each row/column
       double L[5], F[5];
@@ -510,7 +517,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
         if (j0 + j == 0 && bfs[2] >= 0) bf_store(bfs[2], Fy, i, kk);
       }
     }
-    group_sync(bar_id, TGA);
+    sweep_sync(bar_id, TGA);
     // ---- phase 3: difference with the next faces
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
@@ -531,7 +538,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
         bf_store(bfs[3], Fh, i, kk);
       }
     }
-    if (EXBUF == 1) group_sync(bar_id, TGA);
+    if (EXBUF == 1) sweep_sync(bar_id, TGA);
   };
 
   // Runge-Kutta combine eq. (5) + store + optional CFL rate of the new state
@@ -546,7 +553,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
   double* ppx = nullptr;   // x / y push targets of this thread (k = 0, var 0)
   double* ppy = nullptr;
   int nbz0 = -1, nbz1 = -1;
-  if (p.nbr) {
+  if (p.nbr && !(F4_ABL & 4)) {
     const int* nb = p.nbr + (size_t)blk * 6;
     const int jg = j0 + j;
     if (i < NG && nb[0] >= 0) ppx = p.out + (size_t)nb[0] * C::BS + ((jg & ~1) * P + N + 2 * (jg & 1) + i);
@@ -555,6 +562,11 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
     if (jg >= N - NG && nb[3] >= 0) ppy = p.out + (size_t)nb[3] * C::BS + ((jg + 2 * NG) * P + i);
     if (DIM == 3) { nbz0 = nb[4]; nbz1 = nb[5]; }
   }
+  // general instances (BF): up to four previous states in eq. (5) (classical RK4, eq. (11));
+  // the third and fourth are folded into b: b <- b + (w2 c + w3 d) / w1 is avoided by carrying w1 b + w2 c + w3 d
+  const double* pc = (BF && p.prev2) ? p.prev2 + boff + co : nullptr;
+  const double* pd = (BF && p.prev3) ? p.prev3 + boff + co : nullptr;
+  const double w1eff = (BF && pc) ? 1.0 : p.w1;
   auto load_prev = [&](int k, double (&a)[5], double (&b)[5]) {
     const int ko = (DIM == 3 ? k : 0) * PP;
 #pragma unroll
@@ -562,6 +574,12 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
       if (DIM == 2 && q == 3) { a[q] = 0.0; b[q] = 0.0; continue; }
       a[q] = pa[ko + pl(q) * (int)C::VS];
       b[q] = pb ? pb[ko + pl(q) * (int)C::VS] : 0.0;
+      if (BF && pc) {
+        double e = p.w1 * b[q];
+        e = fma(p.w2, pc[ko + pl(q) * (int)C::VS], e);
+        if (pd) e = fma(p.w3, pd[ko + pl(q) * (int)C::VS], e);
+        b[q] = e;
+      }
     }
   };
   auto finish = [&](int k, const double (&tot)[5], const double (&a)[5], const double (&b)[5]) {
@@ -570,7 +588,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
       if (DIM == 2 && q == 3) { u[q] = 0.0; continue; }
-      u[q] = fma(sdt, tot[q], fma(p.w1, b[q], p.w0 * a[q]));
+      u[q] = fma(sdt, tot[q], fma(w1eff, b[q], p.w0 * a[q]));
       po[ko + pl(q) * (int)C::VS] = u[q];
     }
     if (ppx) {
@@ -767,7 +785,7 @@ cudaError_t launch_cfg(const StageParams& p, cudaStream_t s) {
   const int nitems = p.nblocks * C::YT;
   const int grid = (nitems + G - 1) / G;
   const bool fast = p.limiter == F4_LIM_VANLEER && p.flux == F4_FLUX_HLL;
-  if (p.bfslot) {   // flux fixing on: the instances that store boundary fluxes
+  if (p.bfslot || p.prev2) {   // general instances: boundary-flux store (flux fixing) and / or > 2 previous states
     if (HW != 0) return cudaErrorInvalidValue;   // the helper-warp variant has no flux store
     if (fast) stage_kernel<DIM, N, TY, G, EXBUF, HW, true, true><<<grid, C::NT, C::SMEM, s>>>(p);
     else stage_kernel<DIM, N, TY, G, EXBUF, HW, false, true><<<grid, C::NT, C::SMEM, s>>>(p);

@@ -21,11 +21,14 @@ BC_PERIODIC, BC_OUTFLOW, BC_KEEP = 0, 1, 2
 LIM_VANLEER, LIM_MINMOD, LIM_MC = 0, 1, 2
 FLUX_HLL, FLUX_RUSANOV = 0, 1
 CRIT_LOHNER, CRIT_PJUMP = 0, 1
+RK_HEUN, RK_EULER, RK_SSP33, RK_SSP43, RK_RK4 = 0, 1, 2, 3, 4
+RK_STAGES = {RK_HEUN: 2, RK_EULER: 1, RK_SSP33: 3, RK_SSP43: 4, RK_RK4: 4}
+RK_STATES = {RK_HEUN: 2, RK_EULER: 2, RK_SSP33: 3, RK_SSP43: 3, RK_RK4: 4}
 OP_SRL, OP_BC, OP_F2C, OP_C2F = 0, 1, 2, 3
 PROF_NAMES = ("ghost_r1", "ghost_r2", "stage", "dt_reduce", "regrid", "layout")
 
 # every symbol include/f4.h declares
-SYMBOLS = ("f4_mesh_create", "f4_mesh_destroy", "f4_set_options", "f4_set_flux_fix", "f4_storage_bytes", "f4_bind_storage",
+SYMBOLS = ("f4_mesh_create", "f4_mesh_destroy", "f4_set_options", "f4_set_flux_fix", "f4_set_rk_scheme", "f4_storage_bytes", "f4_bind_storage",
            "f4_num_blocks", "f4_get_blocks", "f4_set_state", "f4_get_state", "f4_build_ghost_pattern",
            "f4_pattern_size", "f4_get_pattern", "f4_fill_ghosts", "f4_compute_dt", "f4_advance", "f4_refine_flags", "f4_adapt",
            "f4_conserved_totals", "f4_profile_enable", "f4_profile_get", "f4_launch_count", "f4_last_error",
@@ -58,6 +61,7 @@ def lib():
     L.f4_mesh_destroy.argtypes = [vp]
     L.f4_set_options.argtypes = [vp, C.c_int, C.c_int, C.c_double]
     L.f4_set_flux_fix.argtypes = [vp, C.c_int]
+    L.f4_set_rk_scheme.argtypes = [vp, C.c_int]
     L.f4_refine_flags.argtypes = [vp, C.c_int, C.c_int, C.c_int, dp, ip, dp]
     L.f4_storage_bytes.restype = C.c_size_t
     L.f4_storage_bytes.argtypes = [vp]
@@ -175,6 +179,9 @@ class Mesh:
 
     def set_options(self, limiter=LIM_VANLEER, flux=FLUX_HLL, theta=1.0):
         self._chk(self.L.f4_set_options(self.h, limiter, flux, theta))
+
+    def set_rk_scheme(self, scheme):
+        self._chk(self.L.f4_set_rk_scheme(self.h, int(scheme)))
 
     def set_flux_fix(self, on=True):
         self._chk(self.L.f4_set_flux_fix(self.h, int(on)))

@@ -489,3 +489,77 @@ def test_refine_flags_bit_exact(dim, N, bc):
             assert np.array_equal(ig, io[perm]), (crit, np.abs(ig - io[perm]).max())
             assert np.array_equal(fg, fo[perm])
     lm.close()
+
+
+# ------------------------------------------------------------------ Runge-Kutta schemes of eq. (5)
+RK = [(f4.RK_EULER, "RK_EULER"), (f4.RK_SSP33, "RK_SSP33"), (f4.RK_SSP43, "RK_SSP43"), (f4.RK_RK4, "RK_RK4")]
+
+
+@pytest.mark.parametrize("scheme,name", RK)
+@pytest.mark.parametrize("case", ["config1", "3d16", "amr"])
+def test_rk_schemes_parity(scheme, name, case):
+    nst = f4.RK_STATES[scheme]
+    if case == "config1":
+        cfg, steps, lm, om = W.config(1), 10, None, None
+    elif case == "3d16":
+        cfg, steps = W.config(3, scale=1), 4
+    if case != "amr":
+        lm = f4.Mesh.from_config(cfg, n_states=nst)
+        lm.bind_torch()
+        om = O.OracleMesh.from_config(cfg, n_states=nst)
+        u0, perm = set_both(lm, om, cfg)
+    else:
+        steps = 3
+        cfg = dict(dim=3, block_n=8, n_ghost=2, brick=(2, 2, 2), base_level=0, max_level=2,
+                   bc=[OUT, OUT, PER, PER, OUT, OUT], gamma=1.4)
+        lm = f4.Mesh.from_config(cfg, n_states=nst, max_blocks=600)
+        lm.bind_torch()
+        om = O.OracleMesh.from_config(cfg, n_states=nst)
+        rng = np.random.default_rng(4)
+        for _ in range(2):
+            la, ca = lm.get_blocks()
+            flags = (rng.uniform(size=len(la)) < 0.3).astype(np.int32)
+            flags[0] = 1
+            perm = perm_lib_to_ora(lm, om)
+            fo = np.empty_like(flags)
+            fo[perm] = flags
+            lm.adapt(flags)
+            om.adapt(fo)
+        la, ca = lm.get_blocks()
+        u = _wave_state(dict(cfg, dim=3), la, ca)
+        perm = perm_lib_to_ora(lm, om)
+        uo = np.empty_like(u)
+        uo[perm] = u
+        lm.set_state(0, u)
+        om.set_state(0, uo)
+    lm.set_rk_scheme(scheme)
+    n0 = lm.launch_count()
+    for s in range(steps):
+        dt_o = om.compute_dt(0, 0.4)
+        dt_g = lm.compute_dt(0, 0.4)                  # after the first step: the maximum fused into the last sub-step
+        assert abs(dt_g - dt_o) <= 1e-13 * dt_o, (s, dt_g, dt_o)
+        if scheme == f4.RK_EULER:
+            dt_o *= 0.5                               # forward Euler with a 2nd-order reconstruction: keep it tame
+        om.advance(dt_o, getattr(om, name))
+        lm.advance(dt_o)
+    nl = lm.launch_count() - n0
+    err = H.rel_linf(lm.get_state(0), om.get_state(0)[perm])
+    assert np.all(err <= TOL_STATE), err
+    tg, to = lm.conserved_totals(0), om.totals(0)
+    assert np.all(np.abs(tg - to) <= TOL_TOTALS * np.abs(to).max())
+    if case != "amr":
+        # uniform periodic mesh: one launch per sub-step, plus the first compute_dt's reduction and the first
+        # fill of the freshly set state; afterwards ghosts are pushed and the CFL maximum is fused
+        assert nl == steps * f4.RK_STAGES[scheme] + 2, nl
+    lm.close()
+
+
+def test_rk_scheme_needs_enough_states():
+    lm = f4.Mesh.from_config(W.config(1))            # n_states = 2
+    lm.set_rk_scheme(f4.RK_EULER)
+    for scheme in (f4.RK_SSP33, f4.RK_SSP43, f4.RK_RK4):
+        with pytest.raises(f4.F4Error):
+            lm.set_rk_scheme(scheme)
+    with pytest.raises(f4.F4Error):
+        lm.set_rk_scheme(17)
+    lm.close()

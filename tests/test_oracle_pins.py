@@ -443,6 +443,60 @@ def test_P9_heun_closed_form():
     assert np.allclose(m.get_state(1), 0.1 * lam * u0 + 0.25 * u0 + 0.75 * 2 * u0, rtol=1e-15)
 
 
+@pytest.mark.parametrize("scheme,coef", [
+    ("RK_EULER", [1, 1]), ("RK_HEUN", [1, 1, 1 / 2]), ("RK_SSP33", [1, 1, 1 / 2, 1 / 6]),
+    ("RK_SSP43", [1, 1, 1 / 2, 1 / 6, 1 / 48]), ("RK_RK4", [1, 1, 1 / 2, 1 / 6, 1 / 24])])
+def test_P9_rk_schemes_stability_polynomials(scheme, coef):
+    # eq. (5)-(11) with F(u) = lambda u: one step multiplies u by the scheme's stability polynomial R(z), z = lambda dt
+    # (textbook: Taylor polynomial of the scheme's order; SSPRK(4,3): (1 + z/2)(2/3 + (1 + z/2)^3 / 3)
+    #  = 1 + z + z^2/2 + z^3/6 + z^4/48; RK4 eq. (8)-(11): sum_{k<=4} z^k / k!)
+    m = O.OracleMesh(2, 8, 2, (1, 1), 0, 0, [PER] * 4, 1.4, 4)
+    rng = np.random.default_rng(1)
+    u0 = rng.uniform(1, 2, m.get_state(0).shape)
+    for lam, dt in [(-3.0, 0.05), (0.7, 0.3), (-1.0, 1.0)]:
+        m.set_state(0, u0)
+        m.set_test_rhs(True, lam)
+        m.advance(dt, getattr(m, scheme))
+        z = lam * dt
+        R = sum(c * z ** k for k, c in enumerate(coef))
+        assert np.allclose(m.get_state(0), R * u0, rtol=4e-15, atol=0), scheme
+
+
+@pytest.mark.parametrize("scheme", ["RK_EULER", "RK_SSP33", "RK_SSP43", "RK_RK4"])
+def test_rk_schemes_uniform_state_conservation_and_order(scheme):
+    cfg = W.config(1)
+    # P1: a uniform state is a fixed point of every sub-step, bit for bit
+    m = O.OracleMesh.from_config(cfg, n_states=4)
+    lev, co = m.get_blocks()
+    cu = dict(cfg, ic="uniform", rho0=1.3, vel0=(0.4, -0.2, 0.0), p0=0.9)
+    u = W.initial_state(cu, lev, co)
+    m.set_state(0, u)
+    for _ in range(2):
+        m.advance(1e-2, getattr(m, scheme))
+    assert np.array_equal(m.get_state(0), u)
+    # P2: conservative on a periodic mesh to round-off
+    m.set_state(0, W.initial_state(cfg, lev, co))
+    t0 = m.totals(0)
+    for _ in range(3):
+        m.advance(m.compute_dt(0, 0.4), getattr(m, scheme))
+    assert np.all(np.abs(m.totals(0) - t0) <= 1e-13 * np.abs(t0).max())
+    # temporal order: against a run with dt/8 of the same scheme on the same mesh (the spatial operator is the
+    # same, so the difference is the time-integration error): halving dt divides it by ~2^order
+    order = {"RK_EULER": 1, "RK_SSP33": 3, "RK_SSP43": 3, "RK_RK4": 4}[scheme]
+    u0 = W.initial_state(cfg, lev, co, False)
+    T = 0.04
+    def run(nsteps):
+        m.set_state(0, u0)
+        for _ in range(nsteps):
+            m.advance(T / nsteps, getattr(m, scheme))
+        return m.get_state(0)
+    ref = run(64)
+    e1 = np.abs(run(4) - ref).max()
+    e2 = np.abs(run(8) - ref).max()
+    obs = np.log2(e1 / e2)
+    assert obs > order - 0.6, (scheme, obs, e1, e2)
+
+
 # ---------------------------------------------------------------- P10
 def test_P10_lower_dimensional_data():
     # z-independent 3D data stays z-independent bit-exactly and equals the 2D code to round-off
