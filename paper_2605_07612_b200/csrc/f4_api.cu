@@ -28,11 +28,16 @@ struct f4_mesh {
   int* d_level = nullptr;
   DevRecord* d_r1 = nullptr;
   DevRecord* d_r2 = nullptr;
-  DevRecord* d_r1n = nullptr;  // R1 without the same-level copies (those are pushed by the stage kernel)
+  DevRecord* d_r1n = nullptr;  // R1 without the same-level copies (the stage kernel pushes / gathers those itself)
+  DevRecord* d_r1z = nullptr;  // R1 without the x / y same-level copies: d_r1n plus the z-face same-level copies
   int* d_nbr = nullptr;        // [max_blocks][6] same-level neighbour per face or -1
   size_t cap_r1 = 0, cap_r2 = 0, cap_r1n = 0;
-  int n_r1 = 0, n_r2 = 0, n_r1n = 0;
-  std::vector<char> srl_valid;  // per logical state: same-level face ghosts are up to date (pushed or filled)
+  int n_r1 = 0, n_r2 = 0, n_r1n = 0, n_r1z = 0;
+  size_t cap_r1z = 0;
+  // per logical state, same-level face ghosts: 0 = stale, 1 = x / y faces up to date (pushed by the stage kernel
+  // that produced the state; its z ghost planes were never written because stage kernels fetch them from the
+  // neighbours' interiors), 2 = all faces up to date
+  std::vector<char> srl_valid;
   DevTransfer* d_plan = nullptr;
   size_t cap_plan = 0;
   // flux fixing at refinement boundaries
@@ -121,18 +126,23 @@ int upload_meta(f4_mesh* m) {
     for (size_t q = 0; q < r.size(); ++q)
       out[q] = DevRecord{r[q].dst, r[q].src, r[q].op | r[q].face << 2 | r[q].o1 << 5 | r[q].o2 << 6, 0};
   };
-  std::vector<DevRecord> a, b2, an;
+  std::vector<DevRecord> a, b2, an, az;
   pack(m->hm.r1, a);
   pack(m->hm.r2, b2);
   std::vector<int> nbr((size_t)nb * 6, -1);
   for (const Record& r : m->hm.r1) {
+    const DevRecord dr{r.dst, r.src, r.op | r.face << 2 | r.o1 << 5 | r.o2 << 6, 0};
     if (r.op == F4_OP_SRL) nbr[(size_t)r.dst * 6 + r.face] = r.src;
-    else an.push_back(DevRecord{r.dst, r.src, r.op | r.face << 2 | r.o1 << 5 | r.o2 << 6, 0});
+    else an.push_back(dr);
+    if (r.op != F4_OP_SRL || r.face >= 4) az.push_back(dr);
   }
   int rc;
   if ((rc = ensure(m, m->d_r1, m->cap_r1, a.size()))) return rc;
   if ((rc = ensure(m, m->d_r2, m->cap_r2, b2.size()))) return rc;
   if ((rc = ensure(m, m->d_r1n, m->cap_r1n, an.size()))) return rc;
+  if ((rc = ensure(m, m->d_r1z, m->cap_r1z, az.size()))) return rc;
+  if (!az.empty()) CU(cudaMemcpyAsync(m->d_r1z, az.data(), az.size() * sizeof(DevRecord), cudaMemcpyHostToDevice, m->stream));
+  m->n_r1z = (int)az.size();
   if (!an.empty()) CU(cudaMemcpyAsync(m->d_r1n, an.data(), an.size() * sizeof(DevRecord), cudaMemcpyHostToDevice, m->stream));
   CU(cudaMemcpyAsync(m->d_nbr, nbr.data(), nbr.size() * sizeof(int), cudaMemcpyHostToDevice, m->stream));
   m->n_r1n = (int)an.size();
@@ -186,16 +196,20 @@ int upload_meta(f4_mesh* m) {
   return F4_OK;
 }
 
-// skip_srl: the same-level face ghosts of this state were already pushed by the stage kernel that produced it
-int fill_ghosts_impl(f4_mesh* m, int state, bool skip_srl) {
+// have = srl_valid[state]: which same-level ghosts are already up to date (those records are skipped).
+// need_z: the reader uses same-level z ghost cells (prolongation stencils, refinement criteria, regrid transfer,
+// the caller of f4_fill_ghosts); a stage kernel does not (it fetches those planes from the neighbours' interiors).
+int fill_ghosts_impl(f4_mesh* m, int state, int have, bool need_z) {
   double* st = m->state_ptr(state);
-  const DevRecord* r1 = skip_srl ? m->d_r1n : m->d_r1;
-  const int n1 = skip_srl ? m->n_r1n : m->n_r1;
+  const DevRecord* r1 = m->d_r1;
+  int n1 = m->n_r1, after = 2;
+  if (have == 2 || (have == 1 && (!need_z || m->hm.dim == 2))) { r1 = m->d_r1n; n1 = m->n_r1n; after = have; }
+  else if (have == 1) { r1 = m->d_r1z; n1 = m->n_r1z; }
   if (n1) {
     Scope sc(m, F4_PROF_R1);
     CU(launch_ghost(m->hm.dim, m->hm.N, GhostParams{st, r1, n1, m->theta}, m->stream));
   }
-  m->srl_valid[state] = 1;
+  m->srl_valid[state] = (char)after;
   if (m->n_r2) {
     Scope sc(m, F4_PROF_R2);
     CU(launch_ghost(m->hm.dim, m->hm.N, GhostParams{st, m->d_r2, m->n_r2, m->theta}, m->stream));
@@ -259,6 +273,7 @@ int f4_mesh_destroy(f4_mesh* m) {
   if (m->d_r1) cudaFree(m->d_r1);
   if (m->d_r2) cudaFree(m->d_r2);
   if (m->d_r1n) cudaFree(m->d_r1n);
+  if (m->d_r1z) cudaFree(m->d_r1z);
   if (m->d_nbr) cudaFree(m->d_nbr);
   if (m->d_bfslot) cudaFree(m->d_bfslot);
   if (m->d_fix) cudaFree(m->d_fix);
@@ -425,7 +440,7 @@ int f4_get_pattern(const f4_mesh* m, int* records) {
 int f4_fill_ghosts(f4_mesh* m, int state) {
   int rc = check_state(m, state);
   if (rc) return rc;
-  return fill_ghosts_impl(m, state, false);
+  return fill_ghosts_impl(m, state, 0, true);
 }
 
 int f4_compute_dt(f4_mesh* m, int state, double cfl, double* dt_out) {
@@ -528,7 +543,8 @@ int f4_advance(f4_mesh* m, double dt) {
     const SubStep& ss = sch.sub[q];
     const bool last = (q == sch.n_sub - 1);
     // ghost fill precedes each F evaluation; same-level ghosts of a state a stage produced were pushed
-    if ((rc = fill_ghosts_impl(m, ss.deriv, m->srl_valid[ss.deriv]))) return rc;
+    // (C2F prolongation stencils read the coarse blocks' same-level z ghosts: with such records those are filled too)
+    if ((rc = fill_ghosts_impl(m, ss.deriv, m->srl_valid[ss.deriv], m->n_r2 > 0))) return rc;
     p.deriv = m->state_ptr(ss.deriv);
     p.out = m->state_ptr(ss.out);
     const double* pv[4] = {nullptr, nullptr, nullptr, nullptr};
@@ -554,7 +570,9 @@ int f4_advance(f4_mesh* m, double dt) {
       Scope sc(m, F4_PROF_STAGE);
       CU(launch_fluxfix(dim, N, fp, m->stream));
     }
-    m->srl_valid[ss.out] = ff ? 0 : 1;   // pushed by the stage; BC / F2C / C2F ghosts of `out` are stale until the next fill
+    // x / y same-level ghosts of `out` were pushed by the stage (3D: its z ghost planes were not written);
+    // BC / F2C / C2F ghosts of `out` are stale until the next fill
+    m->srl_valid[ss.out] = ff ? 0 : (dim == 3 ? 1 : 2);
   }
   if (sch.result != 0) std::swap(m->phys[0], m->phys[sch.result]), std::swap(m->srl_valid[0], m->srl_valid[sch.result]);
   m->rate_valid = !ff;
@@ -569,7 +587,7 @@ int f4_refine_flags(f4_mesh* m, int state, int criterion, int var, const double 
   if (criterion != F4_CRIT_LOHNER && criterion != F4_CRIT_PJUMP) return fail(m, F4_EINVAL, "unknown criterion");
   if (criterion == F4_CRIT_LOHNER && (var < 0 || var >= m->nvar)) return fail(m, F4_EINVAL, "variable out of range");
   const int nb = (int)m->hm.leaves.size();
-  if ((rc = fill_ghosts_impl(m, state, m->srl_valid[state]))) return rc;
+  if ((rc = fill_ghosts_impl(m, state, m->srl_valid[state], true))) return rc;
   {
     Scope sc(m, F4_PROF_REGRID);
     CU(launch_flags(m->hm.dim, m->hm.N, m->state_ptr(state), nb, criterion, var, m->gamma, params, m->d_flags,
@@ -586,7 +604,7 @@ int f4_adapt(f4_mesh* m, const int* refine_flags, int* changed_out) {
   if (!m || !refine_flags || !changed_out) return F4_EINVAL;
   *changed_out = 0;
   int rc;
-  if (m->bound && (rc = fill_ghosts_impl(m, 0, m->srl_valid[0]))) return rc;  // prolongation reads the parents' face ghosts
+  if (m->bound && (rc = fill_ghosts_impl(m, 0, m->srl_valid[0], true))) return rc;  // prolongation reads the parents' face ghosts
   std::vector<Transfer> plan;
   bool changed = false;
   std::string err;

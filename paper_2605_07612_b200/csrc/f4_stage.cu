@@ -313,12 +313,20 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
   }
   group_sync(bar_id, TGA);
 
+  // Same-level z neighbours (fused ghost handling, a1 of the pattern): their interior planes ARE this block's z
+  // ghost planes, so the march fetches planes -2,-1 / N,N+1 straight from the neighbour
+  // block instead of from ghost cells somebody would have to write first.  -1: no same-level neighbour (physical
+  // boundary, coarser or finer block): the block's own ghost planes, filled by the pattern executor, are read.
+  int gz0 = -1, gz1 = -1;
+  if (DIM == 3 && p.nbr && !(F4_ABL & 32)) { gz0 = p.nbr[(size_t)blk * 6 + 4]; gz1 = p.nbr[(size_t)blk * 6 + 5]; }
   // issue the bulk copies of z plane c (c in [-2, N+2); 2D: c = 0) into ring slot s
   auto issue_plane = [&](int c, int s) {
     const bool interior = (DIM == 2) || (c >= 0 && c < N);
     const int kslot = (DIM == 3) ? (c < 0 ? c + P : c) : 0;
     const uint32_t dst = ring_u32 + (uint32_t)(s * C::SLOT) * 8u, bar = bars_u32 + 8u * s;
     const double* src = dbase + (size_t)kslot * PP;
+    if (DIM == 3 && c < 0 && gz0 >= 0) src = p.deriv + (size_t)gz0 * C::BS + (size_t)(c + N) * PP;   // its planes N-2, N-1
+    if (DIM == 3 && c >= N && gz1 >= 0) src = p.deriv + (size_t)gz1 * C::BS + (size_t)(c - N) * PP;  // its planes 0, 1
     if (WHOLE) {
       // interior plane: all P slot rows (N interior, 2 high, 2 low ghost rows); z-ghost plane: the N interior rows
       const uint32_t bytes = (uint32_t)(interior ? P : N) * P * 8;
@@ -552,15 +560,13 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
   // (a1 of the pattern).  nbr[f] = same-level neighbour across face f, or -1.
   double* ppx = nullptr;   // x / y push targets of this thread (k = 0, var 0)
   double* ppy = nullptr;
-  int nbz0 = -1, nbz1 = -1;
   if (p.nbr && !(F4_ABL & 4)) {
     const int* nb = p.nbr + (size_t)blk * 6;
     const int jg = j0 + j;
-    if (i < NG && nb[0] >= 0) ppx = p.out + (size_t)nb[0] * C::BS + ((jg & ~1) * P + N + 2 * (jg & 1) + i);
-    if (i >= N - NG && nb[1] >= 0) ppx = p.out + (size_t)nb[1] * C::BS + ((jg | 1) * P + N + 2 * (jg & 1) + (i - (N - NG)));
-    if (jg < NG && nb[2] >= 0) ppy = p.out + (size_t)nb[2] * C::BS + ((N + jg) * P + i);
-    if (jg >= N - NG && nb[3] >= 0) ppy = p.out + (size_t)nb[3] * C::BS + ((jg + 2 * NG) * P + i);
-    if (DIM == 3) { nbz0 = nb[4]; nbz1 = nb[5]; }
+    if (!(F4_ABL & 8) && i < NG && nb[0] >= 0) ppx = p.out + (size_t)nb[0] * C::BS + ((jg & ~1) * P + N + 2 * (jg & 1) + i);
+    if (!(F4_ABL & 8) && i >= N - NG && nb[1] >= 0) ppx = p.out + (size_t)nb[1] * C::BS + ((jg | 1) * P + N + 2 * (jg & 1) + (i - (N - NG)));
+    if (!(F4_ABL & 16) && jg < NG && nb[2] >= 0) ppy = p.out + (size_t)nb[2] * C::BS + ((N + jg) * P + i);
+    if (!(F4_ABL & 16) && jg >= N - NG && nb[3] >= 0) ppy = p.out + (size_t)nb[3] * C::BS + ((jg + 2 * NG) * P + i);
   }
   // general instances (BF): up to four previous states in eq. (5) (classical RK4, eq. (11));
   // the third and fourth are folded into b: b <- b + (w2 c + w3 d) / w1 is avoided by carrying w1 b + w2 c + w3 d
@@ -598,14 +604,6 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
     if (ppy) {
 #pragma unroll
       for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) ppy[ko + pl(q) * (int)C::VS] = u[q];
-    }
-    if (DIM == 3 && (k < NG || k >= N - NG)) {
-      const int nbz = (k < NG) ? nbz0 : nbz1;
-      if (nbz >= 0) {
-        double* pz = p.out + (size_t)nbz * C::BS + (size_t)(k < NG ? N + k : k + 2 * NG) * PP + co;
-#pragma unroll
-        for (int q = 0; q < 5; ++q) pz[pl(q) * (int)C::VS] = u[q];
-      }
     }
     if (p.maxrate) {
       const double ir = rcp_fast(u[0]);

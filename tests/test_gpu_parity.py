@@ -384,8 +384,28 @@ def test_fused_srl_push_equals_pattern_fill(n, scale):
     lm.fill_ghosts(0)                       # full pattern: SRL records included
     filled = lm.get_state(0, with_ghosts=True)
     nc = noncorner_mask(lm)
+    if lm.dim == 3:
+        # z ghost planes are not written by a stage (the next stage fetches them from the neighbours' interiors):
+        # compare the x / y face ghosts and the interior only
+        nc = nc.copy()
+        nc[:, :2] = False
+        nc[:, -2:] = False
     for v in range(lm.nvar):
         assert np.array_equal(pushed[:, v][nc], filled[:, v][nc])
+    # the gathered z planes are the same data the executor would have copied: a step from the ghost-filled state
+    # and a step from the pushed-only state give identical bits
+    a = lm.get_state(0)
+    lm.set_state(0, a)                      # marks every ghost stale: the next advance runs the full pattern first
+    dt = lm.compute_dt(0, 0.4)
+    lm.advance(dt)
+    full = lm.get_state(0)
+    lm.set_state(0, a)
+    lm.advance(dt)
+    lm.advance(dt)                          # second step starts from pushed x / y ghosts + gathered z planes
+    two = lm.get_state(0)
+    lm.set_state(0, full)
+    lm.advance(dt)
+    assert np.array_equal(lm.get_state(0), two)
     lm.close()
 
 
