@@ -362,16 +362,17 @@ def main():
         return
     # ---- roofline of the dominant kernel (fused stage kernel), algorithmic bytes
     peak, peak_src, sm_max = peaks()
-    # per cell update: read s_deriv interior + face halo (bpc*r), write s_out interior + pushed face layers (bpc*r),
-    # extra s_prev read in the second Heun stage (bpc/2 on average); the same-level ghost copy is fused into the
-    # stage kernel, so on a uniform mesh there is no separate ghost-fill traffic.
+    # per cell update: read s_deriv interior + face halo (bpc*r: the y / z halo straight from the neighbours'
+    # interiors), write s_out interior + the x face layers pushed into the neighbours' ghost cells
+    # (bpc*(1 + 2*Ng/N)), extra s_prev reads (bpc/2 on average for Heun); the same-level ghost copy is fused into
+    # the stage kernel, so on a uniform mesh there is no separate ghost-fill traffic.
     r = 1.0 + 2.0 * d * 2 / n
     bpc = 8 * (d + 2)
     st_ms, st_n = prof["stage"]
     cells_per_launch = updates / max(st_n, 1)            # = cells on a static mesh; the average on an adaptive one
     # previous states other than s_deriv read per sub-step, averaged over the scheme's sub-steps (Heun: 0 and 1)
     extra_prev = {"heun": 0.5, "euler": 0.0, "ssp33": 2.0 / 3.0, "ssp43": 0.25, "rk4": 1.25}[args.rk]
-    stage_bytes = cells_per_launch * (2.0 * bpc * r + extra_prev * bpc)
+    stage_bytes = cells_per_launch * (bpc * r + bpc * (1.0 + 2.0 * 2 / n) + extra_prev * bpc)
     g_n = prof["ghost_r1"][1] + prof["ghost_r2"][1]
     g_ms = prof["ghost_r1"][0] + prof["ghost_r2"][0]
     stage_gbs = stage_bytes / (st_ms / max(st_n, 1) * 1e-3) / 1e9 if st_ms > 0 else None

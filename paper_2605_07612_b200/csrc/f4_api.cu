@@ -29,14 +29,14 @@ struct f4_mesh {
   DevRecord* d_r1 = nullptr;
   DevRecord* d_r2 = nullptr;
   DevRecord* d_r1n = nullptr;  // R1 without the same-level copies (the stage kernel pushes / gathers those itself)
-  DevRecord* d_r1z = nullptr;  // R1 without the x / y same-level copies: d_r1n plus the z-face same-level copies
+  DevRecord* d_r1z = nullptr;  // R1 without the x same-level copies: d_r1n plus the y- and z-face same-level copies
   int* d_nbr = nullptr;        // [max_blocks][6] same-level neighbour per face or -1
   size_t cap_r1 = 0, cap_r2 = 0, cap_r1n = 0;
   int n_r1 = 0, n_r2 = 0, n_r1n = 0, n_r1z = 0;
   size_t cap_r1z = 0;
-  // per logical state, same-level face ghosts: 0 = stale, 1 = x / y faces up to date (pushed by the stage kernel
-  // that produced the state; its z ghost planes were never written because stage kernels fetch them from the
-  // neighbours' interiors), 2 = all faces up to date
+  // per logical state, same-level face ghosts: 0 = stale, 1 = x faces up to date (pushed by the stage kernel that
+  // produced the state; its y ghost rows and z ghost planes were never written because stage kernels fetch them
+  // from the neighbours' interiors), 2 = all faces up to date
   std::vector<char> srl_valid;
   DevTransfer* d_plan = nullptr;
   size_t cap_plan = 0;
@@ -134,7 +134,7 @@ int upload_meta(f4_mesh* m) {
     const DevRecord dr{r.dst, r.src, r.op | r.face << 2 | r.o1 << 5 | r.o2 << 6, 0};
     if (r.op == F4_OP_SRL) nbr[(size_t)r.dst * 6 + r.face] = r.src;
     else an.push_back(dr);
-    if (r.op != F4_OP_SRL || r.face >= 4) az.push_back(dr);
+    if (r.op != F4_OP_SRL || r.face >= 2) az.push_back(dr);
   }
   int rc;
   if ((rc = ensure(m, m->d_r1, m->cap_r1, a.size()))) return rc;
@@ -197,13 +197,13 @@ int upload_meta(f4_mesh* m) {
 }
 
 // have = srl_valid[state]: which same-level ghosts are already up to date (those records are skipped).
-// need_z: the reader uses same-level z ghost cells (prolongation stencils, refinement criteria, regrid transfer,
-// the caller of f4_fill_ghosts); a stage kernel does not (it fetches those planes from the neighbours' interiors).
+// need_z: the reader uses same-level y / z ghost cells (prolongation stencils, refinement criteria, regrid transfer,
+// the caller of f4_fill_ghosts); a stage kernel does not (it fetches those rows / planes from the neighbours' interiors).
 int fill_ghosts_impl(f4_mesh* m, int state, int have, bool need_z) {
   double* st = m->state_ptr(state);
   const DevRecord* r1 = m->d_r1;
   int n1 = m->n_r1, after = 2;
-  if (have == 2 || (have == 1 && (!need_z || m->hm.dim == 2))) { r1 = m->d_r1n; n1 = m->n_r1n; after = have; }
+  if (have == 2 || (have == 1 && !need_z)) { r1 = m->d_r1n; n1 = m->n_r1n; after = have; }
   else if (have == 1) { r1 = m->d_r1z; n1 = m->n_r1z; }
   if (n1) {
     Scope sc(m, F4_PROF_R1);
@@ -543,7 +543,7 @@ int f4_advance(f4_mesh* m, double dt) {
     const SubStep& ss = sch.sub[q];
     const bool last = (q == sch.n_sub - 1);
     // ghost fill precedes each F evaluation; same-level ghosts of a state a stage produced were pushed
-    // (C2F prolongation stencils read the coarse blocks' same-level z ghosts: with such records those are filled too)
+    // (C2F prolongation stencils read the coarse blocks' same-level y / z ghosts: with such records those are filled too)
     if ((rc = fill_ghosts_impl(m, ss.deriv, m->srl_valid[ss.deriv], m->n_r2 > 0))) return rc;
     p.deriv = m->state_ptr(ss.deriv);
     p.out = m->state_ptr(ss.out);
@@ -570,9 +570,9 @@ int f4_advance(f4_mesh* m, double dt) {
       Scope sc(m, F4_PROF_STAGE);
       CU(launch_fluxfix(dim, N, fp, m->stream));
     }
-    // x / y same-level ghosts of `out` were pushed by the stage (3D: its z ghost planes were not written);
+    // x same-level ghosts of `out` were pushed by the stage (its y ghost rows / z ghost planes were not written);
     // BC / F2C / C2F ghosts of `out` are stale until the next fill
-    m->srl_valid[ss.out] = ff ? 0 : (dim == 3 ? 1 : 2);
+    m->srl_valid[ss.out] = ff ? 0 : 1;
   }
   if (sch.result != 0) std::swap(m->phys[0], m->phys[sch.result]), std::swap(m->srl_valid[0], m->srl_valid[sch.result]);
   m->rate_valid = !ff;

@@ -317,8 +317,14 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
   // ghost planes, so the march fetches planes -2,-1 / N,N+1 straight from the neighbour
   // block instead of from ghost cells somebody would have to write first.  -1: no same-level neighbour (physical
   // boundary, coarser or finer block): the block's own ghost planes, filled by the pattern executor, are read.
-  int gz0 = -1, gz1 = -1;
+  // The same holds for the y ghost rows of an interior plane: rows N, N+1 are rows 0, 1 of the +y neighbour's
+  // plane, rows -2, -1 are rows N-2, N-1 of the -y neighbour's (two more bulk copies per variable and plane).
+  int gz0 = -1, gz1 = -1, gy0 = -1, gy1 = -1;
   if (DIM == 3 && p.nbr && !(F4_ABL & 32)) { gz0 = p.nbr[(size_t)blk * 6 + 4]; gz1 = p.nbr[(size_t)blk * 6 + 5]; }
+  if (p.nbr && !(F4_ABL & 16)) { gy0 = p.nbr[(size_t)blk * 6 + 2]; gy1 = p.nbr[(size_t)blk * 6 + 3]; }
+  // rows -2,-1 (slots P-2, P-1) and N, N+1 (slots N, N+1) of interior plane kslot: own ghost rows or the neighbours' rows
+  const double* ylo_base = (gy0 >= 0) ? p.deriv + (size_t)gy0 * C::BS + (size_t)(N - 2) * P : dbase + (size_t)(P - 2) * P;
+  const double* yhi_base = (gy1 >= 0) ? p.deriv + (size_t)gy1 * C::BS : dbase + (size_t)N * P;
   // issue the bulk copies of z plane c (c in [-2, N+2); 2D: c = 0) into ring slot s
   auto issue_plane = [&](int c, int s) {
     const bool interior = (DIM == 2) || (c >= 0 && c < N);
@@ -329,21 +335,33 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
     if (DIM == 3 && c >= N && gz1 >= 0) src = p.deriv + (size_t)gz1 * C::BS + (size_t)(c - N) * PP;  // its planes 0, 1
     if (WHOLE) {
       // interior plane: all P slot rows (N interior, 2 high, 2 low ghost rows); z-ghost plane: the N interior rows
-      const uint32_t bytes = (uint32_t)(interior ? P : N) * P * 8;
-      mbar_expect_tx(bar, bytes * NV);
+      constexpr uint32_t bytes = (uint32_t)N * P * 8, gbytes = (uint32_t)2 * P * 8;
+      mbar_expect_tx(bar, (bytes + (interior ? 2 * gbytes : 0u)) * NV);
 #pragma unroll
       for (int v = 0; v < NV; ++v) bulk_g2s(dst + (uint32_t)(v * PLANE) * 8u, src + (size_t)v * C::VS, bytes, bar);
+      if (interior) {
+        const size_t ko = (size_t)kslot * PP;
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+          bulk_g2s(dst + (uint32_t)(v * PLANE + N * P) * 8u, yhi_base + ko + (size_t)v * C::VS, gbytes, bar);
+          bulk_g2s(dst + (uint32_t)(v * PLANE + (P - 2) * P) * 8u, ylo_base + ko + (size_t)v * C::VS, gbytes, bar);
+        }
+      }
     } else {
       // rows y in [ylo, yhi) -> smem rows y - (j0-2); rows with y < 0 live in slots y + P
       const int ylo = interior ? j0 - 2 : j0, yhi = interior ? j0 + TY + 2 : j0 + TY;
-      const int nlow = ylo < 0 ? -ylo : 0;
-      const uint32_t bytes_low = (uint32_t)nlow * P * 8, bytes_hi = (uint32_t)(yhi - ylo - nlow) * P * 8;
-      mbar_expect_tx(bar, (bytes_low + bytes_hi) * NV);
+      const int nlow = ylo < 0 ? -ylo : 0, nhigh = yhi > N ? yhi - N : 0;
+      const uint32_t bytes_low = (uint32_t)nlow * P * 8, bytes_high = (uint32_t)nhigh * P * 8;
+      const uint32_t bytes_mid = (uint32_t)(yhi - ylo - nlow - nhigh) * P * 8;
+      mbar_expect_tx(bar, (bytes_low + bytes_mid + bytes_high) * NV);
+      const size_t ko = (size_t)kslot * PP;
       for (int v = 0; v < NV; ++v) {
         const double* sv = src + (size_t)v * C::VS;
         const uint32_t dv = dst + (uint32_t)(v * PLANE) * 8u;
-        if (nlow) bulk_g2s(dv + (uint32_t)((ylo - (j0 - 2)) * P) * 8u, sv + (size_t)(ylo + P) * P, bytes_low, bar);
-        bulk_g2s(dv + (uint32_t)((ylo + nlow - (j0 - 2)) * P) * 8u, sv + (size_t)(ylo + nlow) * P, bytes_hi, bar);
+        // rows y < 0 and y >= N exist only in interior planes of the first / last tile (ghost rows, see above)
+        if (nlow) bulk_g2s(dv + (uint32_t)((ylo - (j0 - 2)) * P) * 8u, ylo_base + ko + (size_t)v * C::VS, bytes_low, bar);
+        bulk_g2s(dv + (uint32_t)((ylo + nlow - (j0 - 2)) * P) * 8u, sv + (size_t)(ylo + nlow) * P, bytes_mid, bar);
+        if (nhigh) bulk_g2s(dv + (uint32_t)((N - (j0 - 2)) * P) * 8u, yhi_base + ko + (size_t)v * C::VS, bytes_high, bar);
       }
     }
   };
@@ -558,15 +576,12 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
   double* po = p.out + boff + co;
   // fused same-level ghost fill: boundary layers are pushed from registers into the neighbours' ghost cells
   // (a1 of the pattern).  nbr[f] = same-level neighbour across face f, or -1.
-  double* ppx = nullptr;   // x / y push targets of this thread (k = 0, var 0)
-  double* ppy = nullptr;
+  double* ppx = nullptr;   // x push target of this thread (k = 0, var 0); y and z ghosts are gathered by the reader
   if (p.nbr && !(F4_ABL & 4)) {
     const int* nb = p.nbr + (size_t)blk * 6;
     const int jg = j0 + j;
     if (!(F4_ABL & 8) && i < NG && nb[0] >= 0) ppx = p.out + (size_t)nb[0] * C::BS + ((jg & ~1) * P + N + 2 * (jg & 1) + i);
     if (!(F4_ABL & 8) && i >= N - NG && nb[1] >= 0) ppx = p.out + (size_t)nb[1] * C::BS + ((jg | 1) * P + N + 2 * (jg & 1) + (i - (N - NG)));
-    if (!(F4_ABL & 16) && jg < NG && nb[2] >= 0) ppy = p.out + (size_t)nb[2] * C::BS + ((N + jg) * P + i);
-    if (!(F4_ABL & 16) && jg >= N - NG && nb[3] >= 0) ppy = p.out + (size_t)nb[3] * C::BS + ((jg + 2 * NG) * P + i);
   }
   // general instances (BF): up to four previous states in eq. (5) (classical RK4, eq. (11));
   // the third and fourth are folded into b: b <- b + (w2 c + w3 d) / w1 is avoided by carrying w1 b + w2 c + w3 d
@@ -601,10 +616,6 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
 #pragma unroll
       for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) ppx[ko + pl(q) * (int)C::VS] = u[q];
     }
-    if (ppy) {
-#pragma unroll
-      for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) ppy[ko + pl(q) * (int)C::VS] = u[q];
-    }
     if (p.maxrate) {
       const double ir = rcp_fast(u[0]);
       double ke = 0.0, su = 0.0;
@@ -623,7 +634,8 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
     if (is_hc) halo_convert_task(W, th);
   };
 
-  if (DIM == 3 && t == 0) { issue_plane(-2, 0); issue_plane(-1, 1); }
+  constexpr int ISSUER = (TG >= 128) ? 96 : 0;   // lane 0 of a warp without halo roles when the group has one
+  if (DIM == 3 && t == ISSUER) { issue_plane(-2, 0); issue_plane(-1, 1); }
   if (HW == 1 && t >= TG) {
     // ---- helper warp (3D): mirrors the barrier sequence of the march below.  Per plane: convert the halo cells of
     //      plane c, halo slopes of plane c-1 | barrier | last-face fluxes | barrier | refill the freed ring slot.
@@ -666,7 +678,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
 
   if (DIM == 2) {
     double a[5], b[5], w[5], acc[5];
-    if (t == 0) issue_plane(0, 0);
+    if (t == ISSUER) issue_plane(0, 0);
     load_prev(0, a, b);
     mbar_wait(bars_u32, 0);
     convert(ring, own, w);
@@ -742,7 +754,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
         group_sync(bar_id, TGA);
       }
       // every thread is past its last read of plane c-1: refill that slot with plane c+2
-      if (HW == 0 && t == 0 && c + 2 <= N + 1) issue_plane(c + 2, sk);
+      if (HW == 0 && t == ISSUER && c + 2 <= N + 1) issue_plane(c + 2, sk);
       sc = (sc == 2) ? 0 : sc + 1;
     };
     using T = std::true_type;

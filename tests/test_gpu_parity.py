@@ -384,10 +384,12 @@ def test_fused_srl_push_equals_pattern_fill(n, scale):
     lm.fill_ghosts(0)                       # full pattern: SRL records included
     filled = lm.get_state(0, with_ghosts=True)
     nc = noncorner_mask(lm)
+    # y ghost rows and z ghost planes are not written by a stage (the next stage fetches them from the neighbours'
+    # interiors): compare the x face ghosts and the interior only
+    nc = nc.copy()
+    nc[:, :, :2] = False
+    nc[:, :, -2:] = False
     if lm.dim == 3:
-        # z ghost planes are not written by a stage (the next stage fetches them from the neighbours' interiors):
-        # compare the x / y face ghosts and the interior only
-        nc = nc.copy()
         nc[:, :2] = False
         nc[:, -2:] = False
     for v in range(lm.nvar):
