@@ -159,6 +159,11 @@ int f4_fill_ghosts(f4_mesh *m, int state);
  * reduction kernel runs.  Synchronises to read one double back. */
 int f4_compute_dt(f4_mesh *m, int state, double cfl, double *dt_out);
 
+/* Gravitational acceleration g[3] of the source term S = (0, rho g, rho g.u), eq. (20), evaluated
+ * from the primitives of s_deriv in each cell and added to the flux divergence in every sub-step (PAPER.md:334 step i).
+ * Default (0,0,0): no source term, the path every BASELINE config times.  Components beyond `dim` are ignored. */
+int f4_set_gravity(f4_mesh *m, const double g[3]);
+
 /* Select the time integrator used by f4_advance (F4_RK_*).  Every sub-step is one launch of the fused stage kernel
  * in the form of eq. (5), u(s_out) = dt_sub F(u(s_deriv)) + sum_i w_i u(s_prev,i), n_prev <= 4, preceded by the ghost
  * fill of s_deriv; the CFL maximum of the new state is fused into the last sub-step.  GCUPS counts one

@@ -69,6 +69,7 @@ struct Mesh {
   int dim, N, Ng, P, Pz, nvar;
   int brick[3], base_level, max_level, bc[6];
   double gamma, theta;
+  double grav[3] = {0.0, 0.0, 0.0};  // gravitational acceleration g of the source term eq. (20)
   int limiter, flux_scheme;
   int nstates;
   bool test_rhs = false;  // P9 pin: F(u) = lambda*u
@@ -423,7 +424,18 @@ int forward_euler(Mesh& m, int s_out, int s_deriv, double dt_sub, int n_prev, co
     for (int k = 1; k <= kmax; ++k)
       for (int j = 1; j <= N; ++j)
         for (int i = 1; i <= N; ++i) {
-          double Lu[5] = {0, 0, 0, 0, 0};  // i. source term S = 0 for all configs
+          // i. source term ("get_source: compute the source term from primitive variables in one
+          //    cell"): gravity, eq. (20): S = (0, rho g, rho g.u); zero for the BASELINE configs
+          double Lu[5] = {0, 0, 0, 0, 0};
+          if (!m.test_rhs) {
+            const Prim& w0 = W(i, j, k);
+            double gu = 0.0;
+            for (int a = 0; a < dim; ++a) {
+              Lu[1 + a] = w0.rho * m.grav[a];
+              gu = gu + m.grav[a] * w0.u[a];
+            }
+            Lu[nvar - 1] = w0.rho * gu;
+          }
           if (m.test_rhs) {
             for (int v = 0; v < nvar; ++v) Lu[v] = m.test_lambda * m.at(s_deriv, b, v, i, j, k);
           } else {
@@ -826,6 +838,7 @@ void ora_set_options(void* h, int limiter, int flux_scheme, double theta) {
   Mesh* m = (Mesh*)h; m->limiter = limiter; m->flux_scheme = flux_scheme; m->theta = theta;
 }
 void ora_set_flux_fix(void* h, int on) { ((Mesh*)h)->flux_fix = on != 0; }
+void ora_set_gravity(void* h, const double* g) { for (int a = 0; a < 3; ++a) ((Mesh*)h)->grav[a] = g[a]; }
 void ora_set_test_rhs(void* h, int on, double lambda) { Mesh* m = (Mesh*)h; m->test_rhs = on; m->test_lambda = lambda; }
 int ora_num_blocks(void* h) { return (int)((Mesh*)h)->blocks.size(); }
 void ora_get_blocks(void* h, int* level, int* coords) {

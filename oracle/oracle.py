@@ -45,6 +45,7 @@ def lib():
         L.ora_set_options.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double]
         L.ora_set_test_rhs.argtypes = [C.c_void_p, C.c_int, C.c_double]
         L.ora_set_flux_fix.argtypes = [C.c_void_p, C.c_int]
+        L.ora_set_gravity.argtypes = [C.c_void_p, dp]
         L.ora_num_blocks.argtypes = [C.c_void_p]
         L.ora_get_blocks.argtypes = [C.c_void_p, ip, ip]
         L.ora_dx.restype = C.c_double
@@ -119,6 +120,12 @@ class OracleMesh:
 
     def set_options(self, limiter=LIM_VANLEER, flux=FLUX_HLL, theta=1.0):
         self.L.ora_set_options(self.h, limiter, flux, theta)
+
+    def set_gravity(self, g):
+        """Gravitational acceleration of the source term eq. (20); (0,0,0) = no source."""
+        gg = np.zeros(3, dtype=np.float64)
+        gg[:len(g)] = g
+        self.L.ora_set_gravity(self.h, _dp(gg))
 
     def set_flux_fix(self, on=True):
         """Conservative flux correction at refinement boundaries."""

@@ -17,6 +17,7 @@ struct f4_mesh {
   double gamma = 1.4, theta = 1.0;
   int limiter = F4_LIM_VANLEER, flux = F4_FLUX_HLL;
   int rk = F4_RK_HEUN;
+  double grav[3] = {0.0, 0.0, 0.0};
   int n_states = 2;
   int nvar = 5;
   size_t vs = 0, bs = 0, state_doubles = 0;  // doubles per (block,var), per block, per state
@@ -506,6 +507,15 @@ const Scheme& scheme_table(int rk) {
 
 }  // namespace
 
+int f4_set_gravity(f4_mesh* m, const double g[3]) {
+  if (!m || !g) return F4_EINVAL;
+  for (int a = 0; a < 3; ++a) {
+    if (g[a] != g[a]) return fail(m, F4_EINVAL, "gravity is not a number");
+    m->grav[a] = (a < m->hm.dim) ? g[a] : 0.0;
+  }
+  return F4_OK;
+}
+
 int f4_set_rk_scheme(f4_mesh* m, int scheme) {
   if (!m) return F4_EINVAL;
   if (scheme < 0 || scheme >= F4_RK_N) return fail(m, F4_EINVAL, "unknown Runge-Kutta scheme");
@@ -528,6 +538,8 @@ int f4_advance(f4_mesh* m, double dt) {
   p.nblocks = nb;
   p.limiter = m->limiter;
   p.flux = m->flux;
+  for (int a = 0; a < 3; ++a) p.grav[a] = m->grav[a];
+  p.has_grav = (m->grav[0] != 0.0 || m->grav[1] != 0.0 || m->grav[2] != 0.0) ? 1 : 0;
   // flux fixing acts only where the mesh has refinement boundaries.  The corrected cells must be
   // what the neighbours see, so the same-level copy is then left to the pattern executor (no fused push) and the
   // CFL maximum to the standalone reduction (the stage kernel would take it before the correction).

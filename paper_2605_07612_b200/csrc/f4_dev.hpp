@@ -42,6 +42,9 @@ struct StageParams {
   // computation" into bflux[slot][var][t2][t1]; bfslot[blk][6] = slot of that block face or -1; nullptr = off
   const int* bfslot;
   double* bflux;
+  // gravity source term S = (0, rho g, rho g.u), eq. (20) PAPER.md:429-431 (general instances)
+  double grav[3];
+  int has_grav;
 };
 
 // one coarse block with at least one finer face neighbour (flux fixing)

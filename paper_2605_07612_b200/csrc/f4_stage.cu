@@ -3,7 +3,9 @@
 // over every block, F = -div of HLL fluxes of
 // limited primitive reconstructions, optional
 // fused CFL max of the NEW state, fused same-level ghost copy
-// of the new state into the neighbours' ghost cells.
+// (PAPER.md:195, 235-238): y ghost rows and z ghost planes of s_deriv are fetched
+// from the same-level neighbours' interior cells, the x face layers of the new
+// state are pushed into the neighbours' x ghost cells.
 //
 // Design (differs from the paper's gang-per-block / collapse(3) OpenACC loop,
 // PAPER.md:162-189, which converts the whole block to uu_prim in global
@@ -15,7 +17,8 @@
 //    shared-memory ring one plane ahead of use, and converted to primitives in
 //    place (to_primitive once per cell); when the tile is the
 //    whole block the smem plane keeps the store's wrapped row order, so one
-//    bulk copy per variable moves a plane;
+//    bulk copy per variable moves the interior rows of a plane and two more
+//    bring the ghost rows (from the +-y neighbours when they are same-level);
 //  * x/y fluxes exchange reconstructed states and fluxes through shared
 //    memory; the z direction lives in registers along the march;
 //  * fp64 division / sqrt are replaced by MUFU seeds + cubic Newton steps, and
@@ -177,34 +180,36 @@ __device__ __forceinline__ void riemann_flux(const double (&L)[5], const double 
 // Two independent HLL fluxes (van Leer/HLL fast path) written step by step across both faces, so that the
 // rsqrt -> rcp -> rsqrt dependency chains of the two Riemann problems overlap (the kernel is bound by
 // dependent-issue latency, not by instruction count).  Same arithmetic as riemann_flux<DIM, true>.
-template <int DIM>
-__device__ __forceinline__ void riemann_flux2(const double (&L)[2][5], const double (&R)[2][5], double gamma,
-                                              double ig1, double (&F)[2][5]) {
-  double x[4] = {L[0][0], R[0][0], L[1][0], R[1][0]}, y[4];
+template <int DIM, int NF>
+__device__ __forceinline__ void riemann_fluxN(const double (&L)[NF][5], const double (&R)[NF][5], double gamma,
+                                              double ig1, double (&F)[NF][5]) {
+  double x[2 * NF], y[2 * NF];
 #pragma unroll
-  for (int q = 0; q < 4; ++q) asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y[q]) : "d"(x[q]));
+  for (int f = 0; f < NF; ++f) { x[2 * f] = L[f][0]; x[2 * f + 1] = R[f][0]; }
+#pragma unroll
+  for (int q = 0; q < 2 * NF; ++q) asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y[q]) : "d"(x[q]));
   {
-    double e[4];
+    double e[2 * NF];
 #pragma unroll
-    for (int q = 0; q < 4; ++q) e[q] = fma(-(x[q] * y[q]), y[q], 1.0);
+    for (int q = 0; q < 2 * NF; ++q) e[q] = fma(-(x[q] * y[q]), y[q], 1.0);
 #pragma unroll
-    for (int q = 0; q < 4; ++q) y[q] = fma(y[q], fma(0.375, e[q], 0.5) * e[q], y[q]);   // 1/sqrt(rho)
+    for (int q = 0; q < 2 * NF; ++q) y[q] = fma(y[q], fma(0.375, e[q], 0.5) * e[q], y[q]);   // 1/sqrt(rho)
   }
-  double rL[2], rR[2], w[2], sum[2];
+  double rL[NF], rR[NF], w[NF], sum[NF];
 #pragma unroll
-  for (int f = 0; f < 2; ++f) { rL[f] = x[2 * f] * y[2 * f]; rR[f] = x[2 * f + 1] * y[2 * f + 1]; sum[f] = rL[f] + rR[f]; }
+  for (int f = 0; f < NF; ++f) { rL[f] = x[2 * f] * y[2 * f]; rR[f] = x[2 * f + 1] * y[2 * f + 1]; sum[f] = rL[f] + rR[f]; }
 #pragma unroll
-  for (int f = 0; f < 2; ++f) asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(w[f]) : "d"(sum[f]));
+  for (int f = 0; f < NF; ++f) asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(w[f]) : "d"(sum[f]));
   {
-    double e[2];
+    double e[NF];
 #pragma unroll
-    for (int f = 0; f < 2; ++f) e[f] = fma(-sum[f], w[f], 1.0);
+    for (int f = 0; f < NF; ++f) e[f] = fma(-sum[f], w[f], 1.0);
 #pragma unroll
-    for (int f = 0; f < 2; ++f) w[f] = fma(w[f], fma(e[f], e[f], e[f]), w[f]);
+    for (int f = 0; f < NF; ++f) w[f] = fma(w[f], fma(e[f], e[f], e[f]), w[f]);
   }
-  double wl[2], wr[2], uhat[2], d2[2], y2[2];
+  double wl[NF], wr[NF], uhat[NF], d2[NF], y2[NF];
 #pragma unroll
-  for (int f = 0; f < 2; ++f) {
+  for (int f = 0; f < NF; ++f) {
     wl[f] = rL[f] * w[f];
     wr[f] = rR[f] * w[f];
     uhat[f] = fma(wl[f], L[f][1], wr[f] * R[f][1]);
@@ -212,16 +217,16 @@ __device__ __forceinline__ void riemann_flux2(const double (&L)[2][5], const dou
     d2[f] = fma((0.5 * wl[f]) * wr[f], du * du, fma(L[f][4], y[2 * f], R[f][4] * y[2 * f + 1]) * (gamma * w[f]));
   }
 #pragma unroll
-  for (int f = 0; f < 2; ++f) asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y2[f]) : "d"(d2[f]));
+  for (int f = 0; f < NF; ++f) asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y2[f]) : "d"(d2[f]));
   {
-    double e[2];
+    double e[NF];
 #pragma unroll
-    for (int f = 0; f < 2; ++f) e[f] = fma(-(d2[f] * y2[f]), y2[f], 1.0);
+    for (int f = 0; f < NF; ++f) e[f] = fma(-(d2[f] * y2[f]), y2[f], 1.0);
 #pragma unroll
-    for (int f = 0; f < 2; ++f) y2[f] = fma(y2[f], fma(0.375, e[f], 0.5) * e[f], y2[f]);
+    for (int f = 0; f < NF; ++f) y2[f] = fma(y2[f], fma(0.375, e[f], 0.5) * e[f], y2[f]);
   }
 #pragma unroll
-  for (int f = 0; f < 2; ++f) {
+  for (int f = 0; f < NF; ++f) {
     const double a0 = fma(uhat[f], 0.5 * y2[f], 0.5);
     const int ah = __double2hiint(a0);
     const bool neg = ah < 0, big = ah >= 0x3FF00000;
@@ -469,16 +474,26 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
     double tmp[5];
     convert(W, o, tmp);
   };
-  const bool is_hs = (HW == 0) && !(F4_ABL & 2) && t < 2 * NH;
-  const bool is_hf = (HW == 0) && !(F4_ABL & 2) && (t >= 2 * NH) && (t < 3 * NH);
+  const bool is_hs = (HW == 0) && !(F4_ABL & (2 | 64)) && t < 2 * NH;
+  const bool is_hf = (HW == 0) && !(F4_ABL & (2 | 128)) && (t >= 2 * NH) && (t < 3 * NH);
   const int th = t - (TG - C::HALO);
-  const bool is_hc = (HW == 0) && !(F4_ABL & 2) && th >= 0 && th < C::HALO;
+#ifndef F4_HF3
+#define F4_HF3 1
+#endif
+  constexpr bool HF3 = (F4_HF3 != 0) && (HW == 0) && (NH % 32 == 0);   // the last-face flux warp is a whole warp
+  const bool is_hc = (HW == 0) && !(F4_ABL & (2 | 256)) && th >= 0 && th < C::HALO;
 
   // flux fixing: slots of this block's faces at refinement boundaries (BF instances only)
   int bfs[6] = {-1, -1, -1, -1, -1, -1};
   if (BF && p.bfslot) {
 #pragma unroll
     for (int f = 0; f < 2 * DIM; ++f) bfs[f] = p.bfslot[(size_t)blk * 6 + f];
+  }
+  double dxg[3] = {0.0, 0.0, 0.0};                  // dx * g of this block's level (general instances only)
+  if (BF && p.has_grav) {
+    const double dxl = 1.0 / p.inv_dx_l[lvl];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) dxg[d] = dxl * p.grav[d];
   }
   constexpr int BFS = N * ((DIM == 3) ? N : 1);   // cell faces of one block face
   auto bf_store = [&](int slot, const double (&F)[5], int t1, int t2) {
@@ -516,7 +531,32 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
         }
         L2[1][0] = L[0]; L2[1][1] = L[2]; L2[1][2] = L[1]; L2[1][3] = L[3]; L2[1][4] = L[4];
         R2[1][0] = Ry[0]; R2[1][1] = Ry[2]; R2[1][2] = Ry[1]; R2[1][3] = Ry[3]; R2[1][4] = Ry[4];
-        riemann_flux2<DIM>(L2, R2, gamma, ig1, F2);
+        if (HF3 && is_hf) {
+          // the warp that also owns the last-face fluxes of this plane solves its three Riemann problems together:
+          // the extra dependency chain overlaps with the other two instead of following them (the other warps wait
+          // for this one at the barrier below)
+          const int fq = t - 2 * NH;
+          const bool f_isx = fq < TY;
+          const int f_f = f_isx ? fq * (N + 1) + N : TY * N + (fq - TY);
+          double* e = f_isx ? eX : eY;
+          double L3[3][5], R3[3][5], F3[3][5], Lh[5], Rh[5];
+#pragma unroll
+          for (int q = 0; q < 5; ++q) {
+            L3[0][q] = L2[0][q]; L3[1][q] = L2[1][q]; R3[0][q] = R2[0][q]; R3[1][q] = R2[1][q];
+            Lh[q] = (DIM == 2 && q == 3) ? 0.0 : e[pl(q) * EXV + f_f];
+            Rh[q] = (DIM == 2 && q == 3) ? 0.0 : sRh[pl(q) * NH + fq];
+          }
+          L3[2][0] = Lh[0]; L3[2][1] = f_isx ? Lh[1] : Lh[2]; L3[2][2] = f_isx ? Lh[2] : Lh[1]; L3[2][3] = Lh[3]; L3[2][4] = Lh[4];
+          R3[2][0] = Rh[0]; R3[2][1] = f_isx ? Rh[1] : Rh[2]; R3[2][2] = f_isx ? Rh[2] : Rh[1]; R3[2][3] = Rh[3]; R3[2][4] = Rh[4];
+          riemann_fluxN<DIM, 3>(L3, R3, gamma, ig1, F3);
+#pragma unroll
+          for (int q = 0; q < 5; ++q) { F2[0][q] = F3[0][q]; F2[1][q] = F3[1][q]; }
+          const double Fp[5] = {F3[2][0], f_isx ? F3[2][1] : F3[2][2], f_isx ? F3[2][2] : F3[2][1], F3[2][3], F3[2][4]};
+#pragma unroll
+          for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) e[pl(q) * EXV + f_f] = Fp[q];
+        } else {
+          riemann_fluxN<DIM, 2>(L2, R2, gamma, ig1, F2);
+        }
 #pragma unroll
         for (int q = 0; q < 5; ++q) Fx[q] = F2[0][q];
         Fy[0] = F2[1][0]; Fy[1] = F2[1][2]; Fy[2] = F2[1][1]; Fy[3] = F2[1][3]; Fy[4] = F2[1][4];
@@ -537,7 +577,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
       for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eX[pl(q) * EXV + fx] = Fx[q];
 #pragma unroll
       for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eY[pl(q) * EXV + fy] = Fy[q];
-      if (is_hf) halo_flux_task(eX, eY, t - 2 * NH);
+      if (is_hf && !(FAST && HF3)) halo_flux_task(eX, eY, t - 2 * NH);
       if (BF) {
         if (i == 0 && bfs[0] >= 0) bf_store(bfs[0], Fx, j0 + j, kk);
         if (j0 + j == 0 && bfs[2] >= 0) bf_store(bfs[2], Fy, i, kk);
@@ -549,6 +589,18 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
     for (int q = 0; q < 5; ++q) {
       if (DIM == 2 && q == 3) { acc[q] = 0.0; continue; }
       acc[q] = (Fx[q] - eX[pl(q) * EXV + fx + 1]) + (Fy[q] - eY[pl(q) * EXV + fy + N]);
+    }
+    if (BF && p.has_grav) {
+      // source term of eq. (20), S = (0, rho g, rho g.u), from the cell's primitives;
+      // acc is multiplied by dt_sub/dx in the update, so dx S is added here
+      const double rho = W[own];
+      double gu = 0.0;
+#pragma unroll
+      for (int d = 0; d < DIM; ++d) {
+        acc[1 + d] = fma(rho, dxg[d], acc[1 + d]);
+        gu = fma(dxg[d], W[(1 + d) * PLANE + own], gu);
+      }
+      acc[4] = fma(rho, gu, acc[4]);
     }
     if (BF) {
       if (i == N - 1 && bfs[1] >= 0) {
@@ -795,7 +847,7 @@ cudaError_t launch_cfg(const StageParams& p, cudaStream_t s) {
   const int nitems = p.nblocks * C::YT;
   const int grid = (nitems + G - 1) / G;
   const bool fast = p.limiter == F4_LIM_VANLEER && p.flux == F4_FLUX_HLL;
-  if (p.bfslot || p.prev2) {   // general instances: boundary-flux store (flux fixing) and / or > 2 previous states
+  if (p.bfslot || p.prev2 || p.has_grav) {   // general instances: boundary-flux store (flux fixing) and / or > 2 previous states
     if (HW != 0) return cudaErrorInvalidValue;   // the helper-warp variant has no flux store
     if (fast) stage_kernel<DIM, N, TY, G, EXBUF, HW, true, true><<<grid, C::NT, C::SMEM, s>>>(p);
     else stage_kernel<DIM, N, TY, G, EXBUF, HW, false, true><<<grid, C::NT, C::SMEM, s>>>(p);

@@ -28,7 +28,7 @@ OP_SRL, OP_BC, OP_F2C, OP_C2F = 0, 1, 2, 3
 PROF_NAMES = ("ghost_r1", "ghost_r2", "stage", "dt_reduce", "regrid", "layout")
 
 # every symbol include/f4.h declares
-SYMBOLS = ("f4_mesh_create", "f4_mesh_destroy", "f4_set_options", "f4_set_flux_fix", "f4_set_rk_scheme", "f4_storage_bytes", "f4_bind_storage",
+SYMBOLS = ("f4_mesh_create", "f4_mesh_destroy", "f4_set_options", "f4_set_flux_fix", "f4_set_gravity", "f4_set_rk_scheme", "f4_storage_bytes", "f4_bind_storage",
            "f4_num_blocks", "f4_get_blocks", "f4_set_state", "f4_get_state", "f4_build_ghost_pattern",
            "f4_pattern_size", "f4_get_pattern", "f4_fill_ghosts", "f4_compute_dt", "f4_advance", "f4_refine_flags", "f4_adapt",
            "f4_conserved_totals", "f4_profile_enable", "f4_profile_get", "f4_launch_count", "f4_last_error",
@@ -62,6 +62,7 @@ def lib():
     L.f4_set_options.argtypes = [vp, C.c_int, C.c_int, C.c_double]
     L.f4_set_flux_fix.argtypes = [vp, C.c_int]
     L.f4_set_rk_scheme.argtypes = [vp, C.c_int]
+    L.f4_set_gravity.argtypes = [vp, dp]
     L.f4_refine_flags.argtypes = [vp, C.c_int, C.c_int, C.c_int, dp, ip, dp]
     L.f4_storage_bytes.restype = C.c_size_t
     L.f4_storage_bytes.argtypes = [vp]
@@ -179,6 +180,11 @@ class Mesh:
 
     def set_options(self, limiter=LIM_VANLEER, flux=FLUX_HLL, theta=1.0):
         self._chk(self.L.f4_set_options(self.h, limiter, flux, theta))
+
+    def set_gravity(self, g):
+        gg = np.zeros(3, dtype=np.float64)
+        gg[:len(g)] = g
+        self._chk(self.L.f4_set_gravity(self.h, _dp(gg)))
 
     def set_rk_scheme(self, scheme):
         self._chk(self.L.f4_set_rk_scheme(self.h, int(scheme)))
