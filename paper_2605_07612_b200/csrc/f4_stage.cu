@@ -88,6 +88,18 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 __device__ __forceinline__ void group_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+#ifndef F4_MID2
+#define F4_MID2 0    // (measured slower: 20.2 vs 22.4 GCUPS, the live z states spill) SPLIT: z flux + Runge-Kutta combine between arrive and wait of the second exchange barrier
+#endif
+#ifndef F4_LOADEARLY
+#define F4_LOADEARLY 1   // previous states of the finished plane are requested at the start of the iteration
+#endif
+#ifndef F4_SPLIT
+#define F4_SPLIT 1   // 3D march: split arrive / wait on mbarriers around the x/y exchange (0: two bar.sync per plane)
+#endif
 __device__ __forceinline__ void sweep_sync(int id, int nthreads) {
   if (F4_ABL & 1) { __syncwarp(); return; }
   group_sync(id, nthreads);
@@ -267,7 +279,8 @@ struct Cfg {  // FAST (van Leer + HLL fixed at compile time) does not change the
   static constexpr int YT = N / TY;           // y tiles per block
   // ring | exX[EXBUF] | exY[EXBUF] | right states of the high halo cells [NVAR][NH]
   static constexpr int GROUP_DOUBLES = NSLOT * SLOT + 2 * EXBUF * EX + NVAR * NH;
-  static constexpr size_t SMEM = (size_t)G * GROUP_DOUBLES * 8 + (size_t)G * NSLOT * 8;
+  static constexpr int NBAR = NSLOT + 2;     // ring slots + "left states written" + "fluxes written"
+  static constexpr size_t SMEM = (size_t)G * GROUP_DOUBLES * 8 + (size_t)G * NBAR * 8;
   static constexpr int HALO = 4 * TY + 4 * N;  // halo cells of an interior plane
   static_assert(HW == 1 || (HALO <= TG && 3 * NH <= TG), "halo work needs one pass");
   static_assert(HW == 0 || (HW == 1 && DIM == 3), "helper warp: 3D only");
@@ -297,7 +310,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
   double* exY = exX + EXBUF * C::EX;
   double* sRh = exY + EXBUF * C::EX;         // [NV][NH]
   uint64_t* bars = reinterpret_cast<uint64_t*>(reinterpret_cast<double*>(smem_raw) + (size_t)G * C::GROUP_DOUBLES) +
-                   grp * C::NSLOT;
+                   grp * C::NBAR;
   const uint32_t ring_u32 = smem_u32(ring), bars_u32 = smem_u32(bars);
   const int bar_id = 1 + grp;
 
@@ -314,6 +327,8 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
 
   if (t == 0) {
     for (int s = 0; s < C::NSLOT; ++s) mbar_init(&bars[s], 1);
+    mbar_init(&bars[C::NSLOT], TG);       // every cell thread arrives once per plane
+    mbar_init(&bars[C::NSLOT + 1], TG);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   group_sync(bar_id, TGA);
@@ -502,10 +517,32 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
     for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) d[pl(q) * BFS] = F[q];
   };
   // x/y sweep on the converted plane W (z index kk): sum over the x,y faces of (F_in - F_out) of the own cell
-  auto sweep_xy = [&](const double* W, int par, int kk, double (&acc)[5]) {
+  // SPLIT (3D march, double-buffered exchange): the barrier after phase 1 is split into an arrive and a wait on an
+  // mbarrier and `mid` -- the work of the march that does not depend on the exchange (conversion of the next plane,
+  // z slope, z flux, Runge-Kutta combine and store of the finished plane) -- runs in between, so that a warp that is
+  // late with its left states delays the others only by what exceeds that work.  Otherwise mid runs first.
+  constexpr bool SPLIT = (F4_SPLIT != 0) && DIM == 3 && EXBUF == 2 && HW == 0 && !(F4_ABL & 1);
+  uint32_t xph = 0;   // phase parity of the two exchange mbarriers
+  const uint32_t barL = bars_u32 + 8u * C::NSLOT, barF = barL + 8u;
+  auto sweep_xy = [&](const double* W, int par, int kk, double (&acc)[5], auto&& mid, auto&& mid2) {
     double* eX = exX + (EXBUF == 2 ? par : 0) * C::EX;
     double* eY = exY + (EXBUF == 2 ? par : 0) * C::EX;
+    if (!SPLIT) { mid(); mid2(); }
     double Rx[5], Ry[5];
+    double gsrc[4] = {0.0, 0.0, 0.0, 0.0};
+    if (BF && p.has_grav) {
+      // source term of eq. (20) (PAPER.md:431), S = (0, rho g, rho g.u), from the cell's primitives (PAPER.md:334);
+      // acc is multiplied by dt_sub/dx in the update, so dx S is what is added in phase 3.  Read here: after phase 2
+      // the ring slot of this plane may already be refilled
+      const double rho = W[own];
+      double gu = 0.0;
+#pragma unroll
+      for (int d = 0; d < DIM; ++d) {
+        gsrc[d] = rho * dxg[d];
+        gu = fma(dxg[d], W[(1 + d) * PLANE + own], gu);
+      }
+      gsrc[3] = rho * gu;
+    }
     {  // ---- phase 1: slopes -> left states to smem, right states stay in registers
       double L[5];
       slope_states(W, own, own_xm, own_xp, L, Rx);
@@ -516,7 +553,14 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
       for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eY[pl(q) * EXV + fy + N] = L[q];
       if (is_hs) halo_slope_task(W, eX, eY, t);
     }
-    sweep_sync(bar_id, TGA);
+    if (SPLIT) {
+      mbar_arrive(barL);
+      mid();
+      if (!F4_MID2) mid2();
+      mbar_wait(barL, xph);
+    } else {
+      sweep_sync(bar_id, TGA);
+    }
     double Fx[5], Fy[5];
     {  // ---- phase 2: flux at the low x and y face of the own cell, and at the last face of each row/column
       double L[5], F[5];
@@ -583,7 +627,14 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
         if (j0 + j == 0 && bfs[2] >= 0) bf_store(bfs[2], Fy, i, kk);
       }
     }
-    sweep_sync(bar_id, TGA);
+    if (SPLIT) {
+      mbar_arrive(barF);
+      if (F4_MID2) mid2();
+      mbar_wait(barF, xph);
+      xph ^= 1u;
+    } else {
+      sweep_sync(bar_id, TGA);
+    }
     // ---- phase 3: difference with the next faces
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
@@ -591,16 +642,9 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
       acc[q] = (Fx[q] - eX[pl(q) * EXV + fx + 1]) + (Fy[q] - eY[pl(q) * EXV + fy + N]);
     }
     if (BF && p.has_grav) {
-      // source term of eq. (20) (PAPER.md:431), S = (0, rho g, rho g.u), from the cell's primitives (PAPER.md:334);
-      // acc is multiplied by dt_sub/dx in the update, so dx S is added here
-      const double rho = W[own];
-      double gu = 0.0;
 #pragma unroll
-      for (int d = 0; d < DIM; ++d) {
-        acc[1 + d] = fma(rho, dxg[d], acc[1 + d]);
-        gu = fma(dxg[d], W[(1 + d) * PLANE + own], gu);
-      }
-      acc[4] = fma(rho, gu, acc[4]);
+      for (int d = 0; d < DIM; ++d) acc[1 + d] += gsrc[d];
+      acc[4] += gsrc[3];
     }
     if (BF) {
       if (i == N - 1 && bfs[1] >= 0) {
@@ -736,7 +780,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
     convert(ring, own, w);
     convert_halo(ring);
     group_sync(bar_id, TGA);
-    sweep_xy(ring, 0, 0, acc);
+    sweep_xy(ring, 0, 0, acc, [] {}, [] {});
     finish(0, acc, a, b);
   } else {
     double dA[5], Lz[5], accp[5];
@@ -751,8 +795,12 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
       const int sk = (sc == 0) ? 2 : sc - 1;                // slot of plane c-1
       double* Wc = ring + sc * C::SLOT;
       const double* Wk = ring + sk * C::SLOT;
+      double Fz[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+      // the part of the iteration that does not depend on the x/y exchange of plane c-1 (see sweep_xy)
+      double Rz[5], Lf[5];
       double pa5[5], pb5[5];
-      if (FIN) load_prev(c - 2, pa5, pb5);                  // consumed after the z flux: latency hidden
+      auto mid = [&]() {
+      if (F4_LOADEARLY && FIN) load_prev(c - 2, pa5, pb5);  // consumed after the z flux: latency hidden
       if (FIN && pb && c - 1 < N && (i & 3) == 0) {         // stage 2: u_t of the next plane comes from DRAM: pull it into L2 now
 #pragma unroll
         for (int q = 0; q < 5; ++q)
@@ -766,30 +814,32 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
       fence_proxy_async();   // generic-proxy writes before the async-proxy refill of this slot
       // ---- z direction along the march: slope of cell c-1 from w(c-2), w(c-1), w(c);
       //      flux at the face between cells c-2 and c-1 (normal frame (rho, w, u, v, p))
-      double Fz[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
       if (ZSLOPE) {
-        double Rz[5], Ln[5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
           const double wa = Wk[pl(q) * PLANE + own];   // w(c-1), resident in its ring slot
           const double dB = wB[q] - wa;
           const double hs = half_slope<FAST>(dA[q], dB, limiter);  // c == -1: dA = 0 -> hs = 0, result unused
           Rz[q] = wa - hs;
-          Ln[q] = wa + hs;
+          Lf[q] = Lz[q];                               // left state of the face between cells c-2 and c-1
+          Lz[q] = wa + hs;
           dA[q] = dB;
         }
+      }
+      };   // mid
+      auto mid2 = [&]() {
+      if (!F4_LOADEARLY && FIN) load_prev(c - 2, pa5, pb5);
+      if (ZSLOPE) {
         if (ZFLUX) {
-          const double Lf[5] = {Lz[0], Lz[3], Lz[1], Lz[2], Lz[4]}, Rf[5] = {Rz[0], Rz[3], Rz[1], Rz[2], Rz[4]};
+          const double Lfn[5] = {Lf[0], Lf[3], Lf[1], Lf[2], Lf[4]}, Rf[5] = {Rz[0], Rz[3], Rz[1], Rz[2], Rz[4]};
           double F[5];
-          riemann_flux<3, FAST>(Lf, Rf, gamma, ig1, fluxs, F);
+          riemann_flux<3, FAST>(Lfn, Rf, gamma, ig1, fluxs, F);
           Fz[0] = F[0]; Fz[3] = F[1]; Fz[1] = F[2]; Fz[2] = F[3]; Fz[4] = F[4];
           if (BF) {   // the face between cells c-2 and c-1 is the block's low (c = 1) / high (c = N+1) z face
             if (c == 1 && bfs[4] >= 0) bf_store(bfs[4], Fz, i, j0 + j);
             if (c == N + 1 && bfs[5] >= 0) bf_store(bfs[5], Fz, i, j0 + j);
           }
         }
-#pragma unroll
-        for (int q = 0; q < 5; ++q) Lz[q] = Ln[q];
       }
       if (FIN) {
         double tot[5];
@@ -797,12 +847,15 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
         for (int q = 0; q < 5; ++q) tot[q] = accp[q] - Fz[q];
         finish(c - 2, tot, pa5, pb5);
       }
+      };   // mid2
       if (SWEEP) {
         double acc[5];
-        sweep_xy(Wk, c & 1, c - 1, acc);
+        sweep_xy(Wk, c & 1, c - 1, acc, mid, mid2);
 #pragma unroll
         for (int q = 0; q < 5; ++q) accp[q] = acc[q] + Fz[q];
       } else {
+        mid();
+        mid2();
         group_sync(bar_id, TGA);
       }
       // every thread is past its last read of plane c-1: refill that slot with plane c+2
