@@ -91,9 +91,6 @@ __device__ __forceinline__ void group_sync(int id, int nthreads) {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-#ifndef F4_MID2
-#define F4_MID2 0    // (measured slower: 20.2 vs 22.4 GCUPS, the live z states spill) SPLIT: z flux + Runge-Kutta combine between arrive and wait of the second exchange barrier
-#endif
 #ifndef F4_LOADEARLY
 #define F4_LOADEARLY 1   // previous states of the finished plane are requested at the start of the iteration
 #endif
@@ -278,7 +275,7 @@ struct Cfg {  // FAST (van Leer + HLL fixed at compile time) does not change the
   static constexpr int NT = TGA * G;
   static constexpr int YT = N / TY;           // y tiles per block
   // ring | exX[EXBUF] | exY[EXBUF] | right states of the high halo cells [NVAR][NH]
-  static constexpr int GROUP_DOUBLES = NSLOT * SLOT + 2 * EXBUF * EX + NVAR * NH;
+  static constexpr int GROUP_DOUBLES = NSLOT * SLOT + 2 * EXBUF * EX + EXBUF * NVAR * NH;
   static constexpr int NBAR = NSLOT + 2;     // ring slots + "left states written" + "fluxes written"
   static constexpr size_t SMEM = (size_t)G * GROUP_DOUBLES * 8 + (size_t)G * NBAR * 8;
   static constexpr int HALO = 4 * TY + 4 * N;  // halo cells of an interior plane
@@ -308,7 +305,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
   double* ring = reinterpret_cast<double*>(smem_raw) + (size_t)grp * C::GROUP_DOUBLES;
   double* exX = ring + C::NSLOT * C::SLOT;   // [EXBUF][NV][EXV]
   double* exY = exX + EXBUF * C::EX;
-  double* sRh = exY + EXBUF * C::EX;         // [NV][NH]
+  double* sRh0 = exY + EXBUF * C::EX;        // [EXBUF][NV][NH]
   uint64_t* bars = reinterpret_cast<uint64_t*>(reinterpret_cast<double*>(smem_raw) + (size_t)G * C::GROUP_DOUBLES) +
                    grp * C::NBAR;
   const uint32_t ring_u32 = smem_u32(ring), bars_u32 = smem_u32(bars);
@@ -431,7 +428,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
   //      HALO threads convert the halo cells.  With HW = 1 the helper warp loops over all of them, so that the cell
   //      warps (whose dependent-issue latency is the critical path of a plane) all carry the same work.
   // slope task h in [0, 2NH): high halo cell of row/column h (right state -> sRh), low halo cell h-NH (left state -> e)
-  auto halo_slope_task = [&](const double* W, double* eX, double* eY, int h) {
+  auto halo_slope_task = [&](const double* W, double* eX, double* eY, double* sRh, int h) {
     const bool hi = h < NH;
     const int hq = hi ? h : h - NH;
     const bool isx = hq < TY;                          // x halo of row hq, else y halo of column hq-TY
@@ -461,7 +458,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
     }
   };
   // flux task fq in [0, NH): the last face of row fq (x) or of column fq-TY (y)
-  auto halo_flux_task = [&](double* eX, double* eY, int fq) {
+  auto halo_flux_task = [&](double* eX, double* eY, const double* sRh, int fq) {
     const bool f_isx = fq < TY;
     const int f_f = f_isx ? fq * (N + 1) + N : TY * N + (fq - TY);
     double* e = f_isx ? eX : eY;
@@ -517,19 +514,22 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
     for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) d[pl(q) * BFS] = F[q];
   };
   // x/y sweep on the converted plane W (z index kk): sum over the x,y faces of (F_in - F_out) of the own cell
-  // SPLIT (3D march, double-buffered exchange): the barrier after phase 1 is split into an arrive and a wait on an
-  // mbarrier and `mid` -- the work of the march that does not depend on the exchange (conversion of the next plane,
-  // z slope, z flux, Runge-Kutta combine and store of the finished plane) -- runs in between, so that a warp that is
-  // late with its left states delays the others only by what exceeds that work.  Otherwise mid runs first.
+  // SPLIT (3D march, double-buffered exchange): both barriers of the x/y exchange are split into an arrive and a
+  // wait on an mbarrier with exchange-independent work in between, so that a warp that is late delays the others only
+  // by what exceeds that work: the z slope / z flux / Runge-Kutta combine and store of the finished plane between
+  // arrive and wait of "left states written", phase 1 of the NEXT plane between arrive and wait of "fluxes written".
   constexpr bool SPLIT = (F4_SPLIT != 0) && DIM == 3 && EXBUF == 2 && HW == 0 && !(F4_ABL & 1);
   uint32_t xph = 0;   // phase parity of the two exchange mbarriers
   const uint32_t barL = bars_u32 + 8u * C::NSLOT, barF = barL + 8u;
-  auto sweep_xy = [&](const double* W, int par, int kk, double (&acc)[5], auto&& mid, auto&& mid2) {
+  // The x/y sweep of one converted plane W (z index kk, exchange buffers of parity par) in three phases:
+  //   1: slopes -> left states to shared memory, right states (and the gravity source) stay in registers
+  //   2: flux at the low x and y face of the own cell, and at the last face of each row / column
+  //   3: difference with the next faces: acc = sum over the x,y faces of (F_in - F_out) of the own cell
+  auto phase1 = [&](const double* W, int par, double (&Rx)[5], double (&Ry)[5], double (&gsrc)[4]) {
     double* eX = exX + (EXBUF == 2 ? par : 0) * C::EX;
     double* eY = exY + (EXBUF == 2 ? par : 0) * C::EX;
-    if (!SPLIT) { mid(); mid2(); }
-    double Rx[5], Ry[5];
-    double gsrc[4] = {0.0, 0.0, 0.0, 0.0};
+    double* sRh = sRh0 + (EXBUF == 2 ? par : 0) * NV * NH;
+    gsrc[0] = gsrc[1] = gsrc[2] = gsrc[3] = 0.0;
     if (BF && p.has_grav) {
       // source term of eq. (20), S = (0, rho g, rho g.u), from the cell's primitives;
       // acc is multiplied by dt_sub/dx in the update, so dx S is what is added in phase 3.  Read here: after phase 2
@@ -551,17 +551,13 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
       slope_states(W, own, own_ym, own_yp, L, Ry);
 #pragma unroll
       for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eY[pl(q) * EXV + fy + N] = L[q];
-      if (is_hs) halo_slope_task(W, eX, eY, t);
+      if (is_hs) halo_slope_task(W, eX, eY, sRh, t);
     }
-    if (SPLIT) {
-      mbar_arrive(barL);
-      mid();
-      if (!F4_MID2) mid2();
-      mbar_wait(barL, xph);
-    } else {
-      sweep_sync(bar_id, TGA);
-    }
-    double Fx[5], Fy[5];
+  };
+  auto phase2 = [&](int par, int kk, const double (&Rx)[5], const double (&Ry)[5], double (&Fx)[5], double (&Fy)[5]) {
+    double* eX = exX + (EXBUF == 2 ? par : 0) * C::EX;
+    double* eY = exY + (EXBUF == 2 ? par : 0) * C::EX;
+    double* sRh = sRh0 + (EXBUF == 2 ? par : 0) * NV * NH;
     {  // ---- phase 2: flux at the low x and y face of the own cell, and at the last face of each row/column
       double L[5], F[5];
       if (FAST) {
@@ -621,20 +617,18 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
       for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eX[pl(q) * EXV + fx] = Fx[q];
 #pragma unroll
       for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eY[pl(q) * EXV + fy] = Fy[q];
-      if (is_hf && !(FAST && HF3)) halo_flux_task(eX, eY, t - 2 * NH);
+      if (is_hf && !(FAST && HF3)) halo_flux_task(eX, eY, sRh, t - 2 * NH);
       if (BF) {
         if (i == 0 && bfs[0] >= 0) bf_store(bfs[0], Fx, j0 + j, kk);
         if (j0 + j == 0 && bfs[2] >= 0) bf_store(bfs[2], Fy, i, kk);
       }
     }
-    if (SPLIT) {
-      mbar_arrive(barF);
-      if (F4_MID2) mid2();
-      mbar_wait(barF, xph);
-      xph ^= 1u;
-    } else {
-      sweep_sync(bar_id, TGA);
-    }
+  };
+  auto phase3 = [&](int par, int kk, const double (&Fx)[5], const double (&Fy)[5], const double (&gsrc)[4],
+                    double (&acc)[5]) {
+    double* eX = exX + (EXBUF == 2 ? par : 0) * C::EX;
+    double* eY = exY + (EXBUF == 2 ? par : 0) * C::EX;
+    double* sRh = sRh0 + (EXBUF == 2 ? par : 0) * NV * NH;
     // ---- phase 3: difference with the next faces
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
@@ -660,6 +654,15 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
         bf_store(bfs[3], Fh, i, kk);
       }
     }
+  };
+  // the three phases with a group barrier in between (2D, single exchange buffer, F4_SPLIT = 0)
+  auto sweep_xy = [&](const double* W, int par, int kk, double (&acc)[5]) {
+    double Rx[5], Ry[5], Fx[5], Fy[5], gsrc[4];
+    phase1(W, par, Rx, Ry, gsrc);
+    sweep_sync(bar_id, TGA);
+    phase2(par, kk, Rx, Ry, Fx, Fy);
+    sweep_sync(bar_id, TGA);
+    phase3(par, kk, Fx, Fy, gsrc, acc);
     if (EXBUF == 1) sweep_sync(bar_id, TGA);
   };
 
@@ -756,11 +759,11 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
         double* eY = exY + (EXBUF == 2 ? (c & 1) : 0) * C::EX;
 #pragma unroll
         for (int h = 0; h < (2 * NH + 31) / 32; ++h)
-          if (h * 32 + lane < 2 * NH) halo_slope_task(Wk, eX, eY, h * 32 + lane);
+          if (h * 32 + lane < 2 * NH) halo_slope_task(Wk, eX, eY, sRh0 + (EXBUF == 2 ? (c & 1) : 0) * NV * NH, h * 32 + lane);
         group_sync(bar_id, TGA);
 #pragma unroll
         for (int h = 0; h < (NH + 31) / 32; ++h)
-          if (h * 32 + lane < NH) halo_flux_task(eX, eY, h * 32 + lane);
+          if (h * 32 + lane < NH) halo_flux_task(eX, eY, sRh0 + (EXBUF == 2 ? (c & 1) : 0) * NV * NH, h * 32 + lane);
         group_sync(bar_id, TGA);
         if (EXBUF == 1) group_sync(bar_id, TGA);
       } else {
@@ -780,12 +783,14 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
     convert(ring, own, w);
     convert_halo(ring);
     group_sync(bar_id, TGA);
-    sweep_xy(ring, 0, 0, acc, [] {}, [] {});
+    sweep_xy(ring, 0, 0, acc);
     finish(0, acc, a, b);
   } else {
     double dA[5], Lz[5], accp[5];
+    double Rxp[5], Ryp[5], gsp[4];   // SPLIT: right states (and gravity source) of the plane whose phase 1 ran ahead
 #pragma unroll
-    for (int q = 0; q < 5; ++q) { dA[q] = 0.0; Lz[q] = 1.0; accp[q] = 0.0; }
+    for (int q = 0; q < 5; ++q) { dA[q] = 0.0; Lz[q] = 1.0; accp[q] = 0.0; Rxp[q] = 1.0; Ryp[q] = 1.0; }
+    gsp[0] = gsp[1] = gsp[2] = gsp[3] = 0.0;
     int sc = 0;            // ring slot of plane c (planes take the slots 0,1,2,0,...)
     uint32_t ph = 0;       // phase parity of each slot's mbarrier
     // one march iteration; the steady state (c in [2, N]) is the instance with every flag true
@@ -798,20 +803,21 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
       double Fz[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
       // the part of the iteration that does not depend on the x/y exchange of plane c-1 (see sweep_xy)
       double Rz[5], Lf[5];
-      double pa5[5], pb5[5];
-      auto mid = [&]() {
+      double pa5[5], pb5[5], wB[5];
+      auto midA = [&]() {
       if (F4_LOADEARLY && FIN) load_prev(c - 2, pa5, pb5);  // consumed after the z flux: latency hidden
       if (FIN && pb && c - 1 < N && (i & 3) == 0) {         // stage 2: u_t of the next plane comes from DRAM: pull it into L2 now
 #pragma unroll
         for (int q = 0; q < 5; ++q)
           asm volatile("prefetch.global.L2 [%0];" ::"l"(pa + (c - 1) * PP + pl(q) * (int)C::VS));
       }
-      double wB[5];
       mbar_wait(bars_u32 + 8u * sc, (ph >> sc) & 1u);
       ph ^= 1u << sc;
       convert(Wc, own, wB);
       if (c >= 0 && c < N) convert_halo(Wc);
       fence_proxy_async();   // generic-proxy writes before the async-proxy refill of this slot
+      };   // midA
+      auto midB = [&]() {
       // ---- z direction along the march: slope of cell c-1 from w(c-2), w(c-1), w(c);
       //      flux at the face between cells c-2 and c-1 (normal frame (rho, w, u, v, p))
       if (ZSLOPE) {
@@ -826,7 +832,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
           dA[q] = dB;
         }
       }
-      };   // mid
+      };   // midB
       auto mid2 = [&]() {
       if (!F4_LOADEARLY && FIN) load_prev(c - 2, pa5, pb5);
       if (ZSLOPE) {
@@ -848,13 +854,39 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
         finish(c - 2, tot, pa5, pb5);
       }
       };   // mid2
-      if (SWEEP) {
+      if (SWEEP && SPLIT) {
+        // Split barriers, software-pipelined by one plane: the left states of plane c-1 were written in the previous
+        // iteration (phase 1 runs one plane ahead, between arrive and wait of the flux barrier); the z work sits
+        // between arrive and wait of the left-state barrier.  A wait on barL also guarantees that every thread has
+        // converted plane c, which is what phase 1 of plane c reads.
+        if (c == 1) phase1(Wk, c & 1, Rxp, Ryp, gsp);
+        midA();
+        mbar_arrive(barL);
+        midB();
+        mid2();
+        mbar_wait(barL, xph);
+        double Fx[5], Fy[5], gs[4], acc[5];
+        phase2(c & 1, c - 1, Rxp, Ryp, Fx, Fy);
+        mbar_arrive(barF);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) gs[q] = gsp[q];
+        if (c < N) phase1(Wc, (c + 1) & 1, Rxp, Ryp, gsp);
+        mbar_wait(barF, xph);
+        xph ^= 1u;
+        phase3(c & 1, c - 1, Fx, Fy, gs, acc);
+#pragma unroll
+        for (int q = 0; q < 5; ++q) accp[q] = acc[q] + Fz[q];
+      } else if (SWEEP) {
         double acc[5];
-        sweep_xy(Wk, c & 1, c - 1, acc, mid, mid2);
+        midA();
+        midB();
+        mid2();
+        sweep_xy(Wk, c & 1, c - 1, acc);
 #pragma unroll
         for (int q = 0; q < 5; ++q) accp[q] = acc[q] + Fz[q];
       } else {
-        mid();
+        midA();
+        midB();
         mid2();
         group_sync(bar_id, TGA);
       }
