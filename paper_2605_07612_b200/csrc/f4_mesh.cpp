@@ -189,8 +189,45 @@ int HostMesh::adapt(const int* flags, std::vector<Transfer>& plan, bool& changed
       const Leaf& l = leaves[b];
       if (flags[b] < 0 && l.level > base_level) fam[pack(l.level - 1, l.c[0] >> 1, l.c[1] >> 1, l.c[2] >> 1)]++;
     }
+    // A family whose parent would touch a leaf two levels finer is not coarsened: balance (which only refines)
+    // would split the parent again at once.  Checking here keeps the balance work list below to the NEW leaves.
+    auto can_coarsen = [&](const Leaf& par) {
+      for (int dz = (dim == 3 ? -1 : 0); dz <= (dim == 3 ? 1 : 0); ++dz)
+        for (int dy = -1; dy <= 1; ++dy)
+          for (int dx = -1; dx <= 1; ++dx) {
+            if (!dx && !dy && !dz) continue;
+            const int d[3] = {dx, dy, dz};
+            int n[3] = {par.c[0] + dx, par.c[1] + dy, par.c[2] + dz};
+            bool outside = false;
+            for (int a = 0; a < dim; ++a) {
+              int ext = extent(par.level, a);
+              if (n[a] < 0 || n[a] >= ext) {
+                if (bc[2 * a] == F4_BC_PERIODIC) n[a] = (n[a] + ext) % ext; else outside = true;
+              }
+            }
+            if (outside) continue;
+            bool covered = false;   // the neighbour region is a leaf or inside a coarser leaf
+            for (int l = par.level; l >= 0 && !covered; --l) {
+              int sh = par.level - l;
+              covered = S.count(pack(l, n[0] >> sh, n[1] >> sh, n[2] >> sh)) != 0;
+            }
+            if (covered) continue;
+            // subdivided: its children that touch the parent must be leaves (level par.level + 1), not finer
+            for (int cz = 0; cz < (dim == 3 ? 2 : 1); ++cz)
+              for (int cy = 0; cy < 2; ++cy)
+                for (int cx = 0; cx < 2; ++cx) {
+                  const int cc[3] = {cx, cy, cz};
+                  bool touches = true;
+                  for (int a = 0; a < dim; ++a)
+                    if ((d[a] == 1 && cc[a] != 0) || (d[a] == -1 && cc[a] != 1)) touches = false;
+                  if (!touches) continue;
+                  if (!S.count(pack(par.level + 1, 2 * n[0] + cx, 2 * n[1] + cy, dim == 3 ? 2 * n[2] + cz : 0))) return false;
+                }
+          }
+      return true;
+    };
     for (auto& pr : fam)
-      if (pr.second == nch) {
+      if (pr.second == nch && can_coarsen(unpack(pr.first))) {
         Leaf par = unpack(pr.first);
         children(par, ch);
         for (int q = 0; q < nch; ++q) S.erase(ch[q]);
@@ -199,7 +236,10 @@ int HostMesh::adapt(const int* flags, std::vector<Transfer>& plan, bool& changed
   }
   // 3. balance, corner connectivity: ripple from a work queue
   {
-    std::deque<uint64_t> Q(S.begin(), S.end());
+    // the old mesh was balanced, so only a leaf created by this call can be the finer side of a violation
+    std::deque<uint64_t> Q;
+    for (uint64_t k : S)
+      if (!old_index.count(k)) Q.push_back(k);
     while (!Q.empty()) {
       uint64_t ka = Q.front();
       Q.pop_front();
