@@ -76,7 +76,7 @@ class ClockSampler(threading.Thread):
                  "hw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40),
                  "sw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20),
                  "sw_power_cap": getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4)}
-        while not self.stop_flag:
+        while not (self.stop_flag and self.samples):   # at least one sample, also for a very short timed region
             try:
                 self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
                 r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
@@ -306,6 +306,7 @@ def main():
     ev1.record(stream)
     barrier()
     sampler.stop_flag = True
+    sampler.join(timeout=1.0)
     ms = ev0.elapsed_time(ev1)
     launches = mesh.launch_count() - l0
     prof = mesh.profile_get(reset=True)
