@@ -963,7 +963,13 @@ cudaError_t launch_stage(int dim, int n, const StageParams& p, cudaStream_t s) {
 #ifndef F4_HW8
 #define F4_HW8 0
 #endif
-  if (dim == 3 && n == 8) return launch_cfg<3, 8, 8, 4, 1, F4_HW8>(p, s);
+#ifndef F4_G8
+#define F4_G8 4
+#endif
+#ifndef F4_EX8
+#define F4_EX8 1
+#endif
+  if (dim == 3 && n == 8) return launch_cfg<3, 8, 8, F4_G8, F4_EX8, F4_HW8>(p, s);
 #ifndef F4_TY16
 #define F4_TY16 16
 #endif
