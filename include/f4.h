@@ -62,7 +62,11 @@ enum {
 enum {
   F4_BC_PERIODIC = 0, /* via connectivity */
   F4_BC_OUTFLOW = 1,  /* uniform Neumann, zero normal derivative: ghost = nearest interior layer (reading A10) */
-  F4_BC_KEEP = 2      /* ghosts on that face are left as the caller set them (linear-field test) */
+  F4_BC_KEEP = 2,     /* ghosts on that face are left as the caller set them (linear-field test) */
+  F4_BC_DIRICHLET = 3, /* uniform value u_b per face direction and variable (f4_set_bc_values): ghost layer g mirrors
+                          interior layer g through the face, u_ghost = 2 u_b - u_interior (reading A10) */
+  F4_BC_NEUMANN = 4    /* uniform outward normal derivative u_b': ghost layer g = first interior layer + g dx u_b'
+                          (reading A10b; u_b' = 0 is F4_BC_OUTFLOW) */
 };
 
 enum { F4_LIM_VANLEER = 0, F4_LIM_MINMOD = 1, F4_LIM_MC = 2 }; /* PAPER.md:322-326; reading A1 */
@@ -158,6 +162,14 @@ int f4_fill_ghosts(f4_mesh *m, int state);
  * state 0 is already on the device (fused into the last stage); otherwise a
  * reduction kernel runs.  Synchronises to read one double back. */
 int f4_compute_dt(f4_mesh *m, int state, double cfl, double *dt_out);
+
+/* Uniform boundary data of the F4_BC_DIRICHLET / F4_BC_NEUMANN faces ("a Dirichlet boundary condition
+ * with a uniform value u = u_b ... stored per face direction and per variable ... and the same ... for a Neumann
+ * boundary condition with a uniform normal derivative"): values[6][Nvar], face directions -x,+x,-y,+y,-z,+z, stored
+ * (conservative) variables; entries of other faces are ignored.  Default: zeros.  Copied to the device when storage
+ * is bound (host call otherwise); takes effect at the next ghost fill.  Spatially varying bc_data (eq. 4) is not
+ * provided: F4_BC_KEEP lets the caller write such ghosts. */
+int f4_set_bc_values(f4_mesh *m, const double *values);
 
 /* Gravitational acceleration g[3] of the source term S = (0, rho g, rho g.u), eq. (20), evaluated
  * from the primitives of s_deriv in each cell and added to the flux divergence in every sub-step (PAPER.md:334 step i).

@@ -44,7 +44,7 @@
 
 namespace {
 
-enum { BC_PERIODIC = 0, BC_OUTFLOW = 1, BC_KEEP = 2 };
+enum { BC_PERIODIC = 0, BC_OUTFLOW = 1, BC_KEEP = 2, BC_DIRICHLET = 3, BC_NEUMANN = 4 };
 enum { LIM_VANLEER = 0, LIM_MINMOD = 1, LIM_MC = 2 };
 enum { FLUX_HLL = 0, FLUX_RUSANOV = 1 };
 enum { NB_BOUNDARY = 0, NB_SAME = 1, NB_COARSE = 2, NB_FINE = 3 };
@@ -69,6 +69,7 @@ struct Mesh {
   int dim, N, Ng, P, Pz, nvar;
   int brick[3], base_level, max_level, bc[6];
   double gamma, theta;
+  double bcv[6][5] = {};  // uniform boundary value u_b (Dirichlet) or normal derivative u_b' (Neumann) per face direction and variable
   double grav[3] = {0.0, 0.0, 0.0};  // gravitational acceleration g of the source term eq. (20)
   int limiter, flux_scheme;
   int nstates;
@@ -209,7 +210,7 @@ void fill_srl(Mesh& m, int s, int A, int f, int B) {
 void fill_bc(Mesh& m, int s, int A, int f) {
   if (m.bc[f] == BC_KEEP) return;  // ghost values preset by the caller (linear-field test)
   // Outflow = uniform Neumann with zero normal derivative; reading A10:
-  // every ghost layer = nearest interior layer.
+  // every ghost layer = nearest interior layer.  Uniform Dirichlet / Neumann values: m.bcv.
   int a = f / 2, side = f % 2, N = m.N, kmax = (m.dim == 3) ? N : 1;
   for (int v = 0; v < m.nvar; ++v)
     for (int g = 1; g <= m.Ng; ++g)
@@ -218,7 +219,21 @@ void fill_bc(Mesh& m, int s, int A, int f) {
           int di, dj, dk, si, sj, sk;
           if (side) { compose(a, N + g, t1, t2, di, dj, dk); compose(a, N, t1, t2, si, sj, sk); }
           else      { compose(a, 1 - g, t1, t2, di, dj, dk); compose(a, 1, t1, t2, si, sj, sk); }
-          m.at(s, A, v, di, dj, dk) = m.at(s, A, v, si, sj, sk);
+          if (m.bc[f] == BC_OUTFLOW) {
+            m.at(s, A, v, di, dj, dk) = m.at(s, A, v, si, sj, sk);
+          } else if (m.bc[f] == BC_NEUMANN) {
+            // uniform normal derivative u_b' along the outward normal: the centre of ghost layer g is
+            // g dx outside the centre of the first interior cell -> first-order extrapolation with that derivative
+            // (reading A10b; u_b' = 0 is the outflow rule)
+            const double dx = m.dx_of_level(m.blocks[A].level);
+            m.at(s, A, v, di, dj, dk) = m.at(s, A, v, si, sj, sk) + ((double)g * dx) * m.bcv[f][v];
+          } else {  // BC_DIRICHLET
+            // uniform value u_b on the boundary face: ghost layer g mirrors interior layer g through
+            // the face, u_ghost = 2 u_b - u_interior, so that the linear interpolant takes u_b on the face (reading A10)
+            int mi, mj, mk;
+            if (side) compose(a, N + 1 - g, t1, t2, mi, mj, mk); else compose(a, g, t1, t2, mi, mj, mk);
+            m.at(s, A, v, di, dj, dk) = 2.0 * m.bcv[f][v] - m.at(s, A, v, mi, mj, mk);
+          }
         }
 }
 
@@ -838,6 +853,10 @@ void ora_set_options(void* h, int limiter, int flux_scheme, double theta) {
   Mesh* m = (Mesh*)h; m->limiter = limiter; m->flux_scheme = flux_scheme; m->theta = theta;
 }
 void ora_set_flux_fix(void* h, int on) { ((Mesh*)h)->flux_fix = on != 0; }
+void ora_set_bc_values(void* h, const double* v) {   // [6][nvar]
+  Mesh* m = (Mesh*)h;
+  for (int f = 0; f < 6; ++f) for (int q = 0; q < m->nvar; ++q) m->bcv[f][q] = v[f * m->nvar + q];
+}
 void ora_set_gravity(void* h, const double* g) { for (int a = 0; a < 3; ++a) ((Mesh*)h)->grav[a] = g[a]; }
 void ora_set_test_rhs(void* h, int on, double lambda) { Mesh* m = (Mesh*)h; m->test_rhs = on; m->test_lambda = lambda; }
 int ora_num_blocks(void* h) { return (int)((Mesh*)h)->blocks.size(); }

@@ -46,6 +46,7 @@ def lib():
         L.ora_set_test_rhs.argtypes = [C.c_void_p, C.c_int, C.c_double]
         L.ora_set_flux_fix.argtypes = [C.c_void_p, C.c_int]
         L.ora_set_gravity.argtypes = [C.c_void_p, dp]
+        L.ora_set_bc_values.argtypes = [C.c_void_p, dp]
         L.ora_num_blocks.argtypes = [C.c_void_p]
         L.ora_get_blocks.argtypes = [C.c_void_p, ip, ip]
         L.ora_dx.restype = C.c_double
@@ -120,6 +121,12 @@ class OracleMesh:
 
     def set_options(self, limiter=LIM_VANLEER, flux=FLUX_HLL, theta=1.0):
         self.L.ora_set_options(self.h, limiter, flux, theta)
+
+    def set_bc_values(self, values):
+        """values[6][nvar]: u_b of Dirichlet faces / normal derivative u_b' of Neumann faces."""
+        v = np.ascontiguousarray(values, dtype=np.float64)
+        assert v.shape == (6, self.nvar)
+        self.L.ora_set_bc_values(self.h, _dp(v))
 
     def set_gravity(self, g):
         """Gravitational acceleration of the source term eq. (20); (0,0,0) = no source."""

@@ -18,6 +18,8 @@ struct f4_mesh {
   int limiter = F4_LIM_VANLEER, flux = F4_FLUX_HLL;
   int rk = F4_RK_HEUN;
   double grav[3] = {0.0, 0.0, 0.0};
+  double bcv[6 * 5] = {0.0};     // uniform Dirichlet values / Neumann derivatives [6][nvar]
+  double* d_bcv = nullptr;
   int n_states = 2;
   int nvar = 5;
   size_t vs = 0, bs = 0, state_doubles = 0;  // doubles per (block,var), per block, per state
@@ -218,12 +220,14 @@ int fill_ghosts_impl(f4_mesh* m, int state, int have, bool need_z, bool for_stag
   else if (have == 1) { r1 = m->d_r1z; n1 = m->n_r1z; }
   if (n1) {
     Scope sc(m, F4_PROF_R1);
-    CU(launch_ghost(m->hm.dim, m->hm.N, GhostParams{st, r1, n1, m->theta}, m->stream));
+    CU(launch_ghost(m->hm.dim, m->hm.N, GhostParams{st, r1, n1, m->theta, m->d_bcv, m->d_level, m->hm.dx_of_level(0)},
+                    m->stream));
   }
   m->srl_valid[state] = (char)after;
   if (m->n_r2) {
     Scope sc(m, F4_PROF_R2);
-    CU(launch_ghost(m->hm.dim, m->hm.N, GhostParams{st, m->d_r2, m->n_r2, m->theta}, m->stream));
+    CU(launch_ghost(m->hm.dim, m->hm.N,
+                    GhostParams{st, m->d_r2, m->n_r2, m->theta, m->d_bcv, m->d_level, m->hm.dx_of_level(0)}, m->stream));
   }
   return F4_OK;
 }
@@ -294,6 +298,7 @@ int f4_mesh_destroy(f4_mesh* m) {
   if (m->d_maxrate) cudaFree(m->d_maxrate);
   if (m->d_sums) cudaFree(m->d_sums);
   if (m->d_flags) cudaFree(m->d_flags);
+  if (m->d_bcv) cudaFree(m->d_bcv);
   if (m->d_indicator) cudaFree(m->d_indicator);
   if (m->d_stage) cudaFree(m->d_stage);
   delete m;
@@ -335,6 +340,7 @@ int f4_bind_storage(f4_mesh* m, void* dev_ptr, size_t bytes, void* cuda_stream) 
     CU(cudaMalloc((void**)&m->d_maxrate, sizeof(unsigned long long)));
     CU(cudaMalloc((void**)&m->d_sums, (size_t)m->hm.max_blocks * m->nvar * sizeof(double)));
     CU(cudaMalloc((void**)&m->d_flags, (size_t)m->hm.max_blocks * sizeof(int)));
+    CU(cudaMalloc((void**)&m->d_bcv, sizeof(m->bcv)));
     CU(cudaMalloc((void**)&m->d_indicator, (size_t)m->hm.max_blocks * sizeof(double)));
     // staging: whole blocks of the natural padded layout, at most 128 MiB
     size_t per_block = m->bs * sizeof(double);
@@ -345,6 +351,7 @@ int f4_bind_storage(f4_mesh* m, void* dev_ptr, size_t bytes, void* cuda_stream) 
     CU(cudaMalloc((void**)&m->d_stage, m->stage_bytes));
   }
   m->bound = true;
+  CU(cudaMemcpyAsync(m->d_bcv, m->bcv, sizeof(m->bcv), cudaMemcpyHostToDevice, m->stream));
   for (int s = 0; s < m->n_states; ++s) {
     Scope sc(m, F4_PROF_LAYOUT);
     CU(launch_init_benign(m->hm.dim, m->hm.N, m->state_ptr(s), m->hm.max_blocks, m->gamma, m->stream));
@@ -517,6 +524,17 @@ const Scheme& scheme_table(int rk) {
 }
 
 }  // namespace
+
+int f4_set_bc_values(f4_mesh* m, const double* values) {
+  if (!m || !values) return F4_EINVAL;
+  for (int q = 0; q < 6 * m->nvar; ++q) m->bcv[q] = values[q];
+  if (m->bound) {
+    CU(cudaMemcpyAsync(m->d_bcv, m->bcv, sizeof(m->bcv), cudaMemcpyHostToDevice, m->stream));
+    CU(cudaStreamSynchronize(m->stream));
+    for (auto& v : m->srl_valid) v = 0;   // boundary ghosts of every state are stale now
+  }
+  return F4_OK;
+}
 
 int f4_set_gravity(f4_mesh* m, const double g[3]) {
   if (!m || !g) return F4_EINVAL;

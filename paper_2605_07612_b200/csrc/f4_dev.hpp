@@ -59,6 +59,9 @@ struct GhostParams {
   const DevRecord* rec;
   int nrec;
   double theta;
+  const double* bcv;   // [6][Nvar] uniform Dirichlet values / Neumann normal derivatives
+  const int* level;    // per block (Neumann: dx of the block)
+  double dx0;          // cell size of level 0
 };
 
 // every launcher returns the cudaError_t of the launch

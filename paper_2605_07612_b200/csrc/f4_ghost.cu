@@ -177,6 +177,32 @@ __device__ __forceinline__ void do_c2f(double* __restrict__ st, int dst, int src
   }
 }
 
+// Uniform Dirichlet / Neumann boundary face (readings A10, A10b), one record = one block face:
+//   Dirichlet: ghost layer g mirrors interior layer g through the face, u_ghost = 2 u_b - u_interior;
+//   Neumann:   ghost layer g = first interior layer + (g dx) u_b'  (u_b' = outward normal derivative).
+// Individually rounded operations in the order the formulas are written: bit-exact against the oracle.
+template <int DIM, int N>
+__device__ __forceinline__ void do_bc_values(double* __restrict__ st, int blk, int face, bool neumann,
+                                             const double* __restrict__ bcv, double dx) {
+  using G = Geo<DIM, N>;
+  constexpr int NV = G::NVAR, FS = (DIM == 3) ? N * N : N;
+  const int a = face >> 1, side = face & 1;
+  double* db = st + (size_t)blk * G::BS;
+  for (int e = threadIdx.x; e < NV * NG * FS; e += blockDim.x) {
+    const int v = e / (NG * FS), r = e % (NG * FS), g = r / FS + 1, t = r % FS, t1 = t % N, t2 = t / N;
+    const int nd = side ? N - 1 + g : -g;                              // ghost cell along the normal
+    const int ns = neumann ? (side ? N - 1 : 0) : (side ? N - g : g - 1);
+    int di, dj, dk, si, sj, sk;
+    if (a == 0) { di = nd; si = ns; dj = sj = t1; dk = sk = t2; }
+    else if (a == 1) { dj = nd; sj = ns; di = si = t1; dk = sk = t2; }
+    else { dk = nd; sk = ns; di = si = t1; dj = sj = t2; }
+    double* dv = db + (size_t)v * G::VS;
+    const double src = dv[cell_off<DIM, N>(si, sj, sk)], ub = bcv[face * NV + v];
+    dv[cell_off<DIM, N>(di, dj, dk)] =
+        neumann ? __dadd_rn(src, __dmul_rn(__dmul_rn((double)g, dx), ub)) : __dsub_rn(__dmul_rn(2.0, ub), src);
+  }
+}
+
 template <int DIM, int N>
 __global__ void __launch_bounds__(256, 4) ghost_exec_kernel(GhostParams p) {
   using G = Geo<DIM, N>;
@@ -200,7 +226,7 @@ __global__ void __launch_bounds__(256, 4) ghost_exec_kernel(GhostParams p) {
       if (e >= n * PER_VAR) continue;
       const DevRecord rec = recs[e / PER_VAR];
       const int op = rec.meta & 3, face = (rec.meta >> 2) & 7;
-      if (op > F4_OP_BC) continue;
+      if (op > F4_OP_BC || (op == F4_OP_BC && (rec.meta >> 5) & 3)) continue;   // Dirichlet / Neumann faces: below
       const bool outflow = (op == F4_OP_BC);
       int so, d_o;
       copy_unit<DIM, N>(face, outflow, e % PER_VAR, so, d_o);
@@ -226,7 +252,9 @@ __global__ void __launch_bounds__(256, 4) ghost_exec_kernel(GhostParams p) {
   for (int q = 0; q < n; ++q) {
     const DevRecord rec = recs[q];
     const int op = rec.meta & 3, face = (rec.meta >> 2) & 7, o1 = (rec.meta >> 5) & 1, o2 = (rec.meta >> 6) & 1;
-    if (op == F4_OP_F2C) do_f2c<DIM, N>(p.state, rec.dst, rec.src, face, o1, o2);
+    if (op == F4_OP_BC && (o1 | o2))
+      do_bc_values<DIM, N>(p.state, rec.dst, face, o2 != 0, p.bcv, p.dx0 * (1.0 / (double)(1u << p.level[rec.dst])));
+    else if (op == F4_OP_F2C) do_f2c<DIM, N>(p.state, rec.dst, rec.src, face, o1, o2);
     else if (op == F4_OP_C2F) do_c2f<DIM, N>(p.state, rec.dst, rec.src, face, o1, o2, p.theta);
   }
 }

@@ -58,7 +58,7 @@ int HostMesh::init(std::string& err) {
     }
   }
   for (int f = 0; f < 2 * dim; ++f)
-    if (bc[f] < 0 || bc[f] > F4_BC_KEEP) { err = "bad bc_kind"; return F4_EINVAL; }
+    if (bc[f] < 0 || bc[f] > F4_BC_NEUMANN) { err = "bad bc_kind"; return F4_EINVAL; }
   if (dim == 2) brick[2] = 1;
   int64_t nb = 1;
   for (int a = 0; a < dim; ++a) nb *= extent(base_level, a);
@@ -115,7 +115,10 @@ int HostMesh::build_pattern(std::string& err) {
       if (n[a] < 0 || n[a] >= ext) {
         if (bc[f] == F4_BC_PERIODIC) n[a] = (n[a] + ext) % ext;
         else {
+          // o1 / o2 of a boundary record carry its kind: (0,0) outflow, (1,0) Dirichlet, (0,1) Neumann
           if (bc[f] == F4_BC_OUTFLOW) r1.push_back(Record{F4_OP_BC, f, b, b, 0, 0});
+          else if (bc[f] == F4_BC_DIRICHLET) r1.push_back(Record{F4_OP_BC, f, b, b, 1, 0});
+          else if (bc[f] == F4_BC_NEUMANN) r1.push_back(Record{F4_OP_BC, f, b, b, 0, 1});
           continue;  // F4_BC_KEEP: no record
         }
       }

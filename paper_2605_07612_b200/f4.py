@@ -17,7 +17,7 @@ from . import build as _build
 F4_OK = 0
 ERRORS = {-1: "F4_EINVAL", -2: "F4_ENOBLOCKS", -3: "F4_ECUDA", -4: "F4_EUNBOUND", -5: "F4_EUNBALANCED",
           -6: "F4_EUNSUPPORTED"}
-BC_PERIODIC, BC_OUTFLOW, BC_KEEP = 0, 1, 2
+BC_PERIODIC, BC_OUTFLOW, BC_KEEP, BC_DIRICHLET, BC_NEUMANN = 0, 1, 2, 3, 4
 LIM_VANLEER, LIM_MINMOD, LIM_MC = 0, 1, 2
 FLUX_HLL, FLUX_RUSANOV = 0, 1
 CRIT_LOHNER, CRIT_PJUMP = 0, 1
@@ -28,7 +28,7 @@ OP_SRL, OP_BC, OP_F2C, OP_C2F = 0, 1, 2, 3
 PROF_NAMES = ("ghost_r1", "ghost_r2", "stage", "dt_reduce", "regrid", "layout")
 
 # every symbol include/f4.h declares
-SYMBOLS = ("f4_mesh_create", "f4_mesh_destroy", "f4_set_options", "f4_set_flux_fix", "f4_set_gravity", "f4_set_rk_scheme", "f4_storage_bytes", "f4_bind_storage",
+SYMBOLS = ("f4_mesh_create", "f4_mesh_destroy", "f4_set_options", "f4_set_flux_fix", "f4_set_bc_values", "f4_set_gravity", "f4_set_rk_scheme", "f4_storage_bytes", "f4_bind_storage",
            "f4_num_blocks", "f4_get_blocks", "f4_set_state", "f4_get_state", "f4_build_ghost_pattern",
            "f4_pattern_size", "f4_get_pattern", "f4_fill_ghosts", "f4_compute_dt", "f4_advance", "f4_refine_flags", "f4_adapt",
            "f4_conserved_totals", "f4_profile_enable", "f4_profile_get", "f4_launch_count", "f4_last_error",
@@ -63,6 +63,7 @@ def lib():
     L.f4_set_flux_fix.argtypes = [vp, C.c_int]
     L.f4_set_rk_scheme.argtypes = [vp, C.c_int]
     L.f4_set_gravity.argtypes = [vp, dp]
+    L.f4_set_bc_values.argtypes = [vp, dp]
     L.f4_refine_flags.argtypes = [vp, C.c_int, C.c_int, C.c_int, dp, ip, dp]
     L.f4_storage_bytes.restype = C.c_size_t
     L.f4_storage_bytes.argtypes = [vp]
@@ -180,6 +181,11 @@ class Mesh:
 
     def set_options(self, limiter=LIM_VANLEER, flux=FLUX_HLL, theta=1.0):
         self._chk(self.L.f4_set_options(self.h, limiter, flux, theta))
+
+    def set_bc_values(self, values):
+        v = np.ascontiguousarray(values, dtype=np.float64)
+        assert v.shape == (6, self.nvar)
+        self._chk(self.L.f4_set_bc_values(self.h, _dp(v)))
 
     def set_gravity(self, g):
         gg = np.zeros(3, dtype=np.float64)

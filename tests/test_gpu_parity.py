@@ -657,3 +657,55 @@ def test_repeated_runs_are_bit_identical(n, scale):
         else:
             assert np.array_equal(out[0], ref[0]) and np.array_equal(out[1], ref[1]), rep
     lm.close()
+
+
+# ------------------------------------------------------------------ uniform Dirichlet / Neumann faces
+DIR, NEU = W.DIRICHLET, W.NEUMANN
+
+
+@pytest.mark.parametrize("dim,N,bc,amr", [
+    (2, 8, [DIR, NEU, NEU, DIR], False), (2, 16, [DIR, DIR, PER, PER], True), (3, 8, [NEU, DIR, PER, PER, DIR, NEU], True),
+    (3, 16, [DIR, NEU, DIR, NEU, OUT, DIR], False), (3, 32, [PER, PER, NEU, NEU, DIR, DIR], False)])
+def test_dirichlet_neumann_ghosts_bit_exact_and_step_parity(dim, N, bc, amr):
+    if amr:
+        cfg, lm, om = _refined_pair(dim, N, bc, rounds=2, seed=21)
+        cfg = dict(cfg, brick=tuple(cfg["brick"]) + (1,) * (3 - dim))
+    else:
+        cfg = dict(dim=dim, block_n=N, n_ghost=2, brick=(2, 1, 2)[:dim] + (1,) * (3 - dim), base_level=0, max_level=0,
+                   bc=bc + [PER] * (6 - len(bc)), gamma=1.4)
+        lm, om = make_pair(cfg)
+    nvar = dim + 2
+    rng = np.random.default_rng(8)
+    la, ca = lm.get_blocks()
+    u = _wave_state(cfg, la, ca)
+    perm = perm_lib_to_ora(lm, om)
+    uo = np.empty_like(u)
+    uo[perm] = u
+    # boundary data near the state's own values (Dirichlet) / small derivatives (Neumann), different per face and variable
+    vals = np.zeros((6, nvar))
+    mean = u.mean(axis=(0, 2, 3, 4))
+    for f in range(2 * dim):
+        vals[f] = mean * (1.0 + 0.05 * rng.uniform(-1, 1, nvar)) if bc[f] == DIR else 0.3 * rng.uniform(-1, 1, nvar)
+    lm.set_bc_values(vals)
+    om.set_bc_values(vals)
+    lm.set_state(0, u)
+    om.set_state(0, uo)
+    lm.fill_ghosts(0)
+    om.fill_ghosts(0)
+    pg, po = lm.get_state(0, with_ghosts=True), om.get_state(0, with_ghosts=True)[perm]
+    nc = noncorner_mask(lm)
+    if not amr:
+        for v in range(nvar):
+            assert np.array_equal(pg[:, v][nc], po[:, v][nc])          # every face ghost, bit for bit
+    else:
+        _, _, outside = H.padded_coords(dim, N, 2, cfg["brick"], la, ca)
+        for v in range(nvar):
+            assert np.array_equal(pg[:, v][nc & outside], po[:, v][nc & outside])   # the physical-boundary ghosts
+    assert (pg[:, 0][nc] != 0).all()
+    for s in range(3 if N < 32 else 2):
+        dt = 0.5 * om.compute_dt(0, 0.4)
+        om.advance(dt)
+        lm.advance(dt)
+    err = H.rel_linf(lm.get_state(0), om.get_state(0)[perm])
+    assert np.all(err <= TOL_STATE), err
+    lm.close()

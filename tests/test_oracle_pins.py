@@ -897,3 +897,72 @@ def test_gravity_hydrostatic_balance_converges_at_second_order():
         u = m.get_state(0)
         errs.append(np.abs(u[:, 2] / u[:, 0]).max())
     assert errs[0] / errs[1] > 3.0 and errs[1] / errs[2] > 3.0, errs
+
+
+# ---------------------------------------------------------------- uniform Dirichlet / Neumann boundaries
+DIR, NEU = W.DIRICHLET, W.NEUMANN
+
+
+@pytest.mark.parametrize("dim", [2, 3])
+def test_dirichlet_and_neumann_ghosts_reproduce_a_linear_profile(dim):
+    # u_v = a_v + b_v * n along the normal of the boundary, everything in binary fractions so that the expected
+    # ghost values are exact: with u_b = the face value (Dirichlet) or u_b' = the outward derivative (Neumann) the
+    # ghost cells must continue the linear profile (a wrong sign, layer index or mirror cell breaks it)
+    N, P = 8, 12
+    nvar = dim + 2
+    a_v = np.array([1.0, -0.5, 0.25, 2.0, 3.0][:nvar])
+    b_v = np.array([2.0, 1.0, -4.0, 0.5, -1.0][:nvar])
+    dx = 1.0 / N
+    for axis in range(dim):
+        for kind in (DIR, NEU):
+            bc = [PER] * 6
+            bc[2 * axis] = bc[2 * axis + 1] = kind
+            m = O.OracleMesh(dim, N, 2, (1,) * dim, 0, 0, bc, 1.4, 2)
+            x = (np.arange(-2, N + 2) + 0.5) * dx                     # cell centres along the axis, ghosts included
+            shape = [1, 1, 1]
+            shape[2 - axis] = P
+            prof = x.reshape(shape)
+            u = np.zeros((1, nvar, P if dim == 3 else 1, P, P))
+            for v in range(nvar):
+                u[0, v] = a_v[v] + b_v[v] * prof
+            vals = np.zeros((6, nvar))
+            if kind == DIR:
+                vals[2 * axis] = a_v                                   # face at x = 0
+                vals[2 * axis + 1] = a_v + b_v                         # face at x = 1
+            else:
+                vals[2 * axis] = -b_v                                  # outward normal derivative
+                vals[2 * axis + 1] = b_v
+            m.set_bc_values(vals)
+            interior = u[:, :, 2:-2, 2:-2, 2:-2] if dim == 3 else u[:, :, :, 2:-2, 2:-2]
+            m.set_state(0, np.ascontiguousarray(interior))
+            m.fill_ghosts(0)
+            g = m.get_state(0, with_ghosts=True)
+            sl = [slice(None), slice(None)] + ([slice(2, -2)] * 3 if dim == 3 else [slice(0, 1), slice(2, -2), slice(2, -2)])
+            sl[4 - axis] = slice(None)                                 # all cells along the axis, interior transverse
+            assert np.array_equal(g[tuple(sl)], u[tuple(sl)]), (axis, kind)
+
+
+def test_neumann_zero_derivative_is_outflow_and_dirichlet_hand_value():
+    cfg = dict(dim=2, block_n=8, n_ghost=2, brick=(2, 1, 1), base_level=0, max_level=0, gamma=1.4)
+    rng = np.random.default_rng(3)
+    a = O.OracleMesh.from_config(dict(cfg, bc=[OUT] * 6))
+    b = O.OracleMesh.from_config(dict(cfg, bc=[NEU] * 6))
+    c = O.OracleMesh.from_config(dict(cfg, bc=[DIR] * 6))
+    u = rng.uniform(0.5, 2.0, a.get_state(0).shape)
+    vals = np.arange(24, dtype=np.float64).reshape(6, 4) / 8.0
+    for m in (a, b, c):
+        m.set_state(0, u)
+    b.set_bc_values(np.zeros((6, 4)))
+    c.set_bc_values(vals)
+    for m in (a, b, c):
+        m.fill_ghosts(0)
+    ga, gb, gc = (m.get_state(0, with_ghosts=True) for m in (a, b, c))
+    assert np.array_equal(ga, gb)                                      # u_b' = 0: the outflow rule, bit for bit
+    lev, co = c.get_blocks()
+    b0 = int(np.argmax(co[:, 0] == 0))
+    # -x face (direction 0) of the left block, variable 2, row j = 3 (padded 5): ghost layers 1, 2 mirror cells 1, 2
+    for gl in (1, 2):
+        assert gc[b0, 2, 0, 5, 2 - gl] == 2.0 * vals[0, 2] - u[b0, 2, 0, 3, gl - 1]
+    # +y face (direction 3), variable 1, column i = 6 (padded 8)
+    for gl in (1, 2):
+        assert gc[b0, 1, 0, 9 + gl, 8] == 2.0 * vals[3, 1] - u[b0, 1, 0, 8 - gl, 6]
