@@ -593,6 +593,7 @@ int f4_advance(f4_mesh* m, double dt) {
     for (int r = 0; r < ss.np; ++r) { pv[r] = m->state_ptr(ss.prev[r]); w[r] = ss.w[r]; }
     p.prev0 = pv[0]; p.prev1 = pv[1]; p.prev2 = pv[2]; p.prev3 = pv[3];
     p.w0 = w[0]; p.w1 = w[1]; p.w2 = w[2]; p.w3 = w[3];
+    p.grav_from = (ss.prev[0] == ss.deriv) ? 0 : ((ss.np > 1 && ss.prev[1] == ss.deriv) ? 1 : 2);
     p.dt_sub = ss.dtf * dt;
     for (int l = 0; l < MAXL; ++l) {
       p.inv_dx_l[l] = inv_dx0 * (double)(1u << l);

@@ -45,6 +45,7 @@ struct StageParams {
   // gravity source term S = (0, rho g, rho g.u), eq. (20) PAPER.md:429-431 (general instances)
   double grav[3];
   int has_grav;
+  int grav_from;   // where the kernel finds s_deriv's own-cell conservative values: 0 prev0, 1 prev1, 2 load from deriv
 };
 
 // one coarse block with at least one finer face neighbour (flux fixing)

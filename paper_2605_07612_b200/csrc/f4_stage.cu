@@ -284,11 +284,14 @@ struct Cfg {  // FAST (van Leer + HLL fixed at compile time) does not change the
   static_assert(TG % 32 == 0 && N % TY == 0 && GROUP_DOUBLES % 2 == 0, "tile shape");
 };
 
-template <int DIM, int N, int TY, int G, int EXBUF, int HW, bool FAST, bool BF>
+// GEN: 0 = the path every BASELINE config takes; 1 = + gravity source term; 2 = + boundary-flux store (flux fixing)
+// and a third / fourth previous state.
+template <int DIM, int N, int TY, int G, int EXBUF, int HW, bool FAST, int GEN>
 __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
                                   F4_MINB((Cfg<DIM, N, TY, G, EXBUF, HW>::SMEM <= 110 * 1024) ? 2 : 1))
     stage_kernel(const __grid_constant__ StageParams p) {
   using C = Cfg<DIM, N, TY, G, EXBUF, HW>;
+  constexpr bool BF = (GEN == 2), GRAV = (GEN >= 1);
   constexpr int P = C::P, PP = C::P * C::P, NV = C::NVAR, PLANE = C::PLANE, TG = C::TG, EXV = C::EXV, NH = C::NH;
   constexpr int TGA = C::TGA;
   constexpr bool WHOLE = C::WHOLE;
@@ -501,12 +504,6 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
 #pragma unroll
     for (int f = 0; f < 2 * DIM; ++f) bfs[f] = p.bfslot[(size_t)blk * 6 + f];
   }
-  double dxg[3] = {0.0, 0.0, 0.0};                  // dx * g of this block's level (general instances only)
-  if (BF && p.has_grav) {
-    const double dxl = 1.0 / p.inv_dx_l[lvl];
-#pragma unroll
-    for (int d = 0; d < 3; ++d) dxg[d] = dxl * p.grav[d];
-  }
   constexpr int BFS = N * ((DIM == 3) ? N : 1);   // cell faces of one block face
   auto bf_store = [&](int slot, const double (&F)[5], int t1, int t2) {
     double* d = p.bflux + (size_t)slot * NV * BFS + t2 * N + t1;
@@ -522,27 +519,13 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
   uint32_t xph = 0;   // phase parity of the two exchange mbarriers
   const uint32_t barL = bars_u32 + 8u * C::NSLOT, barF = barL + 8u;
   // The x/y sweep of one converted plane W (z index kk, exchange buffers of parity par) in three phases:
-  //   1: slopes -> left states to shared memory, right states (and the gravity source) stay in registers
+  //   1: slopes -> left states to shared memory, right states stay in registers
   //   2: flux at the low x and y face of the own cell, and at the last face of each row / column
   //   3: difference with the next faces: acc = sum over the x,y faces of (F_in - F_out) of the own cell
-  auto phase1 = [&](const double* W, int par, double (&Rx)[5], double (&Ry)[5], double (&gsrc)[4]) {
+  auto phase1 = [&](const double* W, int par, double (&Rx)[5], double (&Ry)[5]) {
     double* eX = exX + (EXBUF == 2 ? par : 0) * C::EX;
     double* eY = exY + (EXBUF == 2 ? par : 0) * C::EX;
     double* sRh = sRh0 + (EXBUF == 2 ? par : 0) * NV * NH;
-    gsrc[0] = gsrc[1] = gsrc[2] = gsrc[3] = 0.0;
-    if (BF && p.has_grav) {
-      // source term of eq. (20), S = (0, rho g, rho g.u), from the cell's primitives;
-      // acc is multiplied by dt_sub/dx in the update, so dx S is what is added in phase 3.  Read here: after phase 2
-      // the ring slot of this plane may already be refilled
-      const double rho = W[own];
-      double gu = 0.0;
-#pragma unroll
-      for (int d = 0; d < DIM; ++d) {
-        gsrc[d] = rho * dxg[d];
-        gu = fma(dxg[d], W[(1 + d) * PLANE + own], gu);
-      }
-      gsrc[3] = rho * gu;
-    }
     {  // ---- phase 1: slopes -> left states to smem, right states stay in registers
       double L[5];
       slope_states(W, own, own_xm, own_xp, L, Rx);
@@ -624,8 +607,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
       }
     }
   };
-  auto phase3 = [&](int par, int kk, const double (&Fx)[5], const double (&Fy)[5], const double (&gsrc)[4],
-                    double (&acc)[5]) {
+  auto phase3 = [&](int par, int kk, const double (&Fx)[5], const double (&Fy)[5], double (&acc)[5]) {
     double* eX = exX + (EXBUF == 2 ? par : 0) * C::EX;
     double* eY = exY + (EXBUF == 2 ? par : 0) * C::EX;
     double* sRh = sRh0 + (EXBUF == 2 ? par : 0) * NV * NH;
@@ -634,11 +616,6 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
     for (int q = 0; q < 5; ++q) {
       if (DIM == 2 && q == 3) { acc[q] = 0.0; continue; }
       acc[q] = (Fx[q] - eX[pl(q) * EXV + fx + 1]) + (Fy[q] - eY[pl(q) * EXV + fy + N]);
-    }
-    if (BF && p.has_grav) {
-#pragma unroll
-      for (int d = 0; d < DIM; ++d) acc[1 + d] += gsrc[d];
-      acc[4] += gsrc[3];
     }
     if (BF) {
       if (i == N - 1 && bfs[1] >= 0) {
@@ -657,12 +634,12 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
   };
   // the three phases with a group barrier in between (2D, single exchange buffer, F4_SPLIT = 0)
   auto sweep_xy = [&](const double* W, int par, int kk, double (&acc)[5]) {
-    double Rx[5], Ry[5], Fx[5], Fy[5], gsrc[4];
-    phase1(W, par, Rx, Ry, gsrc);
+    double Rx[5], Ry[5], Fx[5], Fy[5];
+    phase1(W, par, Rx, Ry);
     sweep_sync(bar_id, TGA);
     phase2(par, kk, Rx, Ry, Fx, Fy);
     sweep_sync(bar_id, TGA);
-    phase3(par, kk, Fx, Fy, gsrc, acc);
+    phase3(par, kk, Fx, Fy, acc);
     if (EXBUF == 1) sweep_sync(bar_id, TGA);
   };
 
@@ -709,6 +686,31 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
     for (int q = 0; q < 5; ++q) {
       if (DIM == 2 && q == 3) { u[q] = 0.0; continue; }
       u[q] = fma(sdt, tot[q], fma(w1eff, b[q], p.w0 * a[q]));
+    }
+    if (GRAV && p.has_grav) {
+      // source term of eq. (20), S = (0, rho g, rho g.u) = (0, rho g, g.m) of s_deriv in this cell
+      // (PAPER.md:334 step i): its conservative values are one of the previous states already in registers
+      // (grav_from 0 / 1) or are loaded (2: s_deriv is not among the first two previous states)
+      double r0, mm[3] = {0.0, 0.0, 0.0};
+      if (p.grav_from == 0) { r0 = a[0]; mm[0] = a[1]; mm[1] = a[2]; mm[2] = a[3]; }
+      else if (p.grav_from == 1 && !(BF && pc)) { r0 = b[0]; mm[0] = b[1]; mm[1] = b[2]; mm[2] = b[3]; }
+      else {
+        const double* pg = p.deriv + boff + co + ko;
+        r0 = pg[0];
+#pragma unroll
+        for (int d = 0; d < DIM; ++d) mm[d] = pg[(1 + d) * (int)C::VS];
+      }
+      double gm = 0.0;
+#pragma unroll
+      for (int d = 0; d < DIM; ++d) {
+        u[1 + d] = fma(p.dt_sub * p.grav[d], r0, u[1 + d]);
+        gm = fma(p.grav[d], mm[d], gm);
+      }
+      u[4] = fma(p.dt_sub, gm, u[4]);
+    }
+#pragma unroll
+    for (int q = 0; q < 5; ++q) {
+      if (DIM == 2 && q == 3) continue;
       po[ko + pl(q) * (int)C::VS] = u[q];
     }
     if (ppx) {
@@ -787,10 +789,9 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
     finish(0, acc, a, b);
   } else {
     double dA[5], Lz[5], accp[5];
-    double Rxp[5], Ryp[5], gsp[4];   // SPLIT: right states (and gravity source) of the plane whose phase 1 ran ahead
+    double Rxp[5], Ryp[5];           // SPLIT: right states of the plane whose phase 1 ran ahead
 #pragma unroll
     for (int q = 0; q < 5; ++q) { dA[q] = 0.0; Lz[q] = 1.0; accp[q] = 0.0; Rxp[q] = 1.0; Ryp[q] = 1.0; }
-    gsp[0] = gsp[1] = gsp[2] = gsp[3] = 0.0;
     int sc = 0;            // ring slot of plane c (planes take the slots 0,1,2,0,...)
     uint32_t ph = 0;       // phase parity of each slot's mbarrier
     // one march iteration; the steady state (c in [2, N]) is the instance with every flag true
@@ -859,21 +860,19 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
         // iteration (phase 1 runs one plane ahead, between arrive and wait of the flux barrier); the z work sits
         // between arrive and wait of the left-state barrier.  A wait on barL also guarantees that every thread has
         // converted plane c, which is what phase 1 of plane c reads.
-        if (c == 1) phase1(Wk, c & 1, Rxp, Ryp, gsp);
+        if (c == 1) phase1(Wk, c & 1, Rxp, Ryp);
         midA();
         mbar_arrive(barL);
         midB();
         mid2();
         mbar_wait(barL, xph);
-        double Fx[5], Fy[5], gs[4], acc[5];
+        double Fx[5], Fy[5], acc[5];
         phase2(c & 1, c - 1, Rxp, Ryp, Fx, Fy);
         mbar_arrive(barF);
-#pragma unroll
-        for (int q = 0; q < 4; ++q) gs[q] = gsp[q];
-        if (c < N) phase1(Wc, (c + 1) & 1, Rxp, Ryp, gsp);
+        if (c < N) phase1(Wc, (c + 1) & 1, Rxp, Ryp);
         mbar_wait(barF, xph);
         xph ^= 1u;
-        phase3(c & 1, c - 1, Fx, Fy, gs, acc);
+        phase3(c & 1, c - 1, Fx, Fy, acc);
 #pragma unroll
         for (int q = 0; q < 5; ++q) accp[q] = acc[q] + Fz[q];
       } else if (SWEEP) {
@@ -922,24 +921,29 @@ cudaError_t launch_cfg(const StageParams& p, cudaStream_t s) {
     auto set = [&](auto* k) {
       if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
     };
-    set(stage_kernel<DIM, N, TY, G, EXBUF, HW, true, false>);
-    set(stage_kernel<DIM, N, TY, G, EXBUF, HW, false, false>);
-    set(stage_kernel<DIM, N, TY, G, EXBUF, HW, true, true>);
-    set(stage_kernel<DIM, N, TY, G, EXBUF, HW, false, true>);
+    set(stage_kernel<DIM, N, TY, G, EXBUF, HW, true, 0>);
+    set(stage_kernel<DIM, N, TY, G, EXBUF, HW, false, 0>);
+    set(stage_kernel<DIM, N, TY, G, EXBUF, HW, true, 1>);
+    set(stage_kernel<DIM, N, TY, G, EXBUF, HW, false, 1>);
+    set(stage_kernel<DIM, N, TY, G, EXBUF, HW, true, 2>);
+    set(stage_kernel<DIM, N, TY, G, EXBUF, HW, false, 2>);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
   const int nitems = p.nblocks * C::YT;
   const int grid = (nitems + G - 1) / G;
   const bool fast = p.limiter == F4_LIM_VANLEER && p.flux == F4_FLUX_HLL;
-  if (p.bfslot || p.prev2 || p.has_grav) {   // general instances: boundary-flux store (flux fixing) and / or > 2 previous states
+  if (p.bfslot || p.prev2) {   // general instances: boundary-flux store (flux fixing) and / or > 2 previous states
     if (HW != 0) return cudaErrorInvalidValue;   // the helper-warp variant has no flux store
-    if (fast) stage_kernel<DIM, N, TY, G, EXBUF, HW, true, true><<<grid, C::NT, C::SMEM, s>>>(p);
-    else stage_kernel<DIM, N, TY, G, EXBUF, HW, false, true><<<grid, C::NT, C::SMEM, s>>>(p);
+    if (fast) stage_kernel<DIM, N, TY, G, EXBUF, HW, true, 2><<<grid, C::NT, C::SMEM, s>>>(p);
+    else stage_kernel<DIM, N, TY, G, EXBUF, HW, false, 2><<<grid, C::NT, C::SMEM, s>>>(p);
+  } else if (p.has_grav) {     // the configs' path + gravity source term
+    if (fast) stage_kernel<DIM, N, TY, G, EXBUF, HW, true, 1><<<grid, C::NT, C::SMEM, s>>>(p);
+    else stage_kernel<DIM, N, TY, G, EXBUF, HW, false, 1><<<grid, C::NT, C::SMEM, s>>>(p);
   } else if (fast) {
-    stage_kernel<DIM, N, TY, G, EXBUF, HW, true, false><<<grid, C::NT, C::SMEM, s>>>(p);
+    stage_kernel<DIM, N, TY, G, EXBUF, HW, true, 0><<<grid, C::NT, C::SMEM, s>>>(p);
   } else {
-    stage_kernel<DIM, N, TY, G, EXBUF, HW, false, false><<<grid, C::NT, C::SMEM, s>>>(p);
+    stage_kernel<DIM, N, TY, G, EXBUF, HW, false, 0><<<grid, C::NT, C::SMEM, s>>>(p);
   }
   return cudaGetLastError();
 }

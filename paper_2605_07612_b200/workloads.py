@@ -83,9 +83,24 @@ def config(n: int, scale: int | None = None) -> dict:
     elif n == 5:
         c = dict(dim=3, block_n=16, brick=(1, 1, 1), base_level=3, max_level=6, bc=out,
                  steps=100, seed=1005, ic="blast", regrid_every=10)
+    elif n == 6:
+        # Not a BASELINE.json config: the paper's own Euler benchmark, the Rayleigh-Taylor set-up of PAPER.md:425-431
+        # as run for Table 1 (3D 512^3, 16^3 blocks, van Leer, Heun, CFL 0.5, gamma = 5/3,
+        # g = (0,0,-1), periodic in x and y).  The paper does not state the top / bottom boundary condition nor the
+        # pressure at the top; reading B5: uniform Neumann faces that continue the hydrostatic state of
+        # a gas at rest -- d(rho)/dn = d(momentum)/dn = 0, dE/dn = -+rho g/(gamma-1) -- and p_top = 1.
+        g1 = 5.0 / 3.0 - 1.0
+        bcv = [[0.0] * 5 for _ in range(6)]
+        bcv[4][4] = 0.1 / g1       # -z face: outward normal is -z, dE/dz = -rho_low/(gamma-1)
+        bcv[5][4] = -1.0 / g1      # +z face: dE/dz = -rho_high/(gamma-1)
+        c = dict(dim=3, block_n=16, brick=(1, 1, 1), base_level=5, max_level=5,
+                 bc=[PERIODIC] * 4 + [NEUMANN] * 2, steps=20, seed=1006, ic="rt",
+                 gravity=(0.0, 0.0, -1.0), bc_values=bcv)
     else:
-        raise ValueError("config 1..5")
+        raise ValueError("config 1..6")
     c.update(n_ghost=2, gamma=1.4, cfl=0.4, name=f"config{n}")
+    if n == 6:
+        c.update(gamma=5.0 / 3.0, cfl=0.5, name="rayleigh-taylor")
     if scale is not None:
         if n == 5:
             c["max_level"] = c["base_level"] + scale
@@ -198,6 +213,13 @@ def initial_primitives(cfg: dict, levels, coords, noise: bool = True) -> np.ndar
         r2 = (x - c[0]) ** 2 + (y - c[1]) ** 2 + (z - c[2]) ** 2
         w[:, 0] = 1.0
         w[:, nvar - 1] = np.where(r2 < 0.05 ** 2, 100.0, 1e-2)
+    elif ic == "rt":  # heavy (rho = 1) over light (rho = 0.1) fluid, interface at
+        # h(x,y) = 0.8 + 0.05 sin(2 pi x) sin(2 pi y), at rest, pressure in hydrostatic balance with g = (0,0,-1)
+        z = xyz[2]
+        h = 0.8 + 0.05 * np.sin(2 * np.pi * x) * np.sin(2 * np.pi * y)
+        above = z > h
+        w[:, 0] = np.where(above, 1.0, 0.1)
+        w[:, nvar - 1] = np.where(above, 1.0 + 1.0 * (1.0 - z), 1.0 + 1.0 * (1.0 - h) + 0.1 * (h - z))
     elif ic == "uniform":
         w[:, 0] = cfg.get("rho0", 1.0)
         for a in range(dim):
@@ -227,6 +249,16 @@ def prim_to_cons(w: np.ndarray, gamma: float) -> np.ndarray:
 def initial_state(cfg: dict, levels, coords, noise: bool = True) -> np.ndarray:
     """Conservative interior state [nb, nvar, Nz, Ny, Nx] (C-contiguous)."""
     return np.ascontiguousarray(prim_to_cons(initial_primitives(cfg, levels, coords, noise), cfg["gamma"]))
+
+
+def apply_physics(cfg: dict, mesh) -> None:
+    """Hand the config's run-time options (gravity, uniform boundary values) to a mesh object of either
+    implementation (same method names); argument passing only."""
+    if "gravity" in cfg:
+        mesh.set_gravity(cfg["gravity"])
+    if "bc_values" in cfg:
+        nvar = cfg["dim"] + 2
+        mesh.set_bc_values(np.asarray(cfg["bc_values"], dtype=np.float64)[:, :nvar])
 
 
 def uniform_blocks(cfg: dict):
