@@ -279,8 +279,9 @@ struct Cfg {  // FAST (van Leer + HLL fixed at compile time) does not change the
   static constexpr int NBAR = NSLOT + 2;     // ring slots + "left states written" + "fluxes written"
   static constexpr size_t SMEM = (size_t)G * GROUP_DOUBLES * 8 + (size_t)G * NBAR * 8;
   static constexpr int HALO = 4 * TY + 4 * N;  // halo cells of an interior plane
-  static_assert(HW == 1 || (HALO <= TG && 3 * NH <= TG), "halo work needs one pass");
-  static_assert(HW == 0 || (HW == 1 && DIM == 3), "helper warp: 3D only");
+  static_assert(HALO <= TG && 3 * NH <= TG, "halo work needs one pass");
+  static_assert(HW == 0, "a ninth helper warp per block for the halo work was measured slower (19.7 vs 20.8 GCUPS: a "
+                         "288-thread CTA puts three warps on one SM sub-partition, which caps registers at 96) and removed");
   static_assert(TG % 32 == 0 && N % TY == 0 && GROUP_DOUBLES % 2 == 0, "tile shape");
 };
 
@@ -426,10 +427,9 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
   const int own_xm = (i == 0) ? (rr | 1) * P + N + 2 * (rr & 1) + 1 : own - 1;
   const int own_xp = (i == N - 1) ? (rr & ~1) * P + N + 2 * (rr & 1) : own + 1;
   const int fx = j * (N + 1) + i, fy = j * N + i;      // own low faces in the exchange arrays
-  // ---- halo tasks (cells and faces outside the tile's own N x TY cells).  Without a helper warp they are roles of
-  //      the cell threads: [0,NH) high halo slopes, [NH,2NH) low halo slopes, [2NH,3NH) last-face fluxes, the last
-  //      HALO threads convert the halo cells.  With HW = 1 the helper warp loops over all of them, so that the cell
-  //      warps (whose dependent-issue latency is the critical path of a plane) all carry the same work.
+  // ---- halo tasks (cells and faces outside the tile's own N x TY cells) are roles of the cell threads:
+  //      [0,NH) high halo slopes, [NH,2NH) low halo slopes, [2NH,3NH) last-face fluxes, the last HALO threads
+  //      convert the halo cells.  (A ninth helper warp looping over all of them was tried and removed, see Cfg.)
   // slope task h in [0, 2NH): high halo cell of row/column h (right state -> sRh), low halo cell h-NH (left state -> e)
   auto halo_slope_task = [&](const double* W, double* eX, double* eY, double* sRh, int h) {
     const bool hi = h < NH;
@@ -737,46 +737,6 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
 
   constexpr int ISSUER = (TG >= 128) ? 96 : 0;   // lane 0 of a warp without halo roles when the group has one
   if (DIM == 3 && t == ISSUER) { issue_plane(-2, 0); issue_plane(-1, 1); }
-  if (HW == 1 && t >= TG) {
-    // ---- helper warp (3D): mirrors the barrier sequence of the march below.  Per plane: convert the halo cells of
-    //      plane c, halo slopes of plane c-1 | barrier | last-face fluxes | barrier | refill the freed ring slot.
-    const int lane = t - TG;
-    int sc = 0;
-    uint32_t ph = 0;
-#pragma unroll 1
-    for (int c = -2; c <= N + 1; ++c) {
-      const int sk = (sc == 0) ? 2 : sc - 1;
-      double* Wc = ring + sc * C::SLOT;
-      const double* Wk = ring + sk * C::SLOT;
-      mbar_wait(bars_u32 + 8u * sc, (ph >> sc) & 1u);
-      ph ^= 1u << sc;
-      if (c >= 0 && c < N) {
-#pragma unroll
-        for (int h = 0; h < (C::HALO + 31) / 32; ++h)
-          if (h * 32 + lane < C::HALO) halo_convert_task(Wc, h * 32 + lane);
-      }
-      fence_proxy_async();
-      if (c >= 1 && c <= N) {
-        double* eX = exX + (EXBUF == 2 ? (c & 1) : 0) * C::EX;
-        double* eY = exY + (EXBUF == 2 ? (c & 1) : 0) * C::EX;
-#pragma unroll
-        for (int h = 0; h < (2 * NH + 31) / 32; ++h)
-          if (h * 32 + lane < 2 * NH) halo_slope_task(Wk, eX, eY, sRh0 + (EXBUF == 2 ? (c & 1) : 0) * NV * NH, h * 32 + lane);
-        group_sync(bar_id, TGA);
-#pragma unroll
-        for (int h = 0; h < (NH + 31) / 32; ++h)
-          if (h * 32 + lane < NH) halo_flux_task(eX, eY, sRh0 + (EXBUF == 2 ? (c & 1) : 0) * NV * NH, h * 32 + lane);
-        group_sync(bar_id, TGA);
-        if (EXBUF == 1) group_sync(bar_id, TGA);
-      } else {
-        group_sync(bar_id, TGA);
-      }
-      if (lane == 0 && c + 2 <= N + 1) issue_plane(c + 2, sk);
-      sc = (sc == 2) ? 0 : sc + 1;
-    }
-    return;
-  }
-
   if (DIM == 2) {
     double a[5], b[5], w[5], acc[5];
     if (t == ISSUER) issue_plane(0, 0);
@@ -934,7 +894,6 @@ cudaError_t launch_cfg(const StageParams& p, cudaStream_t s) {
   const int grid = (nitems + G - 1) / G;
   const bool fast = p.limiter == F4_LIM_VANLEER && p.flux == F4_FLUX_HLL;
   if (p.bfslot || p.prev2) {   // general instances: boundary-flux store (flux fixing) and / or > 2 previous states
-    if (HW != 0) return cudaErrorInvalidValue;   // the helper-warp variant has no flux store
     if (fast) stage_kernel<DIM, N, TY, G, EXBUF, HW, true, 2><<<grid, C::NT, C::SMEM, s>>>(p);
     else stage_kernel<DIM, N, TY, G, EXBUF, HW, false, 2><<<grid, C::NT, C::SMEM, s>>>(p);
   } else if (p.has_grav) {     // the configs' path + gravity source term
@@ -958,22 +917,13 @@ cudaError_t launch_stage(int dim, int n, const StageParams& p, cudaStream_t s) {
   if (p.nblocks <= 0) return cudaSuccess;
   if (dim == 2 && n == 8) return launch_cfg<2, 8, 8, 4, 1>(p, s);
   if (dim == 2 && n == 16) return launch_cfg<2, 16, 16, 1, 1>(p, s);
-  // HW = 1 (a ninth warp per block for all halo work) is correct and halves the barrier stalls, but a CTA of 288
-  // threads is allocated registers as 10 warps, which caps the cell threads at 96 registers (spills, late u_t loads):
-  // measured 19.7 vs 20.8 GCUPS on config 3, so the default keeps the halo roles on cell threads.
-#ifndef F4_HW16
-#define F4_HW16 0
-#endif
-#ifndef F4_HW8
-#define F4_HW8 0
-#endif
 #ifndef F4_G8
 #define F4_G8 4
 #endif
 #ifndef F4_EX8
 #define F4_EX8 1
 #endif
-  if (dim == 3 && n == 8) return launch_cfg<3, 8, 8, F4_G8, F4_EX8, F4_HW8>(p, s);
+  if (dim == 3 && n == 8) return launch_cfg<3, 8, 8, F4_G8, F4_EX8, 0>(p, s);
 #ifndef F4_TY16
 #define F4_TY16 16
 #endif
@@ -983,7 +933,7 @@ cudaError_t launch_stage(int dim, int n, const StageParams& p, cudaStream_t s) {
 #ifndef F4_EX16
 #define F4_EX16 2
 #endif
-  if (dim == 3 && n == 16) return launch_cfg<3, 16, F4_TY16, F4_G16, F4_EX16, F4_HW16>(p, s);
+  if (dim == 3 && n == 16) return launch_cfg<3, 16, F4_TY16, F4_G16, F4_EX16, 0>(p, s);
   if (dim == 3 && n == 32) return launch_cfg<3, 32, 8, 1, 2>(p, s);
   return cudaErrorInvalidValue;
 }
