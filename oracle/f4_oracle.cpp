@@ -8,8 +8,10 @@
 // restriction, C2F prolongation in two rounds) + per-block finite-volume
 // update (primitive reconstruction, HLL flux with Einfeldt speeds,
 // conservative update, Runge-Kutta combine, CFL reduction) + mesh adapt with
-// regrid data transfer; also flux fixing at refinement boundaries
-// and the refinement criteria (eq. (12); config 5's pressure jump).
+// regrid data transfer; also flux fixing at refinement boundaries,
+// the refinement criteria (eq. (12); config 5's pressure jump), the
+// other Runge-Kutta schemes of eq. (5), the gravity source term
+// eq. (20) and uniform Dirichlet / Neumann boundaries.
 //
 // Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
 // --impl reference legs may build, load or call this file.  It shares no code
@@ -25,11 +27,17 @@
 // wave (P4), linear-field ghost/prolong/restrict exactness PAPER.md:433-447
 // (P5), restriction = block average (P6), Appendix-A closed form eq. (24)
 // (P7), block permutation (P8), RK closed form (P9), 1D-in-3D (P10), mirror
-// symmetry (P11), brute-force mesh validity.
+// symmetry (P11), brute-force mesh validity; flux fixing by the paper's conservation
+// test; eq. (12) by hand-worked values (tests/golden/lohner_eq12.txt);
+// RK schemes by their stability polynomials and temporal order; gravity by the free-fall
+// closed form and hydrostatic convergence; Dirichlet / Neumann ghosts by exact
+// continuation of linear profiles.
 // PARITY UNPINNED: the *choice* among readings A1 (van Leer harmonic form),
 // A2 (HLL), A3 (Einfeldt speeds = Roe-average u^ +- d^), A5 (CFL sum over
-// dimensions), A10 (outflow = zero-order extrapolation) cannot be pinned
-// against foap4 itself: the paper prints no formula or worked value for them.
+// dimensions), A10 / A10b (outflow = zero-order extrapolation; Dirichlet mirror,
+// Neumann first-order extrapolation) and the SSPRK(3,3) / SSPRK(4,3) tableaux (taken
+// from the literature the paper cites, [20]) cannot be pinned against foap4 itself:
+// the paper prints no formula or worked value for them.
 // =============================================================================
 #include <algorithm>
 #include <array>
