@@ -69,7 +69,8 @@ enum {
                           (reading A10b; u_b' = 0 is F4_BC_OUTFLOW) */
 };
 
-enum { F4_LIM_VANLEER = 0, F4_LIM_MINMOD = 1, F4_LIM_MC = 2 }; /* PAPER.md:322-326; reading A1 */
+enum { F4_LIM_VANLEER = 0, F4_LIM_MINMOD = 1, F4_LIM_MC = 2, /* PAPER.md:322-326; reading A1 */
+       F4_LIM_KOREN = 3, F4_LIM_WENO3 = 4 };                 /* 2-ghost schemes of PAPER.md:325-326; reading A1b */
 enum { F4_FLUX_HLL = 0, F4_FLUX_RUSANOV = 1 };                 /* PAPER.md:328; reading A2 */
 /* Runge-Kutta schemes of the restricted class eq. (5): Heun = SSPRK(2,2) eq. (6)-(7) (default),
  * forward Euler, SSPRK(3,3), SSPRK(4,3) ("optimal SSP schemes with two, three and four stages"),

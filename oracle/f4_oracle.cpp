@@ -53,7 +53,7 @@
 namespace {
 
 enum { BC_PERIODIC = 0, BC_OUTFLOW = 1, BC_KEEP = 2, BC_DIRICHLET = 3, BC_NEUMANN = 4 };
-enum { LIM_VANLEER = 0, LIM_MINMOD = 1, LIM_MC = 2 };
+enum { LIM_VANLEER = 0, LIM_MINMOD = 1, LIM_MC = 2, LIM_KOREN = 3, LIM_WENO3 = 4 };
 enum { FLUX_HLL = 0, FLUX_RUSANOV = 1 };
 enum { NB_BOUNDARY = 0, NB_SAME = 1, NB_COARSE = 2, NB_FINE = 3 };
 
@@ -133,11 +133,32 @@ double vanleer(double a, double b) {
   if (a * b > 0.0) return 2.0 * a * b / (a + b);
   return 0.0;
 }
+// Koren's limiter (reading A1b): the kappa = 1/3 (third-order) slope (a + 2b)/3 towards the face on the
+// b side, limited to [0, 2a] and [0, 2b]: phi(r) = max(0, min(2r, (2 + r)/3, 2)), r = a/b.  Not symmetric in (a, b).
+double koren(double a, double b) {
+  if (a * b <= 0.0) return 0.0;
+  double m = std::min(std::min(2.0 * std::fabs(a), (std::fabs(a) + 2.0 * std::fabs(b)) / 3.0), 2.0 * std::fabs(b));
+  return (a > 0.0) ? m : -m;
+}
+// Third-order WENO (reading A1b: the classical Jiang-Shu weights, eps = 1e-6): two linear candidates
+// w + a/2 (from the far side) and w + b/2 (from the face side), ideal weights 1/3 and 2/3, smoothness a^2 and b^2.
+// Returned as the equivalent slope s with w_face = w + s/2.
+double weno3(double a, double b) {
+  const double eps = 1e-6;
+  double a0 = (1.0 / 3.0) / ((eps + a * a) * (eps + a * a));
+  double a1 = (2.0 / 3.0) / ((eps + b * b) * (eps + b * b));
+  return (a0 * a + a1 * b) / (a0 + a1);
+}
+// slope of a cell towards the face on the side of difference b (a = the difference on the other side): the left state
+// of the cell's high face is w + s(a,b)/2 with a = w_i - w_{i-1}, b = w_{i+1} - w_i; the right state of its low face
+// is w - s(b,a)/2.  van Leer, minmod and MC are symmetric in (a, b).
 double limited_slope(const Mesh& m, double a, double b) {
   switch (m.limiter) {
     case LIM_VANLEER: return vanleer(a, b);
     case LIM_MINMOD: return minmod_G(a, b, 1.0);
-    default: return minmod_G(a, b, 2.0);          // MC
+    case LIM_MC: return minmod_G(a, b, 2.0);      // MC
+    case LIM_KOREN: return koren(a, b);
+    default: return weno3(a, b);
   }
 }
 
@@ -437,7 +458,7 @@ int forward_euler(Mesh& m, int s_out, int s_deriv, double dt_sub, int n_prev, co
       Prim L{}, R{};
       for (int v = 0; v < nvar; ++v) {
         double sl = limited_slope(m, comp(w0, v) - comp(wm1, v), comp(w1, v) - comp(w0, v));
-        double sr = limited_slope(m, comp(w1, v) - comp(w0, v), comp(w2, v) - comp(w1, v));
+        double sr = limited_slope(m, comp(w2, v) - comp(w1, v), comp(w1, v) - comp(w0, v));  // towards its low face
         setc(L, v, comp(w0, v) + 0.5 * sl);  // w_{i+1/2,L}
         setc(R, v, comp(w1, v) - 0.5 * sr);  // w_{i+1/2,R}
       }
@@ -966,6 +987,8 @@ void ora_face_table(void* h, int* kind, int* nbr, int* off) {
 // elementary functions exposed for the pins
 double ora_minmod_G(double a, double b, double theta) { return minmod_G(a, b, theta); }
 double ora_vanleer(double a, double b) { return vanleer(a, b); }
+double ora_koren(double a, double b) { return koren(a, b); }
+double ora_weno3(double a, double b) { return weno3(a, b); }
 // HLL/Rusanov flux for primitive states wL, wR = (rho, u[dim], p) along dir
 void ora_riemann_flux(int dim, double gamma, int flux_scheme, const double* wL, const double* wR, int dir, double* F) {
   Mesh m{}; m.dim = dim; m.nvar = dim + 2; m.gamma = gamma; m.flux_scheme = flux_scheme;

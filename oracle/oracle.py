@@ -18,7 +18,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "f4_oracle.cpp")
 _LIB = os.path.join(_HERE, "libf4oracle.so")
 
-LIM_VANLEER, LIM_MINMOD, LIM_MC = 0, 1, 2
+LIM_VANLEER, LIM_MINMOD, LIM_MC, LIM_KOREN, LIM_WENO3 = 0, 1, 2, 3, 4
 FLUX_HLL, FLUX_RUSANOV = 0, 1
 NB_BOUNDARY, NB_SAME, NB_COARSE, NB_FINE = 0, 1, 2, 3
 
@@ -72,6 +72,10 @@ def lib():
         L.ora_minmod_G.argtypes = [C.c_double] * 3
         L.ora_vanleer.restype = C.c_double
         L.ora_vanleer.argtypes = [C.c_double] * 2
+        L.ora_koren.restype = C.c_double
+        L.ora_koren.argtypes = [C.c_double] * 2
+        L.ora_weno3.restype = C.c_double
+        L.ora_weno3.argtypes = [C.c_double] * 2
         L.ora_riemann_flux.argtypes = [C.c_int, C.c_double, C.c_int, dp, dp, C.c_int, dp]
         L.ora_wavespeeds.argtypes = [C.c_int, C.c_double, dp, dp, C.c_int, dp, dp]
         _lib = L
@@ -238,6 +242,14 @@ def minmod_G(a, b, theta):
 
 def vanleer(a, b):
     return lib().ora_vanleer(a, b)
+
+
+def koren(a, b):
+    return lib().ora_koren(a, b)
+
+
+def weno3(a, b):
+    return lib().ora_weno3(a, b)
 
 
 def riemann_flux(dim, gamma, wL, wR, direction, flux=FLUX_HLL):

@@ -307,7 +307,7 @@ int f4_mesh_destroy(f4_mesh* m) {
 
 int f4_set_options(f4_mesh* m, int limiter, int flux_scheme, double theta) {
   if (!m) return F4_EINVAL;
-  if (limiter < 0 || limiter > F4_LIM_MC || flux_scheme < 0 || flux_scheme > F4_FLUX_RUSANOV || !(theta >= 1.0))
+  if (limiter < 0 || limiter > F4_LIM_WENO3 || flux_scheme < 0 || flux_scheme > F4_FLUX_RUSANOV || !(theta >= 1.0))
     return fail(m, F4_EINVAL, "bad option");
   m->limiter = limiter;
   m->flux = flux_scheme;

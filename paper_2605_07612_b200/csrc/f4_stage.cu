@@ -119,8 +119,19 @@ __device__ __forceinline__ double half_slope(double a, double b, int limiter) {
     return ab * fma(y, e2, y);
   }
   double r;
+  if (limiter == F4_LIM_WENO3) {
+    // third-order WENO towards the b side (reading A1b): candidates w + a/2, w + b/2, ideal weights
+    // 1/3, 2/3, smoothness a^2, b^2, eps = 1e-6; no sign test (the weights do the limiting)
+    const double ea = 1e-6 + a * a, eb = 1e-6 + b * b;
+    const double a0 = (1.0 / 3.0) / (ea * ea), a1 = (2.0 / 3.0) / (eb * eb);
+    return 0.5 * ((a0 * a + a1 * b) / (a0 + a1));
+  }
   if (limiter == F4_LIM_VANLEER) {
     r = ab * rcp_fast(a + b);
+  } else if (limiter == F4_LIM_KOREN) {
+    // Koren (reading A1b): the kappa = 1/3 slope (a + 2b)/3 towards the b side, limited to [0,2a], [0,2b]
+    double m = fmin(fmin(2.0 * fabs(a), (fabs(a) + 2.0 * fabs(b)) / 3.0), 2.0 * fabs(b));
+    r = 0.5 * ((a > 0.0) ? m : -m);
   } else {
     double th = (limiter == F4_LIM_MC) ? 2.0 : 1.0;   // eq. (1)
     double m = fmin(fmin(fabs(th * a), fabs(th * b)), fabs(a + b) * 0.5);
@@ -412,9 +423,11 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
       if (DIM == 2 && q == 3) { L[q] = 0.0; R[q] = 0.0; continue; }
       const double* Wv = W + pl(q) * PLANE;
       const double w0 = Wv[o0];
-      const double hs = half_slope<FAST>(w0 - Wv[om], Wv[op] - w0, limiter);
+      const double da = w0 - Wv[om], db = Wv[op] - w0;
+      const double hs = half_slope<FAST>(da, db, limiter);
       L[q] = w0 + hs;
-      R[q] = w0 - hs;
+      // Koren / WENO3 are not symmetric in (a, b): the slope towards the low face takes the arguments exchanged
+      R[q] = w0 - ((!FAST && limiter >= F4_LIM_KOREN) ? half_slope<FAST>(db, da, limiter) : hs);
     }
   };
 
@@ -787,7 +800,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
           const double wa = Wk[pl(q) * PLANE + own];   // w(c-1), resident in its ring slot
           const double dB = wB[q] - wa;
           const double hs = half_slope<FAST>(dA[q], dB, limiter);  // c == -1: dA = 0 -> hs = 0, result unused
-          Rz[q] = wa - hs;
+          Rz[q] = wa - ((!FAST && limiter >= F4_LIM_KOREN) ? half_slope<FAST>(dB, dA[q], limiter) : hs);
           Lf[q] = Lz[q];                               // left state of the face between cells c-2 and c-1
           Lz[q] = wa + hs;
           dA[q] = dB;

@@ -18,7 +18,7 @@ F4_OK = 0
 ERRORS = {-1: "F4_EINVAL", -2: "F4_ENOBLOCKS", -3: "F4_ECUDA", -4: "F4_EUNBOUND", -5: "F4_EUNBALANCED",
           -6: "F4_EUNSUPPORTED"}
 BC_PERIODIC, BC_OUTFLOW, BC_KEEP, BC_DIRICHLET, BC_NEUMANN = 0, 1, 2, 3, 4
-LIM_VANLEER, LIM_MINMOD, LIM_MC = 0, 1, 2
+LIM_VANLEER, LIM_MINMOD, LIM_MC, LIM_KOREN, LIM_WENO3 = 0, 1, 2, 3, 4
 FLUX_HLL, FLUX_RUSANOV = 0, 1
 CRIT_LOHNER, CRIT_PJUMP = 0, 1
 RK_HEUN, RK_EULER, RK_SSP33, RK_SSP43, RK_RK4 = 0, 1, 2, 3, 4

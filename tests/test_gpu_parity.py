@@ -197,9 +197,12 @@ def test_ragged_and_nonpow2_bricks(dim, N, brick):
     run_and_compare(cfg, 5)
 
 
-@pytest.mark.parametrize("limiter,flux", [(f4.LIM_MINMOD, f4.FLUX_HLL), (f4.LIM_MC, f4.FLUX_RUSANOV)])
-def test_limiter_and_flux_variants(limiter, flux):
-    cfg = W.config(2, scale=1)
+@pytest.mark.parametrize("n,scale", [(2, 1), (3, 1), (1, None)])
+@pytest.mark.parametrize("limiter,flux", [(f4.LIM_MINMOD, f4.FLUX_HLL), (f4.LIM_MC, f4.FLUX_RUSANOV),
+                                          (f4.LIM_KOREN, f4.FLUX_HLL), (f4.LIM_WENO3, f4.FLUX_HLL),
+                                          (f4.LIM_WENO3, f4.FLUX_RUSANOV)])
+def test_limiter_and_flux_variants(limiter, flux, n, scale):
+    cfg = W.config(n, scale=scale)
     lm, om = make_pair(cfg)
     lm.set_options(limiter, flux, 1.0)
     om.set_options(limiter, flux, 1.0)
