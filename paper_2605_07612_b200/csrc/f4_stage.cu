@@ -947,7 +947,10 @@ cudaError_t launch_stage(int dim, int n, const StageParams& p, cudaStream_t s) {
 #define F4_EX16 2
 #endif
   if (dim == 3 && n == 16) return launch_cfg<3, 16, F4_TY16, F4_G16, F4_EX16, 0>(p, s);
-  if (dim == 3 && n == 32) return launch_cfg<3, 32, 8, 1, 2>(p, s);
+#ifndef F4_TY32
+#define F4_TY32 8
+#endif
+  if (dim == 3 && n == 32) return launch_cfg<3, 32, F4_TY32, 1, 2>(p, s);
   return cudaErrorInvalidValue;
 }
 
