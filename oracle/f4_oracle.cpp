@@ -52,7 +52,7 @@
 
 namespace {
 
-enum { BC_PERIODIC = 0, BC_OUTFLOW = 1, BC_KEEP = 2, BC_DIRICHLET = 3, BC_NEUMANN = 4 };
+enum { BC_PERIODIC = 0, BC_OUTFLOW = 1, BC_KEEP = 2, BC_DIRICHLET = 3, BC_NEUMANN = 4, BC_DATA = 5 };
 enum { LIM_VANLEER = 0, LIM_MINMOD = 1, LIM_MC = 2, LIM_KOREN = 3, LIM_WENO3 = 4 };
 enum { FLUX_HLL = 0, FLUX_RUSANOV = 1 };
 enum { NB_BOUNDARY = 0, NB_SAME = 1, NB_COARSE = 2, NB_FINE = 3 };
@@ -78,6 +78,9 @@ struct Mesh {
   int brick[3], base_level, max_level, bc[6];
   double gamma, theta;
   double bcv[6][5] = {};  // uniform boundary value u_b (Dirichlet) or normal derivative u_b' (Neumann) per face direction and variable
+  // spatially varying boundary values bc_data(i, j, ivar, ibf), eq. (4); here keyed by (block, face),
+  // layout [var][t2][t1] over the cells of the block face
+  std::map<std::pair<int, int>, std::vector<double>> bcdata;
   double grav[3] = {0.0, 0.0, 0.0};  // gravitational acceleration g of the source term eq. (20)
   int limiter, flux_scheme;
   int nstates;
@@ -256,6 +259,13 @@ void fill_bc(Mesh& m, int s, int A, int f) {
             // (reading A10b; u_b' = 0 is the outflow rule)
             const double dx = m.dx_of_level(m.blocks[A].level);
             m.at(s, A, v, di, dj, dk) = m.at(s, A, v, si, sj, sk) + ((double)g * dx) * m.bcv[f][v];
+          } else if (m.bc[f] == BC_DATA) {
+            // spatially varying Dirichlet data, eq. (4): the same mirror rule with the value of this face cell
+            auto it = m.bcdata.find({A, f});
+            double ub = (it == m.bcdata.end()) ? 0.0 : it->second[((size_t)v * kmax + (t2 - 1)) * N + (t1 - 1)];
+            int mi, mj, mk;
+            if (side) compose(a, N + 1 - g, t1, t2, mi, mj, mk); else compose(a, g, t1, t2, mi, mj, mk);
+            m.at(s, A, v, di, dj, dk) = 2.0 * ub - m.at(s, A, v, mi, mj, mk);
           } else {  // BC_DIRICHLET
             // uniform value u_b on the boundary face: ghost layer g mirrors interior layer g through
             // the face, u_ghost = 2 u_b - u_interior, so that the linear interpolant takes u_b on the face (reading A10)
@@ -886,6 +896,13 @@ void ora_set_bc_values(void* h, const double* v) {   // [6][nvar]
   Mesh* m = (Mesh*)h;
   for (int f = 0; f < 6; ++f) for (int q = 0; q < m->nvar; ++q) m->bcv[f][q] = v[f * m->nvar + q];
 }
+// boundary values of one block face of kind BC_DATA: data[nvar][kmax][N]; all entries are dropped by ora_clear_bc_data
+void ora_set_bc_face_data(void* h, int block, int face, const double* data) {
+  Mesh* m = (Mesh*)h;
+  size_t n = (size_t)m->nvar * m->N * (m->dim == 3 ? m->N : 1);
+  m->bcdata[{block, face}] = std::vector<double>(data, data + n);
+}
+void ora_clear_bc_data(void* h) { ((Mesh*)h)->bcdata.clear(); }
 void ora_set_gravity(void* h, const double* g) { for (int a = 0; a < 3; ++a) ((Mesh*)h)->grav[a] = g[a]; }
 void ora_set_test_rhs(void* h, int on, double lambda) { Mesh* m = (Mesh*)h; m->test_rhs = on; m->test_lambda = lambda; }
 int ora_num_blocks(void* h) { return (int)((Mesh*)h)->blocks.size(); }

@@ -47,6 +47,8 @@ def lib():
         L.ora_set_flux_fix.argtypes = [C.c_void_p, C.c_int]
         L.ora_set_gravity.argtypes = [C.c_void_p, dp]
         L.ora_set_bc_values.argtypes = [C.c_void_p, dp]
+        L.ora_set_bc_face_data.argtypes = [C.c_void_p, C.c_int, C.c_int, dp]
+        L.ora_clear_bc_data.argtypes = [C.c_void_p]
         L.ora_num_blocks.argtypes = [C.c_void_p]
         L.ora_get_blocks.argtypes = [C.c_void_p, ip, ip]
         L.ora_dx.restype = C.c_double
@@ -131,6 +133,15 @@ class OracleMesh:
         v = np.ascontiguousarray(values, dtype=np.float64)
         assert v.shape == (6, self.nvar)
         self.L.ora_set_bc_values(self.h, _dp(v))
+
+    def set_bc_data(self, faces, data):
+        """Spatially varying boundary values (eq. 4) of the faces of kind 5 (BC_DATA):
+        faces = [(block, face), ...], data[len(faces)][nvar][kmax][N].  Replaces all earlier data (the block
+        numbering changes with the mesh)."""
+        self.L.ora_clear_bc_data(self.h)
+        d = np.ascontiguousarray(data, dtype=np.float64)
+        for q, (b, f) in enumerate(faces):
+            self.L.ora_set_bc_face_data(self.h, int(b), int(f), _dp(np.ascontiguousarray(d[q])))
 
     def set_gravity(self, g):
         """Gravitational acceleration of the source term eq. (20); (0,0,0) = no source."""

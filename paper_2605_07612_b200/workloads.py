@@ -27,7 +27,7 @@ import numpy as np
 _K1 = np.uint64(0xD6E8FEB86659FD93)
 _K2 = np.uint64(0x9E3779B97F4A7C15)
 
-PERIODIC, OUTFLOW, KEEP, DIRICHLET, NEUMANN = 0, 1, 2, 3, 4  # values of bc_kind, same numbering as include/f4.h
+PERIODIC, OUTFLOW, KEEP, DIRICHLET, NEUMANN, BCDATA = 0, 1, 2, 3, 4, 5  # values of bc_kind, same numbering as include/f4.h
 
 
 def mix64(x: np.ndarray) -> np.ndarray:

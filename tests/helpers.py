@@ -130,3 +130,32 @@ def pressure_jump_flags_numpy(cfg: dict, padded: np.ndarray, hi: float = 0.1, lo
     flags[J > hi] = 1
     flags[J < lo] = -1
     return flags
+
+
+def boundary_faces(dim, N, brick, bc, levels, coords, kind):
+    """(block, face) pairs on the physical boundary whose face direction has bc kind `kind`, in (block, face) order,
+    and the cell-centre coordinates of their face cells: xyz[q][axis] arrays shaped [kmax, N] (t2, t1), with the
+    coordinate along the face normal set ON the face."""
+    maxb = max(brick[:dim])
+    out, xyz = [], []
+    for b, (l, c) in enumerate(zip(levels, coords)):
+        dx = 1.0 / (maxb * 2.0 ** int(l) * N)
+        for f in range(2 * dim):
+            a, side = f // 2, f % 2
+            ext = brick[a] * 2 ** int(l)
+            if bc[f] != kind or (c[a] != (ext - 1 if side else 0)):
+                continue
+            ta = [ax for ax in range(dim) if ax != a]
+            kmax = N if dim == 3 else 1
+            t1 = (c[ta[0]] * N + np.arange(N) + 0.5) * dx
+            X = [None] * 3
+            X[a] = np.full((kmax, N), (c[a] + side) * N * dx)
+            X[ta[0]] = np.broadcast_to(t1[None, :], (kmax, N)).copy()
+            if dim == 3:
+                t2 = (c[ta[1]] * N + np.arange(N) + 0.5) * dx
+                X[ta[1]] = np.broadcast_to(t2[:, None], (kmax, N)).copy()
+            else:
+                X[2] = np.zeros((kmax, N))
+            out.append((b, f))
+            xyz.append(X)
+    return out, xyz

@@ -1051,3 +1051,40 @@ def test_asymmetric_reconstructions_keep_mirror_symmetry(limiter):
     bm[1] = -bm[1]
     assert np.abs(a - bm).max() <= 1e-14, np.abs(a - bm).max()
     assert np.abs(a[0] - a[0][:, ::-1]).max() > 1e-3      # the state itself is not symmetric
+
+
+# ---------------------------------------------------------------- spatially varying boundary data, eq. (4)
+@pytest.mark.parametrize("dim", [2, 3])
+def test_bc_data_reproduces_the_linear_field_on_a_refined_mesh(dim):
+    # the paper's linear-field test (eq. 21) with the boundary values supplied through bc_data:
+    # phi = x + 2y + 3z on the boundary faces; every face ghost (physical boundary, same level, coarse-fine) must
+    # then hold phi to the paper's 1e-15 after a fill
+    N = 8
+    bc = [W.BCDATA] * 6
+    m = mesh(dim, N, (2, 1, 1)[:dim] if dim == 2 else (2, 1, 1), 0, 2, bc)
+    rng = np.random.default_rng(2)
+    for _ in range(2):
+        flags = (rng.uniform(size=m.num_blocks) < 0.4).astype(np.int32)
+        flags[0] = 1
+        m.adapt(flags)
+    lev, co = m.get_blocks()
+    brick = (2, 1, 1)
+    coef = np.array([1.0, 2.0, 3.0][:dim])
+    X, nc, _ = H.padded_coords(dim, N, 2, brick, lev, co)
+    phi = sum(coef[a] * X[a] for a in range(dim))
+    nvar = dim + 2
+    u = np.repeat(phi[:, None], nvar, axis=1) * (1.0 + np.arange(nvar))[None, :, None, None, None]
+    interior = u[:, :, 2:-2, 2:-2, 2:-2] if dim == 3 else u[:, :, :, 2:-2, 2:-2]
+    m.set_state(0, np.ascontiguousarray(interior))
+    faces, xyz = H.boundary_faces(dim, N, brick, bc, lev, co, W.BCDATA)
+    assert len(faces) > 0
+    data = np.zeros((len(faces), nvar, N if dim == 3 else 1, N))
+    for q, Xf in enumerate(xyz):
+        pf = sum(coef[a] * Xf[a] for a in range(dim))
+        for v in range(nvar):
+            data[q, v] = (1.0 + v) * pf
+    m.set_bc_data(faces, data)
+    m.fill_ghosts(0)
+    g = m.get_state(0, with_ghosts=True)
+    for v in range(nvar):
+        assert np.abs(g[:, v][nc] - u[:, v][nc]).max() <= 1e-15 * np.abs(u[:, v]).max() * 4
