@@ -65,8 +65,10 @@ enum {
   F4_BC_KEEP = 2,     /* ghosts on that face are left as the caller set them (linear-field test) */
   F4_BC_DIRICHLET = 3, /* uniform value u_b per face direction and variable (f4_set_bc_values): ghost layer g mirrors
                           interior layer g through the face, u_ghost = 2 u_b - u_interior (reading A10) */
-  F4_BC_NEUMANN = 4    /* uniform outward normal derivative u_b': ghost layer g = first interior layer + g dx u_b'
+  F4_BC_NEUMANN = 4,   /* uniform outward normal derivative u_b': ghost layer g = first interior layer + g dx u_b'
                           (reading A10b; u_b' = 0 is F4_BC_OUTFLOW) */
+  F4_BC_DATA = 5       /* spatially varying boundary values bc_data (eq. 4), one value per face cell
+                          and variable, supplied by a callback (f4_set_bc_callback); same mirror rule as Dirichlet */
 };
 
 enum { F4_LIM_VANLEER = 0, F4_LIM_MINMOD = 1, F4_LIM_MC = 2, /* PAPER.md:322-326; reading A1 */
@@ -171,6 +173,20 @@ int f4_compute_dt(f4_mesh *m, int state, double cfl, double *dt_out);
  * is bound (host call otherwise); takes effect at the next ghost fill.  Spatially varying bc_data (eq. 4) is not
  * provided: F4_BC_KEEP lets the caller write such ghosts. */
 int f4_set_bc_values(f4_mesh *m, const double *values);
+
+/* Spatially varying boundary values, eq. (4): bc_data(i, j, ivar, ibf), ibf = 0 .. n_faces-1 over the
+ * block faces on a physical boundary whose direction has kind F4_BC_DATA, in (block, face) order.  "A callback function
+ * has to be stored so that boundary data is automatically updated when the mesh changes": fn is called by
+ * f4_build_ghost_pattern, f4_bind_storage, f4_adapt (when the mesh changed) and f4_update_bc_data ("for temporally
+ * varying boundary conditions this callback function can be called by the application code whenever necessary") with
+ * the face list block[n_faces], face[n_faces] (block geometry: f4_get_blocks) and must fill the HOST array
+ * bc_data[n_faces][Nvar][N^(dim-1)] (t1 fastest; t1 < t2 the transverse axes in x,y,z order) with stored
+ * (conservative) variables at the face-cell centres; the library copies it to the device.  Ghost layer g then mirrors
+ * interior layer g: u_ghost = 2 bc_data - u_interior.  Without a callback the values are zero. */
+typedef void (*f4_bc_data_fn)(void *user, int n_faces, const int *block, const int *face, double *bc_data);
+int f4_set_bc_callback(f4_mesh *m, f4_bc_data_fn fn, void *user);
+int f4_update_bc_data(f4_mesh *m);
+int f4_num_bc_faces(const f4_mesh *m);
 
 /* Gravitational acceleration g[3] of the source term S = (0, rho g, rho g.u), eq. (20), evaluated
  * from the primitives of s_deriv in each cell and added to the flux divergence in every sub-step (PAPER.md:334 step i).

@@ -20,6 +20,13 @@ struct f4_mesh {
   double grav[3] = {0.0, 0.0, 0.0};
   double bcv[6 * 5] = {0.0};     // uniform Dirichlet values / Neumann derivatives [6][nvar]
   double* d_bcv = nullptr;
+  // spatially varying boundary data (eq. 4): faces in record order, host copy, device copy
+  f4_bc_data_fn bc_fn = nullptr;
+  void* bc_user = nullptr;
+  std::vector<int> bc_block, bc_face;
+  std::vector<double> bc_host;
+  double* d_bcdata = nullptr;
+  size_t cap_bcdata = 0;
   int n_states = 2;
   int nvar = 5;
   size_t vs = 0, bs = 0, state_doubles = 0;  // doubles per (block,var), per block, per state
@@ -119,7 +126,30 @@ int ensure(f4_mesh* m, T*& ptr, size_t& cap, size_t need) {
   return F4_OK;
 }
 
+// (re)evaluate the boundary-data callback for the current face list and copy the values to the device
+int refresh_bc_data(f4_mesh* m) {
+  m->bc_block.clear();
+  m->bc_face.clear();
+  for (const Record& r : m->hm.r1)
+    if (r.op == F4_OP_BC && r.o1 && r.o2) { m->bc_block.push_back(r.dst); m->bc_face.push_back(r.face); }
+  const size_t nf = m->bc_block.size();
+  const size_t per_face = (size_t)m->nvar * m->hm.N * (m->hm.dim == 3 ? m->hm.N : 1);
+  m->bc_host.assign(nf * per_face, 0.0);
+  if (nf && m->bc_fn) m->bc_fn(m->bc_user, (int)nf, m->bc_block.data(), m->bc_face.data(), m->bc_host.data());
+  if (!m->bound || !nf) return F4_OK;
+  int rc;
+  if ((rc = ensure(m, m->d_bcdata, m->cap_bcdata, nf * per_face))) return rc;
+  CU(cudaMemcpyAsync(m->d_bcdata, m->bc_host.data(), nf * per_face * sizeof(double), cudaMemcpyHostToDevice, m->stream));
+  CU(cudaStreamSynchronize(m->stream));
+  std::fill(m->srl_valid.begin(), m->srl_valid.end(), 0);   // boundary ghosts of every state are stale now
+  return F4_OK;
+}
+
 int upload_meta(f4_mesh* m) {
+  {
+    int rc0 = refresh_bc_data(m);
+    if (rc0) return rc0;
+  }
   if (!m->bound) return F4_OK;
   const int nb = (int)m->hm.leaves.size();
   std::vector<int> lev(nb);
@@ -220,14 +250,15 @@ int fill_ghosts_impl(f4_mesh* m, int state, int have, bool need_z, bool for_stag
   else if (have == 1) { r1 = m->d_r1z; n1 = m->n_r1z; }
   if (n1) {
     Scope sc(m, F4_PROF_R1);
-    CU(launch_ghost(m->hm.dim, m->hm.N, GhostParams{st, r1, n1, m->theta, m->d_bcv, m->d_level, m->hm.dx_of_level(0)},
-                    m->stream));
+    CU(launch_ghost(m->hm.dim, m->hm.N,
+                    GhostParams{st, r1, n1, m->theta, m->d_bcv, m->d_bcdata, m->d_level, m->hm.dx_of_level(0)}, m->stream));
   }
   m->srl_valid[state] = (char)after;
   if (m->n_r2) {
     Scope sc(m, F4_PROF_R2);
     CU(launch_ghost(m->hm.dim, m->hm.N,
-                    GhostParams{st, m->d_r2, m->n_r2, m->theta, m->d_bcv, m->d_level, m->hm.dx_of_level(0)}, m->stream));
+                    GhostParams{st, m->d_r2, m->n_r2, m->theta, m->d_bcv, m->d_bcdata, m->d_level, m->hm.dx_of_level(0)},
+                    m->stream));
   }
   return F4_OK;
 }
@@ -299,6 +330,7 @@ int f4_mesh_destroy(f4_mesh* m) {
   if (m->d_sums) cudaFree(m->d_sums);
   if (m->d_flags) cudaFree(m->d_flags);
   if (m->d_bcv) cudaFree(m->d_bcv);
+  if (m->d_bcdata) cudaFree(m->d_bcdata);
   if (m->d_indicator) cudaFree(m->d_indicator);
   if (m->d_stage) cudaFree(m->d_stage);
   delete m;
@@ -536,6 +568,17 @@ int f4_set_bc_values(f4_mesh* m, const double* values) {
   return F4_OK;
 }
 
+int f4_set_bc_callback(f4_mesh* m, f4_bc_data_fn fn, void* user) {
+  if (!m) return F4_EINVAL;
+  m->bc_fn = fn;
+  m->bc_user = user;
+  return refresh_bc_data(m);
+}
+
+int f4_update_bc_data(f4_mesh* m) { return m ? refresh_bc_data(m) : F4_EINVAL; }
+
+int f4_num_bc_faces(const f4_mesh* m) { return m ? (int)m->bc_block.size() : F4_EINVAL; }
+
 int f4_set_gravity(f4_mesh* m, const double g[3]) {
   if (!m || !g) return F4_EINVAL;
   for (int a = 0; a < 3; ++a) {
@@ -654,7 +697,7 @@ int f4_adapt(f4_mesh* m, const int* refine_flags, int* changed_out) {
   if (rc) return fail(m, rc, err);
   if (!changed) return F4_OK;
   *changed_out = 1;
-  if (!m->bound) return F4_OK;
+  if (!m->bound) return refresh_bc_data(m);
   std::vector<DevTransfer> dp(plan.size());
   for (size_t q = 0; q < plan.size(); ++q) {
     dp[q].kind = plan[q].kind;

@@ -61,6 +61,7 @@ struct GhostParams {
   int nrec;
   double theta;
   const double* bcv;   // [6][Nvar] uniform Dirichlet values / Neumann normal derivatives
+  const double* bcdata;  // [n_bc_faces][Nvar][N^(d-1)] spatially varying boundary values, eq. (4)
   const int* level;    // per block (Neumann: dx of the block)
   double dx0;          // cell size of level 0
 };

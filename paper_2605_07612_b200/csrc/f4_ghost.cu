@@ -183,7 +183,8 @@ __device__ __forceinline__ void do_c2f(double* __restrict__ st, int dst, int src
 // Individually rounded operations in the order the formulas are written: bit-exact against the oracle.
 template <int DIM, int N>
 __device__ __forceinline__ void do_bc_values(double* __restrict__ st, int blk, int face, bool neumann,
-                                             const double* __restrict__ bcv, double dx) {
+                                             const double* __restrict__ bcv, double dx,
+                                             const double* __restrict__ data /* this face's bc_data, or nullptr */) {
   using G = Geo<DIM, N>;
   constexpr int NV = G::NVAR, FS = (DIM == 3) ? N * N : N;
   const int a = face >> 1, side = face & 1;
@@ -197,7 +198,7 @@ __device__ __forceinline__ void do_bc_values(double* __restrict__ st, int blk, i
     else if (a == 1) { dj = nd; sj = ns; di = si = t1; dk = sk = t2; }
     else { dk = nd; sk = ns; di = si = t1; dj = sj = t2; }
     double* dv = db + (size_t)v * G::VS;
-    const double src = dv[cell_off<DIM, N>(si, sj, sk)], ub = bcv[face * NV + v];
+    const double src = dv[cell_off<DIM, N>(si, sj, sk)], ub = data ? data[v * FS + t] : bcv[face * NV + v];
     dv[cell_off<DIM, N>(di, dj, dk)] =
         neumann ? __dadd_rn(src, __dmul_rn(__dmul_rn((double)g, dx), ub)) : __dsub_rn(__dmul_rn(2.0, ub), src);
   }
@@ -252,8 +253,10 @@ __global__ void __launch_bounds__(256, 4) ghost_exec_kernel(GhostParams p) {
   for (int q = 0; q < n; ++q) {
     const DevRecord rec = recs[q];
     const int op = rec.meta & 3, face = (rec.meta >> 2) & 7, o1 = (rec.meta >> 5) & 1, o2 = (rec.meta >> 6) & 1;
-    if (op == F4_OP_BC && (o1 | o2))
-      do_bc_values<DIM, N>(p.state, rec.dst, face, o2 != 0, p.bcv, p.dx0 * (1.0 / (double)(1u << p.level[rec.dst])));
+    if (op == F4_OP_BC && (o1 | o2))   // (1,0) Dirichlet, (0,1) Neumann, (1,1) bc_data of face rec.src (mirror rule)
+      do_bc_values<DIM, N>(p.state, rec.dst, face, o2 != 0 && o1 == 0, p.bcv,
+                           p.dx0 * (1.0 / (double)(1u << p.level[rec.dst])),
+                           (o1 & o2) ? p.bcdata + (size_t)rec.src * G::NVAR * ((DIM == 3) ? N * N : N) : nullptr);
     else if (op == F4_OP_F2C) do_f2c<DIM, N>(p.state, rec.dst, rec.src, face, o1, o2);
     else if (op == F4_OP_C2F) do_c2f<DIM, N>(p.state, rec.dst, rec.src, face, o1, o2, p.theta);
   }

@@ -58,7 +58,7 @@ int HostMesh::init(std::string& err) {
     }
   }
   for (int f = 0; f < 2 * dim; ++f)
-    if (bc[f] < 0 || bc[f] > F4_BC_NEUMANN) { err = "bad bc_kind"; return F4_EINVAL; }
+    if (bc[f] < 0 || bc[f] > F4_BC_DATA) { err = "bad bc_kind"; return F4_EINVAL; }
   if (dim == 2) brick[2] = 1;
   int64_t nb = 1;
   for (int a = 0; a < dim; ++a) nb *= extent(base_level, a);
@@ -104,6 +104,7 @@ static inline void transverse(int a, int& ta, int& tb) {
 int HostMesh::build_pattern(std::string& err) {
   r1.clear();
   r2.clear();
+  n_bc_faces = 0;
   const int nb = (int)leaves.size();
   for (int b = 0; b < nb; ++b) {
     const Leaf& L = leaves[b];
@@ -119,6 +120,8 @@ int HostMesh::build_pattern(std::string& err) {
           if (bc[f] == F4_BC_OUTFLOW) r1.push_back(Record{F4_OP_BC, f, b, b, 0, 0});
           else if (bc[f] == F4_BC_DIRICHLET) r1.push_back(Record{F4_OP_BC, f, b, b, 1, 0});
           else if (bc[f] == F4_BC_NEUMANN) r1.push_back(Record{F4_OP_BC, f, b, b, 0, 1});
+          // (1,1): spatially varying data; src is the face's index ibf into bc_data
+          else if (bc[f] == F4_BC_DATA) r1.push_back(Record{F4_OP_BC, f, b, n_bc_faces++, 1, 1});
           continue;  // F4_BC_KEEP: no record
         }
       }

@@ -38,6 +38,7 @@ class HostMesh {
   std::vector<Leaf> leaves;       // Morton order of the anchors at max_level resolution
   std::vector<uint64_t> mkeys;    // sorted Morton keys, parallel to leaves
   std::vector<Record> r1, r2;     // rounds R1 {SRL, BC, F2C} and R2 {C2F}
+  int n_bc_faces = 0;             // block faces with spatially varying boundary data (their records' src = ibf)
 
   int init(std::string& err);
   int extent(int level, int a) const { return brick[a] << level; }

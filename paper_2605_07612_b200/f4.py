@@ -17,7 +17,8 @@ from . import build as _build
 F4_OK = 0
 ERRORS = {-1: "F4_EINVAL", -2: "F4_ENOBLOCKS", -3: "F4_ECUDA", -4: "F4_EUNBOUND", -5: "F4_EUNBALANCED",
           -6: "F4_EUNSUPPORTED"}
-BC_PERIODIC, BC_OUTFLOW, BC_KEEP, BC_DIRICHLET, BC_NEUMANN = 0, 1, 2, 3, 4
+BC_PERIODIC, BC_OUTFLOW, BC_KEEP, BC_DIRICHLET, BC_NEUMANN, BC_DATA = 0, 1, 2, 3, 4, 5
+BC_DATA_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_double))
 LIM_VANLEER, LIM_MINMOD, LIM_MC, LIM_KOREN, LIM_WENO3 = 0, 1, 2, 3, 4
 FLUX_HLL, FLUX_RUSANOV = 0, 1
 CRIT_LOHNER, CRIT_PJUMP = 0, 1
@@ -28,7 +29,8 @@ OP_SRL, OP_BC, OP_F2C, OP_C2F = 0, 1, 2, 3
 PROF_NAMES = ("ghost_r1", "ghost_r2", "stage", "dt_reduce", "regrid", "layout")
 
 # every symbol include/f4.h declares
-SYMBOLS = ("f4_mesh_create", "f4_mesh_destroy", "f4_set_options", "f4_set_flux_fix", "f4_set_bc_values", "f4_set_gravity", "f4_set_rk_scheme", "f4_storage_bytes", "f4_bind_storage",
+SYMBOLS = ("f4_mesh_create", "f4_mesh_destroy", "f4_set_options", "f4_set_flux_fix", "f4_set_bc_values", "f4_set_bc_callback", "f4_update_bc_data",
+           "f4_num_bc_faces", "f4_set_gravity", "f4_set_rk_scheme", "f4_storage_bytes", "f4_bind_storage",
            "f4_num_blocks", "f4_get_blocks", "f4_set_state", "f4_get_state", "f4_build_ghost_pattern",
            "f4_pattern_size", "f4_get_pattern", "f4_fill_ghosts", "f4_compute_dt", "f4_advance", "f4_refine_flags", "f4_adapt",
            "f4_conserved_totals", "f4_profile_enable", "f4_profile_get", "f4_launch_count", "f4_last_error",
@@ -64,6 +66,9 @@ def lib():
     L.f4_set_rk_scheme.argtypes = [vp, C.c_int]
     L.f4_set_gravity.argtypes = [vp, dp]
     L.f4_set_bc_values.argtypes = [vp, dp]
+    L.f4_set_bc_callback.argtypes = [vp, BC_DATA_FN, vp]
+    L.f4_update_bc_data.argtypes = [vp]
+    L.f4_num_bc_faces.argtypes = [vp]
     L.f4_refine_flags.argtypes = [vp, C.c_int, C.c_int, C.c_int, dp, ip, dp]
     L.f4_storage_bytes.restype = C.c_size_t
     L.f4_storage_bytes.argtypes = [vp]
@@ -186,6 +191,27 @@ class Mesh:
         v = np.ascontiguousarray(values, dtype=np.float64)
         assert v.shape == (6, self.nvar)
         self._chk(self.L.f4_set_bc_values(self.h, _dp(v)))
+
+    def set_bc_callback(self, fn):
+        """fn(blocks[n], faces[n], out[n, nvar, kmax, N]) fills the boundary values of the F4_BC_DATA faces
+        (eq. 4); the library calls it whenever the face list changes and on update_bc_data()."""
+        nvar, N, kmax = self.nvar, self.N, (self.N if self.dim == 3 else 1)
+
+        def tramp(_user, n, blk, face, data):
+            b = np.ctypeslib.as_array(blk, shape=(n,)).copy()
+            f = np.ctypeslib.as_array(face, shape=(n,)).copy()
+            out = np.ctypeslib.as_array(data, shape=(n, nvar, kmax, N))
+            fn(b, f, out)
+
+        self._bc_cb = BC_DATA_FN(tramp)          # keep the trampoline alive as long as the mesh
+        self._chk(self.L.f4_set_bc_callback(self.h, self._bc_cb, None))
+
+    def update_bc_data(self):
+        self._chk(self.L.f4_update_bc_data(self.h))
+
+    @property
+    def num_bc_faces(self):
+        return self.L.f4_num_bc_faces(self.h)
 
     def set_gravity(self, g):
         gg = np.zeros(3, dtype=np.float64)

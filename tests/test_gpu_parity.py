@@ -737,3 +737,71 @@ def test_rayleigh_taylor_workload_parity(scale, steps):
     assert np.all(d <= TOL_STATE * scale_v), (d / scale_v, err)
     assert np.abs(uo[:, 3]).max() > 1e-5            # the instability is moving
     lm.close()
+
+
+# ------------------------------------------------------------------ spatially varying boundary data, eq. (4)
+@pytest.mark.parametrize("dim,N", [(2, 8), (3, 8), (3, 16)])
+def test_bc_data_callback_bit_exact_and_linear_field(dim, N):
+    bc = [W.BCDATA] * (2 * dim)
+    cfg, lm, om = _refined_pair(dim, N, bc, rounds=2, seed=13)
+    brick = tuple(cfg["brick"]) + (1,) * (3 - dim)
+    nvar = dim + 2
+    coef = np.array([1.0, 2.0, 3.0][:dim])
+
+    def values(lev, co, blocks, faces):
+        """phi = x + 2y + 3z (times 1 + ivar) at the face-cell centres of the listed faces (eq. 21)"""
+        allf, xyz = H.boundary_faces(dim, N, brick, bc + [PER] * (6 - len(bc)), lev, co, W.BCDATA)
+        idx = {bf: q for q, bf in enumerate(allf)}
+        out = np.zeros((len(blocks), nvar, N if dim == 3 else 1, N))
+        for q, (b, f) in enumerate(zip(blocks, faces)):
+            Xf = xyz[idx[(int(b), int(f))]]
+            pf = sum(coef[a] * Xf[a] for a in range(dim))
+            for v in range(nvar):
+                out[q, v] = (1.0 + v) * pf
+        return out
+
+    calls = []
+
+    def cb(blocks, faces, out):
+        la, ca = lm.get_blocks()
+        out[:] = values(la, ca, blocks, faces)
+        calls.append(len(blocks))
+
+    lm.set_bc_callback(cb)
+    assert calls and calls[-1] == lm.num_bc_faces > 0
+
+    def compare():
+        la, ca = lm.get_blocks()
+        lb, cb_ = om.get_blocks()
+        perm = perm_lib_to_ora(lm, om)
+        of, _ = H.boundary_faces(dim, N, brick, bc + [PER] * (6 - len(bc)), lb, cb_, W.BCDATA)
+        om.set_bc_data(of, values(lb, cb_, [b for b, _ in of], [f for _, f in of]))
+        X, nc, _ = H.padded_coords(dim, N, 2, brick, la, ca)
+        phi = sum(coef[a] * X[a] for a in range(dim))
+        u = np.repeat(phi[:, None], nvar, axis=1) * (1.0 + np.arange(nvar))[None, :, None, None, None]
+        interior = np.ascontiguousarray(u[:, :, 2:-2, 2:-2, 2:-2] if dim == 3 else u[:, :, :, 2:-2, 2:-2])
+        uo = np.empty_like(interior)
+        uo[perm] = interior
+        lm.set_state(0, interior)
+        om.set_state(0, uo)
+        lm.fill_ghosts(0)
+        om.fill_ghosts(0)
+        pg, po = lm.get_state(0, with_ghosts=True), om.get_state(0, with_ghosts=True)[perm]
+        _, _, outside = H.padded_coords(dim, N, 2, brick, la, ca)
+        for v in range(nvar):
+            assert np.array_equal(pg[:, v][nc & outside], po[:, v][nc & outside])      # boundary ghosts: bit-exact
+            assert np.abs(pg[:, v][nc] - u[:, v][nc]).max() <= 4e-15 * np.abs(u[:, v]).max()   # the paper's test
+
+    compare()
+    # the callback is invoked again when the mesh changes ("automatically updated", PAPER.md:158)
+    n_before = len(calls)
+    la, ca = lm.get_blocks()
+    flags = np.zeros(len(la), dtype=np.int32)
+    flags[np.argmin(la)] = 1
+    perm = perm_lib_to_ora(lm, om)
+    fo = np.empty_like(flags)
+    fo[perm] = flags
+    assert lm.adapt(flags) and om.adapt(fo)
+    assert len(calls) > n_before and calls[-1] == lm.num_bc_faces
+    compare()
+    lm.close()
