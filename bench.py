@@ -155,6 +155,9 @@ def adaptive_flags(cfg, mesh):
     """Reading A15: config 5's pressure-jump flags, computed on the device from state 0 (f4_refine_flags fills the
     ghosts and returns one int per block)."""
     from paper_2605_07612_b200 import f4
+    if cfg.get("criterion", ("pjump",))[0] == "lohner":          # config 7: eq. (12), PAPER.md:349-362, 560
+        _, var, params = cfg["criterion"]
+        return mesh.refine_flags(0, f4.CRIT_LOHNER, params, var)[0]
     return mesh.refine_flags(0, f4.CRIT_PJUMP, (0.1, 0.025))[0]
 
 
@@ -228,7 +231,8 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3,
-                    help="1-5: BASELINE.json configs (3 = headline); 6: the paper's own Rayleigh-Taylor benchmark")
+                    help="1-5: BASELINE.json configs (3 = headline); 6: the paper's own Rayleigh-Taylor benchmark; "
+                         "7: the same with AMR driven by the paper's criterion eq. (12)")
     ap.add_argument("--scale", type=int, default=None, help="smaller base level (debug only; invalid as a bench number)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
@@ -266,7 +270,7 @@ def main():
     adaptive = cfg["max_level"] > cfg["base_level"]
     rk = {"heun": f4.RK_HEUN, "euler": f4.RK_EULER, "ssp33": f4.RK_SSP33, "ssp43": f4.RK_SSP43, "rk4": f4.RK_RK4}[args.rk]
     nstages = f4.RK_STAGES[rk]
-    mesh = f4.Mesh.from_config(cfg, n_states=f4.RK_STATES[rk], max_blocks=None if not adaptive else 12000)
+    mesh = f4.Mesh.from_config(cfg, n_states=f4.RK_STATES[rk], max_blocks=None if not adaptive else 40000)
     mesh.set_rk_scheme(rk)
     W.apply_physics(cfg, mesh)
     stream = torch.cuda.Stream(dev)

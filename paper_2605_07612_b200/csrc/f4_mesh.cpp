@@ -7,8 +7,8 @@
 
 #include <algorithm>
 #include <deque>
-#include <unordered_map>
-#include <unordered_set>
+#include <string>
+#include <vector>
 
 #include "../../include/f4.h"
 
@@ -29,6 +29,75 @@ uint64_t morton3(uint32_t x, uint32_t y, uint32_t z) { return spread3(x) | sprea
 static inline uint64_t pack(int level, int cx, int cy, int cz) {
   return (uint64_t)level | (uint64_t)cx << 5 | (uint64_t)cy << 24 | (uint64_t)cz << 43;
 }
+// Open-addressing hash map for packed keys (linear probing, tombstones; keys never reach the two sentinels): the
+// mesh adapt is a few thousand inserts / lookups per call, where std::unordered_* spends its time allocating nodes.
+class KeyMap {
+ public:
+  explicit KeyMap(size_t expected) {
+    size_t cap = 64;
+    while (cap < 2 * expected + 64) cap <<= 1;
+    k_.assign(cap, EMPTY);
+    v_.assign(cap, 0);
+    mask_ = cap - 1;
+  }
+  int* find(uint64_t key) {
+    for (size_t i = hash(key) & mask_;; i = (i + 1) & mask_) {
+      if (k_[i] == key) return &v_[i];
+      if (k_[i] == EMPTY) return nullptr;
+    }
+  }
+  bool count(uint64_t key) { return find(key) != nullptr; }
+  void set(uint64_t key, int val) {
+    if (int* p = find(key)) { *p = val; return; }
+    if (2 * (used_ + 1) > k_.size()) grow();
+    size_t i = hash(key) & mask_;
+    while (k_[i] != EMPTY && k_[i] != TOMB) i = (i + 1) & mask_;
+    if (k_[i] == EMPTY) ++used_;
+    k_[i] = key;
+    v_[i] = val;
+    ++n_;
+  }
+  int& ref(uint64_t key) {   // value of key, inserted as 0 if absent
+    if (!find(key)) set(key, 0);
+    return *find(key);
+  }
+  void erase(uint64_t key) {
+    for (size_t i = hash(key) & mask_;; i = (i + 1) & mask_) {
+      if (k_[i] == key) { k_[i] = TOMB; --n_; return; }
+      if (k_[i] == EMPTY) return;
+    }
+  }
+  size_t size() const { return n_; }
+  template <class F>
+  void for_each(F f) const {
+    for (size_t i = 0; i < k_.size(); ++i)
+      if (k_[i] < TOMB) f(k_[i], v_[i]);
+  }
+
+ private:
+  static constexpr uint64_t EMPTY = ~0ULL, TOMB = ~0ULL - 1;
+  static uint64_t hash(uint64_t x) {
+    x ^= x >> 31;
+    x *= 0x9E3779B97F4A7C15ULL;
+    return x ^ (x >> 29);
+  }
+  void grow() {
+    std::vector<uint64_t> ok;
+    std::vector<int> ov;
+    ok.swap(k_);
+    ov.swap(v_);
+    k_.assign(ok.size() * 2, EMPTY);
+    v_.assign(ok.size() * 2, 0);
+    mask_ = k_.size() - 1;
+    n_ = used_ = 0;
+    for (size_t i = 0; i < ok.size(); ++i)
+      if (ok[i] < TOMB) set(ok[i], ov[i]);
+  }
+  std::vector<uint64_t> k_;
+  std::vector<int> v_;
+  size_t mask_ = 0, n_ = 0, used_ = 0;
+};
+
 static inline Leaf unpack(uint64_t k) {
   Leaf l;
   l.level = (int)(k & 31);
@@ -106,6 +175,11 @@ int HostMesh::build_pattern(std::string& err) {
   r2.clear();
   n_bc_faces = 0;
   const int nb = (int)leaves.size();
+  r1.reserve((size_t)nb * 2 * dim);
+  // (level, coordinates) -> leaf index: on a balanced mesh the neighbour across a face is the same-level region, its
+  // parent, or its children, so one or two hash lookups decide the case
+  KeyMap idx(nb);
+  for (int b = 0; b < nb; ++b) idx.set(pack(leaves[b].level, leaves[b].c[0], leaves[b].c[1], leaves[b].c[2]), b);
   for (int b = 0; b < nb; ++b) {
     const Leaf& L = leaves[b];
     for (int f = 0; f < 2 * dim; ++f) {
@@ -125,9 +199,11 @@ int HostMesh::build_pattern(std::string& err) {
           continue;  // F4_BC_KEEP: no record
         }
       }
-      int q = find_leaf(L.level, n);
-      if (q < 0) { err = "face connectivity: no leaf covers a neighbour region"; return F4_EUNBALANCED; }
-      const int ql = leaves[q].level;
+      int q = -1, ql = L.level + 1;   // neither the region nor its parent is a leaf: refined (or not balanced)
+      if (int* ps = idx.find(pack(L.level, n[0], n[1], n[2]))) { q = *ps; ql = L.level; }
+      else if (L.level > 0) {
+        if (int* pp = idx.find(pack(L.level - 1, n[0] >> 1, n[1] >> 1, n[2] >> 1))) { q = *pp; ql = L.level - 1; }
+      }
       int ta, tb;
       transverse(a, ta, tb);
       if (ql == L.level) {
@@ -143,16 +219,13 @@ int HostMesh::build_pattern(std::string& err) {
             cc[a] += side ? 0 : 1;
             cc[ta] += o1;
             if (dim == 3) cc[tb] += o2;
-            int qf = find_leaf(L.level + 1, cc);
-            if (qf < 0 || leaves[qf].level != L.level + 1) {
-              err = "face connectivity: neighbour more than one level finer (mesh not 2:1 balanced)";
+            int* pf = idx.find(pack(L.level + 1, cc[0], cc[1], cc[2]));
+            if (!pf) {
+              err = "face connectivity: neighbour differs by more than one level (mesh not 2:1 balanced)";
               return F4_EUNBALANCED;
             }
-            r1.push_back(Record{F4_OP_F2C, f, b, qf, o1, o2});
+            r1.push_back(Record{F4_OP_F2C, f, b, *pf, o1, o2});
           }
-      } else {
-        err = "face connectivity: neighbour more than one level coarser (mesh not 2:1 balanced)";
-        return F4_EUNBALANCED;
       }
     }
   }
@@ -164,14 +237,17 @@ int HostMesh::adapt(const int* flags, std::vector<Transfer>& plan, bool& changed
   plan.clear();
   const int nb_old = (int)leaves.size();
   const int nch = 1 << dim;
-  std::unordered_map<uint64_t, int> old_index;
-  old_index.reserve(nb_old * 2);
-  std::unordered_set<uint64_t> S;
-  S.reserve(nb_old * 2);
+  {  // no flag that can take effect: the mesh (already balanced) stays as it is
+    bool any = false;
+    for (int b = 0; b < nb_old && !any; ++b)
+      any = (flags[b] > 0 && leaves[b].level < max_level) || (flags[b] < 0 && leaves[b].level > base_level);
+    if (!any) return F4_OK;
+  }
+  KeyMap old_index(nb_old), S(2 * nb_old);   // old leaves -> index; the leaf set being edited
   for (int b = 0; b < nb_old; ++b) {
     uint64_t k = pack(leaves[b].level, leaves[b].c[0], leaves[b].c[1], leaves[b].c[2]);
-    old_index[k] = b;
-    S.insert(k);
+    old_index.set(k, b);
+    S.set(k, 1);
   }
   auto children = [&](const Leaf& l, uint64_t* out) {
     int q = 0;
@@ -186,14 +262,14 @@ int HostMesh::adapt(const int* flags, std::vector<Transfer>& plan, bool& changed
     if (flags[b] > 0 && leaves[b].level < max_level) {
       S.erase(pack(leaves[b].level, leaves[b].c[0], leaves[b].c[1], leaves[b].c[2]));
       children(leaves[b], ch);
-      for (int q = 0; q < nch; ++q) S.insert(ch[q]);
+      for (int q = 0; q < nch; ++q) S.set(ch[q], 1);
     }
   // 2. coarsen complete families of old leaves, one level, never below base_level
   {
-    std::unordered_map<uint64_t, int> fam;
+    KeyMap fam(nb_old / 4 + 16);
     for (int b = 0; b < nb_old; ++b) {
       const Leaf& l = leaves[b];
-      if (flags[b] < 0 && l.level > base_level) fam[pack(l.level - 1, l.c[0] >> 1, l.c[1] >> 1, l.c[2] >> 1)]++;
+      if (flags[b] < 0 && l.level > base_level) fam.ref(pack(l.level - 1, l.c[0] >> 1, l.c[1] >> 1, l.c[2] >> 1))++;
     }
     // A family whose parent would touch a leaf two levels finer is not coarsened: balance (which only refines)
     // would split the parent again at once.  Checking here keeps the balance work list below to the NEW leaves.
@@ -215,7 +291,7 @@ int HostMesh::adapt(const int* flags, std::vector<Transfer>& plan, bool& changed
             bool covered = false;   // the neighbour region is a leaf or inside a coarser leaf
             for (int l = par.level; l >= 0 && !covered; --l) {
               int sh = par.level - l;
-              covered = S.count(pack(l, n[0] >> sh, n[1] >> sh, n[2] >> sh)) != 0;
+              covered = S.count(pack(l, n[0] >> sh, n[1] >> sh, n[2] >> sh));
             }
             if (covered) continue;
             // subdivided: its children that touch the parent must be leaves (level par.level + 1), not finer
@@ -232,20 +308,22 @@ int HostMesh::adapt(const int* flags, std::vector<Transfer>& plan, bool& changed
           }
       return true;
     };
-    for (auto& pr : fam)
-      if (pr.second == nch && can_coarsen(unpack(pr.first))) {
-        Leaf par = unpack(pr.first);
+    fam.for_each([&](uint64_t kp, int members) {
+      if (members == nch && can_coarsen(unpack(kp))) {
+        Leaf par = unpack(kp);
         children(par, ch);
         for (int q = 0; q < nch; ++q) S.erase(ch[q]);
-        S.insert(pr.first);
+        S.set(kp, 1);
       }
+    });
   }
   // 3. balance, corner connectivity: ripple from a work queue
   {
     // the old mesh was balanced, so only a leaf created by this call can be the finer side of a violation
     std::deque<uint64_t> Q;
-    for (uint64_t k : S)
+    S.for_each([&](uint64_t k, int) {
       if (!old_index.count(k)) Q.push_back(k);
+    });
     while (!Q.empty()) {
       uint64_t ka = Q.front();
       Q.pop_front();
@@ -272,7 +350,7 @@ int HostMesh::adapt(const int* flags, std::vector<Transfer>& plan, bool& changed
                 if (l < A.level - 1) {
                   S.erase(kq);
                   children(unpack(kq), ch);
-                  for (int q = 0; q < nch; ++q) { S.insert(ch[q]); Q.push_back(ch[q]); }
+                  for (int q = 0; q < nch; ++q) { S.set(ch[q], 1); Q.push_back(ch[q]); }
                   Q.push_back(ka);  // look again: the new children may still be too coarse
                   again = true;
                 }
@@ -285,8 +363,7 @@ int HostMesh::adapt(const int* flags, std::vector<Transfer>& plan, bool& changed
   // 4. unchanged? (mesh revision)
   if ((int)S.size() == nb_old) {
     bool same = true;
-    for (auto& pr : old_index)
-      if (!S.count(pr.first)) { same = false; break; }
+    old_index.for_each([&](uint64_t k, int) { if (!S.count(k)) same = false; });
     if (same) return F4_OK;
   }
   if ((int)S.size() > max_blocks) {
@@ -297,29 +374,28 @@ int HostMesh::adapt(const int* flags, std::vector<Transfer>& plan, bool& changed
   std::vector<Leaf> old_leaves;
   old_leaves.swap(leaves);
   leaves.reserve(S.size());
-  for (uint64_t k : S) leaves.push_back(unpack(k));
+  S.for_each([&](uint64_t k, int) { leaves.push_back(unpack(k)); });
   sort_leaves();
   plan.resize(leaves.size());
   for (int b = 0; b < (int)leaves.size(); ++b) {
     const Leaf& l = leaves[b];
     Transfer t{};
     t.dst = b;
-    auto it = old_index.find(pack(l.level, l.c[0], l.c[1], l.c[2]));
-    if (it != old_index.end()) {
+    int* it = old_index.find(pack(l.level, l.c[0], l.c[1], l.c[2]));
+    if (it) {
       t.kind = 0;
-      t.src[0] = it->second;
-    } else if (l.level > 0 &&
-               (it = old_index.find(pack(l.level - 1, l.c[0] >> 1, l.c[1] >> 1, l.c[2] >> 1))) != old_index.end()) {
+      t.src[0] = *it;
+    } else if (l.level > 0 && (it = old_index.find(pack(l.level - 1, l.c[0] >> 1, l.c[1] >> 1, l.c[2] >> 1)))) {
       t.kind = 1;
-      t.src[0] = it->second;
+      t.src[0] = *it;
       t.oct = (l.c[0] & 1) | (l.c[1] & 1) << 1 | (l.c[2] & 1) << 2;
     } else {
       t.kind = 2;
       children(l, ch);
       for (int q = 0; q < nch; ++q) {
-        auto jt = old_index.find(ch[q]);
-        if (jt == old_index.end()) { err = "adapt: block changed by more than one level"; leaves.swap(old_leaves); sort_leaves(); return F4_EINVAL; }
-        t.src[q] = jt->second;
+        int* jt = old_index.find(ch[q]);
+        if (!jt) { err = "adapt: block changed by more than one level"; leaves.swap(old_leaves); sort_leaves(); return F4_EINVAL; }
+        t.src[q] = *jt;
       }
     }
     plan[b] = t;

@@ -96,11 +96,26 @@ def config(n: int, scale: int | None = None) -> dict:
         c = dict(dim=3, block_n=16, brick=(1, 1, 1), base_level=5, max_level=5,
                  bc=[PERIODIC] * 4 + [NEUMANN] * 2, steps=20, seed=1006, ic="rt",
                  gravity=(0.0, 0.0, -1.0), bc_values=bcv)
+    elif n == 7:
+        # Not a BASELINE.json config: the paper's AMR run of the same Rayleigh-Taylor set-up (section
+        # 5.4): refinement criterion eq. (12) on the gas density with c_refine = 5e-2, c_derefine = 6.25e-3,
+        # eps = 1e-2, eps_abs = 1e-10, regrid every four time steps, 16^3 blocks.  Here: base level 2 (64^3 cells),
+        # up to 3 more levels (the paper: levels 0-6 on 64 GPUs).
+        c = config(6)
+        c.update(base_level=2, max_level=5, steps=40, seed=1007, regrid_every=4,
+                 criterion=("lohner", 0, (5e-2, 6.25e-3, 1e-2, 1e-10)))
+        if scale is not None:
+            c["max_level"] = c["base_level"] + scale
+        c["name"] = "rayleigh-taylor-amr"
+        return c
     else:
-        raise ValueError("config 1..6")
+        raise ValueError("config 1..7")
     c.update(n_ghost=2, gamma=1.4, cfl=0.4, name=f"config{n}")
     if n == 6:
         c.update(gamma=5.0 / 3.0, cfl=0.5, name="rayleigh-taylor")
+        if scale is not None:
+            c["base_level"] = c["max_level"] = scale
+        return c
     if scale is not None:
         if n == 5:
             c["max_level"] = c["base_level"] + scale

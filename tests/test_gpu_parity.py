@@ -805,3 +805,47 @@ def test_bc_data_callback_bit_exact_and_linear_field(dim, N):
     assert len(calls) > n_before and calls[-1] == lm.num_bc_faces
     compare()
     lm.close()
+
+
+# ------------------------------------------------------------------ the paper's AMR run: Rayleigh-Taylor + eq. (12)
+def test_rayleigh_taylor_amr_with_lohner_flags():
+    # config 7: gravity, hydrostatic Neumann faces, refinement by eq. (12) on the density, regrid
+    # every 4 steps; flags come from the oracle state and are fed to both sides (reading A15's rule for discrete
+    # decisions); the device's own flags may differ only where the indicator sits on a threshold
+    cfg = W.config(7, scale=1)
+    crit = cfg["criterion"][2]
+    lm, om = make_pair(cfg, max_blocks=4000)
+    W.apply_physics(cfg, lm)
+    W.apply_physics(cfg, om)
+
+    def regrid(check):
+        perm = perm_lib_to_ora(lm, om)
+        om.fill_ghosts(0)
+        fo, io = om.refine_flags(0, om.CRIT_LOHNER, crit, 0)
+        if check:
+            fg, ig = lm.refine_flags(0, f4.CRIT_LOHNER, crit, 0)
+            assert np.all(np.abs(ig - io[perm]) <= 1e-8 * np.maximum(io[perm], 1e-3))
+            near = np.minimum(np.abs(io[perm] - crit[0]), np.abs(io[perm] - crit[1])) <= 1e-8
+            assert not np.any((fg != fo[perm]) & ~near)
+        ch_o = om.adapt(fo)
+        ch_g = lm.adapt(fo[perm])
+        assert ch_o == ch_g
+        return ch_o
+
+    set_both(lm, om, cfg)
+    assert regrid(False)                              # the interface is refined
+    _, perm = set_both(lm, om, cfg)
+    assert lm.get_blocks()[0].max() == cfg["max_level"]
+    for s in range(8):
+        if s and s % cfg["regrid_every"] == 0:
+            regrid(True)
+            perm = perm_lib_to_ora(lm, om)
+        dt = om.compute_dt(0, cfg["cfl"])
+        assert abs(lm.compute_dt(0, cfg["cfl"]) - dt) <= 1e-12 * dt
+        om.advance(dt)
+        lm.advance(dt)
+    ug, uo = lm.get_state(0), om.get_state(0)[perm]
+    scale_v = np.array([np.abs(uo[:, 0]).max()] + [np.abs(uo[:, 0]).max() * 2.0] * 3 + [np.abs(uo[:, 4]).max()])
+    d = np.array([np.abs(ug[:, v] - uo[:, v]).max() for v in range(5)])
+    assert np.all(d <= TOL_STATE * scale_v), d / scale_v
+    lm.close()
