@@ -237,6 +237,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--flux-fix", action="store_true",
+                    help="adaptive configs: conservative flux fixing at refinement boundaries (PAPER.md:253-261)")
     ap.add_argument("--rk", default="heun", choices=["heun", "euler", "ssp33", "ssp43", "rk4"],
                     help="Runge-Kutta scheme of eq. (5) (default: Heun, the configs' scheme); GCUPS counts one cell "
                          "update per sub-step (PAPER.md:453)")
@@ -273,6 +275,7 @@ def main():
     mesh = f4.Mesh.from_config(cfg, n_states=f4.RK_STATES[rk], max_blocks=None if not adaptive else 40000)
     mesh.set_rk_scheme(rk)
     W.apply_physics(cfg, mesh)
+    mesh.set_flux_fix(args.flux_fix)
     stream = torch.cuda.Stream(dev)
     mesh.bind_torch(dev, stream)
     n, d = cfg["block_n"], cfg["dim"]
@@ -409,7 +412,8 @@ def main():
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(cfg), "blocks": nb, "cells": cells,
                    "l2": "state (2 x %.1f GB) is larger than L2; no flush needed" % (mesh.storage_bytes() / 2e9),
-                   "parallelism": "replicas only" if world > 1 else "1 GPU", "rk": args.rk},
+                   "parallelism": "replicas only" if world > 1 else "1 GPU", "rk": args.rk,
+                   "flux_fix": bool(args.flux_fix)},
         "roofline": {"bound": "hbm", "achieved": stage_gbs, "peak": peak, "unit": "GB/s",
                      "frac": (stage_gbs / peak) if stage_gbs else None, "traffic": traffic,
                      "kernel": "stage_kernel", "peak_source": peak_src,

@@ -41,10 +41,11 @@ struct f4_mesh {
   DevRecord* d_r1n = nullptr;  // R1 without the same-level copies (the stage kernel pushes / gathers those itself)
   DevRecord* d_r1z = nullptr;  // R1 without the x same-level copies: d_r1n plus the y- and z-face same-level copies
   DevRecord* d_r1c = nullptr;  // d_r1n plus the y- / z-face same-level copies into blocks that are C2F sources
+  DevRecord* d_r1f = nullptr;  // d_r1c plus all x-face same-level copies (flux-fixing mode: the stage does not push x)
   int* d_nbr = nullptr;        // [max_blocks][6] same-level neighbour per face or -1
   size_t cap_r1 = 0, cap_r2 = 0, cap_r1n = 0;
-  int n_r1 = 0, n_r2 = 0, n_r1n = 0, n_r1z = 0, n_r1c = 0;
-  size_t cap_r1z = 0, cap_r1c = 0;
+  int n_r1 = 0, n_r2 = 0, n_r1n = 0, n_r1z = 0, n_r1c = 0, n_r1f = 0;
+  size_t cap_r1z = 0, cap_r1c = 0, cap_r1f = 0;
   // per logical state, same-level face ghosts: 0 = stale, 1 = x faces up to date (pushed by the stage kernel that
   // produced the state; its y ghost rows and z ghost planes were never written because stage kernels fetch them
   // from the neighbours' interiors), 2 = all faces up to date
@@ -160,7 +161,7 @@ int upload_meta(f4_mesh* m) {
     for (size_t q = 0; q < r.size(); ++q)
       out[q] = DevRecord{r[q].dst, r[q].src, r[q].op | r[q].face << 2 | r[q].o1 << 5 | r[q].o2 << 6, 0};
   };
-  std::vector<DevRecord> a, b2, an, az, ac;
+  std::vector<DevRecord> a, b2, an, az, ac, af;
   std::vector<char> c2f_src(nb, 0);   // coarse blocks whose cells (face ghosts included) a prolongation stencil reads
   for (const Record& r : m->hm.r2) c2f_src[r.src] = 1;
   pack(m->hm.r1, a);
@@ -172,6 +173,7 @@ int upload_meta(f4_mesh* m) {
     else an.push_back(dr);
     if (r.op != F4_OP_SRL || r.face >= 2) az.push_back(dr);
     if (r.op != F4_OP_SRL || (r.face >= 2 && c2f_src[r.dst])) ac.push_back(dr);
+    if (r.op != F4_OP_SRL || r.face < 2 || c2f_src[r.dst]) af.push_back(dr);
   }
   int rc;
   if ((rc = ensure(m, m->d_r1, m->cap_r1, a.size()))) return rc;
@@ -183,6 +185,9 @@ int upload_meta(f4_mesh* m) {
   if ((rc = ensure(m, m->d_r1c, m->cap_r1c, ac.size()))) return rc;
   if (!ac.empty()) CU(cudaMemcpyAsync(m->d_r1c, ac.data(), ac.size() * sizeof(DevRecord), cudaMemcpyHostToDevice, m->stream));
   m->n_r1c = (int)ac.size();
+  if ((rc = ensure(m, m->d_r1f, m->cap_r1f, af.size()))) return rc;
+  if (!af.empty()) CU(cudaMemcpyAsync(m->d_r1f, af.data(), af.size() * sizeof(DevRecord), cudaMemcpyHostToDevice, m->stream));
+  m->n_r1f = (int)af.size();
   if (!an.empty()) CU(cudaMemcpyAsync(m->d_r1n, an.data(), an.size() * sizeof(DevRecord), cudaMemcpyHostToDevice, m->stream));
   CU(cudaMemcpyAsync(m->d_nbr, nbr.data(), nbr.size() * sizeof(int), cudaMemcpyHostToDevice, m->stream));
   m->n_r1n = (int)an.size();
@@ -240,14 +245,16 @@ int upload_meta(f4_mesh* m) {
 // need_z: the reader uses same-level y / z ghost cells (prolongation stencils, refinement criteria, regrid transfer,
 // the caller of f4_fill_ghosts); a stage kernel does not (it fetches those rows / planes from the neighbours' interiors).
 // for_stage: the reader is a stage kernel preceded by this fill's R2 round: of the same-level y / z ghosts only
-// those of C2F source blocks have to be in memory.
-int fill_ghosts_impl(f4_mesh* m, int state, int have, bool need_z, bool for_stage = false) {
+// those of C2F source blocks have to be in memory.  no_push (flux-fixing mode): the stage that produced the state
+// did not push its x layers either (they were corrected afterwards), so the x-face copies run here.
+int fill_ghosts_impl(f4_mesh* m, int state, int have, bool need_z, bool for_stage = false, bool no_push = false) {
   double* st = m->state_ptr(state);
   const DevRecord* r1 = m->d_r1;
   int n1 = m->n_r1, after = 2;
   if (have == 2 || (have == 1 && !need_z)) { r1 = m->d_r1n; n1 = m->n_r1n; after = have; }
   else if (have == 1 && for_stage) { r1 = m->d_r1c; n1 = m->n_r1c; after = 1; }
   else if (have == 1) { r1 = m->d_r1z; n1 = m->n_r1z; }
+  else if (for_stage && no_push) { r1 = m->d_r1f; n1 = m->n_r1f; after = 0; }
   if (n1) {
     Scope sc(m, F4_PROF_R1);
     CU(launch_ghost(m->hm.dim, m->hm.N,
@@ -321,6 +328,7 @@ int f4_mesh_destroy(f4_mesh* m) {
   if (m->d_r1n) cudaFree(m->d_r1n);
   if (m->d_r1z) cudaFree(m->d_r1z);
   if (m->d_r1c) cudaFree(m->d_r1c);
+  if (m->d_r1f) cudaFree(m->d_r1f);
   if (m->d_nbr) cudaFree(m->d_nbr);
   if (m->d_bfslot) cudaFree(m->d_bfslot);
   if (m->d_fix) cudaFree(m->d_fix);
@@ -613,8 +621,9 @@ int f4_advance(f4_mesh* m, double dt) {
   for (int a = 0; a < 3; ++a) p.grav[a] = m->grav[a];
   p.has_grav = (m->grav[0] != 0.0 || m->grav[1] != 0.0 || m->grav[2] != 0.0) ? 1 : 0;
   // flux fixing acts only where the mesh has refinement boundaries.  The corrected cells must be
-  // what the neighbours see, so the same-level copy is then left to the pattern executor (no fused push) and the
-  // CFL maximum to the standalone reduction (the stage kernel would take it before the correction).
+  // what the neighbours see: the stage kernel then does not push its x layers (the executor copies them after the
+  // correction; y / z ghosts are gathered by the next stage from interiors that are corrected by then) and the CFL
+  // maximum is left to the standalone reduction (the stage kernel would take it before the correction).
   const bool ff = m->flux_fix && m->n_fix > 0;
   FixParams fp{};
   fp.fix = m->d_fix;
@@ -622,13 +631,14 @@ int f4_advance(f4_mesh* m, double dt) {
   fp.bflux = m->d_bflux;
   p.bfslot = ff ? m->d_bfslot : nullptr;
   p.bflux = m->d_bflux;
-  p.nbr = ff ? nullptr : m->d_nbr;
+  p.nbr = m->d_nbr;        // y / z ghosts are always gathered from the (already corrected) neighbour interiors
+  p.push_x = ff ? 0 : 1;
   for (int q = 0; q < sch.n_sub; ++q) {
     const SubStep& ss = sch.sub[q];
     const bool last = (q == sch.n_sub - 1);
     // ghost fill precedes each F evaluation; same-level ghosts of a state a stage produced were pushed
     // (C2F prolongation stencils read the coarse blocks' same-level y / z ghosts: with such records those are filled too)
-    if ((rc = fill_ghosts_impl(m, ss.deriv, m->srl_valid[ss.deriv], m->n_r2 > 0, true))) return rc;
+    if ((rc = fill_ghosts_impl(m, ss.deriv, m->srl_valid[ss.deriv], m->n_r2 > 0, true, ff))) return rc;
     p.deriv = m->state_ptr(ss.deriv);
     p.out = m->state_ptr(ss.out);
     const double* pv[4] = {nullptr, nullptr, nullptr, nullptr};

@@ -37,7 +37,8 @@ struct StageParams {
   int nblocks;
   int limiter, flux;
   unsigned long long* maxrate;  // bits of a non-negative double, atomicMax; nullptr = no CFL reduction
-  const int* nbr;               // [nblocks][6] same-level neighbour per face or -1: fused SRL ghost push; nullptr = off
+  const int* nbr;               // [nblocks][6] same-level neighbour per face or -1: fused same-level ghosts; nullptr = off
+  int push_x;                   // with nbr: also push the x face layers of s_out into the neighbours' ghost cells
   // flux fixing: face-normal fluxes at refinement boundaries are stored "during the flux
   // computation" into bflux[slot][var][t2][t1]; bfslot[blk][6] = slot of that block face or -1; nullptr = off
   const int* bfslot;

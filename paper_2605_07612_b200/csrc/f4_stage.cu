@@ -666,7 +666,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
   // fused same-level ghost fill: boundary layers are pushed from registers into the neighbours' ghost cells
   // (a1 of the pattern).  nbr[f] = same-level neighbour across face f, or -1.
   double* ppx = nullptr;   // x push target of this thread (k = 0, var 0); y and z ghosts are gathered by the reader
-  if (p.nbr && !(F4_ABL & 4)) {
+  if (p.nbr && p.push_x && !(F4_ABL & 4)) {
     const int* nb = p.nbr + (size_t)blk * 6;
     const int jg = j0 + j;
     if (!(F4_ABL & 8) && i < NG && nb[0] >= 0) ppx = p.out + (size_t)nb[0] * C::BS + ((jg & ~1) * P + N + 2 * (jg & 1) + i);
