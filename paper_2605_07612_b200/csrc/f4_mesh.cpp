@@ -329,31 +329,37 @@ int HostMesh::adapt(const int* flags, std::vector<Transfer>& plan, bool& changed
       Q.pop_front();
       if (!S.count(ka)) continue;
       Leaf A = unpack(ka);
+      if (A.level < 2) continue;   // nothing can be two levels coarser
+      // A leaf Q that touches A (face, edge or corner) and is more than one level coarser contains the parent region
+      // R' (level A.level-1) of one of A's 26 neighbour regions.  Those parents are A's own parent P shifted by 0 or
+      // by one step TOWARDS the corner of P in which A sits: at most 7 regions.  R' violates iff one of its
+      // ancestors (levels A.level-2 .. 0) is a leaf.
+      const int lp = A.level - 1;
+      const int pc[3] = {A.c[0] >> 1, A.c[1] >> 1, A.c[2] >> 1};
+      const int st[3] = {(A.c[0] & 1) ? 1 : -1, (A.c[1] & 1) ? 1 : -1, (A.c[2] & 1) ? 1 : -1};
       bool again = false;
-      for (int dz = (dim == 3 ? -1 : 0); dz <= (dim == 3 ? 1 : 0) && !again; ++dz)
-        for (int dy = -1; dy <= 1 && !again; ++dy)
-          for (int dx = -1; dx <= 1 && !again; ++dx) {
-            if (!dx && !dy && !dz) continue;
-            int n[3] = {A.c[0] + dx, A.c[1] + dy, A.c[2] + dz};
+      for (int mz = 0; mz <= (dim == 3 ? 1 : 0) && !again; ++mz)
+        for (int my = 0; my <= 1 && !again; ++my)
+          for (int mx = 0; mx <= 1 && !again; ++mx) {
+            if (!mx && !my && !mz) continue;
+            int n[3] = {pc[0] + mx * st[0], pc[1] + my * st[1], pc[2] + mz * st[2]};
             bool outside = false;
             for (int a = 0; a < dim; ++a) {
-              int ext = extent(A.level, a);
+              int ext = extent(lp, a);
               if (n[a] < 0 || n[a] >= ext) {
                 if (bc[2 * a] == F4_BC_PERIODIC) n[a] = (n[a] + ext) % ext; else outside = true;
               }
             }
             if (outside) continue;
-            for (int l = A.level; l >= 0; --l) {
-              int sh = A.level - l;
+            for (int l = lp - 1; l >= 0; --l) {
+              int sh = lp - l;
               uint64_t kq = pack(l, n[0] >> sh, n[1] >> sh, n[2] >> sh);
               if (S.count(kq)) {
-                if (l < A.level - 1) {
-                  S.erase(kq);
-                  children(unpack(kq), ch);
-                  for (int q = 0; q < nch; ++q) { S.set(ch[q], 1); Q.push_back(ch[q]); }
-                  Q.push_back(ka);  // look again: the new children may still be too coarse
-                  again = true;
-                }
+                S.erase(kq);
+                children(unpack(kq), ch);
+                for (int q = 0; q < nch; ++q) { S.set(ch[q], 1); Q.push_back(ch[q]); }
+                Q.push_back(ka);  // look again: the new children may still be too coarse
+                again = true;
                 break;
               }
             }
