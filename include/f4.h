@@ -148,7 +148,9 @@ int f4_build_ghost_pattern(f4_mesh *m);
 int f4_pattern_size(const f4_mesh *m, int *n_r1, int *n_r2);
 /* records[n][6] = {op, face, dst_block, src_block, off_t1, off_t2}, R1 first.
  * face: 0..5 = -x,+x,-y,+y,-z,+z of the DESTINATION block; off_*: hanging-face
- * offset of the fine block within its group. */
+ * offset of the fine block within its group.  F4_OP_BC records
+ * carry the boundary kind in (off_t1, off_t2): (0,0) outflow, (1,0) Dirichlet,
+ * (0,1) Neumann, (1,1) bc_data, whose src_block field is the face index ibf. */
 int f4_get_pattern(const f4_mesh *m, int *records);
 
 /* ---- fill_ghosts -----------------------------------------------------------
