@@ -516,7 +516,8 @@ int f4_compute_dt(f4_mesh* m, int state, double cfl, double* dt_out) {
   CU(cudaMemcpyAsync(&rate, m->d_maxrate, sizeof(double), cudaMemcpyDeviceToHost, m->stream));
   CU(cudaStreamSynchronize(m->stream));
   m->rate_valid = (state == 0);  // d_maxrate now describes this state
-  if (!(rate > 0.0) || rate != rate) return fail(m, F4_EINVAL, "compute_dt: wave speed is zero or not finite");
+  if (!(rate > 0.0) || !(rate <= 1.7976931348623157e308))
+    return fail(m, F4_EINVAL, "compute_dt: wave speed is zero or not finite (a cell with NaN, rho <= 0 or p <= 0?)");
   *dt_out = cfl / rate;
   return F4_OK;
 }

@@ -95,4 +95,5 @@ cudaError_t launch_flags(int dim, int n, const double* state, int nblocks, int c
                          const double params[4], int* flags, double* indicator, cudaStream_t s);
 bool stage_supported(int dim, int n);
 
+
 }  // namespace f4

@@ -29,78 +29,12 @@
 
 #include "../../include/f4.h"
 #include "f4_dev.hpp"
-
-#ifndef F4_MINB
-#define F4_MINB(x) (x)
-#endif
+#include "f4_stage_dev.cuh"
 
 namespace f4 {
 namespace {
 
-// ---- fast fp64 reciprocal / rsqrt: MUFU seed (~2^-22) + one cubic step -> < 2 ulp
-__device__ __forceinline__ double rcp_fast(double x) {
-  double r;
-  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-  double e = fma(-x, r, 1.0);
-  double e2 = fma(e, e, e);
-  return fma(r, e2, r);
-}
-__device__ __forceinline__ double rsqrt_fast(double x) {
-  double y;
-  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  double t = x * y;
-  double e = fma(-t, y, 1.0);
-  double h = fma(0.375, e, 0.5);
-  double he = h * e;
-  return fma(y, he, y);
-}
-
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "WAIT_%=:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra DONE_%=;\n"
-      "bra WAIT_%=;\n"
-      "DONE_%=:\n"
-      "}\n" ::"r"(bar),
-      "r"(parity)
-      : "memory");
-}
-// 1-D bulk async copy global -> shared (TMA engine; SASS UBLKCP), completion counted on the mbarrier
-__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
-               "l"(src), "r"(bytes), "r"(bar)
-               : "memory");
-}
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-#ifndef F4_ABL
-#define F4_ABL 0   // timing ablations (wrong results): 1 no sweep barriers, 2 no halo tasks, 4 no ghost push
-#endif
-__device__ __forceinline__ void group_sync(int id, int nthreads) {
-  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-#ifndef F4_LOADEARLY
-#define F4_LOADEARLY 1   // previous states of the finished plane are requested at the start of the iteration
-#endif
-#ifndef F4_SPLIT
-#define F4_SPLIT 1   // 3D march: split arrive / wait on mbarriers around the x/y exchange (0: two bar.sync per plane)
-#endif
-__device__ __forceinline__ void sweep_sync(int id, int nthreads) {
-  if (F4_ABL & 1) { __syncwarp(); return; }
-  group_sync(id, nthreads);
-}
+__device__ __forceinline__ void sweep_sync(int id, int nthreads) { group_sync(id, nthreads); }
 
 // limited HALF slope 1/2*phi(a,b) for the reconstruction w +- 1/2 phi (reading A1)
 template <bool FAST>
@@ -111,8 +45,7 @@ __device__ __forceinline__ double half_slope(double a, double b, int limiter) {
     // instead of a DSETP on the fp64 pipe); it differs from ab > 0 only for 0 < ab < 2^-1042, where the slope is < 1e-150.
     // the select is taken on the MUFU seed (one 32-bit select: the seed's low word is zero): seed 0 -> rcp 0 -> slope 0
     const double x = a + b;
-    double y;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double y = rcp_seed(x);
     y = __hiloint2double((__double2hiint(ab) > 0) ? __double2hiint(y) : 0, 0);
     const double e = fma(-x, y, 1.0);
     const double e2 = fma(e, e, e);
@@ -145,14 +78,15 @@ __device__ __forceinline__ double half_slope(double a, double b, int limiter) {
 template <int DIM, bool FAST>
 __device__ __forceinline__ void riemann_flux(const double (&L)[5], const double (&R)[5], double gamma, double ig1,
                                              int flux, double (&F)[5]) {
-  const double yL = rsqrt_fast(L[0]), yR = rsqrt_fast(R[0]);  // 1/sqrt(rho)
-  const double rL = L[0] * yL, rR = R[0] * yR;                // sqrt(rho)
-  const double w = rcp_fast(rL + rR);
-  const double wl = rL * w, wr = rR * w;                      // Roe weights
+  // Roe weights from ONE rsqrt: z = 1/sqrt(rho_L rho_R), s = sqrt(rho_R/rho_L) = rho_R z, w_L = 1/(1+s), w_R = s w_L
+  const double z = rsqrt_fast(L[0] * R[0]);
+  const double sr = R[0] * z;
+  const double wl = rcp_fast(1.0 + sr), wr = sr * wl;
   const double uhat = fma(wl, L[1], wr * R[1]);
   const double du = R[1] - L[1];
-  // d^2 = (rL cL^2 + rR cR^2)/(rL+rR) + 1/2 rL rR/(rL+rR)^2 du^2,  r c^2 = gamma p / sqrt(rho)
-  const double d2 = fma((0.5 * wl) * wr, du * du, fma(L[4], yL, R[4] * yR) * (gamma * w));
+  // d^2 = (rL cL^2 + rR cR^2)/(rL+rR) + 1/2 wL wR du^2,  r c^2 = gamma p / sqrt(rho):
+  //   (pL/rL + pR/rR)/(rL+rR) = wL z (pL s + pR)   (1/rho_L = z s, 1/(rL rR) = z)
+  const double d2 = fma((0.5 * wl) * wr, du * du, fma(L[4], sr, R[4]) * ((wl * z) * gamma));
   const double y2 = rsqrt_fast(d2);
   // F = a FL + b FR + c (UR - UL) with a = S+/(S+ - S-), b = -S-/(S+ - S-), c = S+ S-/(S+ - S-)
   double a, b, c;
@@ -194,7 +128,7 @@ __device__ __forceinline__ void riemann_flux(const double (&L)[5], const double 
   F[1] = fma(aL, L[1], fma(aR, R[1], fma(a, L[4], b * R[4])));
   F[2] = fma(aL, L[2], aR * R[2]);
   F[3] = (DIM == 3) ? fma(aL, L[3], aR * R[3]) : 0.0;
-  F[4] = fma(0.5 * aL, hL, fma(0.5 * aR, hR, fma(L[4], fma(bL, ig1, auL), R[4] * fma(bR, ig1, buR))));
+  F[4] = fma(0.5, fma(aL, hL, aR * hR), fma(L[4], fma(bL, ig1, auL), R[4] * fma(bR, ig1, buR)));
 }
 
 // Two independent HLL fluxes (van Leer/HLL fast path) written step by step across both faces, so that the
@@ -203,41 +137,29 @@ __device__ __forceinline__ void riemann_flux(const double (&L)[5], const double 
 template <int DIM, int NF>
 __device__ __forceinline__ void riemann_fluxN(const double (&L)[NF][5], const double (&R)[NF][5], double gamma,
                                               double ig1, double (&F)[NF][5]) {
-  double x[2 * NF], y[2 * NF];
+  double qq[NF], z[NF], sr[NF], x[NF], wl[NF];
 #pragma unroll
-  for (int f = 0; f < NF; ++f) { x[2 * f] = L[f][0]; x[2 * f + 1] = R[f][0]; }
+  for (int f = 0; f < NF; ++f) qq[f] = L[f][0] * R[f][0];
 #pragma unroll
-  for (int q = 0; q < 2 * NF; ++q) asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y[q]) : "d"(x[q]));
-  {
-    double e[2 * NF];
+  for (int f = 0; f < NF; ++f) z[f] = rsqrt_seed(qq[f]);
 #pragma unroll
-    for (int q = 0; q < 2 * NF; ++q) e[q] = fma(-(x[q] * y[q]), y[q], 1.0);
+  for (int f = 0; f < NF; ++f) z[f] = rsqrt_refine(qq[f], z[f]);   // 1/sqrt(rho_L rho_R)
 #pragma unroll
-    for (int q = 0; q < 2 * NF; ++q) y[q] = fma(y[q], fma(0.375, e[q], 0.5) * e[q], y[q]);   // 1/sqrt(rho)
-  }
-  double rL[NF], rR[NF], w[NF], sum[NF];
+  for (int f = 0; f < NF; ++f) { sr[f] = R[f][0] * z[f]; x[f] = 1.0 + sr[f]; }
 #pragma unroll
-  for (int f = 0; f < NF; ++f) { rL[f] = x[2 * f] * y[2 * f]; rR[f] = x[2 * f + 1] * y[2 * f + 1]; sum[f] = rL[f] + rR[f]; }
+  for (int f = 0; f < NF; ++f) wl[f] = rcp_seed(x[f]);
 #pragma unroll
-  for (int f = 0; f < NF; ++f) asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(w[f]) : "d"(sum[f]));
-  {
-    double e[NF];
-#pragma unroll
-    for (int f = 0; f < NF; ++f) e[f] = fma(-sum[f], w[f], 1.0);
-#pragma unroll
-    for (int f = 0; f < NF; ++f) w[f] = fma(w[f], fma(e[f], e[f], e[f]), w[f]);
-  }
-  double wl[NF], wr[NF], uhat[NF], d2[NF], y2[NF];
+  for (int f = 0; f < NF; ++f) wl[f] = rcp_refine(x[f], wl[f]);
+  double uhat[NF], d2[NF], y2[NF];
 #pragma unroll
   for (int f = 0; f < NF; ++f) {
-    wl[f] = rL[f] * w[f];
-    wr[f] = rR[f] * w[f];
-    uhat[f] = fma(wl[f], L[f][1], wr[f] * R[f][1]);
+    const double wr = sr[f] * wl[f];
+    uhat[f] = fma(wl[f], L[f][1], wr * R[f][1]);
     const double du = R[f][1] - L[f][1];
-    d2[f] = fma((0.5 * wl[f]) * wr[f], du * du, fma(L[f][4], y[2 * f], R[f][4] * y[2 * f + 1]) * (gamma * w[f]));
+    d2[f] = fma((0.5 * wl[f]) * wr, du * du, fma(L[f][4], sr[f], R[f][4]) * ((wl[f] * z[f]) * gamma));
   }
 #pragma unroll
-  for (int f = 0; f < NF; ++f) asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y2[f]) : "d"(d2[f]));
+  for (int f = 0; f < NF; ++f) y2[f] = rsqrt_seed(d2[f]);
   {
     double e[NF];
 #pragma unroll
@@ -262,11 +184,11 @@ __device__ __forceinline__ void riemann_fluxN(const double (&L)[NF][5], const do
     F[f][1] = fma(aL, L[f][1], fma(aR, R[f][1], fma(a, L[f][4], b * R[f][4])));
     F[f][2] = fma(aL, L[f][2], aR * R[f][2]);
     F[f][3] = (DIM == 3) ? fma(aL, L[f][3], aR * R[f][3]) : 0.0;
-    F[f][4] = fma(0.5 * aL, hL, fma(0.5 * aR, hR, fma(L[f][4], fma(bL, ig1, auL), R[f][4] * fma(bR, ig1, buR))));
+    F[f][4] = fma(0.5, fma(aL, hL, aR * hR), fma(L[f][4], fma(bL, ig1, auL), R[f][4] * fma(bR, ig1, buR)));
   }
 }
 
-template <int DIM, int N, int TY, int G, int EXBUF, int HW = 0>
+template <int DIM, int N, int TY, int G, int EXBUF>
 struct Cfg {  // FAST (van Leer + HLL fixed at compile time) does not change the geometry
   static constexpr int P = N + 2 * NG;
   static constexpr int PZ = (DIM == 3) ? P : 1;
@@ -282,8 +204,7 @@ struct Cfg {  // FAST (van Leer + HLL fixed at compile time) does not change the
   static constexpr int EX = NVAR * EXV;
   static constexpr int NH = TY + N;           // halo cells per side (x rows + y columns)
   static constexpr int TG = N * TY;           // cell threads per group
-  static constexpr int TGA = TG + 32 * HW;    // + HW helper warps (halo conversion, halo slopes, last-face fluxes, TMA issue)
-  static constexpr int NT = TGA * G;
+  static constexpr int NT = TG * G;
   static constexpr int YT = N / TY;           // y tiles per block
   // ring | exX[EXBUF] | exY[EXBUF] | right states of the high halo cells [NVAR][NH]
   static constexpr int GROUP_DOUBLES = NSLOT * SLOT + 2 * EXBUF * EX + EXBUF * NVAR * NH;
@@ -291,25 +212,21 @@ struct Cfg {  // FAST (van Leer + HLL fixed at compile time) does not change the
   static constexpr size_t SMEM = (size_t)G * GROUP_DOUBLES * 8 + (size_t)G * NBAR * 8;
   static constexpr int HALO = 4 * TY + 4 * N;  // halo cells of an interior plane
   static_assert(HALO <= TG && 3 * NH <= TG, "halo work needs one pass");
-  static_assert(HW == 0, "a ninth helper warp per block for the halo work was measured slower (19.7 vs 20.8 GCUPS: a "
-                         "288-thread CTA puts three warps on one SM sub-partition, which caps registers at 96) and removed");
   static_assert(TG % 32 == 0 && N % TY == 0 && GROUP_DOUBLES % 2 == 0, "tile shape");
 };
 
 // GEN: 0 = the path every BASELINE config takes; 1 = + gravity source term; 2 = + boundary-flux store (flux fixing)
 // and a third / fourth previous state.
-template <int DIM, int N, int TY, int G, int EXBUF, int HW, bool FAST, int GEN>
-__global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
-                                  F4_MINB((Cfg<DIM, N, TY, G, EXBUF, HW>::SMEM <= 110 * 1024) ? 2 : 1))
+template <int DIM, int N, int TY, int G, int EXBUF, bool FAST, int GEN>
+__global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY, G, EXBUF>::SMEM <= 110 * 1024) ? 2 : 1)
     stage_kernel(const __grid_constant__ StageParams p) {
-  using C = Cfg<DIM, N, TY, G, EXBUF, HW>;
+  using C = Cfg<DIM, N, TY, G, EXBUF>;
   constexpr bool BF = (GEN == 2), GRAV = (GEN >= 1);
   constexpr int P = C::P, PP = C::P * C::P, NV = C::NVAR, PLANE = C::PLANE, TG = C::TG, EXV = C::EXV, NH = C::NH;
-  constexpr int TGA = C::TGA;
   constexpr bool WHOLE = C::WHOLE;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  const int grp = (G == 1) ? 0 : (int)threadIdx.x / TGA;
-  const int t = (G == 1) ? (int)threadIdx.x : (int)threadIdx.x % TGA;
+  const int grp = (G == 1) ? 0 : (int)threadIdx.x / TG;
+  const int t = (G == 1) ? (int)threadIdx.x : (int)threadIdx.x % TG;
   const int item = blockIdx.x * G + grp;
   // a whole group leaves together: its named barrier and mbarriers are private to the group
   if (item >= p.nblocks * C::YT) return;
@@ -343,7 +260,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
     mbar_init(&bars[C::NSLOT + 1], TG);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  group_sync(bar_id, TGA);
+  group_sync(bar_id, TG);
 
   // Same-level z neighbours (fused ghost handling, a1 of the pattern): their interior planes ARE this block's z
   // ghost planes, so the march fetches planes -2,-1 / N,N+1 straight from the neighbour
@@ -352,8 +269,8 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
   // The same holds for the y ghost rows of an interior plane: rows N, N+1 are rows 0, 1 of the +y neighbour's
   // plane, rows -2, -1 are rows N-2, N-1 of the -y neighbour's (two more bulk copies per variable and plane).
   int gz0 = -1, gz1 = -1, gy0 = -1, gy1 = -1;
-  if (DIM == 3 && p.nbr && !(F4_ABL & 32)) { gz0 = p.nbr[(size_t)blk * 6 + 4]; gz1 = p.nbr[(size_t)blk * 6 + 5]; }
-  if (p.nbr && !(F4_ABL & 16)) { gy0 = p.nbr[(size_t)blk * 6 + 2]; gy1 = p.nbr[(size_t)blk * 6 + 3]; }
+  if (DIM == 3 && p.nbr) { gz0 = p.nbr[(size_t)blk * 6 + 4]; gz1 = p.nbr[(size_t)blk * 6 + 5]; }
+  if (p.nbr) { gy0 = p.nbr[(size_t)blk * 6 + 2]; gy1 = p.nbr[(size_t)blk * 6 + 3]; }
   // rows -2,-1 (slots P-2, P-1) and N, N+1 (slots N, N+1) of interior plane kslot: own ghost rows or the neighbours' rows
   const double* ylo_base = (gy0 >= 0) ? p.deriv + (size_t)gy0 * C::BS + (size_t)(N - 2) * P : dbase + (size_t)(P - 2) * P;
   const double* yhi_base = (gy1 >= 0) ? p.deriv + (size_t)gy1 * C::BS : dbase + (size_t)N * P;
@@ -417,12 +334,14 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
   };
 
   // limited reconstruction of one cell from its two neighbours along a line (offsets o0, om, op)
-  auto slope_states = [&](const double* W, int o0, int om, int op, double (&L)[5], double (&R)[5]) {
+  // w0v: the cell's own primitives when the caller already holds them in registers (else read at offset o0)
+  auto slope_states = [&](const double* W, int o0, int om, int op, double (&L)[5], double (&R)[5],
+                          const double* w0v = nullptr) {
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
       if (DIM == 2 && q == 3) { L[q] = 0.0; R[q] = 0.0; continue; }
       const double* Wv = W + pl(q) * PLANE;
-      const double w0 = Wv[o0];
+      const double w0 = w0v ? w0v[q] : Wv[o0];
       const double da = w0 - Wv[om], db = Wv[op] - w0;
       const double hs = half_slope<FAST>(da, db, limiter);
       L[q] = w0 + hs;
@@ -502,14 +421,11 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
     double tmp[5];
     convert(W, o, tmp);
   };
-  const bool is_hs = (HW == 0) && !(F4_ABL & (2 | 64)) && t < 2 * NH;
-  const bool is_hf = (HW == 0) && !(F4_ABL & (2 | 128)) && (t >= 2 * NH) && (t < 3 * NH);
+  const bool is_hs = t < 2 * NH;
+  const bool is_hf = (t >= 2 * NH) && (t < 3 * NH);
   const int th = t - (TG - C::HALO);
-#ifndef F4_HF3
-#define F4_HF3 1
-#endif
-  constexpr bool HF3 = (F4_HF3 != 0) && (HW == 0) && (NH % 32 == 0);   // the last-face flux warp is a whole warp
-  const bool is_hc = (HW == 0) && !(F4_ABL & (2 | 256)) && th >= 0 && th < C::HALO;
+  constexpr bool HF3 = (NH % 32 == 0);   // the last-face flux warp is a whole warp
+  const bool is_hc = th >= 0 && th < C::HALO;
 
   // flux fixing: slots of this block's faces at refinement boundaries (BF instances only)
   int bfs[6] = {-1, -1, -1, -1, -1, -1};
@@ -528,23 +444,25 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
   // wait on an mbarrier with exchange-independent work in between, so that a warp that is late delays the others only
   // by what exceeds that work: the z slope / z flux / Runge-Kutta combine and store of the finished plane between
   // arrive and wait of "left states written", phase 1 of the NEXT plane between arrive and wait of "fluxes written".
-  constexpr bool SPLIT = (F4_SPLIT != 0) && DIM == 3 && EXBUF == 2 && HW == 0 && !(F4_ABL & 1);
+  constexpr bool SPLIT = DIM == 3 && EXBUF == 2;
   uint32_t xph = 0;   // phase parity of the two exchange mbarriers
   const uint32_t barL = bars_u32 + 8u * C::NSLOT, barF = barL + 8u;
   // The x/y sweep of one converted plane W (z index kk, exchange buffers of parity par) in three phases:
   //   1: slopes -> left states to shared memory, right states stay in registers
   //   2: flux at the low x and y face of the own cell, and at the last face of each row / column
   //   3: difference with the next faces: acc = sum over the x,y faces of (F_in - F_out) of the own cell
-  auto phase1 = [&](const double* W, int par, double (&Rx)[5], double (&Ry)[5]) {
+  auto phase1 = [&](const double* W, int par, double (&Rx)[5], double (&Ry)[5], const double* w0v = nullptr) {
     double* eX = exX + (EXBUF == 2 ? par : 0) * C::EX;
     double* eY = exY + (EXBUF == 2 ? par : 0) * C::EX;
     double* sRh = sRh0 + (EXBUF == 2 ? par : 0) * NV * NH;
     {  // ---- phase 1: slopes -> left states to smem, right states stay in registers
-      double L[5];
-      slope_states(W, own, own_xm, own_xp, L, Rx);
+      double L[5], w0[5];
+#pragma unroll
+      for (int q = 0; q < 5; ++q) w0[q] = (DIM == 2 && q == 3) ? 0.0 : (w0v ? w0v[q] : W[pl(q) * PLANE + own]);   // read once
+      slope_states(W, own, own_xm, own_xp, L, Rx, w0);
 #pragma unroll
       for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eX[pl(q) * EXV + fx + 1] = L[q];
-      slope_states(W, own, own_ym, own_yp, L, Ry);
+      slope_states(W, own, own_ym, own_yp, L, Ry, w0);
 #pragma unroll
       for (int q = 0; q < 5; ++q) if (!(DIM == 2 && q == 3)) eY[pl(q) * EXV + fy + N] = L[q];
       if (is_hs) halo_slope_task(W, eX, eY, sRh, t);
@@ -645,15 +563,15 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
       }
     }
   };
-  // the three phases with a group barrier in between (2D, single exchange buffer, F4_SPLIT = 0)
+  // the three phases with a group barrier in between (2D, single exchange buffer)
   auto sweep_xy = [&](const double* W, int par, int kk, double (&acc)[5]) {
     double Rx[5], Ry[5], Fx[5], Fy[5];
     phase1(W, par, Rx, Ry);
-    sweep_sync(bar_id, TGA);
+    sweep_sync(bar_id, TG);
     phase2(par, kk, Rx, Ry, Fx, Fy);
-    sweep_sync(bar_id, TGA);
+    sweep_sync(bar_id, TG);
     phase3(par, kk, Fx, Fy, acc);
-    if (EXBUF == 1) sweep_sync(bar_id, TGA);
+    if (EXBUF == 1) sweep_sync(bar_id, TG);
   };
 
   // Runge-Kutta combine eq. (5) + store + optional CFL rate of the new state
@@ -666,11 +584,11 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
   // fused same-level ghost fill: boundary layers are pushed from registers into the neighbours' ghost cells
   // (a1 of the pattern).  nbr[f] = same-level neighbour across face f, or -1.
   double* ppx = nullptr;   // x push target of this thread (k = 0, var 0); y and z ghosts are gathered by the reader
-  if (p.nbr && p.push_x && !(F4_ABL & 4)) {
+  if (p.nbr && p.push_x) {
     const int* nb = p.nbr + (size_t)blk * 6;
     const int jg = j0 + j;
-    if (!(F4_ABL & 8) && i < NG && nb[0] >= 0) ppx = p.out + (size_t)nb[0] * C::BS + ((jg & ~1) * P + N + 2 * (jg & 1) + i);
-    if (!(F4_ABL & 8) && i >= N - NG && nb[1] >= 0) ppx = p.out + (size_t)nb[1] * C::BS + ((jg | 1) * P + N + 2 * (jg & 1) + (i - (N - NG)));
+    if (i < NG && nb[0] >= 0) ppx = p.out + (size_t)nb[0] * C::BS + ((jg & ~1) * P + N + 2 * (jg & 1) + i);
+    if (i >= N - NG && nb[1] >= 0) ppx = p.out + (size_t)nb[1] * C::BS + ((jg | 1) * P + N + 2 * (jg & 1) + (i - (N - NG)));
   }
   // general instances (BF): up to four previous states in eq. (5) (classical RK4, eq. (11));
   // the third and fourth are folded into b: b <- b + (w2 c + w3 d) / w1 is avoided by carrying w1 b + w2 c + w3 d
@@ -741,7 +659,9 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
       }
       const double pr = gm1 * fma(-0.5 * u[0], ke, u[4]);
       const double c2 = gamma * pr * ir;
-      rate_max = fmax(rate_max, fma((double)DIM, c2 * rsqrt_fast(c2), su));
+      // a cell that is not a valid gas state (NaN, rho <= 0, p <= 0) makes the maximum +inf: compute_dt reports it
+      const double rate = fma((double)DIM, c2 * rsqrt_fast(c2), su);
+      rate_max = fmax(rate_max, (u[0] > 0.0 && pr > 0.0 && rate == rate) ? rate : __longlong_as_double(0x7ff0000000000000LL));
     }
   };
   auto convert_halo = [&](double* W) {
@@ -757,7 +677,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
     mbar_wait(bars_u32, 0);
     convert(ring, own, w);
     convert_halo(ring);
-    group_sync(bar_id, TGA);
+    group_sync(bar_id, TG);
     sweep_xy(ring, 0, 0, acc);
     finish(0, acc, a, b);
   } else {
@@ -779,7 +699,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
       double Rz[5], Lf[5];
       double pa5[5], pb5[5], wB[5];
       auto midA = [&]() {
-      if (F4_LOADEARLY && FIN) load_prev(c - 2, pa5, pb5);  // consumed after the z flux: latency hidden
+      if (FIN) load_prev(c - 2, pa5, pb5);  // consumed after the z flux: latency hidden
       if (FIN && pb && c - 1 < N && (i & 3) == 0) {         // stage 2: u_t of the next plane comes from DRAM: pull it into L2 now
 #pragma unroll
         for (int q = 0; q < 5; ++q)
@@ -808,7 +728,6 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
       }
       };   // midB
       auto mid2 = [&]() {
-      if (!F4_LOADEARLY && FIN) load_prev(c - 2, pa5, pb5);
       if (ZSLOPE) {
         if (ZFLUX) {
           const double Lfn[5] = {Lf[0], Lf[3], Lf[1], Lf[2], Lf[4]}, Rf[5] = {Rz[0], Rz[3], Rz[1], Rz[2], Rz[4]};
@@ -842,7 +761,7 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
         double Fx[5], Fy[5], acc[5];
         phase2(c & 1, c - 1, Rxp, Ryp, Fx, Fy);
         mbar_arrive(barF);
-        if (c < N) phase1(Wc, (c + 1) & 1, Rxp, Ryp);
+        if (c < N) phase1(Wc, (c + 1) & 1, Rxp, Ryp, wB);   // own cell of plane c: still in registers
         mbar_wait(barF, xph);
         xph ^= 1u;
         phase3(c & 1, c - 1, Fx, Fy, acc);
@@ -860,10 +779,10 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
         midA();
         midB();
         mid2();
-        group_sync(bar_id, TGA);
+        group_sync(bar_id, TG);
       }
       // every thread is past its last read of plane c-1: refill that slot with plane c+2
-      if (HW == 0 && t == ISSUER && c + 2 <= N + 1) issue_plane(c + 2, sk);
+      if (t == ISSUER && c + 2 <= N + 1) issue_plane(c + 2, sk);
       sc = (sc == 2) ? 0 : sc + 1;
     };
     using T = std::true_type;
@@ -885,72 +804,41 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF, HW>::NT,
   }
 }
 
-template <int DIM, int N, int TY, int G, int EXBUF, int HW = 0>
+template <int DIM, int N, int TY, int G, int EXBUF>
 cudaError_t launch_cfg(const StageParams& p, cudaStream_t s) {
-  using C = Cfg<DIM, N, TY, G, EXBUF, HW>;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaSuccess;
-    auto set = [&](auto* k) {
-      if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
-    };
-    set(stage_kernel<DIM, N, TY, G, EXBUF, HW, true, 0>);
-    set(stage_kernel<DIM, N, TY, G, EXBUF, HW, false, 0>);
-    set(stage_kernel<DIM, N, TY, G, EXBUF, HW, true, 1>);
-    set(stage_kernel<DIM, N, TY, G, EXBUF, HW, false, 1>);
-    set(stage_kernel<DIM, N, TY, G, EXBUF, HW, true, 2>);
-    set(stage_kernel<DIM, N, TY, G, EXBUF, HW, false, 2>);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  using C = Cfg<DIM, N, TY, G, EXBUF>;
   const int nitems = p.nblocks * C::YT;
   const int grid = (nitems + G - 1) / G;
   const bool fast = p.limiter == F4_LIM_VANLEER && p.flux == F4_FLUX_HLL;
-  if (p.bfslot || p.prev2) {   // general instances: boundary-flux store (flux fixing) and / or > 2 previous states
-    if (fast) stage_kernel<DIM, N, TY, G, EXBUF, HW, true, 2><<<grid, C::NT, C::SMEM, s>>>(p);
-    else stage_kernel<DIM, N, TY, G, EXBUF, HW, false, 2><<<grid, C::NT, C::SMEM, s>>>(p);
-  } else if (p.has_grav) {     // the configs' path + gravity source term
-    if (fast) stage_kernel<DIM, N, TY, G, EXBUF, HW, true, 1><<<grid, C::NT, C::SMEM, s>>>(p);
-    else stage_kernel<DIM, N, TY, G, EXBUF, HW, false, 1><<<grid, C::NT, C::SMEM, s>>>(p);
-  } else if (fast) {
-    stage_kernel<DIM, N, TY, G, EXBUF, HW, true, 0><<<grid, C::NT, C::SMEM, s>>>(p);
-  } else {
-    stage_kernel<DIM, N, TY, G, EXBUF, HW, false, 0><<<grid, C::NT, C::SMEM, s>>>(p);
-  }
+  // general instances (2): boundary-flux store (flux fixing) and / or > 2 previous states; (1): the configs' path +
+  // gravity source term; (0): the configs' path
+  const int gen = (p.bfslot || p.prev2) ? 2 : (p.has_grav ? 1 : 0);
+  void (*k)(StageParams) =
+      gen == 2 ? (fast ? stage_kernel<DIM, N, TY, G, EXBUF, true, 2> : stage_kernel<DIM, N, TY, G, EXBUF, false, 2>)
+      : gen == 1 ? (fast ? stage_kernel<DIM, N, TY, G, EXBUF, true, 1> : stage_kernel<DIM, N, TY, G, EXBUF, false, 1>)
+                 : (fast ? stage_kernel<DIM, N, TY, G, EXBUF, true, 0> : stage_kernel<DIM, N, TY, G, EXBUF, false, 0>);
+  // the opt-in dynamic shared-memory size is an attribute of the function ON THE CURRENT DEVICE: set it before every
+  // launch (a host-side call without synchronisation) instead of caching "done" per process
+  cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+  if (e != cudaSuccess) return e;
+  k<<<grid, C::NT, C::SMEM, s>>>(p);
   return cudaGetLastError();
 }
 
 }  // namespace
 
 bool stage_supported(int dim, int n) {
-  return (dim == 2 && (n == 8 || n == 16)) || (dim == 3 && (n == 8 || n == 16 || n == 32));
+  return (dim == 2 && (n == 8 || n == 16 || n == 32)) || (dim == 3 && (n == 8 || n == 16 || n == 32));
 }
 
 cudaError_t launch_stage(int dim, int n, const StageParams& p, cudaStream_t s) {
   if (p.nblocks <= 0) return cudaSuccess;
   if (dim == 2 && n == 8) return launch_cfg<2, 8, 8, 4, 1>(p, s);
   if (dim == 2 && n == 16) return launch_cfg<2, 16, 16, 1, 1>(p, s);
-#ifndef F4_G8
-#define F4_G8 4
-#endif
-#ifndef F4_EX8
-#define F4_EX8 1
-#endif
-  if (dim == 3 && n == 8) return launch_cfg<3, 8, 8, F4_G8, F4_EX8, 0>(p, s);
-#ifndef F4_TY16
-#define F4_TY16 16
-#endif
-#ifndef F4_G16
-#define F4_G16 1
-#endif
-#ifndef F4_EX16
-#define F4_EX16 2
-#endif
-  if (dim == 3 && n == 16) return launch_cfg<3, 16, F4_TY16, F4_G16, F4_EX16, 0>(p, s);
-#ifndef F4_TY32
-#define F4_TY32 8
-#endif
-  if (dim == 3 && n == 32) return launch_cfg<3, 32, F4_TY32, 1, 2>(p, s);
+  if (dim == 2 && n == 32) return launch_cfg<2, 32, 8, 1, 1>(p, s);
+  if (dim == 3 && n == 8) return launch_cfg<3, 8, 8, 4, 1>(p, s);      // four blocks per CTA
+  if (dim == 3 && n == 16) return launch_cfg<3, 16, 16, 1, 2>(p, s);   // one block per CTA, double-buffered exchange
+  if (dim == 3 && n == 32) return launch_cfg<3, 32, 8, 1, 2>(p, s);    // 32 x 8 tiles
   return cudaErrorInvalidValue;
 }
 
