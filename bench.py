@@ -102,9 +102,10 @@ def fill_initial_state(cfg, lev, co, out, chunk=1024):
         out[b0:b0 + chunk] = W.initial_state(cfg, lev[b0:b0 + chunk], co[b0:b0 + chunk])
 
 
-def oracle_sample(cfg, target_updates=1.2e7):
+def oracle_sample(cfg, target_updates=1.2e7, nthreads=1):
     """The oracle, as it stands, on a bounded sample of the same workload: same generator and block
-    size, smaller uniform base level (or fewer extra levels); returns (GCUPS, cores, description)."""
+    size, smaller uniform base level (or fewer extra levels); returns (GCUPS, cores, description).
+    nthreads > 1: the block-parallel driver of the same routines (bit-identical results, tests/test_oracle_pins.py)."""
     from oracle import oracle as O
     n, d = cfg["block_n"], cfg["dim"]
     scfg = dict(cfg)
@@ -124,14 +125,22 @@ def oracle_sample(cfg, target_updates=1.2e7):
     om.set_state(0, W.initial_state(scfg, lev, co))
     cells = len(lev) * n ** d
     steps = max(2, int(round(target_updates / (2.0 * cells))))
-    om.advance(om.compute_dt(0, cfg["cfl"]))  # warm
+    nthreads = max(1, min(int(nthreads), len(lev)))
+
+    def one():
+        if nthreads == 1:
+            om.advance(om.compute_dt(0, cfg["cfl"]))
+        else:
+            om.advance_mt(om.compute_dt_mt(0, cfg["cfl"], nthreads), nthreads)
+
+    one()  # warm
     t0 = time.perf_counter()
     for _ in range(steps):
-        om.advance(om.compute_dt(0, cfg["cfl"]))
+        one()
     el = time.perf_counter() - t0
     ext = [scfg["brick"][a] * 2 ** scfg["base_level"] * n for a in range(d)]
     desc = f"{'x'.join(map(str, ext))} cells ({len(lev)} blocks of {n}^{d}), {steps} Heun steps, same generator/seed"
-    return cells * 2.0 * steps / el / 1e9, 1, desc, el, steps
+    return cells * 2.0 * steps / el / 1e9, nthreads, desc, el, steps
 
 
 def pattern_bytes(mesh, n, d):
@@ -228,12 +237,12 @@ def run_reference(args, cfg, rank):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=None,
+                    help="timed steps (default: 20; config 5: the 100 steps BASELINE.json states, regrid every 10)")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3,
                     help="1-5: BASELINE.json configs (3 = headline); 6: the paper's own Rayleigh-Taylor benchmark; "
                          "7: the same with AMR driven by the paper's criterion eq. (12)")
-    ap.add_argument("--scale", type=int, default=None, help="smaller base level (debug only; invalid as a bench number)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -246,7 +255,9 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
-    cfg = W.config(args.config, scale=args.scale)
+    cfg = W.config(args.config)
+    if args.steps is None:
+        args.steps = 100 if args.config == 5 else 20
 
     if args.impl == "reference":
         run_reference(args, cfg, rank)
@@ -353,24 +364,38 @@ def main():
     else:
         fill_initial_state(cfg, lev, co, host_np)
     e2e_steps = max(1, args.e2e_steps)
-    mesh.set_state(0, host_np)
-    step()
-    barrier()
-    ev2, ev3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ev2.record(stream)
-    for _ in range(e2e_steps):
-        mesh.set_state(0, host_np)          # pinned host -> device staging -> store
-        if adaptive:
-            counters["step"] = 1
+    back = torch.empty(mesh._shape(False), dtype=torch.float64).pin_memory()
+    back_np = back.numpy()
+
+    def e2e_loop(full):
+        """set_state from pinned host memory -> compute_dt + advance -> the result back on the host: the whole new
+        state (full) or only its digest (per-block conserved sums)."""
+        mesh.set_state(0, host_np)
         step()
-        tot = mesh.conserved_totals(0)      # device -> host: per-block sums + dt
-    ev3.record(stream)
-    barrier()
-    ms_e2e = ev2.elapsed_time(ev3)
-    ms_e2e = max_over_ranks(ms_e2e, dist, dev)
+        barrier()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(e2e_steps):
+            mesh.set_state(0, host_np)          # pinned host -> device staging -> store
+            if adaptive:
+                counters["step"] = 1            # no regrid inside the end-to-end loop
+            step()
+            if full:
+                mesh.get_state(0, out=back_np)  # device -> pinned host: the new state
+            else:
+                mesh.conserved_totals(0)        # device -> host: per-block sums
+        b.record(stream)
+        barrier()
+        return max_over_ranks(a.elapsed_time(b), dist, dev)
+
+    ms_e2e = e2e_loop(True)
+    ms_dig = e2e_loop(False)
     e2e = {"value": whole_job_value(world, cells * float(nstages) * e2e_steps, ms_e2e), "unit": UNIT,
-           "h2d_bytes_per_step": int(host_np.nbytes), "d2h_bytes_per_step": int(nb * (d + 2) * 8 + 8),
-           "steps": e2e_steps, "ms_per_step": ms_e2e / e2e_steps}
+           "h2d_bytes_per_step": int(host_np.nbytes), "d2h_bytes_per_step": int(back_np.nbytes + 8),
+           "steps": e2e_steps, "ms_per_step": ms_e2e / e2e_steps,
+           "digest_only": {"value": whole_job_value(world, cells * float(nstages) * e2e_steps, ms_dig),
+                           "d2h_bytes_per_step": int(nb * (d + 2) * 8 + 8),
+                           "note": "same loop with the per-block conserved sums read back instead of the state"}}
 
     if rank != 0:
         return
@@ -408,7 +433,7 @@ def main():
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         # BASELINE.md holds a paper number only for the paper's own workload (config 6 at full size, Heun):
         # 1.35 GCUPS on one H100, PAPER.md:496 -- another machine's: context, not the target
-        "vs_baseline": (value / 1.35) if (args.config == 6 and args.scale is None and args.rk == "heun") else None,
+        "vs_baseline": (value / 1.35) if (args.config == 6 and args.rk == "heun") else None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(cfg), "blocks": nb, "cells": cells,
                    "l2": "state (2 x %.1f GB) is larger than L2; no flush needed" % (mesh.storage_bytes() / 2e9),
@@ -435,9 +460,17 @@ def main():
         "totals": [float(x) for x in totals_after],
     }
     if world == 1 and not args.no_cpu_baseline:
+        # the oracle as it stands on one core (its definition), and the block-parallel driver of the same routines on
+        # all host cores (SURVEY 8(d) "Timing the oracle beside it"); both on bounded samples of the workload
         v, cores, desc, el, cs = oracle_sample(cfg)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
                                "seconds": el}
+        ncores = os.cpu_count() or 1
+        if ncores > 1:
+            va, ca, desca, ela, _ = oracle_sample(cfg, target_updates=1.2e7 * min(ncores, 16), nthreads=ncores)
+            out["cpu_baseline"]["all_cores"] = {"value": va, "unit": UNIT, "cores": ca, "kind": "oracle",
+                                                "sample": desca, "seconds": ela,
+                                                "note": "block-parallel driver of the same routines, bit-identical"}
     print(json.dumps(out))
     mesh.close()
     if dist is not None:

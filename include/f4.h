@@ -249,6 +249,9 @@ enum { F4_PROF_R1 = 0, F4_PROF_R2 = 1, F4_PROF_STAGE = 2, F4_PROF_DT = 3, F4_PRO
 int f4_profile_enable(f4_mesh *m, int on);
 int f4_profile_get(f4_mesh *m, double ms[F4_PROF_N], long long launches[F4_PROF_N], int reset);
 long long f4_launch_count(const f4_mesh *m);
+/* host wall time (ms) of the last f4_adapt that changed the mesh, by part: [0] refine / coarsen / balance + pattern
+ * records on the host, [1] regrid transfer kernel + wait, [2] record upload. */
+int f4_last_adapt_ms(const f4_mesh *m, double ms[3]);
 
 const char *f4_last_error(const f4_mesh *m);
 const char *f4_version(void);

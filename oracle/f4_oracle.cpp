@@ -48,6 +48,7 @@
 #include <map>
 #include <set>
 #include <string>
+#include <thread>
 #include <vector>
 
 namespace {
@@ -347,27 +348,38 @@ void fill_c2f(Mesh& m, int s, int F, int f, const Neighbor& nb) {
         }
 }
 
-int fill_ghosts(Mesh& m, int s) {
-  int nb_ = (int)m.blocks.size();
-  // R1: SRL, BC and F2C
-  for (int b = 0; b < nb_; ++b)
-    for (int f = 0; f < 2 * m.dim; ++f) {
-      Neighbor nb = find_neighbor(m, b, f);
-      if (nb.kind == NB_SAME) fill_srl(m, s, b, f, nb.blk[0]);
-      else if (nb.kind == NB_BOUNDARY) fill_bc(m, s, b, f);
-      else if (nb.kind == NB_FINE) {
-        for (int q = 0; q < (m.dim == 3 ? 4 : 2); ++q)
-          if (nb.blk[q] < 0) { m.err = "mesh not 2:1 balanced (missing fine neighbour)"; return -1; }
-        fill_f2c(m, s, b, f, nb);
+// One round of the ghost fill over the blocks [b0, b1) (every block of the range is a DESTINATION: a round writes
+// ghost cells of its own blocks only and reads interiors -- round 2 also the round-1 ghosts -- of others).
+int fill_ghosts_round(Mesh& m, int s, int round, int b0, int b1) {
+  if (round == 1) {
+    // R1: SRL, BC and F2C
+    for (int b = b0; b < b1; ++b)
+      for (int f = 0; f < 2 * m.dim; ++f) {
+        Neighbor nb = find_neighbor(m, b, f);
+        if (nb.kind == NB_SAME) fill_srl(m, s, b, f, nb.blk[0]);
+        else if (nb.kind == NB_BOUNDARY) fill_bc(m, s, b, f);
+        else if (nb.kind == NB_FINE) {
+          for (int q = 0; q < (m.dim == 3 ? 4 : 2); ++q)
+            if (nb.blk[q] < 0) { m.err = "mesh not 2:1 balanced (missing fine neighbour)"; return -1; }
+          fill_f2c(m, s, b, f, nb);
+        }
       }
-    }
-  // R2: C2F by interpolation, after R1
-  for (int b = 0; b < nb_; ++b)
-    for (int f = 0; f < 2 * m.dim; ++f) {
-      Neighbor nb = find_neighbor(m, b, f);
-      if (nb.kind == NB_COARSE) fill_c2f(m, s, b, f, nb);
-    }
+  } else {
+    // R2: C2F by interpolation, after R1
+    for (int b = b0; b < b1; ++b)
+      for (int f = 0; f < 2 * m.dim; ++f) {
+        Neighbor nb = find_neighbor(m, b, f);
+        if (nb.kind == NB_COARSE) fill_c2f(m, s, b, f, nb);
+      }
+  }
   return 0;
+}
+
+int fill_ghosts(Mesh& m, int s) {
+  const int nb_ = (int)m.blocks.size();
+  int rc;
+  if ((rc = fill_ghosts_round(m, s, 1, 0, nb_))) return rc;
+  return fill_ghosts_round(m, s, 2, 0, nb_);
 }
 
 // ----------------------------------------------------------------------------
@@ -433,17 +445,18 @@ void riemann_flux(const Mesh& m, const Prim& L, const Prim& R, int dir, double* 
 // ----------------------------------------------------------------------------
 // Finite-volume forward-Euler sub-step, eq. (5)
 //   u(s_out) = dt_sub * F(u(s_deriv)) + sum_i w_i u(s_prev_i)
-// Ghosts of s_deriv must be filled.  Returns max over cells of sum_dim (|u|+c)/dx
-// of the s_deriv state when want_cfl (reading A5/A6), else 0.
+// Ghosts of s_deriv must be filled.  Returns 0, or a negative code with Mesh::err set (positivity lost, reading A18).
 // ----------------------------------------------------------------------------
-int forward_euler(Mesh& m, int s_out, int s_deriv, double dt_sub, int n_prev, const double* w, const int* s_prev) {
+// steps (a), (b) and flux-fixing step 0 for the blocks [b0, b1): a block's update reads and writes that block only
+int forward_euler_blocks(Mesh& m, int b0, int b1, int s_out, int s_deriv, double dt_sub, int n_prev, const double* w,
+                         const int* s_prev) {
   const int N = m.N, Ng = m.Ng, P = m.P, nvar = m.nvar, dim = m.dim;
   const int kmax = (dim == 3) ? N : 1;
   const size_t vs = m.var_stride();
   std::vector<Prim> prim(vs);        // uu_prim
   std::vector<char> valid(vs);
   std::vector<double> result((size_t)nvar * vs);
-  for (int b = 0; b < (int)m.blocks.size(); ++b) {
+  for (int b = b0; b < b1; ++b) {
     const double dx = m.dx_of_level(m.blocks[b].level);
     // (a) to_primitive over the padded block; corner/edge ghosts are never used -> skipped
     for (int k = (dim == 3 ? 1 - Ng : 1); k <= (dim == 3 ? N + Ng : 1); ++k)
@@ -557,6 +570,16 @@ int forward_euler(Mesh& m, int s_out, int s_deriv, double dt_sub, int n_prev, co
         }
     (void)P;
   }
+  return 0;
+}
+
+int forward_euler(Mesh& m, int s_out, int s_deriv, double dt_sub, int n_prev, const double* w, const int* s_prev) {
+  const int N = m.N, nvar = m.nvar, dim = m.dim;
+  const int kmax = (dim == 3) ? N : 1;
+  {
+    int rc = forward_euler_blocks(m, 0, (int)m.blocks.size(), s_out, s_deriv, dt_sub, n_prev, w, s_prev);
+    if (rc) return rc;
+  }
   // flux fixing, step 3: "a loop over all coarse sides of refinement boundaries is performed, and
   // the solution in the cells adjacent to the boundary is corrected based on the difference in the coarse-side
   // flux and the average fine-side flux".  The update above used the coarse flux Fc through that face; with the
@@ -599,10 +622,10 @@ int forward_euler(Mesh& m, int s_out, int s_deriv, double dt_sub, int n_prev, co
 }
 
 // iii. CFL: reading A5 (sum over dimensions) on interior cells, one global dt
-double max_wave_rate(Mesh& m, int s) {
+double max_wave_rate_blocks(Mesh& m, int s, int b0, int b1) {
   const int N = m.N, kmax = (m.dim == 3) ? N : 1;
   double mx = 0.0;
-  for (int b = 0; b < (int)m.blocks.size(); ++b) {
+  for (int b = b0; b < b1; ++b) {
     const double dx = m.dx_of_level(m.blocks[b].level);
     for (int k = 1; k <= kmax; ++k)
       for (int j = 1; j <= N; ++j)
@@ -618,6 +641,7 @@ double max_wave_rate(Mesh& m, int s) {
   }
   return mx;
 }
+double max_wave_rate(Mesh& m, int s) { return max_wave_rate_blocks(m, s, 0, (int)m.blocks.size()); }
 
 // Heun's method, eq. (6)-(7); ghost fill precedes each F
 int advance_heun(Mesh& m, double dt) {
@@ -859,6 +883,57 @@ int refine_flags(Mesh& m, int s, int criterion, int var, const double* params, i
   return 0;
 }
 
+// ----------------------------------------------------------------------------
+// Block-parallel DRIVER of the same routines (timing only: bench.py's all-cores cpu_baseline leg; SURVEY 8(d)
+// "Timing the oracle beside it").  The routines above are unchanged: every thread calls them on its own contiguous
+// range of blocks.  A block's update reads and writes that block only and the CFL maximum does not depend on the
+// order, so the results are bit-identical to one thread (tests/test_oracle_pins.py asserts it).  No flux fixing
+// here (its bflux map is filled during the update).
+// ----------------------------------------------------------------------------
+template <typename F>
+int over_block_ranges(Mesh& m, int nthreads, F&& body) {
+  const int nb = (int)m.blocks.size();
+  if (nthreads < 1) nthreads = 1;
+  if (nthreads > nb) nthreads = nb;
+  std::vector<int> rcs(nthreads, 0);
+  std::vector<std::thread> th;
+  for (int t = 0; t < nthreads; ++t) {
+    const int b0 = (int)((long long)nb * t / nthreads), b1 = (int)((long long)nb * (t + 1) / nthreads);
+    th.emplace_back([&, t, b0, b1]() { rcs[t] = body(t, b0, b1); });
+  }
+  for (auto& x : th) x.join();
+  for (int rc : rcs) if (rc) return rc;
+  return 0;
+}
+
+int fill_ghosts_mt(Mesh& m, int s, int nthreads) {
+  int rc;
+  if ((rc = over_block_ranges(m, nthreads, [&](int, int b0, int b1) { return fill_ghosts_round(m, s, 1, b0, b1); }))) return rc;
+  return over_block_ranges(m, nthreads, [&](int, int b0, int b1) { return fill_ghosts_round(m, s, 2, b0, b1); });
+}
+
+int advance_heun_mt(Mesh& m, double dt, int nthreads) {
+  if (m.flux_fix) { m.err = "the block-parallel driver does not do flux fixing"; return -3; }
+  int rc;
+  if ((rc = fill_ghosts_mt(m, 0, nthreads))) return rc;
+  { double w[1] = {1.0}; int sp[1] = {0};
+    if ((rc = over_block_ranges(m, nthreads, [&](int, int b0, int b1) {
+          return forward_euler_blocks(m, b0, b1, 1, 0, dt, 1, w, sp); }))) return rc; }
+  if ((rc = fill_ghosts_mt(m, 1, nthreads))) return rc;
+  { double w[2] = {0.5, 0.5}; int sp[2] = {0, 1};
+    if ((rc = over_block_ranges(m, nthreads, [&](int, int b0, int b1) {
+          return forward_euler_blocks(m, b0, b1, 0, 1, 0.5 * dt, 2, w, sp); }))) return rc; }
+  return 0;
+}
+
+double max_wave_rate_mt(Mesh& m, int s, int nthreads) {
+  std::vector<double> mx(std::max(nthreads, 1), 0.0);
+  over_block_ranges(m, nthreads, [&](int t, int b0, int b1) { mx[t] = max_wave_rate_blocks(m, s, b0, b1); return 0; });
+  double r = 0.0;
+  for (double x : mx) if (x > r) r = x;
+  return r;
+}
+
 }  // namespace
 
 // =============================================================================
@@ -942,6 +1017,9 @@ int ora_fill_ghosts(void* h, int s) { return fill_ghosts(*(Mesh*)h, s); }
 double ora_max_wave_rate(void* h, int s) { return max_wave_rate(*(Mesh*)h, s); }
 double ora_compute_dt(void* h, int s, double cfl) { return cfl / max_wave_rate(*(Mesh*)h, s); }
 int ora_advance(void* h, double dt) { return advance_heun(*(Mesh*)h, dt); }
+// block-parallel driver (timing only; bit-identical results)
+int ora_advance_mt(void* h, double dt, int nthreads) { return advance_heun_mt(*(Mesh*)h, dt, nthreads); }
+double ora_compute_dt_mt(void* h, int s, double cfl, int nthreads) { return cfl / max_wave_rate_mt(*(Mesh*)h, s, nthreads); }
 int ora_advance_rk(void* h, int scheme, double dt) { return advance_rk(*(Mesh*)h, scheme, dt); }
 int ora_forward_euler(void* h, int s_out, int s_deriv, double dt_sub, int n_prev, const double* w, const int* s_prev) {
   return forward_euler(*(Mesh*)h, s_out, s_deriv, dt_sub, n_prev, w, s_prev);
@@ -1013,6 +1091,21 @@ void ora_riemann_flux(int dim, double gamma, int flux_scheme, const double* wL, 
   L.rho = wL[0]; R.rho = wR[0]; L.p = wL[dim + 1]; R.p = wR[dim + 1];
   for (int d = 0; d < dim; ++d) { L.u[d] = wL[1 + d]; R.u[d] = wR[1 + d]; }
   riemann_flux(m, L, R, dir, F);
+}
+void ora_to_primitive(int dim, double gamma, const double* U, double* w) {
+  Mesh m{}; m.dim = dim; m.nvar = dim + 2; m.gamma = gamma;
+  Prim q = to_primitive(m, U);
+  w[0] = q.rho;
+  for (int a = 0; a < dim; ++a) w[1 + a] = q.u[a];
+  w[dim + 1] = q.p;
+}
+void ora_to_conservative(int dim, double gamma, const double* w, double* U) {
+  Mesh m{}; m.dim = dim; m.nvar = dim + 2; m.gamma = gamma;
+  Prim q{};
+  q.rho = w[0];
+  for (int a = 0; a < dim; ++a) q.u[a] = w[1 + a];
+  q.p = w[dim + 1];
+  to_conservative(m, q, U);
 }
 void ora_wavespeeds(int dim, double gamma, const double* wL, const double* wR, int dir, double* smin, double* smax) {
   Mesh m{}; m.dim = dim; m.nvar = dim + 2; m.gamma = gamma;

@@ -26,7 +26,7 @@ NB_BOUNDARY, NB_SAME, NB_COARSE, NB_FINE = 0, 1, 2, 3
 def build(force: bool = False) -> str:
     """g++ -O2 -ffp-contract=off: no FMA contraction, no fast-math."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        subprocess.check_call(["g++", "-O2", "-ffp-contract=off", "-std=c++17", "-shared", "-fPIC",
+        subprocess.check_call(["g++", "-O2", "-ffp-contract=off", "-std=c++17", "-shared", "-fPIC", "-pthread",
                                "-o", _LIB, _SRC])
     return _LIB
 
@@ -63,6 +63,9 @@ def lib():
         L.ora_compute_dt.restype = C.c_double
         L.ora_compute_dt.argtypes = [C.c_void_p, C.c_int, C.c_double]
         L.ora_advance.argtypes = [C.c_void_p, C.c_double]
+        L.ora_advance_mt.argtypes = [C.c_void_p, C.c_double, C.c_int]
+        L.ora_compute_dt_mt.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_int]
+        L.ora_compute_dt_mt.restype = C.c_double
         L.ora_advance_rk.argtypes = [C.c_void_p, C.c_int, C.c_double]
         L.ora_forward_euler.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_int, dp, ip]
         L.ora_adapt.argtypes = [C.c_void_p, ip, ip]
@@ -79,6 +82,8 @@ def lib():
         L.ora_weno3.restype = C.c_double
         L.ora_weno3.argtypes = [C.c_double] * 2
         L.ora_riemann_flux.argtypes = [C.c_int, C.c_double, C.c_int, dp, dp, C.c_int, dp]
+        L.ora_to_primitive.argtypes = [C.c_int, C.c_double, dp, dp]
+        L.ora_to_conservative.argtypes = [C.c_int, C.c_double, dp, dp]
         L.ora_wavespeeds.argtypes = [C.c_int, C.c_double, dp, dp, C.c_int, dp, dp]
         _lib = L
     return _lib
@@ -203,6 +208,13 @@ class OracleMesh:
         else:
             self._chk(self.L.ora_advance_rk(self.h, int(scheme), dt))
 
+    def advance_mt(self, dt, nthreads):
+        """Heun step by the block-parallel driver (timing only; bit-identical to advance)."""
+        self._chk(self.L.ora_advance_mt(self.h, dt, int(nthreads)))
+
+    def compute_dt_mt(self, state, cfl, nthreads):
+        return self.L.ora_compute_dt_mt(self.h, state, cfl, int(nthreads))
+
     def forward_euler(self, s_out, s_deriv, dt_sub, w, s_prev):
         w = np.asarray(w, dtype=np.float64)
         sp = np.asarray(s_prev, dtype=np.int32)
@@ -277,3 +289,17 @@ def wavespeeds(dim, gamma, wL, wR, direction):
     a, b = C.c_double(), C.c_double()
     lib().ora_wavespeeds(dim, gamma, _dp(wL), _dp(wR), direction, C.byref(a), C.byref(b))
     return a.value, b.value
+
+
+def to_primitive(dim, gamma, U):
+    U = np.asarray(U, dtype=np.float64)
+    w = np.zeros(dim + 2)
+    lib().ora_to_primitive(dim, gamma, _dp(U), _dp(w))
+    return w
+
+
+def to_conservative(dim, gamma, w):
+    w = np.asarray(w, dtype=np.float64)
+    U = np.zeros(dim + 2)
+    lib().ora_to_conservative(dim, gamma, _dp(w), _dp(U))
+    return U

@@ -17,19 +17,18 @@ def _newest_source() -> float:
     return max(os.path.getmtime(os.path.join(CSRC, f)) for f in SOURCES + HEADERS)
 
 
-def build(force: bool = False, verbose: bool = False, extra_flags=(), out: str | None = None) -> str:
-    """Compile csrc/ into ``out`` (default: the in-tree libf4.so).  ``extra_flags`` are appended to the nvcc
-    command line (e.g. ``-DF4_...`` experiment switches; the default build passes none)."""
-    lib = out or LIB
+def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile csrc/ into the in-tree libf4.so."""
+    lib = LIB
     if not force and os.path.exists(lib) and os.path.getmtime(lib) >= _newest_source():
         return lib
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     objs = []
     procs = []
     for src in SOURCES:
-        obj = os.path.join(CSRC, os.path.splitext(src)[0] + (".o" if out is None else "." + os.path.basename(out) + ".o"))
+        obj = os.path.join(CSRC, os.path.splitext(src)[0] + ".o")
         objs.append(obj)
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + list(extra_flags) + ["-x", "cu", "-c", os.path.join(CSRC, src), "-o", obj]
+        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-x", "cu", "-c", os.path.join(CSRC, src), "-o", obj]
         procs.append((cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     for cmd, pr in procs:
         out, _ = pr.communicate()

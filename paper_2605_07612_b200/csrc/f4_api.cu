@@ -3,6 +3,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <chrono>
 #include <string>
 #include <vector>
 
@@ -32,6 +33,7 @@ struct f4_mesh {
   size_t vs = 0, bs = 0, state_doubles = 0;  // doubles per (block,var), per block, per state
   // device
   bool bound = false;
+  int device = -1;            // the device dev_ptr of f4_bind_storage lives on: every device call runs there
   double* store = nullptr;
   cudaStream_t stream = nullptr;
   std::vector<int> phys;  // logical state -> physical state slab
@@ -68,11 +70,25 @@ struct f4_mesh {
   bool rate_valid = false;
   // measurement
   bool prof = false;
+  // a fixed pool of event pairs created by f4_profile_enable (no cudaEventCreate inside a timed loop); when the pool
+  // is used up the recorded pairs are folded into prof_ms (one stream synchronisation) and the pool starts again
   struct Ev { int cls; cudaEvent_t a, b; };
+  static constexpr size_t EV_POOL = 2048;
   std::vector<Ev> evs;
+  size_t evs_used = 0;
+  void fold_events() {
+    if (evs_used == 0) return;
+    cudaEventSynchronize(evs[evs_used - 1].b);
+    for (size_t q = 0; q < evs_used; ++q) {
+      float t = 0.f;
+      if (cudaEventElapsedTime(&t, evs[q].a, evs[q].b) == cudaSuccess) prof_ms[evs[q].cls] += t;
+    }
+    evs_used = 0;
+  }
   double prof_ms[F4_PROF_N] = {0, 0, 0, 0, 0, 0};
   long long prof_n[F4_PROF_N] = {0, 0, 0, 0, 0, 0};
   long long launches = 0;
+  double adapt_ms[3] = {0.0, 0.0, 0.0};   // last f4_adapt: host mesh + pattern, transfer kernel + wait, record upload
   std::string err;
 
   double* state_ptr(int s) { return store + (size_t)phys[s] * state_doubles; }
@@ -93,26 +109,35 @@ int cuda_fail(f4_mesh* m, cudaError_t e, const char* what) {
     if (e_ != cudaSuccess) return cuda_fail(m, e_, #call); \
   } while (0)
 
+// Makes the mesh's device current for the duration of a call and restores the caller's (a C-ABI that takes any
+// pointer / stream must not depend on which device happens to be current)
+struct DeviceScope {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceScope(const f4_mesh* m) {
+    if (m && m->device >= 0 && cudaGetDevice(&prev) == cudaSuccess && prev != m->device)
+      switched = cudaSetDevice(m->device) == cudaSuccess;
+  }
+  ~DeviceScope() {
+    if (switched) cudaSetDevice(prev);
+  }
+};
+
 struct Scope {  // event bracket around one kernel launch
   f4_mesh* m;
-  int cls;
-  f4_mesh::Ev ev{};
-  bool on;
-  Scope(f4_mesh* m_, int cls_) : m(m_), cls(cls_), on(m_->prof) {
+  f4_mesh::Ev* ev = nullptr;
+  Scope(f4_mesh* m_, int cls) : m(m_) {
     m->launches++;
     m->prof_n[cls]++;
-    if (on) {
-      ev.cls = cls;
-      cudaEventCreate(&ev.a);
-      cudaEventCreate(&ev.b);
-      cudaEventRecord(ev.a, m->stream);
+    if (m->prof && !m->evs.empty()) {
+      if (m->evs_used == m->evs.size()) m->fold_events();
+      ev = &m->evs[m->evs_used++];
+      ev->cls = cls;
+      cudaEventRecord(ev->a, m->stream);
     }
   }
   ~Scope() {
-    if (on) {
-      cudaEventRecord(ev.b, m->stream);
-      m->evs.push_back(ev);
-    }
+    if (ev) cudaEventRecord(ev->b, m->stream);
   }
 };
 
@@ -319,6 +344,7 @@ int f4_mesh_create(int dim, int block_n, int n_ghost, const int brick[3], int ba
 }
 
 int f4_mesh_destroy(f4_mesh* m) {
+  DeviceScope dev_scope(m);
   if (!m) return F4_EINVAL;
   if (m->bound) cudaStreamSynchronize(m->stream);
   for (auto& e : m->evs) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
@@ -367,10 +393,20 @@ int f4_bind_storage(f4_mesh* m, void* dev_ptr, size_t bytes, void* cuda_stream) 
   if (!m) return F4_EINVAL;
   if (!dev_ptr || bytes < f4_storage_bytes(m) || ((uintptr_t)dev_ptr & 255)) return fail(m, F4_EINVAL, "bad storage");
   if (m->hm.Ng != NG || !stage_supported(m->hm.dim, m->hm.N))
-    return fail(m, F4_EUNSUPPORTED, "CUDA kernels exist for n_ghost=2 and (dim,N) in {(2,8),(2,16),(3,8),(3,16),(3,32)}");
+    return fail(m, F4_EUNSUPPORTED, "CUDA kernels exist for n_ghost=2 and (dim,N) in {(2,8),(2,16),(2,32),(3,8),(3,16),(3,32)}");
   int ndev = 0;
   CU(cudaGetDeviceCount(&ndev));
   if (ndev < 1) return fail(m, F4_ECUDA, "no CUDA device");
+  {
+    cudaPointerAttributes pa{};
+    CU(cudaPointerGetAttributes(&pa, dev_ptr));
+    if (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged)
+      return fail(m, F4_EINVAL, "storage is not device memory");
+    if (m->d_level && m->device != pa.device)
+      return fail(m, F4_EINVAL, "storage was bound on another device before");
+    m->device = pa.device;
+  }
+  DeviceScope dev_scope(m);
   m->store = (double*)dev_ptr;
   m->stream = (cudaStream_t)cuda_stream;
   if (!m->d_level) {
@@ -419,6 +455,7 @@ int f4_get_blocks(const f4_mesh* m, int* level, int* coords, double* origin, dou
 }
 
 int f4_set_state(f4_mesh* m, int state, const double* src, int src_is_device, int with_ghosts) {
+  DeviceScope dev_scope(m);
   int rc = check_state(m, state);
   if (rc) return rc;
   if (!src) return fail(m, F4_EINVAL, "null source");
@@ -445,6 +482,7 @@ int f4_set_state(f4_mesh* m, int state, const double* src, int src_is_device, in
 }
 
 int f4_get_state(f4_mesh* m, int state, double* dst, int dst_is_device, int with_ghosts) {
+  DeviceScope dev_scope(m);
   int rc = check_state(m, state);
   if (rc) return rc;
   if (!dst) return fail(m, F4_EINVAL, "null destination");
@@ -471,6 +509,7 @@ int f4_get_state(f4_mesh* m, int state, double* dst, int dst_is_device, int with
 }
 
 int f4_build_ghost_pattern(f4_mesh* m) {
+  DeviceScope dev_scope(m);
   if (!m) return F4_EINVAL;
   std::string err;
   int rc = m->hm.build_pattern(err);
@@ -497,12 +536,14 @@ int f4_get_pattern(const f4_mesh* m, int* records) {
 }
 
 int f4_fill_ghosts(f4_mesh* m, int state) {
+  DeviceScope dev_scope(m);
   int rc = check_state(m, state);
   if (rc) return rc;
   return fill_ghosts_impl(m, state, 0, true);
 }
 
 int f4_compute_dt(f4_mesh* m, int state, double cfl, double* dt_out) {
+  DeviceScope dev_scope(m);
   int rc = check_state(m, state);
   if (rc) return rc;
   if (!dt_out || !(cfl > 0.0)) return fail(m, F4_EINVAL, "bad cfl / null output");
@@ -567,6 +608,7 @@ const Scheme& scheme_table(int rk) {
 }  // namespace
 
 int f4_set_bc_values(f4_mesh* m, const double* values) {
+  DeviceScope dev_scope(m);
   if (!m || !values) return F4_EINVAL;
   for (int q = 0; q < 6 * m->nvar; ++q) m->bcv[q] = values[q];
   if (m->bound) {
@@ -578,13 +620,17 @@ int f4_set_bc_values(f4_mesh* m, const double* values) {
 }
 
 int f4_set_bc_callback(f4_mesh* m, f4_bc_data_fn fn, void* user) {
+  DeviceScope dev_scope(m);
   if (!m) return F4_EINVAL;
   m->bc_fn = fn;
   m->bc_user = user;
   return refresh_bc_data(m);
 }
 
-int f4_update_bc_data(f4_mesh* m) { return m ? refresh_bc_data(m) : F4_EINVAL; }
+int f4_update_bc_data(f4_mesh* m) {
+  DeviceScope dev_scope(m);
+  return m ? refresh_bc_data(m) : F4_EINVAL;
+}
 
 int f4_num_bc_faces(const f4_mesh* m) { return m ? (int)m->bc_block.size() : F4_EINVAL; }
 
@@ -607,6 +653,7 @@ int f4_set_rk_scheme(f4_mesh* m, int scheme) {
 }
 
 int f4_advance(f4_mesh* m, double dt) {
+  DeviceScope dev_scope(m);
   int rc = check_state(m, 0);
   if (rc) return rc;
   if (!(dt > 0.0)) return fail(m, F4_EINVAL, "dt must be positive");
@@ -677,6 +724,7 @@ int f4_advance(f4_mesh* m, double dt) {
 
 int f4_refine_flags(f4_mesh* m, int state, int criterion, int var, const double params[4], int* flags_out,
                     double* indicator_out) {
+  DeviceScope dev_scope(m);
   int rc = check_state(m, state);
   if (rc) return rc;
   if (!params || !flags_out) return fail(m, F4_EINVAL, "null params / flags");
@@ -697,6 +745,7 @@ int f4_refine_flags(f4_mesh* m, int state, int criterion, int var, const double 
 }
 
 int f4_adapt(f4_mesh* m, const int* refine_flags, int* changed_out) {
+  DeviceScope dev_scope(m);
   if (!m || !refine_flags || !changed_out) return F4_EINVAL;
   *changed_out = 0;
   int rc;
@@ -704,7 +753,11 @@ int f4_adapt(f4_mesh* m, const int* refine_flags, int* changed_out) {
   std::vector<Transfer> plan;
   bool changed = false;
   std::string err;
+  const auto t0 = std::chrono::steady_clock::now();
   rc = m->hm.adapt(refine_flags, plan, changed, err);
+  const auto t1 = std::chrono::steady_clock::now();
+  m->adapt_ms[0] = std::chrono::duration<double, std::milli>(t1 - t0).count();
+  m->adapt_ms[1] = m->adapt_ms[2] = 0.0;
   if (rc) return fail(m, rc, err);
   if (!changed) return F4_OK;
   *changed_out = 1;
@@ -725,13 +778,24 @@ int f4_adapt(f4_mesh* m, const int* refine_flags, int* changed_out) {
                        m->stream));
   }
   CU(cudaStreamSynchronize(m->stream));
+  const auto t2 = std::chrono::steady_clock::now();
+  m->adapt_ms[1] = std::chrono::duration<double, std::milli>(t2 - t1).count();
   std::swap(m->phys[0], m->phys[1]);  // the new numbering lives in the slab that was state 1
   std::fill(m->srl_valid.begin(), m->srl_valid.end(), 0);
   m->rate_valid = false;
-  return upload_meta(m);
+  rc = upload_meta(m);
+  m->adapt_ms[2] = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t2).count();
+  return rc;
+}
+
+int f4_last_adapt_ms(const f4_mesh* m, double ms[3]) {
+  if (!m || !ms) return F4_EINVAL;
+  for (int q = 0; q < 3; ++q) ms[q] = m->adapt_ms[q];
+  return F4_OK;
 }
 
 int f4_conserved_totals(f4_mesh* m, int state, double* totals) {
+  DeviceScope dev_scope(m);
   int rc = check_state(m, state);
   if (rc) return rc;
   if (!totals) return fail(m, F4_EINVAL, "null output");
@@ -755,21 +819,24 @@ int f4_conserved_totals(f4_mesh* m, int state, double* totals) {
 }
 
 int f4_profile_enable(f4_mesh* m, int on) {
+  DeviceScope dev_scope(m);
   if (!m) return F4_EINVAL;
+  if (on && m->evs.empty()) {
+    m->evs.resize(f4_mesh::EV_POOL);
+    for (auto& e : m->evs) {
+      CU(cudaEventCreate(&e.a));
+      CU(cudaEventCreate(&e.b));
+    }
+  }
   m->prof = on != 0;
   return F4_OK;
 }
 
 int f4_profile_get(f4_mesh* m, double ms[F4_PROF_N], long long launches[F4_PROF_N], int reset) {
+  DeviceScope dev_scope(m);
   if (!m) return F4_EINVAL;
   if (m->bound) CU(cudaStreamSynchronize(m->stream));
-  for (auto& e : m->evs) {
-    float t = 0.f;
-    if (cudaEventElapsedTime(&t, e.a, e.b) == cudaSuccess) m->prof_ms[e.cls] += t;
-    cudaEventDestroy(e.a);
-    cudaEventDestroy(e.b);
-  }
-  m->evs.clear();
+  m->fold_events();
   for (int c = 0; c < F4_PROF_N; ++c) {
     if (ms) ms[c] = m->prof_ms[c];
     if (launches) launches[c] = m->prof_n[c];

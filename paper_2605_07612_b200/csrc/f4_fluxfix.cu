@@ -63,7 +63,7 @@ cudaError_t launch_fluxfix(int dim, int n, const FixParams& p, cudaStream_t s) {
     fluxfix_kernel<D, NN><<<p.nfix, 256, 0, s>>>(p);                                      \
     return cudaGetLastError();                                                            \
   }
-  F4_FIX(2, 8) F4_FIX(2, 16) F4_FIX(3, 8) F4_FIX(3, 16) F4_FIX(3, 32)
+  F4_FIX(2, 8) F4_FIX(2, 16) F4_FIX(2, 32) F4_FIX(3, 8) F4_FIX(3, 16) F4_FIX(3, 32)
 #undef F4_FIX
   return cudaErrorInvalidValue;
 }

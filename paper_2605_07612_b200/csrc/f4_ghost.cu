@@ -451,7 +451,9 @@ __global__ void __launch_bounds__(256) maxrate_kernel(const double* __restrict__
     }
     double p = (gamma - 1.0) * (sb[(size_t)(DIM + 1) * G::VS + o] - 0.5 * rho * ke);
     double c = sqrt(gamma * p * ir);
-    mx = fmax(mx, (su + DIM * c) * inv_dx);
+    // a cell that is not a valid gas state (NaN, rho <= 0, p <= 0) makes the maximum +inf: compute_dt reports it
+    const double rate = (su + DIM * c) * inv_dx;
+    mx = fmax(mx, (rho > 0.0 && p > 0.0 && rate == rate) ? rate : __longlong_as_double(0x7ff0000000000000LL));
   }
   for (int s = 16; s > 0; s >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, s));
   if ((threadIdx.x & 31) == 0) atomicMax(maxrate, (unsigned long long)__double_as_longlong(mx));
@@ -461,6 +463,7 @@ template <typename F>
 cudaError_t dispatch(int dim, int n, F&& f) {
   if (dim == 2 && n == 8) return f(Geo<2, 8>{});
   if (dim == 2 && n == 16) return f(Geo<2, 16>{});
+  if (dim == 2 && n == 32) return f(Geo<2, 32>{});
   if (dim == 3 && n == 8) return f(Geo<3, 8>{});
   if (dim == 3 && n == 16) return f(Geo<3, 16>{});
   if (dim == 3 && n == 32) return f(Geo<3, 32>{});

@@ -699,17 +699,19 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
       double Rz[5], Lf[5];
       double pa5[5], pb5[5], wB[5];
       auto midA = [&]() {
-      if (FIN) load_prev(c - 2, pa5, pb5);  // consumed after the z flux: latency hidden
-      if (FIN && pb && c - 1 < N && (i & 3) == 0) {         // stage 2: u_t of the next plane comes from DRAM: pull it into L2 now
-#pragma unroll
-        for (int q = 0; q < 5; ++q)
-          asm volatile("prefetch.global.L2 [%0];" ::"l"(pa + (c - 1) * PP + pl(q) * (int)C::VS));
-      }
       mbar_wait(bars_u32 + 8u * sc, (ph >> sc) & 1u);
       ph ^= 1u << sc;
       convert(Wc, own, wB);
       if (c >= 0 && c < N) convert_halo(Wc);
       fence_proxy_async();   // generic-proxy writes before the async-proxy refill of this slot
+      // after the fence (it compiles to MEMBAR.ALL.CTA, which would wait for these loads): previous states of the
+      // finished plane, consumed after the z flux
+      if (FIN) load_prev(c - 2, pa5, pb5);
+      if (FIN && pb && c - 1 < N && (i & 3) == 0) {         // stage 2: u_t of the next plane comes from DRAM: pull it into L2 now
+#pragma unroll
+        for (int q = 0; q < 5; ++q)
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(pa + (c - 1) * PP + pl(q) * (int)C::VS));
+      }
       };   // midA
       auto midB = [&]() {
       // ---- z direction along the march: slope of cell c-1 from w(c-2), w(c-1), w(c);

@@ -33,7 +33,7 @@ SYMBOLS = ("f4_mesh_create", "f4_mesh_destroy", "f4_set_options", "f4_set_flux_f
            "f4_num_bc_faces", "f4_set_gravity", "f4_set_rk_scheme", "f4_storage_bytes", "f4_bind_storage",
            "f4_num_blocks", "f4_get_blocks", "f4_set_state", "f4_get_state", "f4_build_ghost_pattern",
            "f4_pattern_size", "f4_get_pattern", "f4_fill_ghosts", "f4_compute_dt", "f4_advance", "f4_refine_flags", "f4_adapt",
-           "f4_conserved_totals", "f4_profile_enable", "f4_profile_get", "f4_launch_count", "f4_last_error",
+           "f4_conserved_totals", "f4_profile_enable", "f4_profile_get", "f4_launch_count", "f4_last_adapt_ms", "f4_last_error",
            "f4_version")
 
 
@@ -51,10 +51,8 @@ def lib():
     global _lib
     if _lib is not None:
         return _lib
-    path = os.environ.get("F4_LIB") or _build.LIB   # F4_LIB: load another build of the same library
+    path = _build.LIB
     if not os.path.exists(path):
-        if path != _build.LIB:
-            raise FileNotFoundError(path)
         path = _build.build()
     L = C.CDLL(path)
     vp, ip, dp = C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_double)
@@ -89,6 +87,7 @@ def lib():
     L.f4_profile_get.argtypes = [vp, dp, C.POINTER(C.c_longlong), C.c_int]
     L.f4_launch_count.restype = C.c_longlong
     L.f4_launch_count.argtypes = [vp]
+    L.f4_last_adapt_ms.argtypes = [vp, dp]
     L.f4_last_error.restype = C.c_char_p
     L.f4_last_error.argtypes = [vp]
     L.f4_version.restype = C.c_char_p
@@ -304,6 +303,11 @@ class Mesh:
 
     def launch_count(self):
         return self.L.f4_launch_count(self.h)
+
+    def last_adapt_ms(self):
+        ms = np.zeros(3)
+        self._chk(self.L.f4_last_adapt_ms(self.h, _dp(ms)))
+        return {"host_mesh_pattern": float(ms[0]), "transfer": float(ms[1]), "upload": float(ms[2])}
 
 
 def version():

@@ -2,7 +2,8 @@
 against the CPU oracle on the same seeded inputs.  Bars (BASELINE.json
 north_star): ghost copies and restriction bit-exact; fp64 state within 1e-11
 relative L-inf (reading A16) after 10 steps; conserved totals within 1e-12
-relative; compute_dt within 1e-14 relative."""
+relative; compute_dt within 1e-14 relative on equal states (the stand-alone test;
+inside a run the two states differ by ~1e-13 and dt is compared at 1e-13)."""
 from __future__ import annotations
 
 import numpy as np
@@ -72,7 +73,7 @@ def run_and_compare(cfg, nsteps, max_blocks=None, tol=TOL_STATE):
 
 
 # ------------------------------------------------------------------ layout
-@pytest.mark.parametrize("dim,N", [(2, 8), (3, 8), (3, 16), (3, 32), (2, 16)])
+@pytest.mark.parametrize("dim,N", [(2, 8), (3, 8), (3, 16), (3, 32), (2, 16), (2, 32)])
 def test_layout_roundtrip(dim, N):
     import torch
     rng = np.random.default_rng(dim * 100 + N)
@@ -101,6 +102,7 @@ def test_layout_roundtrip(dim, N):
 @pytest.mark.parametrize("dim,N,brick,bc", [
     (2, 8, (2, 2), [PER] * 4),
     (2, 16, (3, 2), [OUT, OUT, PER, PER]),
+    (2, 32, (2, 3), [PER, PER, OUT, OUT]),
     (3, 8, (3, 2, 2), [PER, PER, OUT, OUT, PER, PER]),
     (3, 16, (2, 2, 3), [OUT, OUT, PER, PER, OUT, OUT]),
     (3, 32, (2, 1, 2), [PER, PER, PER, PER, OUT, OUT]),
@@ -142,7 +144,7 @@ def _refined_pair(dim, N, bc, rounds=2, seed=3):
 
 
 @pytest.mark.parametrize("dim,N,bc", [
-    (2, 8, [PER] * 4), (2, 16, [OUT] * 4), (3, 8, [PER] * 6), (3, 16, [OUT, OUT, PER, PER, OUT, OUT]), (3, 32, [PER] * 6)])
+    (2, 8, [PER] * 4), (2, 16, [OUT] * 4), (2, 32, [OUT, OUT, PER, PER]), (3, 8, [PER] * 6), (3, 16, [OUT, OUT, PER, PER, OUT, OUT]), (3, 32, [PER] * 6)])
 def test_fill_ghosts_amr(dim, N, bc):
     cfg, lm, om = _refined_pair(dim, N, bc, rounds=2 if N < 32 else 1)
     rec, n1, n2 = lm.pattern()
@@ -183,13 +185,14 @@ def test_config1_full_2d():
     print("config1 rel Linf", err)
 
 
-@pytest.mark.parametrize("n,scale,steps", [(2, 2, 10), (3, 1, 10), (3, 2, 3), (4, 1, 4)])
+@pytest.mark.parametrize("n,scale,steps", [(2, 2, 10), (3, 1, 10), (3, 2, 3), (4, 1, 10)])
 def test_configs_3d_small(n, scale, steps):
     err = run_and_compare(W.config(n, scale=scale), steps)
     print(f"config{n} scale {scale} rel Linf", err)
 
 
-@pytest.mark.parametrize("dim,N,brick", [(3, 8, (3, 1, 2)), (3, 8, (1, 1, 1)), (2, 8, (3, 1)), (3, 16, (1, 2, 1)), (2, 16, (2, 3))])
+@pytest.mark.parametrize("dim,N,brick", [(3, 8, (3, 1, 2)), (3, 8, (1, 1, 1)), (2, 8, (3, 1)), (3, 16, (1, 2, 1)), (2, 16, (2, 3)), (2, 32, (3, 2)),
+                                           (2, 32, (1, 1))])
 def test_ragged_and_nonpow2_bricks(dim, N, brick):
     # block counts that are not a multiple of the groups per CTA; single-block periodic wrap onto itself
     cfg = dict(W.config(2 if dim == 3 else 1), dim=dim, block_n=N, brick=tuple(brick) + (1,) * (3 - len(brick)),
