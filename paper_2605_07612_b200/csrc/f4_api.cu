@@ -45,9 +45,12 @@ struct f4_mesh {
   DevRecord* d_r1c = nullptr;  // d_r1n plus the y- / z-face same-level copies into blocks that are C2F sources
   DevRecord* d_r1f = nullptr;  // d_r1c plus all x-face same-level copies (flux-fixing mode: the stage does not push x)
   int* d_nbr = nullptr;        // [max_blocks][6] same-level neighbour per face or -1
-  size_t cap_r1 = 0, cap_r2 = 0, cap_r1n = 0;
+  // all of the above (and d_bfslot, d_fix) point into one device blob, uploaded from one pinned host buffer
+  char* d_meta = nullptr;
+  char* h_meta = nullptr;
+  size_t cap_meta = 0;
+  cudaEvent_t meta_ev = nullptr;
   int n_r1 = 0, n_r2 = 0, n_r1n = 0, n_r1z = 0, n_r1c = 0, n_r1f = 0;
-  size_t cap_r1z = 0, cap_r1c = 0, cap_r1f = 0;
   // per logical state, same-level face ghosts: 0 = stale, 1 = x faces up to date (pushed by the stage kernel that
   // produced the state; its y ghost rows and z ghost planes were never written because stage kernels fetch them
   // from the neighbours' interiors), 2 = all faces up to date
@@ -59,7 +62,7 @@ struct f4_mesh {
   int* d_bfslot = nullptr;       // [max_blocks][6] bflux slot of a block face at a refinement boundary, or -1
   DevFixBlock* d_fix = nullptr;  // coarse blocks with a finer face neighbour
   double* d_bflux = nullptr;     // [n_bfslots][nvar][N^(d-1)]
-  size_t cap_fix = 0, cap_bflux = 0;
+  size_t cap_bflux = 0;
   int n_fix = 0, n_bfslots = 0;
   unsigned long long* d_maxrate = nullptr;
   double* d_sums = nullptr;
@@ -171,6 +174,9 @@ int refresh_bc_data(f4_mesh* m) {
   return F4_OK;
 }
 
+// Pattern records, block levels, neighbour table and flux-fixing tables of the current mesh go to the device as ONE
+// blob: packed into a pinned host buffer and sent by a single asynchronous copy on the bound stream (kernels enqueued
+// afterwards are ordered behind it; the host buffer is guarded by an event until the copy has finished).
 int upload_meta(f4_mesh* m) {
   {
     int rc0 = refresh_bc_data(m);
@@ -178,91 +184,119 @@ int upload_meta(f4_mesh* m) {
   }
   if (!m->bound) return F4_OK;
   const int nb = (int)m->hm.leaves.size();
-  std::vector<int> lev(nb);
-  for (int b = 0; b < nb; ++b) lev[b] = m->hm.leaves[b].level;
-  CU(cudaMemcpyAsync(m->d_level, lev.data(), nb * sizeof(int), cudaMemcpyHostToDevice, m->stream));
-  auto pack = [](const std::vector<Record>& r, std::vector<DevRecord>& out) {
-    out.resize(r.size());
-    for (size_t q = 0; q < r.size(); ++q)
-      out[q] = DevRecord{r[q].dst, r[q].src, r[q].op | r[q].face << 2 | r[q].o1 << 5 | r[q].o2 << 6, 0};
-  };
-  std::vector<DevRecord> a, b2, an, az, ac, af;
+  auto dev = [](const Record& r) { return DevRecord{r.dst, r.src, r.op | r.face << 2 | r.o1 << 5 | r.o2 << 6, 0}; };
   std::vector<char> c2f_src(nb, 0);   // coarse blocks whose cells (face ghosts included) a prolongation stencil reads
   for (const Record& r : m->hm.r2) c2f_src[r.src] = 1;
-  pack(m->hm.r1, a);
-  pack(m->hm.r2, b2);
-  std::vector<int> nbr((size_t)nb * 6, -1);
+  // sizes of the record lists (see the d_r1* members)
+  size_t n_a = m->hm.r1.size(), n_b2 = m->hm.r2.size(), n_an = 0, n_az = 0, n_ac = 0, n_af = 0;
   for (const Record& r : m->hm.r1) {
-    const DevRecord dr{r.dst, r.src, r.op | r.face << 2 | r.o1 << 5 | r.o2 << 6, 0};
-    if (r.op == F4_OP_SRL) nbr[(size_t)r.dst * 6 + r.face] = r.src;
-    else an.push_back(dr);
-    if (r.op != F4_OP_SRL || r.face >= 2) az.push_back(dr);
-    if (r.op != F4_OP_SRL || (r.face >= 2 && c2f_src[r.dst])) ac.push_back(dr);
-    if (r.op != F4_OP_SRL || r.face < 2 || c2f_src[r.dst]) af.push_back(dr);
+    const bool srl = r.op == F4_OP_SRL;
+    n_an += !srl;
+    n_az += (!srl || r.face >= 2);
+    n_ac += (!srl || (r.face >= 2 && c2f_src[r.dst]));
+    n_af += (!srl || r.face < 2 || c2f_src[r.dst]);
   }
-  int rc;
-  if ((rc = ensure(m, m->d_r1, m->cap_r1, a.size()))) return rc;
-  if ((rc = ensure(m, m->d_r2, m->cap_r2, b2.size()))) return rc;
-  if ((rc = ensure(m, m->d_r1n, m->cap_r1n, an.size()))) return rc;
-  if ((rc = ensure(m, m->d_r1z, m->cap_r1z, az.size()))) return rc;
-  if (!az.empty()) CU(cudaMemcpyAsync(m->d_r1z, az.data(), az.size() * sizeof(DevRecord), cudaMemcpyHostToDevice, m->stream));
-  m->n_r1z = (int)az.size();
-  if ((rc = ensure(m, m->d_r1c, m->cap_r1c, ac.size()))) return rc;
-  if (!ac.empty()) CU(cudaMemcpyAsync(m->d_r1c, ac.data(), ac.size() * sizeof(DevRecord), cudaMemcpyHostToDevice, m->stream));
-  m->n_r1c = (int)ac.size();
-  if ((rc = ensure(m, m->d_r1f, m->cap_r1f, af.size()))) return rc;
-  if (!af.empty()) CU(cudaMemcpyAsync(m->d_r1f, af.data(), af.size() * sizeof(DevRecord), cudaMemcpyHostToDevice, m->stream));
-  m->n_r1f = (int)af.size();
-  if (!an.empty()) CU(cudaMemcpyAsync(m->d_r1n, an.data(), an.size() * sizeof(DevRecord), cudaMemcpyHostToDevice, m->stream));
-  CU(cudaMemcpyAsync(m->d_nbr, nbr.data(), nbr.size() * sizeof(int), cudaMemcpyHostToDevice, m->stream));
-  m->n_r1n = (int)an.size();
-  std::fill(m->srl_valid.begin(), m->srl_valid.end(), 0);
-  if (!a.empty()) CU(cudaMemcpyAsync(m->d_r1, a.data(), a.size() * sizeof(DevRecord), cudaMemcpyHostToDevice, m->stream));
-  if (!b2.empty()) CU(cudaMemcpyAsync(m->d_r2, b2.data(), b2.size() * sizeof(DevRecord), cudaMemcpyHostToDevice, m->stream));
-  m->n_r1 = (int)a.size();
-  m->n_r2 = (int)b2.size();
   // flux fixing: a bflux slot for every block face whose neighbour is finer (F2C records end there) or coarser
   // (a C2F record ends there); one DevFixBlock per coarse block with a finer face neighbour
-  std::vector<int> bfslot((size_t)nb * 6, -1);
-  std::vector<DevFixBlock> fix;
-  {
-    int nslots = 0;
-    for (const Record& r : m->hm.r1)
-      if (r.op == F4_OP_F2C && bfslot[(size_t)r.dst * 6 + r.face] < 0) bfslot[(size_t)r.dst * 6 + r.face] = nslots++;
-    for (const Record& r : m->hm.r2)
-      if (r.op == F4_OP_C2F) bfslot[(size_t)r.dst * 6 + r.face] = nslots++;
-    std::vector<int> fix_of(nb, -1);
-    for (const Record& r : m->hm.r1) {
-      if (r.op != F4_OP_F2C) continue;
-      if (fix_of[r.dst] < 0) {
-        fix_of[r.dst] = (int)fix.size();
-        DevFixBlock fb;
-        fb.blk = r.dst;
-        fb.level = m->hm.leaves[r.dst].level;
-        for (int f = 0; f < 6; ++f) {
-          fb.slot_c[f] = -1;
-          for (int o = 0; o < 4; ++o) fb.slot_f[f][o] = -1;
-        }
-        fix.push_back(fb);
-      }
-      DevFixBlock& fb = fix[fix_of[r.dst]];
-      fb.slot_c[r.face] = bfslot[(size_t)r.dst * 6 + r.face];
-      fb.slot_f[r.face][r.o1 + 2 * r.o2] = bfslot[(size_t)r.src * 6 + (r.face ^ 1)];   // the fine block's face towards us
-    }
-    for (const DevFixBlock& fb : fix)
-      for (int f = 0; f < 2 * m->hm.dim; ++f)
-        if (fb.slot_c[f] >= 0)
-          for (int o = 0; o < (m->hm.dim == 3 ? 4 : 2); ++o)
-            if (fb.slot_f[f][o] < 0) return fail(m, F4_EUNBALANCED, "flux fixing: a fine face has no coarse-to-fine record");
-    m->n_bfslots = nslots;
-    m->n_fix = (int)fix.size();
-    size_t face_doubles = (size_t)m->nvar * m->hm.N * (m->hm.dim == 3 ? m->hm.N : 1);
-    if ((rc = ensure(m, m->d_fix, m->cap_fix, fix.size()))) return rc;
-    if ((rc = ensure(m, m->d_bflux, m->cap_bflux, (size_t)nslots * face_doubles))) return rc;
-    CU(cudaMemcpyAsync(m->d_bfslot, bfslot.data(), bfslot.size() * sizeof(int), cudaMemcpyHostToDevice, m->stream));
-    if (!fix.empty()) CU(cudaMemcpyAsync(m->d_fix, fix.data(), fix.size() * sizeof(DevFixBlock), cudaMemcpyHostToDevice, m->stream));
+  std::vector<int> fix_of(nb, -1);
+  size_t n_fix = 0;
+  for (const Record& r : m->hm.r1)
+    if (r.op == F4_OP_F2C && fix_of[r.dst] < 0) fix_of[r.dst] = (int)n_fix++;
+  // blob layout (every section 256-byte aligned)
+  size_t off = 0;
+  auto section = [&](size_t bytes) { size_t o = off; off += (bytes + 255) & ~(size_t)255; return o; };
+  const size_t o_level = section((size_t)nb * sizeof(int)), o_nbr = section((size_t)nb * 6 * sizeof(int)),
+               o_bfs = section((size_t)nb * 6 * sizeof(int)), o_a = section(n_a * sizeof(DevRecord)),
+               o_b2 = section(n_b2 * sizeof(DevRecord)), o_an = section(n_an * sizeof(DevRecord)),
+               o_az = section(n_az * sizeof(DevRecord)), o_ac = section(n_ac * sizeof(DevRecord)),
+               o_af = section(n_af * sizeof(DevRecord)), o_fix = section(n_fix * sizeof(DevFixBlock));
+  const size_t total = off;
+  if (m->meta_ev) CU(cudaEventSynchronize(m->meta_ev));   // the previous upload has left the host buffer
+  if (total > m->cap_meta) {
+    CU(cudaStreamSynchronize(m->stream));   // kernels in flight still read the old blob
+    if (m->d_meta) cudaFree(m->d_meta);
+    if (m->h_meta) cudaFreeHost(m->h_meta);
+    m->d_meta = m->h_meta = nullptr;
+    m->cap_meta = 0;
+    const size_t ncap = total + total / 2 + 4096;
+    CU(cudaMalloc((void**)&m->d_meta, ncap));
+    CU(cudaHostAlloc((void**)&m->h_meta, ncap, cudaHostAllocDefault));
+    m->cap_meta = ncap;
   }
-  CU(cudaStreamSynchronize(m->stream));  // host vectors go out of scope
+  if (!m->meta_ev) CU(cudaEventCreateWithFlags(&m->meta_ev, cudaEventDisableTiming));
+  char* h = m->h_meta;
+  int* lev = (int*)(h + o_level);
+  int* nbr = (int*)(h + o_nbr);
+  int* bfslot = (int*)(h + o_bfs);
+  DevRecord *a = (DevRecord*)(h + o_a), *b2 = (DevRecord*)(h + o_b2), *an = (DevRecord*)(h + o_an),
+            *az = (DevRecord*)(h + o_az), *ac = (DevRecord*)(h + o_ac), *af = (DevRecord*)(h + o_af);
+  DevFixBlock* fix = (DevFixBlock*)(h + o_fix);
+  for (int b = 0; b < nb; ++b) lev[b] = m->hm.leaves[b].level;
+  for (int q = 0; q < nb * 6; ++q) { nbr[q] = -1; bfslot[q] = -1; }
+  {
+    size_t qa = 0, qn = 0, qz = 0, qc = 0, qf = 0;
+    for (const Record& r : m->hm.r1) {
+      const DevRecord dr = dev(r);
+      const bool srl = r.op == F4_OP_SRL;
+      a[qa++] = dr;
+      if (srl) nbr[(size_t)r.dst * 6 + r.face] = r.src;
+      else an[qn++] = dr;
+      if (!srl || r.face >= 2) az[qz++] = dr;
+      if (!srl || (r.face >= 2 && c2f_src[r.dst])) ac[qc++] = dr;
+      if (!srl || r.face < 2 || c2f_src[r.dst]) af[qf++] = dr;
+    }
+    size_t qb = 0;
+    for (const Record& r : m->hm.r2) b2[qb++] = dev(r);
+  }
+  int nslots = 0;
+  for (const Record& r : m->hm.r1)
+    if (r.op == F4_OP_F2C && bfslot[(size_t)r.dst * 6 + r.face] < 0) bfslot[(size_t)r.dst * 6 + r.face] = nslots++;
+  for (const Record& r : m->hm.r2)
+    if (r.op == F4_OP_C2F) bfslot[(size_t)r.dst * 6 + r.face] = nslots++;
+  for (int b = 0; b < nb; ++b)
+    if (fix_of[b] >= 0) {
+      DevFixBlock& fb = fix[fix_of[b]];
+      fb.blk = b;
+      fb.level = m->hm.leaves[b].level;
+      for (int f = 0; f < 6; ++f) {
+        fb.slot_c[f] = -1;
+        for (int o = 0; o < 4; ++o) fb.slot_f[f][o] = -1;
+      }
+    }
+  for (const Record& r : m->hm.r1) {
+    if (r.op != F4_OP_F2C) continue;
+    DevFixBlock& fb = fix[fix_of[r.dst]];
+    fb.slot_c[r.face] = bfslot[(size_t)r.dst * 6 + r.face];
+    fb.slot_f[r.face][r.o1 + 2 * r.o2] = bfslot[(size_t)r.src * 6 + (r.face ^ 1)];   // the fine block's face towards us
+  }
+  for (size_t q = 0; q < n_fix; ++q)
+    for (int f = 0; f < 2 * m->hm.dim; ++f)
+      if (fix[q].slot_c[f] >= 0)
+        for (int o = 0; o < (m->hm.dim == 3 ? 4 : 2); ++o)
+          if (fix[q].slot_f[f][o] < 0) return fail(m, F4_EUNBALANCED, "flux fixing: a fine face has no coarse-to-fine record");
+  m->n_bfslots = nslots;
+  m->n_fix = (int)n_fix;
+  {
+    int rc;
+    const size_t face_doubles = (size_t)m->nvar * m->hm.N * (m->hm.dim == 3 ? m->hm.N : 1);
+    if ((rc = ensure(m, m->d_bflux, m->cap_bflux, (size_t)nslots * face_doubles))) return rc;
+  }
+  CU(cudaMemcpyAsync(m->d_meta, m->h_meta, total, cudaMemcpyHostToDevice, m->stream));
+  CU(cudaEventRecord(m->meta_ev, m->stream));
+  char* d = m->d_meta;
+  m->d_level = (int*)(d + o_level);
+  m->d_nbr = (int*)(d + o_nbr);
+  m->d_bfslot = (int*)(d + o_bfs);
+  m->d_r1 = (DevRecord*)(d + o_a);
+  m->d_r2 = (DevRecord*)(d + o_b2);
+  m->d_r1n = (DevRecord*)(d + o_an);
+  m->d_r1z = (DevRecord*)(d + o_az);
+  m->d_r1c = (DevRecord*)(d + o_ac);
+  m->d_r1f = (DevRecord*)(d + o_af);
+  m->d_fix = (DevFixBlock*)(d + o_fix);
+  m->n_r1 = (int)n_a; m->n_r2 = (int)n_b2; m->n_r1n = (int)n_an; m->n_r1z = (int)n_az; m->n_r1c = (int)n_ac;
+  m->n_r1f = (int)n_af;
+  std::fill(m->srl_valid.begin(), m->srl_valid.end(), 0);
   return F4_OK;
 }
 
@@ -348,16 +382,9 @@ int f4_mesh_destroy(f4_mesh* m) {
   if (!m) return F4_EINVAL;
   if (m->bound) cudaStreamSynchronize(m->stream);
   for (auto& e : m->evs) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
-  if (m->d_level) cudaFree(m->d_level);
-  if (m->d_r1) cudaFree(m->d_r1);
-  if (m->d_r2) cudaFree(m->d_r2);
-  if (m->d_r1n) cudaFree(m->d_r1n);
-  if (m->d_r1z) cudaFree(m->d_r1z);
-  if (m->d_r1c) cudaFree(m->d_r1c);
-  if (m->d_r1f) cudaFree(m->d_r1f);
-  if (m->d_nbr) cudaFree(m->d_nbr);
-  if (m->d_bfslot) cudaFree(m->d_bfslot);
-  if (m->d_fix) cudaFree(m->d_fix);
+  if (m->d_meta) cudaFree(m->d_meta);
+  if (m->h_meta) cudaFreeHost(m->h_meta);
+  if (m->meta_ev) cudaEventDestroy(m->meta_ev);
   if (m->d_bflux) cudaFree(m->d_bflux);
   if (m->d_plan) cudaFree(m->d_plan);
   if (m->d_maxrate) cudaFree(m->d_maxrate);
@@ -402,17 +429,14 @@ int f4_bind_storage(f4_mesh* m, void* dev_ptr, size_t bytes, void* cuda_stream) 
     CU(cudaPointerGetAttributes(&pa, dev_ptr));
     if (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged)
       return fail(m, F4_EINVAL, "storage is not device memory");
-    if (m->d_level && m->device != pa.device)
+    if (m->d_maxrate && m->device != pa.device)
       return fail(m, F4_EINVAL, "storage was bound on another device before");
     m->device = pa.device;
   }
   DeviceScope dev_scope(m);
   m->store = (double*)dev_ptr;
   m->stream = (cudaStream_t)cuda_stream;
-  if (!m->d_level) {
-    CU(cudaMalloc((void**)&m->d_level, (size_t)m->hm.max_blocks * sizeof(int)));
-    CU(cudaMalloc((void**)&m->d_nbr, (size_t)m->hm.max_blocks * 6 * sizeof(int)));
-    CU(cudaMalloc((void**)&m->d_bfslot, (size_t)m->hm.max_blocks * 6 * sizeof(int)));
+  if (!m->d_maxrate) {
     CU(cudaMalloc((void**)&m->d_maxrate, sizeof(unsigned long long)));
     CU(cudaMalloc((void**)&m->d_sums, (size_t)m->hm.max_blocks * m->nvar * sizeof(double)));
     CU(cudaMalloc((void**)&m->d_flags, (size_t)m->hm.max_blocks * sizeof(int)));
@@ -749,7 +773,6 @@ int f4_adapt(f4_mesh* m, const int* refine_flags, int* changed_out) {
   if (!m || !refine_flags || !changed_out) return F4_EINVAL;
   *changed_out = 0;
   int rc;
-  if (m->bound && (rc = fill_ghosts_impl(m, 0, m->srl_valid[0], true))) return rc;  // prolongation reads the parents' face ghosts
   std::vector<Transfer> plan;
   bool changed = false;
   std::string err;
@@ -762,6 +785,9 @@ int f4_adapt(f4_mesh* m, const int* refine_flags, int* changed_out) {
   if (!changed) return F4_OK;
   *changed_out = 1;
   if (!m->bound) return refresh_bc_data(m);
+  // prolongation reads the parents' face ghosts: fill them now (only when the mesh does change), with the records
+  // of the OLD mesh, which are the ones still on the device
+  if ((rc = fill_ghosts_impl(m, 0, m->srl_valid[0], true))) return rc;
   std::vector<DevTransfer> dp(plan.size());
   for (size_t q = 0; q < plan.size(); ++q) {
     dp[q].kind = plan[q].kind;

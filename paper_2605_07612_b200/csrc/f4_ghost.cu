@@ -118,63 +118,63 @@ __device__ __forceinline__ void copy_unit(int face, bool outflow, int r, int& so
   } else { d_o = dl * P + 2 * h; so = sl * P + 2 * h; }
 }
 
+// one coarse ghost cell of an F2C record: e in [0, NVAR * NG * H^(d-1)); returns the destination, the value in val
 template <int DIM, int N>
-__device__ __forceinline__ void do_f2c(double* __restrict__ st, int dst, int src, int face, int o1, int o2) {
+__device__ __forceinline__ double* f2c_item(double* __restrict__ st, const DevRecord& rec, int e, double& val) {
   using G = Geo<DIM, N>;
-  constexpr int H = G::H, NV = G::NVAR;
+  constexpr int H = G::H;
+  const int face = (rec.meta >> 2) & 7, o1 = (rec.meta >> 5) & 1, o2 = (rec.meta >> 6) & 1;
   const int a = face >> 1, side = face & 1;
   constexpr int PER_VAR = NG * ((DIM == 3) ? H * H : H);
-  double* db = st + (size_t)dst * G::BS;
-  const double* sb = st + (size_t)src * G::BS;
-  for (int e = threadIdx.x; e < NV * PER_VAR; e += blockDim.x) {
-    int v = e / PER_VAR, r = e % PER_VAR;
-    int tt1 = r % H, tt2 = (DIM == 3) ? (r / H) % H : 0, q = r / ((DIM == 3) ? H * H : H);
-    // coarse ghost cell: normal index N+q (high) or -2+q (low); its fine children along the normal
-    int nc = side ? N + q : -2 + q;
-    int nf = side ? 2 * q : N - 4 + 2 * q;
-    int t1c = o1 * H + tt1, t2c = o2 * H + tt2;
-    int ci, cj, ck, fi, fj, fk;
-    if (a == 0) { ci = nc; cj = t1c; ck = t2c; fi = nf; fj = 2 * tt1; fk = 2 * tt2; }
-    else if (a == 1) { cj = nc; ci = t1c; ck = t2c; fj = nf; fi = 2 * tt1; fk = 2 * tt2; }
-    else { ck = nc; ci = t1c; cj = t2c; fk = nf; fi = 2 * tt1; fj = 2 * tt2; }
-    if (DIM == 2) { ck = 0; fk = 0; }
-    db[(size_t)v * G::VS + cell_off<DIM, N>(ci, cj, ck)] = restrict_mean<DIM, N>(sb + (size_t)v * G::VS, fi, fj, fk);
-  }
+  double* db = st + (size_t)rec.dst * G::BS;
+  const double* sb = st + (size_t)rec.src * G::BS;
+  const int v = e / PER_VAR, r = e % PER_VAR;
+  const int tt1 = r % H, tt2 = (DIM == 3) ? (r / H) % H : 0, q = r / ((DIM == 3) ? H * H : H);
+  // coarse ghost cell: normal index N+q (high) or -2+q (low); its fine children along the normal
+  const int nc = side ? N + q : -2 + q;
+  const int nf = side ? 2 * q : N - 4 + 2 * q;
+  const int t1c = o1 * H + tt1, t2c = o2 * H + tt2;
+  int ci, cj, ck, fi, fj, fk;
+  if (a == 0) { ci = nc; cj = t1c; ck = t2c; fi = nf; fj = 2 * tt1; fk = 2 * tt2; }
+  else if (a == 1) { cj = nc; ci = t1c; ck = t2c; fj = nf; fi = 2 * tt1; fk = 2 * tt2; }
+  else { ck = nc; ci = t1c; cj = t2c; fk = nf; fi = 2 * tt1; fj = 2 * tt2; }
+  if (DIM == 2) { ck = 0; fk = 0; }
+  val = restrict_mean<DIM, N>(sb + (size_t)v * G::VS, fi, fj, fk);
+  return db + (size_t)v * G::VS + cell_off<DIM, N>(ci, cj, ck);
 }
 
+// one coarse cell of a C2F record (its 2^d... the NG x 2^(d-1) fine ghost cells it covers): e in [0, NVAR * H^(d-1))
 template <int DIM, int N>
-__device__ __forceinline__ void do_c2f(double* __restrict__ st, int dst, int src, int face, int o1, int o2,
-                                       double theta) {
+__device__ __forceinline__ void c2f_item(double* __restrict__ st, const DevRecord& rec, int e, double theta) {
   using G = Geo<DIM, N>;
-  constexpr int H = G::H, NV = G::NVAR;
+  constexpr int H = G::H;
+  const int face = (rec.meta >> 2) & 7, o1 = (rec.meta >> 5) & 1, o2 = (rec.meta >> 6) & 1;
   const int a = face >> 1, side = face & 1;
   constexpr int PER_VAR = (DIM == 3) ? H * H : H;  // coarse cells of the one coarse layer (NG/2 = 1)
-  double* db = st + (size_t)dst * G::BS;
-  const double* sb = st + (size_t)src * G::BS;
+  double* db = st + (size_t)rec.dst * G::BS;
+  const double* sb = st + (size_t)rec.src * G::BS;
   const int ncoarse = side ? 0 : N - 1;   // F's high ghosts are covered by C's first cell, low ghosts by its last
   const int nfine = side ? N : -2;        // lower of the two fine ghost cells (lower half of the coarse cell)
-  for (int e = threadIdx.x; e < NV * PER_VAR; e += blockDim.x) {
-    int v = e / PER_VAR, r = e % PER_VAR;
-    int tt1 = r % H, tt2 = (DIM == 3) ? r / H : 0;
-    int t1c = o1 * H + tt1, t2c = o2 * H + tt2;
-    int ic, jc, kc, fi, fj, fk;
-    if (a == 0) { ic = ncoarse; jc = t1c; kc = t2c; fi = nfine; fj = 2 * tt1; fk = 2 * tt2; }
-    else if (a == 1) { jc = ncoarse; ic = t1c; kc = t2c; fj = nfine; fi = 2 * tt1; fk = 2 * tt2; }
-    else { kc = ncoarse; ic = t1c; jc = t2c; fk = nfine; fi = 2 * tt1; fj = 2 * tt2; }
-    if (DIM == 2) { kc = 0; fk = 0; }
-    double uc, sx, sy, sz;
-    coarse_slopes<DIM, N>(sb + (size_t)v * G::VS, ic, jc, kc, theta, uc, sx, sy, sz);
-    double* dv = db + (size_t)v * G::VS;
+  const int v = e / PER_VAR, r = e % PER_VAR;
+  const int tt1 = r % H, tt2 = (DIM == 3) ? r / H : 0;
+  const int t1c = o1 * H + tt1, t2c = o2 * H + tt2;
+  int ic, jc, kc, fi, fj, fk;
+  if (a == 0) { ic = ncoarse; jc = t1c; kc = t2c; fi = nfine; fj = 2 * tt1; fk = 2 * tt2; }
+  else if (a == 1) { jc = ncoarse; ic = t1c; kc = t2c; fj = nfine; fi = 2 * tt1; fk = 2 * tt2; }
+  else { kc = ncoarse; ic = t1c; jc = t2c; fk = nfine; fi = 2 * tt1; fj = 2 * tt2; }
+  if (DIM == 2) { kc = 0; fk = 0; }
+  double uc, sx, sy, sz;
+  coarse_slopes<DIM, N>(sb + (size_t)v * G::VS, ic, jc, kc, theta, uc, sx, sy, sz);
+  double* dv = db + (size_t)v * G::VS;
 #pragma unroll
-    for (int pz = 0; pz < (DIM == 3 ? 2 : 1); ++pz)
+  for (int pz = 0; pz < (DIM == 3 ? 2 : 1); ++pz)
 #pragma unroll
-      for (int py = 0; py < 2; ++py) {
-        double2 w;
-        w.x = child_value<DIM>(uc, sx, sy, sz, 0, py, pz);
-        w.y = child_value<DIM>(uc, sx, sy, sz, 1, py, pz);
-        st2(dv + cell_off<DIM, N>(fi, fj + py, fk + pz), w);   // fi even or -2: the x pair is 16-byte aligned
-      }
-  }
+    for (int py = 0; py < 2; ++py) {
+      double2 w;
+      w.x = child_value<DIM>(uc, sx, sy, sz, 0, py, pz);
+      w.y = child_value<DIM>(uc, sx, sy, sz, 1, py, pz);
+      st2(dv + cell_off<DIM, N>(fi, fj + py, fk + pz), w);   // fi even or -2: the x pair is 16-byte aligned
+    }
 }
 
 // Uniform Dirichlet / Neumann boundary face (readings A10, A10b), one record = one block face:
@@ -248,7 +248,39 @@ __global__ void __launch_bounds__(256, 4) ghost_exec_kernel(GhostParams p) {
         for (int v = 0; v < NV; ++v) st2(dptr[u] + (size_t)v * G::VS, val[u][v]);
       }
   }
-  // ---- restriction / prolongation records
+  // ---- restriction / prolongation records of this CTA, flattened over (record, cell) like the copies above, so that
+  //      a CTA with several such records (refinement boundaries) keeps all its threads and loads busy
+  __shared__ int lst_f2c[CH], lst_c2f[CH], cnt[2];
+  if (threadIdx.x == 0) {
+    int nf = 0, nc = 0;
+    for (int q = 0; q < n; ++q) {
+      const int op = recs[q].meta & 3;
+      if (op == F4_OP_F2C) lst_f2c[nf++] = q;
+      else if (op == F4_OP_C2F) lst_c2f[nc++] = q;
+    }
+    cnt[0] = nf;
+    cnt[1] = nc;
+  }
+  __syncthreads();
+  {
+    constexpr int ITEMS = NV * NG * ((DIM == 3) ? G::H * G::H : G::H);
+    const int tot = cnt[0] * ITEMS;
+    for (int e0 = threadIdx.x; e0 < tot; e0 += 2 * blockDim.x) {   // two cells (2 x 2^d loads) in flight per thread
+      const int e1 = e0 + blockDim.x;
+      double v0, v1 = 0.0;
+      double* d0 = f2c_item<DIM, N>(p.state, recs[lst_f2c[e0 / ITEMS]], e0 % ITEMS, v0);
+      double* d1 = (e1 < tot) ? f2c_item<DIM, N>(p.state, recs[lst_f2c[e1 / ITEMS]], e1 % ITEMS, v1) : nullptr;
+      *d0 = v0;
+      if (d1) *d1 = v1;
+    }
+  }
+  {
+    constexpr int ITEMS = NV * ((DIM == 3) ? G::H * G::H : G::H);
+    const int tot = cnt[1] * ITEMS;
+    for (int e = threadIdx.x; e < tot; e += blockDim.x)
+      c2f_item<DIM, N>(p.state, recs[lst_c2f[e / ITEMS]], e % ITEMS, p.theta);
+  }
+  // ---- uniform Dirichlet / Neumann / bc_data faces
 #pragma unroll 1
   for (int q = 0; q < n; ++q) {
     const DevRecord rec = recs[q];
@@ -257,8 +289,6 @@ __global__ void __launch_bounds__(256, 4) ghost_exec_kernel(GhostParams p) {
       do_bc_values<DIM, N>(p.state, rec.dst, face, o2 != 0 && o1 == 0, p.bcv,
                            p.dx0 * (1.0 / (double)(1u << p.level[rec.dst])),
                            (o1 & o2) ? p.bcdata + (size_t)rec.src * G::NVAR * ((DIM == 3) ? N * N : N) : nullptr);
-    else if (op == F4_OP_F2C) do_f2c<DIM, N>(p.state, rec.dst, rec.src, face, o1, o2);
-    else if (op == F4_OP_C2F) do_c2f<DIM, N>(p.state, rec.dst, rec.src, face, o1, o2, p.theta);
   }
 }
 
