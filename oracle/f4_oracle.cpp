@@ -12,6 +12,10 @@
 // the refinement criteria (eq. (12); config 5's pressure jump), the
 // other Runge-Kutta schemes of eq. (5), the gravity source term
 // eq. (20) and uniform Dirichlet / Neumann boundaries.
+// Second physics: scalar advection eq. (13) with a uniform velocity field, one variable per cell,
+// wave speeds min(v,0) / max(v,0); pinned (tests/test_oracle_advection.py) by upwind hand values, the dt closed form,
+// the paper's Gaussian convergence test (L1 order ~ 2) and its flux-fixing conservation test in the
+// original scalar form.
 //
 // Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
 // --impl reference legs may build, load or call this file.  It shares no code
@@ -57,6 +61,7 @@ enum { BC_PERIODIC = 0, BC_OUTFLOW = 1, BC_KEEP = 2, BC_DIRICHLET = 3, BC_NEUMAN
 enum { LIM_VANLEER = 0, LIM_MINMOD = 1, LIM_MC = 2, LIM_KOREN = 3, LIM_WENO3 = 4 };
 enum { FLUX_HLL = 0, FLUX_RUSANOV = 1 };
 enum { NB_BOUNDARY = 0, NB_SAME = 1, NB_COARSE = 2, NB_FINE = 3 };
+enum { PHYS_EULER = 0, PHYS_ADVECTION = 1 };
 
 struct Key {
   int level;
@@ -83,6 +88,10 @@ struct Mesh {
   // layout [var][t2][t1] over the cells of the block face
   std::map<std::pair<int, int>, std::vector<double>> bcdata;
   double grav[3] = {0.0, 0.0, 0.0};  // gravitational acceleration g of the source term eq. (20)
+  // physics: 0 = Euler gas dynamics (nvar = dim + 2), 1 = scalar advection eq. (13) with the uniform
+  // velocity field vel (nvar = 1: the scalar sits in Prim::rho)
+  int physics = 0;
+  double vel[3] = {0.0, 0.0, 0.0};
   int limiter, flux_scheme;
   int nstates;
   bool test_rhs = false;  // P9 pin: F(u) = lambda*u
@@ -391,6 +400,7 @@ struct Prim { double rho, u[3], p; };
 Prim to_primitive(const Mesh& m, const double* U) {
   Prim w{};
   w.rho = U[0];
+  if (m.physics == PHYS_ADVECTION) return w;   // "primitive and conservative variables are identical"
   double ke = 0.0;
   for (int d = 0; d < m.dim; ++d) { w.u[d] = U[1 + d] / w.rho; ke += w.u[d] * w.u[d]; }
   w.p = (m.gamma - 1.0) * (U[m.nvar - 1] - 0.5 * w.rho * ke);
@@ -400,11 +410,13 @@ Prim to_primitive(const Mesh& m, const double* U) {
 void to_conservative(const Mesh& m, const Prim& w, double* U) {
   double ke = 0.0;
   U[0] = w.rho;
+  if (m.physics == PHYS_ADVECTION) return;
   for (int d = 0; d < m.dim; ++d) { U[1 + d] = w.rho * w.u[d]; ke += w.u[d] * w.u[d]; }
   U[m.nvar - 1] = w.p / (m.gamma - 1.0) + 0.5 * w.rho * ke;
 }
 // get_flux: flux of eq. (14) along direction dir from primitive variables
 void get_flux(const Mesh& m, const Prim& w, int dir, double* F) {
+  if (m.physics == PHYS_ADVECTION) { F[0] = w.rho * m.vel[dir]; return; }   // eq. (13): flux rho v
   double U[5];
   to_conservative(m, w, U);
   double un = w.u[dir];
@@ -414,6 +426,11 @@ void get_flux(const Mesh& m, const Prim& w, int dir, double* F) {
 }
 // get_min_max_wavespeed: Einfeldt, reading A3: Roe averages u^ -+ d^
 void get_min_max_wavespeed(const Mesh& m, const Prim& L, const Prim& R, int dir, double& smin, double& smax) {
+  if (m.physics == PHYS_ADVECTION) {   // "the minimum and maximum wave speeds in direction i are min(v_i, 0) and max(v_i, 0)"
+    smin = std::min(m.vel[dir], 0.0);
+    smax = std::max(m.vel[dir], 0.0);
+    return;
+  }
   double rL = std::sqrt(L.rho), rR = std::sqrt(R.rho);
   double cL2 = m.gamma * L.p / L.rho, cR2 = m.gamma * R.p / R.rho;  // eq. (16)
   double uL = L.u[dir], uR = R.u[dir];
@@ -438,6 +455,10 @@ void riemann_flux(const Mesh& m, const Prim& L, const Prim& R, int dir, double* 
   double FL[5], FR[5], UL[5], UR[5];
   get_flux(m, L, dir, FL); get_flux(m, R, dir, FR);
   to_conservative(m, L, UL); to_conservative(m, R, UR);
+  if (Sp - Sm == 0.0) {   // scalar advection with v_dir = 0: no wave crosses the face, F_L = F_R = 0
+    for (int v = 0; v < m.nvar; ++v) F[v] = 0.0;
+    return;
+  }
   for (int v = 0; v < m.nvar; ++v)
     F[v] = (Sp * FL[v] - Sm * FR[v] + Sp * Sm * (UR[v] - UL[v])) / (Sp - Sm);
 }
@@ -494,7 +515,7 @@ int forward_euler_blocks(Mesh& m, int b0, int b1, int s_out, int s_deriv, double
           // i. source term ("get_source: compute the source term from primitive variables in one
           //    cell"): gravity, eq. (20): S = (0, rho g, rho g.u); zero for the BASELINE configs
           double Lu[5] = {0, 0, 0, 0, 0};
-          if (!m.test_rhs) {
+          if (!m.test_rhs && m.physics == PHYS_EULER) {
             const Prim& w0 = W(i, j, k);
             double gu = 0.0;
             for (int a = 0; a < dim; ++a) {
@@ -557,7 +578,7 @@ int forward_euler_blocks(Mesh& m, int b0, int b1, int s_out, int s_deriv, double
     for (int k = 1; k <= kmax; ++k)
       for (int j = 1; j <= N; ++j)
         for (int i = 1; i <= N; ++i) {
-          if (m.test_rhs) continue;
+          if (m.test_rhs || m.physics != PHYS_EULER) continue;
           double U[5];
           for (int v = 0; v < nvar; ++v) U[v] = m.at(s_out, b, v, i, j, k);
           Prim q = to_primitive(m, U);
@@ -633,9 +654,13 @@ double max_wave_rate_blocks(Mesh& m, int s, int b0, int b1) {
           double U[5];
           for (int v = 0; v < m.nvar; ++v) U[v] = m.at(s, b, v, i, j, k);
           Prim q = to_primitive(m, U);
-          double c = std::sqrt(m.gamma * q.p / q.rho);  // eq. (16)
           double r = 0.0;
-          for (int d = 0; d < m.dim; ++d) r += (std::fabs(q.u[d]) + c) / dx;
+          if (m.physics == PHYS_ADVECTION) {   // the only wave speed is v; reading A5: sum over dimensions
+            for (int d = 0; d < m.dim; ++d) r += std::fabs(m.vel[d]) / dx;
+          } else {
+            double c = std::sqrt(m.gamma * q.p / q.rho);  // eq. (16)
+            for (int d = 0; d < m.dim; ++d) r += (std::fabs(q.u[d]) + c) / dx;
+          }
           if (r > mx) mx = r;
         }
   }
@@ -838,6 +863,7 @@ enum { CRIT_LOHNER = 0, CRIT_PJUMP = 1 };
 int refine_flags(Mesh& m, int s, int criterion, int var, const double* params, int* flags, double* indicator) {
   const int N = m.N, dim = m.dim, kmax = (dim == 3) ? N : 1;
   if (criterion == CRIT_LOHNER && (var < 0 || var >= m.nvar)) { m.err = "refine_flags: bad variable"; return -1; }
+  if (criterion == CRIT_PJUMP && m.physics != PHYS_EULER) { m.err = "refine_flags: the pressure-jump rule needs Euler"; return -1; }
   auto pressure = [&](int b, int i, int j, int k) {
     double rho = m.at(s, b, 0, i, j, k), ke = 0.0;
     for (int a = 0; a < dim; ++a) { double mom = m.at(s, b, 1 + a, i, j, k); ke = ke + mom * mom; }
@@ -978,6 +1004,17 @@ void ora_set_bc_face_data(void* h, int block, int face, const double* data) {
   m->bcdata[{block, face}] = std::vector<double>(data, data + n);
 }
 void ora_clear_bc_data(void* h) { ((Mesh*)h)->bcdata.clear(); }
+// physics 1 = scalar advection eq. (13) with uniform velocity vel: one variable per cell.  Call
+// right after ora_create (the block store is re-allocated for the new number of variables).
+int ora_set_physics(void* h, int physics, const double* vel) {
+  Mesh* m = (Mesh*)h;
+  if (physics != PHYS_EULER && physics != PHYS_ADVECTION) return -1;
+  m->physics = physics;
+  m->nvar = (physics == PHYS_ADVECTION) ? 1 : m->dim + 2;
+  for (int a = 0; a < 3; ++a) m->vel[a] = (vel && a < m->dim) ? vel[a] : 0.0;
+  for (auto& u : m->uu) u.assign(m->blocks.size() * m->block_stride(), 0.0);
+  return 0;
+}
 void ora_set_gravity(void* h, const double* g) { for (int a = 0; a < 3; ++a) ((Mesh*)h)->grav[a] = g[a]; }
 void ora_set_test_rhs(void* h, int on, double lambda) { Mesh* m = (Mesh*)h; m->test_rhs = on; m->test_lambda = lambda; }
 int ora_num_blocks(void* h) { return (int)((Mesh*)h)->blocks.size(); }
@@ -1106,6 +1143,16 @@ void ora_to_conservative(int dim, double gamma, const double* w, double* U) {
   for (int a = 0; a < dim; ++a) q.u[a] = w[1 + a];
   q.p = w[dim + 1];
   to_conservative(m, q, U);
+}
+// face flux of scalar advection eq. (13) with velocity vel between the states rhoL, rhoR (test hook)
+double ora_advection_flux(int dim, const double* vel, int flux_scheme, double rhoL, double rhoR, int dir) {
+  Mesh m{}; m.dim = dim; m.nvar = 1; m.physics = PHYS_ADVECTION; m.flux_scheme = flux_scheme;
+  for (int a = 0; a < 3; ++a) m.vel[a] = (a < dim) ? vel[a] : 0.0;
+  Prim L{}, R{};
+  L.rho = rhoL; R.rho = rhoR;
+  double F[5];
+  riemann_flux(m, L, R, dir, F);
+  return F[0];
 }
 void ora_wavespeeds(int dim, double gamma, const double* wL, const double* wR, int dir, double* smin, double* smax) {
   Mesh m{}; m.dim = dim; m.nvar = dim + 2; m.gamma = gamma;

@@ -46,6 +46,7 @@ def lib():
         L.ora_set_test_rhs.argtypes = [C.c_void_p, C.c_int, C.c_double]
         L.ora_set_flux_fix.argtypes = [C.c_void_p, C.c_int]
         L.ora_set_gravity.argtypes = [C.c_void_p, dp]
+        L.ora_set_physics.argtypes = [C.c_void_p, C.c_int, dp]
         L.ora_set_bc_values.argtypes = [C.c_void_p, dp]
         L.ora_set_bc_face_data.argtypes = [C.c_void_p, C.c_int, C.c_int, dp]
         L.ora_clear_bc_data.argtypes = [C.c_void_p]
@@ -84,6 +85,8 @@ def lib():
         L.ora_riemann_flux.argtypes = [C.c_int, C.c_double, C.c_int, dp, dp, C.c_int, dp]
         L.ora_to_primitive.argtypes = [C.c_int, C.c_double, dp, dp]
         L.ora_to_conservative.argtypes = [C.c_int, C.c_double, dp, dp]
+        L.ora_advection_flux.argtypes = [C.c_int, dp, C.c_int, C.c_double, C.c_double, C.c_int]
+        L.ora_advection_flux.restype = C.c_double
         L.ora_wavespeeds.argtypes = [C.c_int, C.c_double, dp, dp, C.c_int, dp, dp]
         _lib = L
     return _lib
@@ -118,8 +121,19 @@ class OracleMesh:
 
     @classmethod
     def from_config(cls, cfg, n_states=2):
-        return cls(cfg["dim"], cfg["block_n"], cfg["n_ghost"], cfg["brick"], cfg["base_level"],
-                   cfg["max_level"], cfg["bc"], cfg["gamma"], n_states)
+        m = cls(cfg["dim"], cfg["block_n"], cfg["n_ghost"], cfg["brick"], cfg["base_level"],
+                cfg["max_level"], cfg["bc"], cfg["gamma"], n_states)
+        if cfg.get("physics") == "advection":
+            m.set_advection(cfg["velocity"])
+        return m
+
+    def set_advection(self, velocity):
+        """Scalar advection eq. (13) with a uniform velocity field: one variable per cell.  Call
+        before any state is set."""
+        v = np.zeros(3)
+        v[:self.dim] = np.asarray(velocity, dtype=np.float64)[:self.dim]
+        self._chk(self.L.ora_set_physics(self.h, 1, _dp(v)))
+        self.nvar = 1
 
     def __del__(self):
         if getattr(self, "h", None):
@@ -303,3 +317,9 @@ def to_conservative(dim, gamma, w):
     U = np.zeros(dim + 2)
     lib().ora_to_conservative(dim, gamma, _dp(w), _dp(U))
     return U
+
+
+def advection_flux(dim, vel, rhoL, rhoR, direction, flux=FLUX_HLL):
+    v = np.zeros(3)
+    v[:dim] = vel
+    return lib().ora_advection_flux(dim, _dp(v), flux, rhoL, rhoR, direction)

@@ -108,8 +108,18 @@ def config(n: int, scale: int | None = None) -> dict:
             c["max_level"] = c["base_level"] + scale
         c["name"] = "rayleigh-taylor-amr"
         return c
+    elif n == 8:
+        # Not a BASELINE.json config: the paper's second physics, scalar advection eq. (13) with v = (1,1,1) on the
+        # periodic unit cube, initial condition eq. (17), van Leer, Heun, CFL 0.5,
+        # 3D 512^3 in 16^3 blocks as in Table 1 (10.89 GCUPS on one H100)
+        c = dict(dim=3, block_n=16, brick=(1, 1, 1), base_level=5, max_level=5, bc=per, steps=20, seed=1008,
+                 ic="bump", physics="advection", velocity=(1.0, 1.0, 1.0))
+        c.update(n_ghost=2, gamma=1.4, cfl=0.5, name="advection")
+        if scale is not None:
+            c["base_level"] = c["max_level"] = scale
+        return c
     else:
-        raise ValueError("config 1..7")
+        raise ValueError("config 1..8")
     c.update(n_ghost=2, gamma=1.4, cfl=0.4, name=f"config{n}")
     if n == 6:
         c.update(gamma=5.0 / 3.0, cfl=0.5, name="rayleigh-taylor")
@@ -261,8 +271,28 @@ def prim_to_cons(w: np.ndarray, gamma: float) -> np.ndarray:
     return u
 
 
+def scalar_field(cfg: dict, levels, coords) -> np.ndarray:
+    """Scalar advection inputs (one variable), [nb, 1, Nz, Ny, Nx]: the paper's compact bump eq. (17) (PAPER.md:398:
+    R = 0.1, delta = 0.05) or the Gaussian of its convergence test eq. (19) (R = 0.1), both centred in the
+    unit domain, evaluated at the cell centres."""
+    xyz, gid = cell_centres(cfg, levels, coords)
+    d2 = sum((c - 0.5) ** 2 for c in xyz)
+    if cfg["ic"] == "gauss":
+        rho = np.exp(-d2 / 0.1 ** 2)
+    elif cfg["ic"] == "bump":
+        R, delta = 0.1, 0.05
+        d = np.sqrt(d2)
+        q = 1.0 + (d - R) / delta
+        rho = np.where(d < R - delta, 1.0, np.where(d < R, 1.0 - 3.0 * q ** 2 + 2.0 * q ** 3, 0.0))
+    else:
+        raise ValueError(cfg["ic"])
+    return np.ascontiguousarray(np.broadcast_to(rho, gid.shape)[:, None].astype(np.float64))
+
+
 def initial_state(cfg: dict, levels, coords, noise: bool = True) -> np.ndarray:
     """Conservative interior state [nb, nvar, Nz, Ny, Nx] (C-contiguous)."""
+    if cfg.get("physics") == "advection":
+        return scalar_field(cfg, levels, coords)
     return np.ascontiguousarray(prim_to_cons(initial_primitives(cfg, levels, coords, noise), cfg["gamma"]))
 
 
