@@ -149,7 +149,7 @@ def pattern_bytes(mesh, n, d):
     1/2^(d-1) share of a coarse face and reads 2^d fine cells per ghost; a C2F record writes a fine face and
     reads the (Ng/2+2) x (N/2+2)^(d-1) coarse cells of its slope stencils."""
     rec, n1, n2 = mesh.pattern()
-    nvar, ng = d + 2, 2
+    nvar, ng = mesh.nvar, 2
     face = ng * n ** (d - 1) * nvar * 8
     ops = rec[:, 0]
     n_copy = int(np.sum((ops == 0) | (ops == 1)))
@@ -242,7 +242,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3,
                     help="1-5: BASELINE.json configs (3 = headline); 6: the paper's own Rayleigh-Taylor benchmark; "
-                         "7: the same with AMR driven by the paper's criterion eq. (12)")
+                         "7: the same with AMR driven by the paper's criterion eq. (12); 8: the paper's 3D scalar "
+                         "advection benchmark (eq. 13, 512^3 in 16^3 blocks)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -406,7 +407,7 @@ def main():
     # (bpc*(1 + 2*Ng/N)), extra s_prev reads (bpc/2 on average for Heun); the same-level ghost copy is fused into
     # the stage kernel, so on a uniform mesh there is no separate ghost-fill traffic.
     r = 1.0 + 2.0 * d * 2 / n
-    bpc = 8 * (d + 2)
+    bpc = 8 * mesh.nvar                                   # Euler: d + 2 variables; scalar advection: 1
     st_ms, st_n = prof["stage"]
     cells_per_launch = updates / max(st_n, 1)            # = cells on a static mesh; the average on an adaptive one
     # previous states other than s_deriv read per sub-step, averaged over the scheme's sub-steps (Heun: 0 and 1)
@@ -433,15 +434,18 @@ def main():
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         # BASELINE.md holds a paper number only for the paper's own workload (config 6 at full size, Heun):
         # 1.35 GCUPS on one H100, PAPER.md:496 -- another machine's: context, not the target
-        "vs_baseline": (value / 1.35) if (args.config == 6 and args.rk == "heun") else None,
+        # (config 6) and 10.89 GCUPS for its 3D scalar advection row (config 8)
+        "vs_baseline": (value / 1.35) if (args.config == 6 and args.rk == "heun") else
+                       ((value / 10.89) if (args.config == 8 and args.rk == "heun") else None),
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(cfg), "blocks": nb, "cells": cells,
+        "config": {"workload": workload_name(cfg), "physics": cfg.get("physics", "euler"), "blocks": nb, "cells": cells,
                    "l2": "state (2 x %.1f GB) is larger than L2; no flush needed" % (mesh.storage_bytes() / 2e9),
                    "parallelism": "replicas only" if world > 1 else "1 GPU", "rk": args.rk,
                    "flux_fix": bool(args.flux_fix)},
         "roofline": {"bound": "hbm", "achieved": stage_gbs, "peak": peak, "unit": "GB/s",
                      "frac": (stage_gbs / peak) if stage_gbs else None, "traffic": traffic,
-                     "kernel": "stage_kernel", "peak_source": peak_src,
+                     "kernel": "advect_kernel" if cfg.get("physics") == "advection" else "stage_kernel",
+                     "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": stage_bytes, "avg_launch_ms": st_ms / max(st_n, 1)},
         "ghost_fill": {"GBps": ghost_gbs, "frac_of_hbm_peak": (ghost_gbs / peak) if ghost_gbs else None,
                        "ms_per_fill": fill_ms, "bytes_read": int(rd_b), "bytes_written": int(wr_b),

@@ -112,6 +112,18 @@ int f4_set_options(f4_mesh *m, int limiter, int flux_scheme, double theta);
  * takes exactly the same path as with the switch off.  Host only; takes effect at the next f4_advance. */
 int f4_set_flux_fix(f4_mesh *m, int on);
 
+/* Physics (default Euler gas dynamics, Nvar = dim + 2).  F4_PHYS_ADVECTION: the scalar advection
+ * equation (13) of PAPER.md:364-370, d(rho)/dt + div(rho v) = 0 with the uniform velocity field `velocity` (host,
+ * [3], the first dim entries are used): ONE variable per cell, primitive = conservative, wave speeds min(v_i, 0) and
+ * max(v_i, 0), i.e. the upwind flux; f4_compute_dt = CFL dx_finest / sum_i |v_i| without a device pass.  Limiters:
+ * van Leer, minmod, MC; Runge-Kutta schemes with at most two previous states; no gravity; the pressure-jump
+ * criterion is not defined.  Must be called before f4_bind_storage (the storage size changes with Nvar).
+ * Errors: F4_EINVAL (unknown physics, NaN velocity, already bound). */
+enum { F4_PHYS_EULER = 0, F4_PHYS_ADVECTION = 1 };
+int f4_set_physics(f4_mesh *m, int physics, const double velocity[3]);
+/* variables per cell of the mesh's physics */
+int f4_num_vars(const f4_mesh *m);
+
 /* bytes of the block store: n_states*max_blocks*Nvar*P^dim*8. */
 size_t f4_storage_bytes(const f4_mesh *m);
 

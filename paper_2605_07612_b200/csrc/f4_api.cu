@@ -1,5 +1,6 @@
 // C-ABI of the f4 library (include/f4.h): argument checking, device metadata,
 // launch sequencing.  All arithmetic of the path lives in f4_ghost.cu / f4_stage.cu.
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -19,6 +20,8 @@ struct f4_mesh {
   int limiter = F4_LIM_VANLEER, flux = F4_FLUX_HLL;
   int rk = F4_RK_HEUN;
   double grav[3] = {0.0, 0.0, 0.0};
+  int physics = F4_PHYS_EULER;           // F4_PHYS_ADVECTION: scalar advection eq. (13) with the uniform velocity vel
+  double vel[3] = {0.0, 0.0, 0.0};
   double bcv[6 * 5] = {0.0};     // uniform Dirichlet values / Neumann derivatives [6][nvar]
   double* d_bcv = nullptr;
   // spatially varying boundary data (eq. 4): faces in record order, host copy, device copy
@@ -316,13 +319,13 @@ int fill_ghosts_impl(f4_mesh* m, int state, int have, bool need_z, bool for_stag
   else if (for_stage && no_push) { r1 = m->d_r1f; n1 = m->n_r1f; after = 0; }
   if (n1) {
     Scope sc(m, F4_PROF_R1);
-    CU(launch_ghost(m->hm.dim, m->hm.N,
+    CU(launch_ghost(m->hm.dim, m->hm.N, m->nvar,
                     GhostParams{st, r1, n1, m->theta, m->d_bcv, m->d_bcdata, m->d_level, m->hm.dx_of_level(0)}, m->stream));
   }
   m->srl_valid[state] = (char)after;
   if (m->n_r2) {
     Scope sc(m, F4_PROF_R2);
-    CU(launch_ghost(m->hm.dim, m->hm.N,
+    CU(launch_ghost(m->hm.dim, m->hm.N, m->nvar,
                     GhostParams{st, m->d_r2, m->n_r2, m->theta, m->d_bcv, m->d_bcdata, m->d_level, m->hm.dx_of_level(0)},
                     m->stream));
   }
@@ -414,6 +417,26 @@ int f4_set_flux_fix(f4_mesh* m, int on) {
   return F4_OK;
 }
 
+int f4_set_physics(f4_mesh* m, int physics, const double velocity[3]) {
+  if (!m) return F4_EINVAL;
+  if (physics != F4_PHYS_EULER && physics != F4_PHYS_ADVECTION) return fail(m, F4_EINVAL, "unknown physics");
+  if (m->bound) return fail(m, F4_EINVAL, "f4_set_physics must precede f4_bind_storage (it changes the storage size)");
+  if (physics == F4_PHYS_ADVECTION) {
+    if (!velocity) return fail(m, F4_EINVAL, "scalar advection needs a velocity");
+    for (int a = 0; a < 3; ++a) {
+      if (velocity[a] != velocity[a]) return fail(m, F4_EINVAL, "velocity is not a number");
+      m->vel[a] = (a < m->hm.dim) ? velocity[a] : 0.0;
+    }
+  }
+  m->physics = physics;
+  m->nvar = (physics == F4_PHYS_ADVECTION) ? 1 : m->hm.dim + 2;
+  m->bs = m->vs * m->nvar;
+  m->state_doubles = m->bs * (size_t)m->hm.max_blocks;
+  return F4_OK;
+}
+
+int f4_num_vars(const f4_mesh* m) { return m ? m->nvar : F4_EINVAL; }
+
 size_t f4_storage_bytes(const f4_mesh* m) { return m ? m->state_doubles * (size_t)m->n_states * sizeof(double) : 0; }
 
 int f4_bind_storage(f4_mesh* m, void* dev_ptr, size_t bytes, void* cuda_stream) {
@@ -454,7 +477,7 @@ int f4_bind_storage(f4_mesh* m, void* dev_ptr, size_t bytes, void* cuda_stream) 
   CU(cudaMemcpyAsync(m->d_bcv, m->bcv, sizeof(m->bcv), cudaMemcpyHostToDevice, m->stream));
   for (int s = 0; s < m->n_states; ++s) {
     Scope sc(m, F4_PROF_LAYOUT);
-    CU(launch_init_benign(m->hm.dim, m->hm.N, m->state_ptr(s), m->hm.max_blocks, m->gamma, m->stream));
+    CU(launch_init_benign(m->hm.dim, m->hm.N, m->nvar, m->state_ptr(s), m->hm.max_blocks, m->gamma, m->stream));
   }
   m->rate_valid = false;
   return upload_meta(m);
@@ -490,7 +513,7 @@ int f4_set_state(f4_mesh* m, int state, const double* src, int src_is_device, in
   m->srl_valid[state] = 0;
   if (src_is_device) {
     Scope sc(m, F4_PROF_LAYOUT);
-    CU(launch_pack(dim, N, m->state_ptr(state), src, 0, nb, with_ghosts, m->stream));
+    CU(launch_pack(dim, N, m->nvar, m->state_ptr(state), src, 0, nb, with_ghosts, m->stream));
     return F4_OK;
   }
   const int chunk = (int)(m->stage_bytes / (per_block * sizeof(double)));
@@ -499,7 +522,7 @@ int f4_set_state(f4_mesh* m, int state, const double* src, int src_is_device, in
     CU(cudaMemcpyAsync(m->d_stage, src + (size_t)b0 * per_block, (size_t)n * per_block * sizeof(double),
                        cudaMemcpyHostToDevice, m->stream));
     Scope sc(m, F4_PROF_LAYOUT);
-    CU(launch_pack(dim, N, m->state_ptr(state), m->d_stage, b0, n, with_ghosts, m->stream));
+    CU(launch_pack(dim, N, m->nvar, m->state_ptr(state), m->d_stage, b0, n, with_ghosts, m->stream));
   }
   CU(cudaStreamSynchronize(m->stream));
   return F4_OK;
@@ -515,7 +538,7 @@ int f4_get_state(f4_mesh* m, int state, double* dst, int dst_is_device, int with
   const size_t per_block = (size_t)m->nvar * E * E * (dim == 3 ? E : 1);
   if (dst_is_device) {
     Scope sc(m, F4_PROF_LAYOUT);
-    CU(launch_unpack(dim, N, m->state_ptr(state), dst, 0, nb, with_ghosts, m->stream));
+    CU(launch_unpack(dim, N, m->nvar, m->state_ptr(state), dst, 0, nb, with_ghosts, m->stream));
     return F4_OK;
   }
   const int chunk = (int)(m->stage_bytes / (per_block * sizeof(double)));
@@ -523,7 +546,7 @@ int f4_get_state(f4_mesh* m, int state, double* dst, int dst_is_device, int with
     const int n = (nb - b0 < chunk) ? nb - b0 : chunk;
     {
       Scope sc(m, F4_PROF_LAYOUT);
-      CU(launch_unpack(dim, N, m->state_ptr(state), m->d_stage, b0, n, with_ghosts, m->stream));
+      CU(launch_unpack(dim, N, m->nvar, m->state_ptr(state), m->d_stage, b0, n, with_ghosts, m->stream));
     }
     CU(cudaMemcpyAsync(dst + (size_t)b0 * per_block, m->d_stage, (size_t)n * per_block * sizeof(double),
                        cudaMemcpyDeviceToHost, m->stream));
@@ -571,6 +594,17 @@ int f4_compute_dt(f4_mesh* m, int state, double cfl, double* dt_out) {
   int rc = check_state(m, state);
   if (rc) return rc;
   if (!dt_out || !(cfl > 0.0)) return fail(m, F4_EINVAL, "bad cfl / null output");
+  if (m->physics == F4_PHYS_ADVECTION) {
+    // the only wave speed is v: max over cells of sum_d |v_d| / dx is taken on the finest level present
+    int lmax = 0;
+    for (const Leaf& l : m->hm.leaves) lmax = l.level > lmax ? l.level : lmax;
+    double sv = 0.0;
+    for (int a = 0; a < m->hm.dim; ++a) sv += std::fabs(m->vel[a]);
+    const double rate = sv / m->hm.dx_of_level(lmax);
+    if (!(rate > 0.0)) return fail(m, F4_EINVAL, "compute_dt: the advection velocity is zero");
+    *dt_out = cfl / rate;
+    return F4_OK;
+  }
   if (!(state == 0 && m->rate_valid)) {
     CU(cudaMemsetAsync(m->d_maxrate, 0, sizeof(unsigned long long), m->stream));
     Scope sc(m, F4_PROF_DT);
@@ -690,6 +724,8 @@ int f4_advance(f4_mesh* m, double dt) {
   p.nblocks = nb;
   p.limiter = m->limiter;
   p.flux = m->flux;
+  const bool adv = m->physics == F4_PHYS_ADVECTION;
+  for (int a = 0; a < 3; ++a) p.vel[a] = m->vel[a];
   for (int a = 0; a < 3; ++a) p.grav[a] = m->grav[a];
   p.has_grav = (m->grav[0] != 0.0 || m->grav[1] != 0.0 || m->grav[2] != 0.0) ? 1 : 0;
   // flux fixing acts only where the mesh has refinement boundaries.  The corrected cells must be
@@ -725,24 +761,30 @@ int f4_advance(f4_mesh* m, double dt) {
       p.sdt_l[l] = p.dt_sub * p.inv_dx_l[l];
     }
     // CFL max of the new state fused into the last sub-step ("a limit for the next time step")
-    p.maxrate = (last && !ff) ? m->d_maxrate : nullptr;
+    p.maxrate = (last && !ff && !adv) ? m->d_maxrate : nullptr;
     if (p.maxrate) CU(cudaMemsetAsync(m->d_maxrate, 0, sizeof(unsigned long long), m->stream));
     {
       Scope sc(m, F4_PROF_STAGE);
-      CU(launch_stage(dim, N, p, m->stream));
+      if (adv) {
+        if (!advect_supported(p))
+          return fail(m, F4_EUNSUPPORTED, "scalar advection: van Leer / minmod / MC limiters and at most two previous states");
+        CU(launch_advect(dim, N, p, m->stream));
+      } else {
+        CU(launch_stage(dim, N, p, m->stream));
+      }
     }
     if (ff) {
       fp.out = p.out;
       for (int l = 0; l < MAXL; ++l) fp.sdt_l[l] = p.sdt_l[l];
       Scope sc(m, F4_PROF_STAGE);
-      CU(launch_fluxfix(dim, N, fp, m->stream));
+      CU(launch_fluxfix(dim, N, m->nvar, fp, m->stream));
     }
     // x same-level ghosts of `out` were pushed by the stage (its y ghost rows / z ghost planes were not written);
     // BC / F2C / C2F ghosts of `out` are stale until the next fill
     m->srl_valid[ss.out] = ff ? 0 : 1;
   }
   if (sch.result != 0) std::swap(m->phys[0], m->phys[sch.result]), std::swap(m->srl_valid[0], m->srl_valid[sch.result]);
-  m->rate_valid = !ff;
+  m->rate_valid = !ff && !adv;
   return F4_OK;
 }
 
@@ -754,11 +796,12 @@ int f4_refine_flags(f4_mesh* m, int state, int criterion, int var, const double 
   if (!params || !flags_out) return fail(m, F4_EINVAL, "null params / flags");
   if (criterion != F4_CRIT_LOHNER && criterion != F4_CRIT_PJUMP) return fail(m, F4_EINVAL, "unknown criterion");
   if (criterion == F4_CRIT_LOHNER && (var < 0 || var >= m->nvar)) return fail(m, F4_EINVAL, "variable out of range");
+  if (criterion == F4_CRIT_PJUMP && m->physics != F4_PHYS_EULER) return fail(m, F4_EINVAL, "the pressure-jump rule needs Euler");
   const int nb = (int)m->hm.leaves.size();
   if ((rc = fill_ghosts_impl(m, state, m->srl_valid[state], true))) return rc;
   {
     Scope sc(m, F4_PROF_REGRID);
-    CU(launch_flags(m->hm.dim, m->hm.N, m->state_ptr(state), nb, criterion, var, m->gamma, params, m->d_flags,
+    CU(launch_flags(m->hm.dim, m->hm.N, m->nvar, m->state_ptr(state), nb, criterion, var, m->gamma, params, m->d_flags,
                     m->d_indicator, m->stream));
   }
   CU(cudaMemcpyAsync(flags_out, m->d_flags, (size_t)nb * sizeof(int), cudaMemcpyDeviceToHost, m->stream));
@@ -800,7 +843,7 @@ int f4_adapt(f4_mesh* m, const int* refine_flags, int* changed_out) {
   CU(cudaMemcpyAsync(m->d_plan, dp.data(), dp.size() * sizeof(DevTransfer), cudaMemcpyHostToDevice, m->stream));
   {
     Scope sc(m, F4_PROF_REGRID);
-    CU(launch_transfer(m->hm.dim, m->hm.N, m->state_ptr(0), m->state_ptr(1), m->d_plan, (int)dp.size(), m->theta,
+    CU(launch_transfer(m->hm.dim, m->hm.N, m->nvar, m->state_ptr(0), m->state_ptr(1), m->d_plan, (int)dp.size(), m->theta,
                        m->stream));
   }
   CU(cudaStreamSynchronize(m->stream));
@@ -828,7 +871,7 @@ int f4_conserved_totals(f4_mesh* m, int state, double* totals) {
   const int nb = (int)m->hm.leaves.size();
   {
     Scope sc(m, F4_PROF_LAYOUT);
-    CU(launch_block_sums(m->hm.dim, m->hm.N, m->state_ptr(state), nb, m->d_sums, m->stream));
+    CU(launch_block_sums(m->hm.dim, m->hm.N, m->nvar, m->state_ptr(state), nb, m->d_sums, m->stream));
   }
   std::vector<double> sums((size_t)nb * m->nvar);
   CU(cudaMemcpyAsync(sums.data(), m->d_sums, sums.size() * sizeof(double), cudaMemcpyDeviceToHost, m->stream));

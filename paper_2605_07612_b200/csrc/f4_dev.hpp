@@ -45,6 +45,7 @@ struct StageParams {
   double* bflux;
   // gravity source term S = (0, rho g, rho g.u), eq. (20) PAPER.md:429-431 (general instances)
   double grav[3];
+  double vel[3];   // scalar advection eq. (13): the uniform velocity field (f4_advect.cu)
   int has_grav;
   int grav_from;   // where the kernel finds s_deriv's own-cell conservative values: 0 prev0, 1 prev1, 2 load from deriv
 };
@@ -68,19 +69,19 @@ struct GhostParams {
 };
 
 // every launcher returns the cudaError_t of the launch
-cudaError_t launch_ghost(int dim, int n, const GhostParams& p, cudaStream_t s);
+cudaError_t launch_ghost(int dim, int n, int nvar, const GhostParams& p, cudaStream_t s);
 cudaError_t launch_stage(int dim, int n, const StageParams& p, cudaStream_t s);
 cudaError_t launch_maxrate(int dim, int n, const double* state, const int* level, int nblocks, double gamma,
                            double inv_dx0, unsigned long long* maxrate, cudaStream_t s);
-cudaError_t launch_transfer(int dim, int n, const double* old_state, double* new_state, const DevTransfer* plan,
+cudaError_t launch_transfer(int dim, int n, int nvar, const double* old_state, double* new_state, const DevTransfer* plan,
                             int nplan, double theta, cudaStream_t s);
 // layout kernels: natural (interior or padded) <-> wrapped padded store
-cudaError_t launch_pack(int dim, int n, double* store_state, const double* src, int b0, int nb, int with_ghosts,
+cudaError_t launch_pack(int dim, int n, int nvar, double* store_state, const double* src, int b0, int nb, int with_ghosts,
                         cudaStream_t s);
-cudaError_t launch_unpack(int dim, int n, const double* store_state, double* dst, int b0, int nb, int with_ghosts,
+cudaError_t launch_unpack(int dim, int n, int nvar, const double* store_state, double* dst, int b0, int nb, int with_ghosts,
                           cudaStream_t s);
-cudaError_t launch_init_benign(int dim, int n, double* store_state, int nb, double gamma, cudaStream_t s);
-cudaError_t launch_block_sums(int dim, int n, const double* state, int nb, double* sums /*[nb][nvar]*/, cudaStream_t s);
+cudaError_t launch_init_benign(int dim, int n, int nvar, double* store_state, int nb, double gamma, cudaStream_t s);
+cudaError_t launch_block_sums(int dim, int n, int nvar, const double* state, int nb, double* sums /*[nb][nvar]*/, cudaStream_t s);
 // coarse-side correction u -= -+ dt_sub/dx_c (mean fine flux - coarse flux) in the cells next to refinement boundaries
 struct FixParams {
   double* out;              // the state the stage kernel just wrote
@@ -89,11 +90,14 @@ struct FixParams {
   const double* bflux;
   double sdt_l[MAXL];       // dt_sub/dx per level
 };
-cudaError_t launch_fluxfix(int dim, int n, const FixParams& p, cudaStream_t s);
+cudaError_t launch_fluxfix(int dim, int n, int nvar, const FixParams& p, cudaStream_t s);
 // per-block refinement flags and indicator (device arrays) from a ghost-filled state
-cudaError_t launch_flags(int dim, int n, const double* state, int nblocks, int criterion, int var, double gamma,
+cudaError_t launch_flags(int dim, int n, int nvar, const double* state, int nblocks, int criterion, int var, double gamma,
                          const double params[4], int* flags, double* indicator, cudaStream_t s);
 bool stage_supported(int dim, int n);
+// scalar advection eq. (13), PAPER.md:364-370 (f4_advect.cu): symmetric limiters, at most two previous states
+bool advect_supported(const StageParams& p);
+cudaError_t launch_advect(int dim, int n, const StageParams& p, cudaStream_t s);
 
 
 }  // namespace f4

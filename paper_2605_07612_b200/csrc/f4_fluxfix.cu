@@ -14,9 +14,9 @@
 namespace f4 {
 namespace {
 
-template <int DIM, int N>
+template <int DIM, int N, int NV>
 __global__ void __launch_bounds__(256) fluxfix_kernel(const __grid_constant__ FixParams p) {
-  constexpr int P = N + 2 * NG, NV = DIM + 2, H = N / 2;
+  constexpr int P = N + 2 * NG, H = N / 2;
   constexpr int KM = (DIM == 3) ? N : 1;       // cells along t2
   constexpr int FS = N * KM;                   // cells of one block face
   constexpr size_t VS = (size_t)P * P * ((DIM == 3) ? P : 1);
@@ -56,11 +56,12 @@ __global__ void __launch_bounds__(256) fluxfix_kernel(const __grid_constant__ Fi
 
 }  // namespace
 
-cudaError_t launch_fluxfix(int dim, int n, const FixParams& p, cudaStream_t s) {
+cudaError_t launch_fluxfix(int dim, int n, int nvar, const FixParams& p, cudaStream_t s) {
   if (p.nfix <= 0) return cudaSuccess;
 #define F4_FIX(D, NN)                                                                     \
   if (dim == D && n == NN) {                                                              \
-    fluxfix_kernel<D, NN><<<p.nfix, 256, 0, s>>>(p);                                      \
+    if (nvar == 1) fluxfix_kernel<D, NN, 1><<<p.nfix, 256, 0, s>>>(p);                    \
+    else fluxfix_kernel<D, NN, D + 2><<<p.nfix, 256, 0, s>>>(p);                          \
     return cudaGetLastError();                                                            \
   }
   F4_FIX(2, 8) F4_FIX(2, 16) F4_FIX(2, 32) F4_FIX(3, 8) F4_FIX(3, 16) F4_FIX(3, 32)

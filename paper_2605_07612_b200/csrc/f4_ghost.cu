@@ -15,12 +15,13 @@
 namespace f4 {
 namespace {
 
-template <int DIM, int N>
+// NV: variables per cell (Euler: DIM + 2; scalar advection eq. (13): 1)
+template <int DIM, int N, int NV = DIM + 2>
 struct Geo {
   static constexpr int P = N + 2 * NG;
   static constexpr int PZ = (DIM == 3) ? P : 1;
   static constexpr int NZ = (DIM == 3) ? N : 1;
-  static constexpr int NVAR = DIM + 2;
+  static constexpr int NVAR = NV;
   static constexpr int H = N / 2;
   static constexpr size_t VS = (size_t)P * P * PZ;   // doubles per (block, var)
   static constexpr size_t BS = VS * NVAR;            // doubles per block
@@ -119,9 +120,9 @@ __device__ __forceinline__ void copy_unit(int face, bool outflow, int r, int& so
 }
 
 // one coarse ghost cell of an F2C record: e in [0, NVAR * NG * H^(d-1)); returns the destination, the value in val
-template <int DIM, int N>
+template <int DIM, int N, int NV>
 __device__ __forceinline__ double* f2c_item(double* __restrict__ st, const DevRecord& rec, int e, double& val) {
-  using G = Geo<DIM, N>;
+  using G = Geo<DIM, N, NV>;
   constexpr int H = G::H;
   const int face = (rec.meta >> 2) & 7, o1 = (rec.meta >> 5) & 1, o2 = (rec.meta >> 6) & 1;
   const int a = face >> 1, side = face & 1;
@@ -144,9 +145,9 @@ __device__ __forceinline__ double* f2c_item(double* __restrict__ st, const DevRe
 }
 
 // one coarse cell of a C2F record (its 2^d... the NG x 2^(d-1) fine ghost cells it covers): e in [0, NVAR * H^(d-1))
-template <int DIM, int N>
+template <int DIM, int N, int NV>
 __device__ __forceinline__ void c2f_item(double* __restrict__ st, const DevRecord& rec, int e, double theta) {
-  using G = Geo<DIM, N>;
+  using G = Geo<DIM, N, NV>;
   constexpr int H = G::H;
   const int face = (rec.meta >> 2) & 7, o1 = (rec.meta >> 5) & 1, o2 = (rec.meta >> 6) & 1;
   const int a = face >> 1, side = face & 1;
@@ -181,12 +182,12 @@ __device__ __forceinline__ void c2f_item(double* __restrict__ st, const DevRecor
 //   Dirichlet: ghost layer g mirrors interior layer g through the face, u_ghost = 2 u_b - u_interior;
 //   Neumann:   ghost layer g = first interior layer + (g dx) u_b'  (u_b' = outward normal derivative).
 // Individually rounded operations in the order the formulas are written: bit-exact against the oracle.
-template <int DIM, int N>
+template <int DIM, int N, int NV>
 __device__ __forceinline__ void do_bc_values(double* __restrict__ st, int blk, int face, bool neumann,
                                              const double* __restrict__ bcv, double dx,
                                              const double* __restrict__ data /* this face's bc_data, or nullptr */) {
-  using G = Geo<DIM, N>;
-  constexpr int NV = G::NVAR, FS = (DIM == 3) ? N * N : N;
+  using G = Geo<DIM, N, NV>;
+  constexpr int FS = (DIM == 3) ? N * N : N;
   const int a = face >> 1, side = face & 1;
   double* db = st + (size_t)blk * G::BS;
   for (int e = threadIdx.x; e < NV * NG * FS; e += blockDim.x) {
@@ -204,10 +205,10 @@ __device__ __forceinline__ void do_bc_values(double* __restrict__ st, int blk, i
   }
 }
 
-template <int DIM, int N>
+template <int DIM, int N, int NV>
 __global__ void __launch_bounds__(256, 4) ghost_exec_kernel(GhostParams p) {
-  using G = Geo<DIM, N>;
-  constexpr int CH = 2 * DIM, NV = G::NVAR;
+  using G = Geo<DIM, N, NV>;
+  constexpr int CH = 2 * DIM;
   constexpr int PER_VAR = (DIM == 3) ? N * N : N;   // 16-byte units per variable of one face copy
   __shared__ DevRecord recs[CH];
   const int r0 = blockIdx.x * CH;
@@ -268,8 +269,8 @@ __global__ void __launch_bounds__(256, 4) ghost_exec_kernel(GhostParams p) {
     for (int e0 = threadIdx.x; e0 < tot; e0 += 2 * blockDim.x) {   // two cells (2 x 2^d loads) in flight per thread
       const int e1 = e0 + blockDim.x;
       double v0, v1 = 0.0;
-      double* d0 = f2c_item<DIM, N>(p.state, recs[lst_f2c[e0 / ITEMS]], e0 % ITEMS, v0);
-      double* d1 = (e1 < tot) ? f2c_item<DIM, N>(p.state, recs[lst_f2c[e1 / ITEMS]], e1 % ITEMS, v1) : nullptr;
+      double* d0 = f2c_item<DIM, N, NV>(p.state, recs[lst_f2c[e0 / ITEMS]], e0 % ITEMS, v0);
+      double* d1 = (e1 < tot) ? f2c_item<DIM, N, NV>(p.state, recs[lst_f2c[e1 / ITEMS]], e1 % ITEMS, v1) : nullptr;
       *d0 = v0;
       if (d1) *d1 = v1;
     }
@@ -278,7 +279,7 @@ __global__ void __launch_bounds__(256, 4) ghost_exec_kernel(GhostParams p) {
     constexpr int ITEMS = NV * ((DIM == 3) ? G::H * G::H : G::H);
     const int tot = cnt[1] * ITEMS;
     for (int e = threadIdx.x; e < tot; e += blockDim.x)
-      c2f_item<DIM, N>(p.state, recs[lst_c2f[e / ITEMS]], e % ITEMS, p.theta);
+      c2f_item<DIM, N, NV>(p.state, recs[lst_c2f[e / ITEMS]], e % ITEMS, p.theta);
   }
   // ---- uniform Dirichlet / Neumann / bc_data faces
 #pragma unroll 1
@@ -286,7 +287,7 @@ __global__ void __launch_bounds__(256, 4) ghost_exec_kernel(GhostParams p) {
     const DevRecord rec = recs[q];
     const int op = rec.meta & 3, face = (rec.meta >> 2) & 7, o1 = (rec.meta >> 5) & 1, o2 = (rec.meta >> 6) & 1;
     if (op == F4_OP_BC && (o1 | o2))   // (1,0) Dirichlet, (0,1) Neumann, (1,1) bc_data of face rec.src (mirror rule)
-      do_bc_values<DIM, N>(p.state, rec.dst, face, o2 != 0 && o1 == 0, p.bcv,
+      do_bc_values<DIM, N, NV>(p.state, rec.dst, face, o2 != 0 && o1 == 0, p.bcv,
                            p.dx0 * (1.0 / (double)(1u << p.level[rec.dst])),
                            (o1 & o2) ? p.bcdata + (size_t)rec.src * G::NVAR * ((DIM == 3) ? N * N : N) : nullptr);
   }
@@ -295,11 +296,11 @@ __global__ void __launch_bounds__(256, 4) ghost_exec_kernel(GhostParams p) {
 // ---------------------------------------------------------------------------
 // regrid transfer: one CTA per new block
 // ---------------------------------------------------------------------------
-template <int DIM, int N>
+template <int DIM, int N, int NV>
 __global__ void __launch_bounds__(256) transfer_kernel(const double* __restrict__ old_st, double* __restrict__ new_st,
                                                        const DevTransfer* __restrict__ plan, double theta) {
-  using G = Geo<DIM, N>;
-  constexpr int H = G::H, NV = G::NVAR, NZ = G::NZ;
+  using G = Geo<DIM, N, NV>;
+  constexpr int H = G::H, NZ = G::NZ;
   const DevTransfer t = plan[blockIdx.x];
   double* db = new_st + (size_t)t.dst * G::BS;
   if (t.kind == 0) {  // unaltered: copy the interior
@@ -345,10 +346,10 @@ __global__ void __launch_bounds__(256) transfer_kernel(const double* __restrict_
 // ---------------------------------------------------------------------------
 // layout kernels (not on the per-step path)
 // ---------------------------------------------------------------------------
-template <int DIM, int N, bool PACK>
+template <int DIM, int N, int NV, bool PACK>
 __global__ void __launch_bounds__(256) layout_kernel(double* __restrict__ store, double* __restrict__ user, int b0,
                                                      int with_ghosts) {
-  using G = Geo<DIM, N>;
+  using G = Geo<DIM, N, NV>;
   const int E = with_ghosts ? G::P : N, EZ = (DIM == 3) ? E : 1, lo = with_ghosts ? -NG : 0;
   const int b = blockIdx.x, v = blockIdx.y;
   const size_t ubase = ((size_t)b * G::NVAR + v) * (size_t)(E * E * EZ);
@@ -361,9 +362,9 @@ __global__ void __launch_bounds__(256) layout_kernel(double* __restrict__ store,
   }
 }
 
-template <int DIM, int N>
+template <int DIM, int N, int NV>
 __global__ void __launch_bounds__(256) init_benign_kernel(double* __restrict__ store, double gamma) {
-  using G = Geo<DIM, N>;
+  using G = Geo<DIM, N, NV>;
   const int b = blockIdx.x, v = blockIdx.y;
   double val = (v == 0) ? 1.0 : (v == G::NVAR - 1 ? 1.0 / (gamma - 1.0) : 0.0);  // rho=1, u=0, p=1
   double* sv = store + ((size_t)b * G::NVAR + v) * G::VS;
@@ -371,9 +372,9 @@ __global__ void __launch_bounds__(256) init_benign_kernel(double* __restrict__ s
 }
 
 // per-(block,var) interior sums, fixed order inside the CTA (for f4_conserved_totals)
-template <int DIM, int N>
+template <int DIM, int N, int NV>
 __global__ void __launch_bounds__(256) block_sums_kernel(const double* __restrict__ st, double* __restrict__ sums) {
-  using G = Geo<DIM, N>;
+  using G = Geo<DIM, N, NV>;
   __shared__ double sh[256];
   const int b = blockIdx.x, v = blockIdx.y;
   const double* sv = st + ((size_t)b * G::NVAR + v) * G::VS;
@@ -397,11 +398,11 @@ __global__ void __launch_bounds__(256) block_sums_kernel(const double* __restric
 // are read, so the state must be ghost-filled.  The flag is a discrete decision taken from floating point: every
 // operation is an explicitly rounded IEEE add / mul / div / sqrt in the order the paper writes the formula, no
 // contraction, so that the indicator does not depend on compiler choices.
-template <int DIM, int N>
+template <int DIM, int N, int NV>
 __global__ void __launch_bounds__(256) flags_kernel(const double* __restrict__ st, int criterion, int var, double gamma,
                                                     double p0, double p1, double p2, double p3,
                                                     int* __restrict__ flags, double* __restrict__ indicator) {
-  using G = Geo<DIM, N>;
+  using G = Geo<DIM, N, NV>;
   __shared__ double sh[8];
   const int b = blockIdx.x;
   const double* sb = st + (size_t)b * G::BS;
@@ -490,68 +491,73 @@ __global__ void __launch_bounds__(256) maxrate_kernel(const double* __restrict__
 }
 
 template <typename F>
-cudaError_t dispatch(int dim, int n, F&& f) {
-  if (dim == 2 && n == 8) return f(Geo<2, 8>{});
-  if (dim == 2 && n == 16) return f(Geo<2, 16>{});
-  if (dim == 2 && n == 32) return f(Geo<2, 32>{});
-  if (dim == 3 && n == 8) return f(Geo<3, 8>{});
-  if (dim == 3 && n == 16) return f(Geo<3, 16>{});
-  if (dim == 3 && n == 32) return f(Geo<3, 32>{});
+cudaError_t dispatch(int dim, int n, int nvar, F&& f) {
+#define F4_CASE(D, NN)                                                   \
+  if (dim == D && n == NN) {                                             \
+    if (nvar == D + 2) return f(Geo<D, NN, D + 2>{});                    \
+    if (nvar == 1) return f(Geo<D, NN, 1>{});                            \
+  }
+  F4_CASE(2, 8) F4_CASE(2, 16) F4_CASE(2, 32) F4_CASE(3, 8) F4_CASE(3, 16) F4_CASE(3, 32)
+#undef F4_CASE
   return cudaErrorInvalidValue;
 }
-template <int D, int N>
-constexpr int dim_of(Geo<D, N>) { return D; }
-template <int D, int N>
-constexpr int n_of(Geo<D, N>) { return N; }
+template <int D, int N, int V>
+constexpr int dim_of(Geo<D, N, V>) { return D; }
+template <int D, int N, int V>
+constexpr int n_of(Geo<D, N, V>) { return N; }
+template <int D, int N, int V>
+constexpr int nv_of(Geo<D, N, V>) { return V; }
 
 }  // namespace
 
-#define F4_DISPATCH(body)                                   \
-  return dispatch(dim, n, [&](auto g) -> cudaError_t {      \
-    constexpr int D = dim_of(decltype(g){});                \
-    constexpr int NN = n_of(decltype(g){});                 \
-    body;                                                   \
-    return cudaGetLastError();                              \
+#define F4_DISPATCH(body)                                        \
+  return dispatch(dim, n, nvar, [&](auto g) -> cudaError_t {     \
+    constexpr int D = dim_of(decltype(g){});                     \
+    constexpr int NN = n_of(decltype(g){});                      \
+    constexpr int NVV = nv_of(decltype(g){});                    \
+    body;                                                        \
+    return cudaGetLastError();                                   \
   })
 
-cudaError_t launch_ghost(int dim, int n, const GhostParams& p, cudaStream_t s) {
+cudaError_t launch_ghost(int dim, int n, int nvar, const GhostParams& p, cudaStream_t s) {
   if (p.nrec <= 0) return cudaSuccess;
-  F4_DISPATCH((ghost_exec_kernel<D, NN><<<(p.nrec + 2 * D - 1) / (2 * D), 256, 0, s>>>(p)));
+  F4_DISPATCH((ghost_exec_kernel<D, NN, NVV><<<(p.nrec + 2 * D - 1) / (2 * D), 256, 0, s>>>(p)));
 }
-cudaError_t launch_transfer(int dim, int n, const double* old_state, double* new_state, const DevTransfer* plan,
+cudaError_t launch_transfer(int dim, int n, int nvar, const double* old_state, double* new_state, const DevTransfer* plan,
                             int nplan, double theta, cudaStream_t s) {
   if (nplan <= 0) return cudaSuccess;
-  F4_DISPATCH((transfer_kernel<D, NN><<<nplan, 256, 0, s>>>(old_state, new_state, plan, theta)));
+  F4_DISPATCH((transfer_kernel<D, NN, NVV><<<nplan, 256, 0, s>>>(old_state, new_state, plan, theta)));
 }
-cudaError_t launch_pack(int dim, int n, double* store_state, const double* src, int b0, int nb, int with_ghosts,
+cudaError_t launch_pack(int dim, int n, int nvar, double* store_state, const double* src, int b0, int nb, int with_ghosts,
                         cudaStream_t s) {
   if (nb <= 0) return cudaSuccess;
-  F4_DISPATCH((layout_kernel<D, NN, true><<<dim3(nb, D + 2), 256, 0, s>>>(store_state, const_cast<double*>(src), b0,
+  F4_DISPATCH((layout_kernel<D, NN, NVV, true><<<dim3(nb, NVV), 256, 0, s>>>(store_state, const_cast<double*>(src), b0,
                                                                            with_ghosts)));
 }
-cudaError_t launch_unpack(int dim, int n, const double* store_state, double* dst, int b0, int nb, int with_ghosts,
+cudaError_t launch_unpack(int dim, int n, int nvar, const double* store_state, double* dst, int b0, int nb, int with_ghosts,
                           cudaStream_t s) {
   if (nb <= 0) return cudaSuccess;
-  F4_DISPATCH((layout_kernel<D, NN, false><<<dim3(nb, D + 2), 256, 0, s>>>(const_cast<double*>(store_state), dst, b0,
+  F4_DISPATCH((layout_kernel<D, NN, NVV, false><<<dim3(nb, NVV), 256, 0, s>>>(const_cast<double*>(store_state), dst, b0,
                                                                             with_ghosts)));
 }
-cudaError_t launch_init_benign(int dim, int n, double* store_state, int nb, double gamma, cudaStream_t s) {
+cudaError_t launch_init_benign(int dim, int n, int nvar, double* store_state, int nb, double gamma, cudaStream_t s) {
   if (nb <= 0) return cudaSuccess;
-  F4_DISPATCH((init_benign_kernel<D, NN><<<dim3(nb, D + 2), 256, 0, s>>>(store_state, gamma)));
+  F4_DISPATCH((init_benign_kernel<D, NN, NVV><<<dim3(nb, NVV), 256, 0, s>>>(store_state, gamma)));
 }
-cudaError_t launch_block_sums(int dim, int n, const double* state, int nb, double* sums, cudaStream_t s) {
+cudaError_t launch_block_sums(int dim, int n, int nvar, const double* state, int nb, double* sums, cudaStream_t s) {
   if (nb <= 0) return cudaSuccess;
-  F4_DISPATCH((block_sums_kernel<D, NN><<<dim3(nb, D + 2), 256, 0, s>>>(state, sums)));
+  F4_DISPATCH((block_sums_kernel<D, NN, NVV><<<dim3(nb, NVV), 256, 0, s>>>(state, sums)));
 }
-cudaError_t launch_flags(int dim, int n, const double* state, int nblocks, int criterion, int var, double gamma,
+cudaError_t launch_flags(int dim, int n, int nvar, const double* state, int nblocks, int criterion, int var, double gamma,
                          const double params[4], int* flags, double* indicator, cudaStream_t s) {
   if (nblocks <= 0) return cudaSuccess;
-  F4_DISPATCH((flags_kernel<D, NN><<<nblocks, 256, 0, s>>>(state, criterion, var, gamma, params[0], params[1],
+  F4_DISPATCH((flags_kernel<D, NN, NVV><<<nblocks, 256, 0, s>>>(state, criterion, var, gamma, params[0], params[1],
                                                            params[2], params[3], flags, indicator)));
 }
 cudaError_t launch_maxrate(int dim, int n, const double* state, const int* level, int nblocks, double gamma,
                            double inv_dx0, unsigned long long* maxrate, cudaStream_t s) {
   if (nblocks <= 0) return cudaSuccess;
+  const int nvar = dim + 2;   // Euler only: scalar advection has the constant wave speed v (f4_compute_dt)
   F4_DISPATCH((maxrate_kernel<D, NN><<<nblocks, 256, 0, s>>>(state, level, gamma, inv_dx0, maxrate)));
 }
 

@@ -36,43 +36,6 @@ namespace {
 
 __device__ __forceinline__ void sweep_sync(int id, int nthreads) { group_sync(id, nthreads); }
 
-// limited HALF slope 1/2*phi(a,b) for the reconstruction w +- 1/2 phi (reading A1)
-template <bool FAST>
-__device__ __forceinline__ double half_slope(double a, double b, int limiter) {
-  double ab = a * b;
-  if (FAST) {
-    // van Leer: 1/2 * 2ab/(a+b) where ab > 0.  The sign test is taken on the high word of ab (an integer compare
-    // instead of a DSETP on the fp64 pipe); it differs from ab > 0 only for 0 < ab < 2^-1042, where the slope is < 1e-150.
-    // the select is taken on the MUFU seed (one 32-bit select: the seed's low word is zero): seed 0 -> rcp 0 -> slope 0
-    const double x = a + b;
-    double y = rcp_seed(x);
-    y = __hiloint2double((__double2hiint(ab) > 0) ? __double2hiint(y) : 0, 0);
-    const double e = fma(-x, y, 1.0);
-    const double e2 = fma(e, e, e);
-    return ab * fma(y, e2, y);
-  }
-  double r;
-  if (limiter == F4_LIM_WENO3) {
-    // third-order WENO towards the b side (reading A1b): candidates w + a/2, w + b/2, ideal weights
-    // 1/3, 2/3, smoothness a^2, b^2, eps = 1e-6; no sign test (the weights do the limiting)
-    const double ea = 1e-6 + a * a, eb = 1e-6 + b * b;
-    const double a0 = (1.0 / 3.0) / (ea * ea), a1 = (2.0 / 3.0) / (eb * eb);
-    return 0.5 * ((a0 * a + a1 * b) / (a0 + a1));
-  }
-  if (limiter == F4_LIM_VANLEER) {
-    r = ab * rcp_fast(a + b);
-  } else if (limiter == F4_LIM_KOREN) {
-    // Koren (reading A1b): the kappa = 1/3 slope (a + 2b)/3 towards the b side, limited to [0,2a], [0,2b]
-    double m = fmin(fmin(2.0 * fabs(a), (fabs(a) + 2.0 * fabs(b)) / 3.0), 2.0 * fabs(b));
-    r = 0.5 * ((a > 0.0) ? m : -m);
-  } else {
-    double th = (limiter == F4_LIM_MC) ? 2.0 : 1.0;   // eq. (1)
-    double m = fmin(fmin(fabs(th * a), fabs(th * b)), fabs(a + b) * 0.5);
-    r = 0.5 * ((a > 0.0) ? m : -m);
-  }
-  return (ab > 0.0) ? r : 0.0;
-}
-
 // HLL / Rusanov flux in the face-normal frame (readings A2-A3).
 // q = (rho, un, ut1, ut2, p); F = (mass, normal momentum, tangential momenta, energy).
 template <int DIM, bool FAST>

@@ -29,12 +29,15 @@ OP_SRL, OP_BC, OP_F2C, OP_C2F = 0, 1, 2, 3
 PROF_NAMES = ("ghost_r1", "ghost_r2", "stage", "dt_reduce", "regrid", "layout")
 
 # every symbol include/f4.h declares
-SYMBOLS = ("f4_mesh_create", "f4_mesh_destroy", "f4_set_options", "f4_set_flux_fix", "f4_set_bc_values", "f4_set_bc_callback", "f4_update_bc_data",
+SYMBOLS = ("f4_mesh_create", "f4_mesh_destroy", "f4_set_options", "f4_set_flux_fix", "f4_set_physics", "f4_num_vars", "f4_set_bc_values", "f4_set_bc_callback", "f4_update_bc_data",
            "f4_num_bc_faces", "f4_set_gravity", "f4_set_rk_scheme", "f4_storage_bytes", "f4_bind_storage",
            "f4_num_blocks", "f4_get_blocks", "f4_set_state", "f4_get_state", "f4_build_ghost_pattern",
            "f4_pattern_size", "f4_get_pattern", "f4_fill_ghosts", "f4_compute_dt", "f4_advance", "f4_refine_flags", "f4_adapt",
            "f4_conserved_totals", "f4_profile_enable", "f4_profile_get", "f4_launch_count", "f4_last_adapt_ms", "f4_last_error",
            "f4_version")
+
+
+PHYS_EULER, PHYS_ADVECTION = 0, 1
 
 
 class F4Error(RuntimeError):
@@ -61,6 +64,8 @@ def lib():
     L.f4_mesh_destroy.argtypes = [vp]
     L.f4_set_options.argtypes = [vp, C.c_int, C.c_int, C.c_double]
     L.f4_set_flux_fix.argtypes = [vp, C.c_int]
+    L.f4_set_physics.argtypes = [vp, C.c_int, dp]
+    L.f4_num_vars.argtypes = [vp]
     L.f4_set_rk_scheme.argtypes = [vp, C.c_int]
     L.f4_set_gravity.argtypes = [vp, dp]
     L.f4_set_bc_values.argtypes = [vp, dp]
@@ -128,6 +133,14 @@ class Mesh:
 
     @classmethod
     def from_config(cls, cfg, n_states=2, max_blocks=None):
+        if cfg.get("physics") == "advection":
+            m = cls._from_config_base(cfg, n_states, max_blocks)
+            m.set_advection(cfg["velocity"])
+            return m
+        return cls._from_config_base(cfg, n_states, max_blocks)
+
+    @classmethod
+    def _from_config_base(cls, cfg, n_states=2, max_blocks=None):
         return cls(cfg["dim"], cfg["block_n"], cfg["n_ghost"], cfg["brick"], cfg["base_level"], cfg["max_level"],
                    cfg["bc"], cfg["gamma"], n_states, max_blocks)
 
@@ -211,6 +224,14 @@ class Mesh:
     @property
     def num_bc_faces(self):
         return self.L.f4_num_bc_faces(self.h)
+
+    def set_advection(self, velocity):
+        """Scalar advection eq. (13) with a uniform velocity field: one variable per cell.
+        Before bind_storage / bind_torch."""
+        v = np.zeros(3)
+        v[:self.dim] = np.asarray(velocity, dtype=np.float64)[:self.dim]
+        self._chk(self.L.f4_set_physics(self.h, PHYS_ADVECTION, _dp(v)))
+        self.nvar = 1
 
     def set_gravity(self, g):
         gg = np.zeros(3, dtype=np.float64)
