@@ -5,7 +5,7 @@
 //
 // One variable, 8 bytes per cell: the kernel is bound by HBM bandwidth.  Same data path as the Euler stage kernel
 // (f4_stage.cu): a thread group of N x TY threads owns a (block, y-tile) and marches through the z planes; padded
-// planes arrive by bulk async copies (TMA engine, completion on an mbarrier) in a 4-slot shared-memory ring two
+// planes arrive by bulk async copies (TMA engine, completion on an mbarrier) in an 8-slot shared-memory ring six
 // planes ahead of use; z ghost planes / y ghost rows of same-level neighbours are fetched straight from their interior
 // cells and the x face layers of the new state are pushed into the neighbours' ghost cells (a1 of the pattern,
 // PAPER.md:195, 235-238).  Primitive and conservative variables are identical: nothing is converted,
@@ -27,7 +27,7 @@ struct CfgA {
   static constexpr size_t VS = (size_t)P * P * PZ;   // one variable: VS doubles per block
   static constexpr bool WHOLE = (TY == N);
   static constexpr int ROWS = TY + 4, PLANE = ROWS * P;
-  static constexpr int NSLOT = (DIM == 3) ? 4 : 1;
+  static constexpr int NSLOT = (DIM == 3) ? 8 : 1;     // ring depth (the march is unrolled by 8): planes c-1, c and six in flight
   static constexpr int TG = N * TY, NT = TG * G, YT = N / TY;
   // half slopes of the cells (-1 .. N) x rows (x direction) and columns x rows (-1 .. TY) (y direction), two buffers
   static constexpr int HX = TY * (N + 2), HY = (TY + 2) * N, EXD = HX + HY;
@@ -39,7 +39,7 @@ struct CfgA {
 
 // FAST: van Leer fixed at compile time; BF: store the face fluxes at refinement boundaries (flux fixing)
 template <int DIM, int N, int TY, int G, bool FAST, bool BF>
-__global__ void __launch_bounds__(CfgA<DIM, N, TY, G>::NT) advect_kernel(const __grid_constant__ StageParams p) {
+__global__ void __launch_bounds__(CfgA<DIM, N, TY, G>::NT, 1024 / CfgA<DIM, N, TY, G>::NT) advect_kernel(const __grid_constant__ StageParams p) {
   using C = CfgA<DIM, N, TY, G>;
   constexpr int P = C::P, PP = C::PP, PLANE = C::PLANE, TG = C::TG;
   constexpr bool WHOLE = C::WHOLE;
@@ -124,12 +124,28 @@ __global__ void __launch_bounds__(CfgA<DIM, N, TY, G>::NT) advect_kernel(const _
   const int gcol = N + 2 * (rr & 1);
   const int own_xm = (i == 0) ? (rr | 1) * P + gcol + 1 : own - 1;
   const int own_xp = (i == N - 1) ? (rr & ~1) * P + gcol : own + 1;
-  // edge threads also take the half slope of the halo cell next to them (cell -1 / N of the row, row -1 / TY of the
-  // column): xfar / yfar = the cell two steps outside
-  const bool xlo = (i == 0), xedge = xlo || (i == N - 1);
-  const bool ylo = (j == 0), yedge = ylo || (j == TY - 1);
-  const int own_xfar = xlo ? (rr | 1) * P + gcol : (rr & ~1) * P + gcol + 1;
-  const int own_yfar = rown(ylo ? j0 - 2 : j0 + TY + 1) * P + i;
+  // halo role of the first 2*TY + 2*N threads: the half slope of one halo cell (cell -1 / N of a row, row -1 / TY of a
+  // column): offsets of that cell (h0), its low (hm) and high (hp) neighbour, and where its half slope goes (hdst)
+  constexpr int NHALO = 2 * TY + 2 * N;
+  static_assert(NHALO <= TG, "halo roles need one pass");
+  const bool is_h = t < NHALO;
+  int h0 = 0, hm = 0, hp = 0, hdst = 0;
+  if (is_h) {
+    if (t < 2 * TY) {
+      const int r = t >> 1, hi = t & 1, sr = rown(j0 + r), gc = N + 2 * (sr & 1);
+      const int olo = (sr | 1) * P + gc, ohi = (sr & ~1) * P + gc;   // ghost pairs (-2,-1) and (N,N+1) of the row
+      h0 = hi ? ohi : olo + 1;
+      hm = hi ? sr * P + N - 1 : olo;
+      hp = hi ? ohi + 1 : sr * P;
+      hdst = r * (N + 2) + (hi ? N + 1 : 0);
+    } else {
+      const int q = t - 2 * TY, col = q >> 1, hi = q & 1, y = hi ? j0 + TY : j0 - 1;
+      h0 = rown(y) * P + col;
+      hm = rown(y - 1) * P + col;
+      hp = rown(y + 1) * P + col;
+      hdst = C::HX + (hi ? TY + 1 : 0) * N + col;
+    }
+  }
   const int hxo = j * (N + 2) + i + 1, hyo = C::HX + (j + 1) * N + i;   // own entries of the half-slope arrays
 
   int bfs[6] = {-1, -1, -1, -1, -1, -1};
@@ -148,13 +164,9 @@ __global__ void __launch_bounds__(CfgA<DIM, N, TY, G>::NT) advect_kernel(const _
     const double hsy = half_slope<FAST>(wa - wym, wyp - wa, limiter);
     ex[hxo] = hsx;
     ex[hyo] = hsy;
-    if (xedge) {
-      const double wf = W[own_xfar];
-      ex[xlo ? hxo - 1 : hxo + 1] = xlo ? half_slope<FAST>(wxm - wf, wa - wxm, limiter) : half_slope<FAST>(wxp - wa, wf - wxp, limiter);
-    }
-    if (yedge) {
-      const double wf = W[own_yfar];
-      ex[ylo ? hyo - N : hyo + N] = ylo ? half_slope<FAST>(wym - wf, wa - wym, limiter) : half_slope<FAST>(wyp - wa, wf - wyp, limiter);
+    if (is_h) {
+      const double w0 = W[h0];
+      ex[hdst] = half_slope<FAST>(w0 - W[hm], W[hp] - w0, limiter);
     }
     gsync();
     after_barrier();
@@ -200,15 +212,22 @@ __global__ void __launch_bounds__(CfgA<DIM, N, TY, G>::NT) advect_kernel(const _
     const double acc = sweep_xy(ring, ring[own], ex0, 0, []() {});
     finish(0, acc, a, b);
   } else {
-    if (t == ISSUER) { issue_plane(-2, 0); issue_plane(-1, 1); issue_plane(0, 2); issue_plane(1, 3); }
+    constexpr int NS = C::NSLOT;
+    if (t == ISSUER) {
+      for (int q = 0; q < NS && q - 2 <= N + 1; ++q) issue_plane(q - 2, q);
+    }
     double dA = 0.0, Lz = 0.0, accp = 0.0, wa = 0.0;
-    int sc = 0;            // ring slot of plane c: (c + 2) & 3
+    // previous states of plane c are requested in iteration c and consumed two iterations later (finish of cell c)
+    double aq0 = 0.0, aq1 = 0.0, bq0 = 0.0, bq1 = 0.0;
     uint32_t ph = 0;       // phase parity of each slot's mbarrier
-    auto march = [&](int c, auto zflux_t, auto fin_t, auto sweep_t) {
+    // sc_t: ring slot of plane c, (c + 2) & (NS - 1), as a compile-time constant (shared-memory addresses become
+    // register + immediate)
+    auto march = [&](int c, auto sc_t, auto zflux_t, auto fin_t, auto sweep_t) {
       constexpr bool ZFLUX = decltype(zflux_t)::value, FIN = decltype(fin_t)::value, SWEEP = decltype(sweep_t)::value;
-      const int sk = (sc + 3) & 3;                          // slot of plane c-1
-      double a = 0.0, b = 0.0;
-      if (FIN) { a = pa[(c - 2) * PP]; b = pb ? pb[(c - 2) * PP] : 0.0; }
+      constexpr int sc = decltype(sc_t)::value;
+      constexpr int sk = (sc + NS - 1) & (NS - 1);          // slot of plane c-1
+      double a_new = 0.0, b_new = 0.0;
+      if (c >= 0 && c < N) { a_new = pa[c * PP]; b_new = pb ? pb[c * PP] : 0.0; }
       mbar_wait(bars_u32 + 8u * sc, (ph >> sc) & 1u);
       ph ^= 1u << sc;
       const double wB = ring[sc * PLANE + own];
@@ -222,25 +241,37 @@ __global__ void __launch_bounds__(CfgA<DIM, N, TY, G>::NT) advect_kernel(const _
         if (c == 1 && bfs[4] >= 0) bf_store(bfs[4], Fz, i, j0 + j);
         if (c == N + 1 && bfs[5] >= 0) bf_store(bfs[5], Fz, i, j0 + j);
       }
-      if (FIN) finish(c - 2, accp - Fz, a, b);
-      // after this iteration's barrier every thread is past its reads of plane c-2: its slot takes plane c+2
+      if (FIN) finish(c - 2, accp - Fz, aq1, bq1);
+      aq1 = aq0; aq0 = a_new;
+      bq1 = bq0; bq0 = b_new;
+      // after this iteration's barrier every thread is past its reads of plane c-2: its slot takes the next plane of the ring
       auto refill = [&]() {
-        if (t == ISSUER && c >= 0 && c + 2 <= N + 1) issue_plane(c + 2, (sc + 2) & 3);   // (c + 4) & 3: plane c-2's slot
+        if (t == ISSUER && c >= 0 && c - 2 + NS <= N + 1) issue_plane(c - 2 + NS, (sc + NS - 2) & (NS - 1));   // plane c-2's slot
       };
       if (SWEEP) accp = sweep_xy(ring + sk * PLANE, wa, ex0 + (c & 1) * C::EXD, c - 1, refill) + Fz;
       else { gsync(); refill(); }
       wa = wB;
-      sc = (sc + 1) & 3;
     };
     using T = std::true_type;
     using F_ = std::false_type;
-    march(-2, F_{}, F_{}, F_{});
-    march(-1, F_{}, F_{}, F_{});
-    march(0, F_{}, F_{}, F_{});
-    march(1, T{}, F_{}, T{});
+    auto slot = [](auto c_t) { return std::integral_constant<int, (decltype(c_t)::value + 2) & (NS - 1)>{}; };
+    march(-2, slot(std::integral_constant<int, -2>{}), F_{}, F_{}, F_{});
+    march(-1, slot(std::integral_constant<int, -1>{}), F_{}, F_{}, F_{});
+    march(0, slot(std::integral_constant<int, 0>{}), F_{}, F_{}, F_{});
+    march(1, slot(std::integral_constant<int, 1>{}), T{}, F_{}, T{});
+    // steady state c = 2 .. N, unrolled by the ring depth: plane c0 + u sits in slot (4 + u) & (NS - 1)
 #pragma unroll 1
-    for (int c = 2; c <= N; ++c) march(c, T{}, T{}, T{});
-    march(N + 1, T{}, T{}, F_{});
+    for (int c0 = 2; c0 <= N; c0 += NS) {
+      auto body = [&](auto u_t) {
+        constexpr int u = decltype(u_t)::value;
+        if (c0 + u <= N) march(c0 + u, std::integral_constant<int, (4 + u) & (NS - 1)>{}, T{}, T{}, T{});
+      };
+      body(std::integral_constant<int, 0>{}); body(std::integral_constant<int, 1>{});
+      body(std::integral_constant<int, 2>{}); body(std::integral_constant<int, 3>{});
+      body(std::integral_constant<int, 4>{}); body(std::integral_constant<int, 5>{});
+      body(std::integral_constant<int, 6>{}); body(std::integral_constant<int, 7>{});
+    }
+    march(N + 1, slot(std::integral_constant<int, N + 1>{}), T{}, T{}, F_{});
   }
 }
 
