@@ -247,6 +247,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sync-regrid", action="store_true",
+                    help="adaptive configs: blocking f4_adapt before the step instead of f4_adapt_begin / f4_adapt_end "
+                         "around it (host mesh work overlapped with the step, new mesh one step later)")
     ap.add_argument("--flux-fix", action="store_true",
                     help="adaptive configs: conservative flux fixing at refinement boundaries (PAPER.md:253-261)")
     ap.add_argument("--rk", default="heun", choices=["heun", "euler", "ssp33", "ssp43", "rk4"],
@@ -304,16 +307,29 @@ def main():
     counters = {"step": 0, "updates": 0.0, "adapt_s": 0.0, "regrids": 0, "changed": 0}
 
     def step():
-        # config 5: regrid on the host every cfg["regrid_every"] steps (rule A15), inside the timed region
+        # config 5: regrid on the host every cfg["regrid_every"] steps (rule A15), inside the timed region.  Default:
+        # the flags of step s start the host part of the regrid on a worker thread (f4_adapt_begin), the device
+        # advances step s on the current mesh meanwhile, and the new mesh takes over after that step (f4_adapt_end);
+        # --sync-regrid: the blocking f4_adapt before the step
+        pend = False
         if adaptive and counters["step"] and counters["step"] % cfg["regrid_every"] == 0:
             t0 = time.perf_counter()
-            counters["changed"] += int(mesh.adapt(adaptive_flags(cfg, mesh)))
+            flags = adaptive_flags(cfg, mesh)
+            if args.sync_regrid:
+                counters["changed"] += int(mesh.adapt(flags))
+            else:
+                mesh.adapt_begin(flags)
+                pend = True
             counters["regrids"] += 1
             counters["adapt_s"] += time.perf_counter() - t0
         dt = mesh.compute_dt(0, cfg["cfl"])
         mesh.advance(dt)
         counters["step"] += 1
-        counters["updates"] += float(nstages) * mesh.num_blocks * n ** d
+        counters["updates"] += float(nstages) * mesh.num_blocks * n ** d     # the blocks this step advanced
+        if pend:
+            t0 = time.perf_counter()
+            counters["changed"] += int(mesh.adapt_end())
+            counters["adapt_s"] += time.perf_counter() - t0
 
     for _ in range(max(args.warmup, 0)):
         step()
@@ -458,6 +474,8 @@ def main():
         "step_algorithmic_GBps": (nstages * stage_bytes) / (ms / args.steps * 1e-3) / 1e9,
         "adaptive": ({"regrids": adapt_info["regrids"], "mesh_changed": adapt_info["changed"],
                       "adapt_ms_total": 1e3 * adapt_info["adapt_s"], "blocks_at_end": nb,
+                      "regrid_mode": "blocking f4_adapt before the step" if args.sync_regrid else
+                                     "f4_adapt_begin before / f4_adapt_end after the step (host part overlapped)",
                       "value_excluding_adapt": world * updates / max(ms * 1e-3 - adapt_info["adapt_s"], 1e-9) / 1e9}
                      if adaptive else None),
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,

@@ -62,7 +62,12 @@ enum {
 enum {
   F4_BC_PERIODIC = 0, /* via connectivity */
   F4_BC_OUTFLOW = 1,  /* uniform Neumann, zero normal derivative: ghost = nearest interior layer (reading A10) */
-  F4_BC_KEEP = 2,     /* ghosts on that face are left as the caller set them (linear-field test) */
+  F4_BC_KEEP = 2,     /* no record: ghosts on that face stay as the caller wrote them (the "boundary values set
+                         analytically" of the linear-field test).  Contract: the library never writes
+                         these ghost cells, so the caller must set them (f4_set_state with_ghosts = 1) in EVERY temporal
+                         state that f4_advance differentiates (intermediate Runge-Kutta states start from a benign
+                         constant, rho = 1, u = 0, p = 1), and again after f4_adapt (the regrid transfer carries
+                         interior cells only). */
   F4_BC_DIRICHLET = 3, /* uniform value u_b per face direction and variable (f4_set_bc_values): ghost layer g mirrors
                           interior layer g through the face, u_ghost = 2 u_b - u_interior (reading A10) */
   F4_BC_NEUMANN = 4,   /* uniform outward normal derivative u_b': ghost layer g = first interior layer + g dx u_b'
@@ -184,8 +189,8 @@ int f4_compute_dt(f4_mesh *m, int state, double cfl, double *dt_out);
  * with a uniform value u = u_b ... stored per face direction and per variable ... and the same ... for a Neumann
  * boundary condition with a uniform normal derivative"): values[6][Nvar], face directions -x,+x,-y,+y,-z,+z, stored
  * (conservative) variables; entries of other faces are ignored.  Default: zeros.  Copied to the device when storage
- * is bound (host call otherwise); takes effect at the next ghost fill.  Spatially varying bc_data (eq. 4) is not
- * provided: F4_BC_KEEP lets the caller write such ghosts. */
+ * is bound (host call otherwise); takes effect at the next ghost fill.  Spatially varying values (eq. 4) are the
+ * F4_BC_DATA kind below. */
 int f4_set_bc_values(f4_mesh *m, const double *values);
 
 /* Spatially varying boundary values, eq. (4): bc_data(i, j, ivar, ibf), ibf = 0 .. n_faces-1 over the
@@ -247,6 +252,16 @@ int f4_refine_flags(f4_mesh *m, int state, int criterion, int var, const double 
  * the topology changes.  Other states become undefined.  Synchronises.
  * Errors: F4_ENOBLOCKS (nothing modified), F4_ECUDA. */
 int f4_adapt(f4_mesh *m, const int *refine_flags, int *changed_out);
+
+/* The same regrid split in two, so that the host part (refine / coarsen / balance and the pattern records of the new
+ * mesh) overlaps device work: f4_adapt_begin copies the flags and starts that part on a
+ * worker thread, on a copy of the mesh; the mesh in use stays valid, so f4_compute_dt / f4_advance (and nothing that
+ * changes the mesh or its state layout) may be called in between.  f4_adapt_end waits for the worker and, if the mesh
+ * changes, does what f4_adapt does on the device (ghost fill, transfer of state 0 AS IT IS NOW, record upload).  The
+ * new mesh is the one f4_adapt would have built from the same flags; only the moment of the switch differs.
+ * Errors: F4_EINVAL (begin while pending, end without begin, f4_adapt while pending), else as f4_adapt. */
+int f4_adapt_begin(f4_mesh *m, const int *refine_flags);
+int f4_adapt_end(f4_mesh *m, int *changed_out);
 
 /* sum over interior cells of u * dx^dim, per variable [Nvar] (for conservation tests). */
 int f4_conserved_totals(f4_mesh *m, int state, double *totals);

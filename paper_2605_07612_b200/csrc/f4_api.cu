@@ -6,6 +6,7 @@
 #include <new>
 #include <chrono>
 #include <string>
+#include <thread>
 #include <vector>
 
 #include "../../include/f4.h"
@@ -94,6 +95,15 @@ struct f4_mesh {
   double prof_ms[F4_PROF_N] = {0, 0, 0, 0, 0, 0};
   long long prof_n[F4_PROF_N] = {0, 0, 0, 0, 0, 0};
   long long launches = 0;
+  // asynchronous regrid (f4_adapt_begin / f4_adapt_end): the host part runs on a worker thread on a copy of the mesh
+  std::thread worker;
+  bool pending = false;
+  HostMesh hm_next;
+  std::vector<int> flags_next;
+  std::vector<Transfer> plan_next;
+  bool changed_next = false;
+  int rc_next = 0;
+  std::string err_next;
   double adapt_ms[3] = {0.0, 0.0, 0.0};   // last f4_adapt: host mesh + pattern, transfer kernel + wait, record upload
   std::string err;
 
@@ -383,6 +393,7 @@ int f4_mesh_create(int dim, int block_n, int n_ghost, const int brick[3], int ba
 int f4_mesh_destroy(f4_mesh* m) {
   DeviceScope dev_scope(m);
   if (!m) return F4_EINVAL;
+  if (m->pending) m->worker.join();
   if (m->bound) cudaStreamSynchronize(m->stream);
   for (auto& e : m->evs) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
   if (m->d_meta) cudaFree(m->d_meta);
@@ -811,25 +822,14 @@ int f4_refine_flags(f4_mesh* m, int state, int criterion, int var, const double 
   return F4_OK;
 }
 
-int f4_adapt(f4_mesh* m, const int* refine_flags, int* changed_out) {
-  DeviceScope dev_scope(m);
-  if (!m || !refine_flags || !changed_out) return F4_EINVAL;
-  *changed_out = 0;
+namespace {
+
+// device side of a regrid whose host part (m->hm already is the new mesh) produced `plan`: ghost fill of state 0
+// with the records of the OLD mesh (still the ones on the device; prolongation reads the parents' face ghosts),
+// transfer into the other slab, record upload
+int commit_adapt(f4_mesh* m, const std::vector<Transfer>& plan) {
   int rc;
-  std::vector<Transfer> plan;
-  bool changed = false;
-  std::string err;
-  const auto t0 = std::chrono::steady_clock::now();
-  rc = m->hm.adapt(refine_flags, plan, changed, err);
   const auto t1 = std::chrono::steady_clock::now();
-  m->adapt_ms[0] = std::chrono::duration<double, std::milli>(t1 - t0).count();
-  m->adapt_ms[1] = m->adapt_ms[2] = 0.0;
-  if (rc) return fail(m, rc, err);
-  if (!changed) return F4_OK;
-  *changed_out = 1;
-  if (!m->bound) return refresh_bc_data(m);
-  // prolongation reads the parents' face ghosts: fill them now (only when the mesh does change), with the records
-  // of the OLD mesh, which are the ones still on the device
   if ((rc = fill_ghosts_impl(m, 0, m->srl_valid[0], true))) return rc;
   std::vector<DevTransfer> dp(plan.size());
   for (size_t q = 0; q < plan.size(); ++q) {
@@ -855,6 +855,61 @@ int f4_adapt(f4_mesh* m, const int* refine_flags, int* changed_out) {
   rc = upload_meta(m);
   m->adapt_ms[2] = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t2).count();
   return rc;
+}
+
+}  // namespace
+
+int f4_adapt(f4_mesh* m, const int* refine_flags, int* changed_out) {
+  DeviceScope dev_scope(m);
+  if (!m || !refine_flags || !changed_out) return F4_EINVAL;
+  *changed_out = 0;
+  if (m->pending) return fail(m, F4_EINVAL, "f4_adapt: an asynchronous regrid is pending (f4_adapt_end)");
+  std::vector<Transfer> plan;
+  bool changed = false;
+  std::string err;
+  const auto t0 = std::chrono::steady_clock::now();
+  int rc = m->hm.adapt(refine_flags, plan, changed, err);
+  m->adapt_ms[0] = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+  m->adapt_ms[1] = m->adapt_ms[2] = 0.0;
+  if (rc) return fail(m, rc, err);
+  if (!changed) return F4_OK;
+  *changed_out = 1;
+  if (!m->bound) return refresh_bc_data(m);
+  return commit_adapt(m, plan);
+}
+
+int f4_adapt_begin(f4_mesh* m, const int* refine_flags) {
+  if (!m || !refine_flags) return F4_EINVAL;
+  if (m->pending) return fail(m, F4_EINVAL, "f4_adapt_begin: a regrid is already pending");
+  m->flags_next.assign(refine_flags, refine_flags + m->hm.leaves.size());
+  m->hm_next = m->hm;   // the worker edits a copy: the mesh in use stays valid for compute_dt / advance
+  m->plan_next.clear();
+  m->changed_next = false;
+  m->rc_next = F4_OK;
+  m->err_next.clear();
+  m->pending = true;
+  m->worker = std::thread([m]() {
+    const auto t0 = std::chrono::steady_clock::now();
+    m->rc_next = m->hm_next.adapt(m->flags_next.data(), m->plan_next, m->changed_next, m->err_next);
+    m->adapt_ms[0] = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+  });
+  return F4_OK;
+}
+
+int f4_adapt_end(f4_mesh* m, int* changed_out) {
+  DeviceScope dev_scope(m);
+  if (!m || !changed_out) return F4_EINVAL;
+  *changed_out = 0;
+  if (!m->pending) return fail(m, F4_EINVAL, "f4_adapt_end: no regrid pending");
+  m->worker.join();
+  m->pending = false;
+  m->adapt_ms[1] = m->adapt_ms[2] = 0.0;
+  if (m->rc_next) return fail(m, m->rc_next, m->err_next);
+  if (!m->changed_next) return F4_OK;
+  *changed_out = 1;
+  m->hm = std::move(m->hm_next);
+  if (!m->bound) return refresh_bc_data(m);
+  return commit_adapt(m, m->plan_next);
 }
 
 int f4_last_adapt_ms(const f4_mesh* m, double ms[3]) {

@@ -32,7 +32,7 @@ PROF_NAMES = ("ghost_r1", "ghost_r2", "stage", "dt_reduce", "regrid", "layout")
 SYMBOLS = ("f4_mesh_create", "f4_mesh_destroy", "f4_set_options", "f4_set_flux_fix", "f4_set_physics", "f4_num_vars", "f4_set_bc_values", "f4_set_bc_callback", "f4_update_bc_data",
            "f4_num_bc_faces", "f4_set_gravity", "f4_set_rk_scheme", "f4_storage_bytes", "f4_bind_storage",
            "f4_num_blocks", "f4_get_blocks", "f4_set_state", "f4_get_state", "f4_build_ghost_pattern",
-           "f4_pattern_size", "f4_get_pattern", "f4_fill_ghosts", "f4_compute_dt", "f4_advance", "f4_refine_flags", "f4_adapt",
+           "f4_pattern_size", "f4_get_pattern", "f4_fill_ghosts", "f4_compute_dt", "f4_advance", "f4_refine_flags", "f4_adapt", "f4_adapt_begin", "f4_adapt_end",
            "f4_conserved_totals", "f4_profile_enable", "f4_profile_get", "f4_launch_count", "f4_last_adapt_ms", "f4_last_error",
            "f4_version")
 
@@ -87,6 +87,8 @@ def lib():
     L.f4_compute_dt.argtypes = [vp, C.c_int, C.c_double, dp]
     L.f4_advance.argtypes = [vp, C.c_double]
     L.f4_adapt.argtypes = [vp, ip, ip]
+    L.f4_adapt_begin.argtypes = [vp, ip]
+    L.f4_adapt_end.argtypes = [vp, ip]
     L.f4_conserved_totals.argtypes = [vp, C.c_int, dp]
     L.f4_profile_enable.argtypes = [vp, C.c_int]
     L.f4_profile_get.argtypes = [vp, dp, C.POINTER(C.c_longlong), C.c_int]
@@ -269,6 +271,17 @@ class Mesh:
         assert f.shape[0] == self.num_blocks
         ch = C.c_int(0)
         self._chk(self.L.f4_adapt(self.h, _ip(f), C.byref(ch)))
+        return bool(ch.value)
+
+    def adapt_begin(self, flags):
+        """Start the host part of a regrid on a worker thread (compute_dt / advance may follow); adapt_end() commits."""
+        f = np.ascontiguousarray(flags, dtype=np.int32)
+        assert f.shape[0] == self.num_blocks
+        self._chk(self.L.f4_adapt_begin(self.h, _ip(f)))
+
+    def adapt_end(self):
+        ch = C.c_int(0)
+        self._chk(self.L.f4_adapt_end(self.h, C.byref(ch)))
         return bool(ch.value)
 
     # -- state -------------------------------------------------------------

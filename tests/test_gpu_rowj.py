@@ -179,3 +179,43 @@ def test_invalid_cell_is_reported_by_compute_dt(poison):
         with pytest.raises(f4.F4Error):
             lm.compute_dt(0, cfg["cfl"])
     lm.close()
+
+
+def test_asynchronous_regrid_matches_the_oracle_with_the_same_lag():
+    """f4_adapt_begin / f4_adapt_end: the host part of the regrid runs on a worker thread while the device advances a
+    step on the current mesh; the new mesh (the one f4_adapt builds from the same flags) takes over afterwards.  The
+    oracle mirrors it -- flags at step s, advance, then adapt -- and the two runs agree to 1e-11."""
+    cfg = dict(W.config(5), base_level=1, max_level=3)
+    lm = f4.Mesh.from_config(cfg, max_blocks=3000)
+    lm.bind_torch()
+    om = O.OracleMesh.from_config(cfg)
+    perm = _set_both(lm, om, cfg)
+    om.fill_ghosts(0)
+    fo, _ = om.refine_flags(0, om.CRIT_PJUMP, PJUMP)
+    assert om.adapt(fo) == lm.adapt(fo[perm])
+    perm = _set_both(lm, om, cfg)
+    changed = 0
+    for s in range(9):
+        pend = None
+        if s % 3 == 0:
+            om.fill_ghosts(0)
+            pend, _ = om.refine_flags(0, om.CRIT_PJUMP, PJUMP)
+            lm.adapt_begin(pend[perm])
+            with pytest.raises(f4.F4Error):
+                lm.adapt(pend[perm])                   # no second regrid while one is pending
+        dt = om.compute_dt(0, cfg["cfl"])
+        assert abs(lm.compute_dt(0, cfg["cfl"]) - dt) <= 1e-12 * dt
+        om.advance(dt)
+        lm.advance(dt)
+        if pend is not None:
+            ch_g, ch_o = lm.adapt_end(), om.adapt(pend)
+            assert ch_g == ch_o
+            changed += ch_o
+            perm = _perm(lm, om)
+            assert np.all(H.rel_linf(lm.get_state(0), om.get_state(0)[perm]) <= TOL_STATE)
+    assert changed >= 1 and lm.get_blocks()[0].max() == 3
+    err = H.rel_linf(lm.get_state(0), om.get_state(0)[perm])
+    assert np.all(err <= TOL_STATE), err
+    with pytest.raises(f4.F4Error):
+        lm.adapt_end()                                 # nothing pending
+    lm.close()
