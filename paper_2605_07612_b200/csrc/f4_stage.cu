@@ -13,8 +13,8 @@
 //  * a thread group of N x TY threads owns a (block, y-tile) and marches
 //    through the z planes; every face flux is evaluated once;
 //  * padded planes of the conservative state are fetched by bulk async copies
-//    (cp.async.bulk, the TMA engine, completion on an mbarrier) into a 3-slot
-//    shared-memory ring one plane ahead of use, and converted to primitives in
+//    (cp.async.bulk, the TMA engine, completion on an mbarrier) into a 4-slot (3 where two CTAs per SM would not fit otherwise)
+//    shared-memory ring two planes ahead of use, and converted to primitives in
 //    place (to_primitive once per cell); when the tile is the
 //    whole block the smem plane keeps the store's wrapped row order, so one
 //    bulk copy per variable moves the interior rows of a plane and two more
@@ -162,7 +162,14 @@ struct Cfg {  // FAST (van Leer + HLL fixed at compile time) does not change the
   static constexpr int ROWS = TY + 4;
   static constexpr int PLANE = ROWS * P;      // doubles per variable in one ring slot
   static constexpr int SLOT = NVAR * PLANE;
-  static constexpr int NSLOT = (DIM == 3) ? 3 : 1;
+  // ring depth: planes c-1 (swept), c (converted) and two in flight; all four are requested when the block starts, so
+  // the DRAM latency of the first planes is paid once (with three slots every short prologue iteration waited for it)
+  static constexpr size_t smem_for(int nslot) {
+    return (size_t)G * (nslot * (NVAR * (TY + 4) * P) + 2 * EXBUF * (NVAR * (N + 1) * (TY + 1)) + EXBUF * NVAR * (TY + N)) * 8 +
+           (size_t)G * (nslot + 2) * 8;
+  }
+  static constexpr size_t TWO_CTAS = 113 * 1024;   // two CTAs per SM: 2 x (SMEM + 1 KB reserved) <= 228 KB
+  static constexpr int NSLOT = (DIM == 3) ? (smem_for(4) <= TWO_CTAS ? 4 : 3) : 1;
   static constexpr int EXV = (N + 1) * (TY + 1);  // exchange entries per variable
   static constexpr int EX = NVAR * EXV;
   static constexpr int NH = TY + N;           // halo cells per side (x rows + y columns)
@@ -181,7 +188,7 @@ struct Cfg {  // FAST (van Leer + HLL fixed at compile time) does not change the
 // GEN: 0 = the path every BASELINE config takes; 1 = + gravity source term; 2 = + boundary-flux store (flux fixing)
 // and a third / fourth previous state.
 template <int DIM, int N, int TY, int G, int EXBUF, bool FAST, int GEN>
-__global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY, G, EXBUF>::SMEM <= 110 * 1024) ? 2 : 1)
+__global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY, G, EXBUF>::SMEM <= Cfg<DIM, N, TY, G, EXBUF>::TWO_CTAS) ? 2 : 1)
     stage_kernel(const __grid_constant__ StageParams p) {
   using C = Cfg<DIM, N, TY, G, EXBUF>;
   constexpr bool BF = (GEN == 2), GRAV = (GEN >= 1);
@@ -632,7 +639,9 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
   };
 
   constexpr int ISSUER = (TG >= 128) ? 96 : 0;   // lane 0 of a warp without halo roles when the group has one
-  if (DIM == 3 && t == ISSUER) { issue_plane(-2, 0); issue_plane(-1, 1); }
+  if (DIM == 3 && t == ISSUER) {
+    for (int q = 0; q < C::NSLOT; ++q) issue_plane(q - 2, q);
+  }
   if (DIM == 2) {
     double a[5], b[5], w[5], acc[5];
     if (t == ISSUER) issue_plane(0, 0);
@@ -648,13 +657,14 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
     double Rxp[5], Ryp[5];           // SPLIT: right states of the plane whose phase 1 ran ahead
 #pragma unroll
     for (int q = 0; q < 5; ++q) { dA[q] = 0.0; Lz[q] = 1.0; accp[q] = 0.0; Rxp[q] = 1.0; Ryp[q] = 1.0; }
-    int sc = 0;            // ring slot of plane c (planes take the slots 0,1,2,0,...)
+    constexpr int NS = C::NSLOT;
+    int sc = 0;            // ring slot of plane c: (c + 2) % NS
     uint32_t ph = 0;       // phase parity of each slot's mbarrier
     // one march iteration; the steady state (c in [2, N]) is the instance with every flag true
     auto march = [&](int c, auto zslope_t, auto zflux_t, auto fin_t, auto sweep_t) {
       constexpr bool ZSLOPE = decltype(zslope_t)::value, ZFLUX = decltype(zflux_t)::value;
       constexpr bool FIN = decltype(fin_t)::value, SWEEP = decltype(sweep_t)::value;
-      const int sk = (sc == 0) ? 2 : sc - 1;                // slot of plane c-1
+      const int sk = (sc == 0) ? NS - 1 : sc - 1;           // slot of plane c-1
       double* Wc = ring + sc * C::SLOT;
       const double* Wk = ring + sk * C::SLOT;
       double Fz[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
@@ -746,9 +756,9 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
         mid2();
         group_sync(bar_id, TG);
       }
-      // every thread is past its last read of plane c-1: refill that slot with plane c+2
-      if (t == ISSUER && c + 2 <= N + 1) issue_plane(c + 2, sk);
-      sc = (sc == 2) ? 0 : sc + 1;
+      // every thread is past its last read of plane c-1: refill that slot with the next plane of the ring
+      if (t == ISSUER && c >= -1 && c + NS - 1 <= N + 1) issue_plane(c + NS - 1, sk);
+      sc = (sc == NS - 1) ? 0 : sc + 1;
     };
     using T = std::true_type;
     using F_ = std::false_type;
