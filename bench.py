@@ -247,6 +247,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--host-dt", action="store_true",
+                    help="step = f4_compute_dt (dt read back) + f4_advance(dt) instead of f4_advance_cfl (dt stays on the device)")
     ap.add_argument("--sync-regrid", action="store_true",
                     help="adaptive configs: blocking f4_adapt before the step instead of f4_adapt_begin / f4_adapt_end "
                          "around it (host mesh work overlapped with the step, new mesh one step later)")
@@ -322,8 +324,11 @@ def main():
                 pend = True
             counters["regrids"] += 1
             counters["adapt_s"] += time.perf_counter() - t0
-        dt = mesh.compute_dt(0, cfg["cfl"])
-        mesh.advance(dt)
+        if args.host_dt:
+            dt = mesh.compute_dt(0, cfg["cfl"])      # reads the CFL maximum back: one host round trip per step
+            mesh.advance(dt)
+        else:
+            mesh.advance_cfl(cfg["cfl"])             # the same two calls with dt kept on the device (no round trip)
         counters["step"] += 1
         counters["updates"] += float(nstages) * mesh.num_blocks * n ** d     # the blocks this step advanced
         if pend:
@@ -457,6 +462,7 @@ def main():
         "config": {"workload": workload_name(cfg), "physics": cfg.get("physics", "euler"), "blocks": nb, "cells": cells,
                    "l2": "state (2 x %.1f GB) is larger than L2; no flush needed" % (mesh.storage_bytes() / 2e9),
                    "parallelism": "replicas only" if world > 1 else "1 GPU", "rk": args.rk,
+                   "step": "f4_compute_dt + f4_advance(dt)" if args.host_dt else "f4_advance_cfl (compute_dt + advance, dt on the device)",
                    "flux_fix": bool(args.flux_fix)},
         "roofline": {"bound": "hbm", "achieved": stage_gbs, "peak": peak, "unit": "GB/s",
                      "frac": (stage_gbs / peak) if stage_gbs else None, "traffic": traffic,
@@ -476,7 +482,11 @@ def main():
                       "adapt_ms_total": 1e3 * adapt_info["adapt_s"], "blocks_at_end": nb,
                       "regrid_mode": "blocking f4_adapt before the step" if args.sync_regrid else
                                      "f4_adapt_begin before / f4_adapt_end after the step (host part overlapped)",
-                      "value_excluding_adapt": world * updates / max(ms * 1e-3 - adapt_info["adapt_s"], 1e-9) / 1e9}
+                      # host wall time inside the regrid calls; with f4_advance_cfl the host runs ahead of the device,
+                      # so this includes waiting for queued steps: only with --host-dt --sync-regrid is
+                      # (time - adapt time) the time of the steps alone
+                      "value_excluding_adapt": (world * updates / max(ms * 1e-3 - adapt_info["adapt_s"], 1e-9) / 1e9)
+                      if (args.host_dt and args.sync_regrid) else None}
                      if adaptive else None),
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         "totals": [float(x) for x in totals_after],

@@ -227,6 +227,17 @@ int f4_set_rk_scheme(f4_mesh *m, int scheme);
  * Asynchronous; result in state 0, whose ghosts are then stale. */
 int f4_advance(f4_mesh *m, double dt);
 
+/* compute_dt + advance in one call without a host round trip: dt = cfl / (CFL maximum of state 0) stays on the device.
+ * The maximum is the one the previous f4_advance / f4_advance_cfl fused into its last stage (forward
+ * Euler "provide[s] a limit for the next time step"), else one reduction pass runs first; a one-thread kernel turns
+ * it into dt, and the stage kernels read dt from device memory (same operations and order as with a host dt: the
+ * results are those of f4_compute_dt followed by f4_advance).  Nothing synchronises: a step loop of f4_advance_cfl
+ * calls is enqueued as fast as the host can launch.  f4_last_dt reads the last step's dt back (synchronises);
+ * it returns F4_EINVAL if the wave speed was zero or not finite -- that step then ran with dt = 0.
+ * Scalar advection: dt is known on the host (constant wave speed); same call, no device scalar. */
+int f4_advance_cfl(f4_mesh *m, double cfl);
+int f4_last_dt(f4_mesh *m, double *dt_out);
+
 /* ---- refinement flags on the device ----------------------------------------
  * Per-block flags for f4_adapt from state `state` (its ghosts are filled first: the criteria read the first layer
  * of face ghosts, never edge / corner ghosts).

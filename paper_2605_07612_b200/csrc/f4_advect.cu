@@ -185,7 +185,7 @@ __global__ void __launch_bounds__(CfgA<DIM, N, TY, G>::NT, 1024 / CfgA<DIM, N, T
   };
 
   // ---- Runge-Kutta combine eq. (5), store, x push
-  const double sdt = p.sdt_l[lvl];                          // dt_sub / dx of this block's level
+  const double sdt = p.dt_dev ? (p.dtf * *p.dt_dev) * p.inv_dx_l[lvl] : p.sdt_l[lvl];   // dt_sub / dx of this block's level
   const int co = (j0 + j) * P + i;
   const double* pa = p.prev0 + boff + co;
   const double* pb = p.prev1 ? p.prev1 + boff + co : nullptr;

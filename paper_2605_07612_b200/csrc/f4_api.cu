@@ -69,6 +69,9 @@ struct f4_mesh {
   size_t cap_bflux = 0;
   int n_fix = 0, n_bfslots = 0;
   unsigned long long* d_maxrate = nullptr;
+  double* d_dt = nullptr;        // [2]: time step of f4_advance_cfl, error flag
+  bool dt_on_device = false;
+  double host_dt = 0.0;
   double* d_sums = nullptr;
   int* d_flags = nullptr;        // [max_blocks] refinement flags
   double* d_indicator = nullptr; // [max_blocks] block maxima of the refinement indicator
@@ -402,6 +405,7 @@ int f4_mesh_destroy(f4_mesh* m) {
   if (m->d_bflux) cudaFree(m->d_bflux);
   if (m->d_plan) cudaFree(m->d_plan);
   if (m->d_maxrate) cudaFree(m->d_maxrate);
+  if (m->d_dt) cudaFree(m->d_dt);
   if (m->d_sums) cudaFree(m->d_sums);
   if (m->d_flags) cudaFree(m->d_flags);
   if (m->d_bcv) cudaFree(m->d_bcv);
@@ -472,6 +476,7 @@ int f4_bind_storage(f4_mesh* m, void* dev_ptr, size_t bytes, void* cuda_stream) 
   m->stream = (cudaStream_t)cuda_stream;
   if (!m->d_maxrate) {
     CU(cudaMalloc((void**)&m->d_maxrate, sizeof(unsigned long long)));
+    CU(cudaMalloc((void**)&m->d_dt, 2 * sizeof(double)));
     CU(cudaMalloc((void**)&m->d_sums, (size_t)m->hm.max_blocks * m->nvar * sizeof(double)));
     CU(cudaMalloc((void**)&m->d_flags, (size_t)m->hm.max_blocks * sizeof(int)));
     CU(cudaMalloc((void**)&m->d_bcv, sizeof(m->bcv)));
@@ -721,11 +726,60 @@ int f4_set_rk_scheme(f4_mesh* m, int scheme) {
   return F4_OK;
 }
 
+namespace {
+// one step of the chosen Runge-Kutta scheme; dev_dt: the time step is the device-resident m->d_dt[0] (f4_advance_cfl)
+int advance_impl(f4_mesh* m, double dt, bool dev_dt);
+}
+
 int f4_advance(f4_mesh* m, double dt) {
   DeviceScope dev_scope(m);
   int rc = check_state(m, 0);
   if (rc) return rc;
   if (!(dt > 0.0)) return fail(m, F4_EINVAL, "dt must be positive");
+  return advance_impl(m, dt, false);
+}
+
+int f4_advance_cfl(f4_mesh* m, double cfl) {
+  DeviceScope dev_scope(m);
+  int rc = check_state(m, 0);
+  if (rc) return rc;
+  if (!(cfl > 0.0)) return fail(m, F4_EINVAL, "cfl must be positive");
+  if (m->physics == F4_PHYS_ADVECTION) {   // constant wave speed: dt is known on the host without a device pass
+    double dt = 0.0;
+    if ((rc = f4_compute_dt(m, 0, cfl, &dt))) return rc;
+    m->dt_on_device = false;
+    m->host_dt = dt;
+    return advance_impl(m, dt, false);
+  }
+  if (!m->rate_valid) {   // no fused CFL maximum of state 0 at hand (first step, after set_state / adapt / flux fixing)
+    CU(cudaMemsetAsync(m->d_maxrate, 0, sizeof(unsigned long long), m->stream));
+    Scope sc(m, F4_PROF_DT);
+    CU(launch_maxrate(m->hm.dim, m->hm.N, m->state_ptr(0), m->d_level, (int)m->hm.leaves.size(), m->gamma,
+                      1.0 / m->hm.dx_of_level(0), m->d_maxrate, m->stream));
+  }
+  {
+    Scope sc(m, F4_PROF_DT);
+    CU(launch_dt_from_rate(m->d_maxrate, cfl, m->d_dt, m->stream));
+  }
+  m->dt_on_device = true;
+  return advance_impl(m, 0.0, true);
+}
+
+int f4_last_dt(f4_mesh* m, double* dt_out) {
+  DeviceScope dev_scope(m);
+  if (!m || !dt_out) return F4_EINVAL;
+  if (!m->dt_on_device) { *dt_out = m->host_dt; return F4_OK; }
+  double h[2] = {0.0, 0.0};
+  CU(cudaMemcpyAsync(h, m->d_dt, sizeof(h), cudaMemcpyDeviceToHost, m->stream));
+  CU(cudaStreamSynchronize(m->stream));
+  *dt_out = h[0];
+  if (h[1] != 0.0) return fail(m, F4_EINVAL, "advance_cfl: wave speed is zero or not finite (a cell with NaN, rho <= 0 or p <= 0?)");
+  return F4_OK;
+}
+
+namespace {
+int advance_impl(f4_mesh* m, double dt, bool dev_dt) {
+  int rc;
   const int dim = m->hm.dim, N = m->hm.N, nb = (int)m->hm.leaves.size();
   const Scheme& sch = scheme_table(m->rk);
   StageParams p{};
@@ -767,6 +821,8 @@ int f4_advance(f4_mesh* m, double dt) {
     p.w0 = w[0]; p.w1 = w[1]; p.w2 = w[2]; p.w3 = w[3];
     p.grav_from = (ss.prev[0] == ss.deriv) ? 0 : ((ss.np > 1 && ss.prev[1] == ss.deriv) ? 1 : 2);
     p.dt_sub = ss.dtf * dt;
+    p.dt_dev = dev_dt ? m->d_dt : nullptr;
+    p.dtf = ss.dtf;
     for (int l = 0; l < MAXL; ++l) {
       p.inv_dx_l[l] = inv_dx0 * (double)(1u << l);
       p.sdt_l[l] = p.dt_sub * p.inv_dx_l[l];
@@ -786,7 +842,9 @@ int f4_advance(f4_mesh* m, double dt) {
     }
     if (ff) {
       fp.out = p.out;
-      for (int l = 0; l < MAXL; ++l) fp.sdt_l[l] = p.sdt_l[l];
+      for (int l = 0; l < MAXL; ++l) { fp.sdt_l[l] = p.sdt_l[l]; fp.inv_dx_l[l] = p.inv_dx_l[l]; }
+      fp.dt_dev = p.dt_dev;
+      fp.dtf = p.dtf;
       Scope sc(m, F4_PROF_STAGE);
       CU(launch_fluxfix(dim, N, m->nvar, fp, m->stream));
     }
@@ -798,6 +856,7 @@ int f4_advance(f4_mesh* m, double dt) {
   m->rate_valid = !ff && !adv;
   return F4_OK;
 }
+}  // namespace
 
 int f4_refine_flags(f4_mesh* m, int state, int criterion, int var, const double params[4], int* flags_out,
                     double* indicator_out) {

@@ -30,6 +30,11 @@ struct StageParams {
   const double* prev3;
   double* out;
   double w0, w1, w2, w3, dt_sub;
+  // time step resident on the device (f4_advance_cfl): when dt_dev != nullptr the kernels take dt_sub = dtf * *dt_dev and
+  // dt_sub / dx = dt_sub * inv_dx_l[level] themselves (same operations, same order as the host path) and ignore
+  // dt_sub / sdt_l
+  const double* dt_dev;
+  double dtf;
   double gamma;
   double inv_dx_l[MAXL];  // 1/dx per refinement level (1/dx_0 * 2^l, exact)
   double sdt_l[MAXL];     // dt_sub/dx per level: the factor of the flux difference in eq. (5)
@@ -71,6 +76,9 @@ struct GhostParams {
 // every launcher returns the cudaError_t of the launch
 cudaError_t launch_ghost(int dim, int n, int nvar, const GhostParams& p, cudaStream_t s);
 cudaError_t launch_stage(int dim, int n, const StageParams& p, cudaStream_t s);
+// dt[0] = cfl / rate with rate = the CFL maximum as bits of a double (0 and dt[1] = 1 if the rate is not a positive finite
+// number); one thread
+cudaError_t launch_dt_from_rate(const unsigned long long* maxrate, double cfl, double* dt, cudaStream_t s);
 cudaError_t launch_maxrate(int dim, int n, const double* state, const int* level, int nblocks, double gamma,
                            double inv_dx0, unsigned long long* maxrate, cudaStream_t s);
 cudaError_t launch_transfer(int dim, int n, int nvar, const double* old_state, double* new_state, const DevTransfer* plan,
@@ -89,6 +97,9 @@ struct FixParams {
   int nfix;
   const double* bflux;
   double sdt_l[MAXL];       // dt_sub/dx per level
+  const double* dt_dev;     // see StageParams: dt_sub / dx = (dtf * *dt_dev) * inv_dx_l[level]
+  double dtf;
+  double inv_dx_l[MAXL];
 };
 cudaError_t launch_fluxfix(int dim, int n, int nvar, const FixParams& p, cudaStream_t s);
 // per-block refinement flags and indicator (device arrays) from a ghost-filled state

@@ -21,7 +21,7 @@ __global__ void __launch_bounds__(256) fluxfix_kernel(const __grid_constant__ Fi
   constexpr int FS = N * KM;                   // cells of one block face
   constexpr size_t VS = (size_t)P * P * ((DIM == 3) ? P : 1);
   const DevFixBlock fb = p.fix[blockIdx.x];
-  const double sdt = p.sdt_l[fb.level];
+  const double sdt = p.dt_dev ? (p.dtf * *p.dt_dev) * p.inv_dx_l[fb.level] : p.sdt_l[fb.level];
   const double* bflux = p.bflux;
   double* blk = p.out + (size_t)fb.blk * VS * NV;
   for (int f = 0; f < 2 * DIM; ++f) {

@@ -490,6 +490,13 @@ __global__ void __launch_bounds__(256) maxrate_kernel(const double* __restrict__
   if ((threadIdx.x & 31) == 0) atomicMax(maxrate, (unsigned long long)__double_as_longlong(mx));
 }
 
+__global__ void dt_from_rate_kernel(const unsigned long long* __restrict__ maxrate, double cfl, double* __restrict__ dt) {
+  const double rate = __longlong_as_double((long long)*maxrate);
+  const bool ok = rate > 0.0 && rate <= 1.7976931348623157e308;
+  dt[0] = ok ? cfl / rate : 0.0;      // dt = 0: the stages leave the state as it is; f4_last_dt reports the failure
+  dt[1] = ok ? 0.0 : 1.0;
+}
+
 template <typename F>
 cudaError_t dispatch(int dim, int n, int nvar, F&& f) {
 #define F4_CASE(D, NN)                                                   \
@@ -519,6 +526,10 @@ constexpr int nv_of(Geo<D, N, V>) { return V; }
     return cudaGetLastError();                                   \
   })
 
+cudaError_t launch_dt_from_rate(const unsigned long long* maxrate, double cfl, double* dt, cudaStream_t s) {
+  dt_from_rate_kernel<<<1, 1, 0, s>>>(maxrate, cfl, dt);
+  return cudaGetLastError();
+}
 cudaError_t launch_ghost(int dim, int n, int nvar, const GhostParams& p, cudaStream_t s) {
   if (p.nrec <= 0) return cudaSuccess;
   F4_DISPATCH((ghost_exec_kernel<D, NN, NVV><<<(p.nrec + 2 * D - 1) / (2 * D), 256, 0, s>>>(p)));

@@ -546,7 +546,9 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
 
   // Runge-Kutta combine eq. (5) + store + optional CFL rate of the new state
   double rate_max = 0.0;
-  const double sdt = p.sdt_l[lvl];                          // dt_sub / dx of this block's level
+  // dt_sub and dt_sub / dx of this block's level: from the host, or from the time step resident on the device
+  const double dt_sub = p.dt_dev ? p.dtf * *p.dt_dev : p.dt_sub;
+  const double sdt = p.dt_dev ? dt_sub * p.inv_dx_l[lvl] : p.sdt_l[lvl];
   const int co = (j0 + j) * P + i;                          // own cell inside a (block, var) box, + k*PP + v*VS
   const double* pa = p.prev0 + boff + co;
   const double* pb = p.prev1 ? p.prev1 + boff + co : nullptr;
@@ -604,10 +606,10 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
       double gm = 0.0;
 #pragma unroll
       for (int d = 0; d < DIM; ++d) {
-        u[1 + d] = fma(p.dt_sub * p.grav[d], r0, u[1 + d]);
+        u[1 + d] = fma(dt_sub * p.grav[d], r0, u[1 + d]);
         gm = fma(p.grav[d], mm[d], gm);
       }
-      u[4] = fma(p.dt_sub, gm, u[4]);
+      u[4] = fma(dt_sub, gm, u[4]);
     }
 #pragma unroll
     for (int q = 0; q < 5; ++q) {

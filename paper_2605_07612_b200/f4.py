@@ -32,7 +32,7 @@ PROF_NAMES = ("ghost_r1", "ghost_r2", "stage", "dt_reduce", "regrid", "layout")
 SYMBOLS = ("f4_mesh_create", "f4_mesh_destroy", "f4_set_options", "f4_set_flux_fix", "f4_set_physics", "f4_num_vars", "f4_set_bc_values", "f4_set_bc_callback", "f4_update_bc_data",
            "f4_num_bc_faces", "f4_set_gravity", "f4_set_rk_scheme", "f4_storage_bytes", "f4_bind_storage",
            "f4_num_blocks", "f4_get_blocks", "f4_set_state", "f4_get_state", "f4_build_ghost_pattern",
-           "f4_pattern_size", "f4_get_pattern", "f4_fill_ghosts", "f4_compute_dt", "f4_advance", "f4_refine_flags", "f4_adapt", "f4_adapt_begin", "f4_adapt_end",
+           "f4_pattern_size", "f4_get_pattern", "f4_fill_ghosts", "f4_compute_dt", "f4_advance", "f4_advance_cfl", "f4_last_dt", "f4_refine_flags", "f4_adapt", "f4_adapt_begin", "f4_adapt_end",
            "f4_conserved_totals", "f4_profile_enable", "f4_profile_get", "f4_launch_count", "f4_last_adapt_ms", "f4_last_error",
            "f4_version")
 
@@ -87,6 +87,8 @@ def lib():
     L.f4_compute_dt.argtypes = [vp, C.c_int, C.c_double, dp]
     L.f4_advance.argtypes = [vp, C.c_double]
     L.f4_adapt.argtypes = [vp, ip, ip]
+    L.f4_advance_cfl.argtypes = [vp, C.c_double]
+    L.f4_last_dt.argtypes = [vp, dp]
     L.f4_adapt_begin.argtypes = [vp, ip]
     L.f4_adapt_end.argtypes = [vp, ip]
     L.f4_conserved_totals.argtypes = [vp, C.c_int, dp]
@@ -272,6 +274,15 @@ class Mesh:
         ch = C.c_int(0)
         self._chk(self.L.f4_adapt(self.h, _ip(f), C.byref(ch)))
         return bool(ch.value)
+
+    def advance_cfl(self, cfl):
+        """compute_dt + advance without a host round trip (dt stays on the device); last_dt() reads it back."""
+        self._chk(self.L.f4_advance_cfl(self.h, float(cfl)))
+
+    def last_dt(self):
+        dt = C.c_double(0.0)
+        self._chk(self.L.f4_last_dt(self.h, C.byref(dt)))
+        return dt.value
 
     def adapt_begin(self, flags):
         """Start the host part of a regrid on a worker thread (compute_dt / advance may follow); adapt_end() commits."""

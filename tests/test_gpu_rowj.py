@@ -219,3 +219,61 @@ def test_asynchronous_regrid_matches_the_oracle_with_the_same_lag():
     with pytest.raises(f4.F4Error):
         lm.adapt_end()                                 # nothing pending
     lm.close()
+
+
+@pytest.mark.parametrize("n,scale,flux_fix", [(1, None, False), (3, 1, False), (5, 1, False), (5, 1, True)])
+def test_advance_cfl_equals_compute_dt_then_advance(n, scale, flux_fix):
+    """f4_advance_cfl keeps dt on the device (no host round trip per step); it must be compute_dt followed by advance:
+    bit-identical states and the same dt against a second mesh stepped the two-call way, and the oracle's state to 1e-11."""
+    cfg = W.config(n, scale=scale)
+    a = f4.Mesh.from_config(cfg, max_blocks=3000)
+    b = f4.Mesh.from_config(cfg, max_blocks=3000)
+    a.bind_torch()
+    b.bind_torch()
+    om = O.OracleMesh.from_config(cfg)
+    if n == 5:
+        fl = np.zeros(a.num_blocks, dtype=np.int32)
+        fl[[0, 3, 5]] = 1
+        perm0 = _perm(a, om)
+        fo = np.empty_like(fl)
+        fo[perm0] = fl
+        assert a.adapt(fl) and b.adapt(fl) and om.adapt(fo)
+        a.set_flux_fix(flux_fix)
+        b.set_flux_fix(flux_fix)
+        om.set_flux_fix(flux_fix)
+    lev, co = a.get_blocks()
+    u = W.initial_state(cfg, lev, co)
+    a.set_state(0, u)
+    b.set_state(0, u)
+    perm = _perm(a, om)
+    uo = np.empty_like(u)
+    uo[perm] = u
+    om.set_state(0, uo)
+    for s in range(6):
+        a.advance_cfl(cfg["cfl"])
+        dt = b.compute_dt(0, cfg["cfl"])
+        b.advance(dt)
+        om.advance(om.compute_dt(0, cfg["cfl"]))
+        if s in (0, 5):
+            assert a.last_dt() == dt
+    assert np.array_equal(a.get_state(0), b.get_state(0))
+    err = H.rel_linf(a.get_state(0), om.get_state(0)[perm])
+    assert np.all(err <= TOL_STATE), err
+    a.close()
+    b.close()
+
+
+def test_advance_cfl_reports_an_invalid_state():
+    cfg = W.config(3, scale=1)
+    lm = f4.Mesh.from_config(cfg)
+    lm.bind_torch()
+    lev, co = lm.get_blocks()
+    u = W.initial_state(cfg, lev, co)
+    u[2, 0, 3, 3, 3] = -1.0
+    lm.set_state(0, u)
+    lm.advance_cfl(cfg["cfl"])              # runs with dt = 0 (and NaN fluxes around the bad cell)
+    with pytest.raises(f4.F4Error):
+        lm.last_dt()
+    far = lm.get_state(0)[40:]              # blocks away from the bad cell: u + 0 * F(u) = u
+    assert np.array_equal(far, u[40:])
+    lm.close()
