@@ -7,7 +7,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libf4.so")
-SOURCES = ["f4_mesh.cpp", "f4_ghost.cu", "f4_stage.cu", "f4_advect.cu", "f4_fluxfix.cu", "f4_api.cu"]
+SOURCES = ["f4_mesh.cpp", "f4_ghost.cu", "f4_stage.cu", "f4_advect.cu", "f4_advect2.cu", "f4_fluxfix.cu", "f4_api.cu"]
 HEADERS = ["f4_mesh.hpp", "f4_dev.hpp", "f4_stage_dev.cuh", os.path.join("..", "..", "include", "f4.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-cudart", "static", "-Wno-deprecated-gpu-targets"]

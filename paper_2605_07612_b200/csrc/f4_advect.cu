@@ -299,9 +299,7 @@ cudaError_t launch_advect(int dim, int n, const StageParams& p, cudaStream_t s) 
   if (dim == 2 && n == 8) return launch_cfgA<2, 8, 8, 4>(p, s);
   if (dim == 2 && n == 16) return launch_cfgA<2, 16, 16, 1>(p, s);
   if (dim == 2 && n == 32) return launch_cfgA<2, 32, 8, 1>(p, s);
-  if (dim == 3 && n == 8) return launch_cfgA<3, 8, 8, 4>(p, s);
-  if (dim == 3 && n == 16) return launch_cfgA<3, 16, 16, 1>(p, s);
-  if (dim == 3 && n == 32) return launch_cfgA<3, 32, 8, 1>(p, s);
+  if (dim == 3) return launch_advect2(n, p, s);   // two cells per thread (f4_advect2.cu)
   return cudaErrorInvalidValue;
 }
 

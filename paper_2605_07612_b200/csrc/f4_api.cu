@@ -329,7 +329,9 @@ int fill_ghosts_impl(f4_mesh* m, int state, int have, bool need_z, bool for_stag
   if (have == 2 || (have == 1 && !need_z)) { r1 = m->d_r1n; n1 = m->n_r1n; after = have; }
   else if (have == 1 && for_stage) { r1 = m->d_r1c; n1 = m->n_r1c; after = 1; }
   else if (have == 1) { r1 = m->d_r1z; n1 = m->n_r1z; }
-  else if (for_stage && no_push) { r1 = m->d_r1f; n1 = m->n_r1f; after = 0; }
+  // nothing valid and the reader is a stage kernel: of the same-level copies it needs the x faces only (and the y / z
+  // ones into C2F source blocks); its y / z halos come from the neighbours' interiors
+  else if (for_stage) { r1 = m->d_r1f; n1 = m->n_r1f; after = no_push ? 0 : 1; }
   if (n1) {
     Scope sc(m, F4_PROF_R1);
     CU(launch_ghost(m->hm.dim, m->hm.N, m->nvar,

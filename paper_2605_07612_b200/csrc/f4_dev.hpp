@@ -109,6 +109,7 @@ bool stage_supported(int dim, int n);
 // scalar advection eq. (13), PAPER.md:364-370 (f4_advect.cu): symmetric limiters, at most two previous states
 bool advect_supported(const StageParams& p);
 cudaError_t launch_advect(int dim, int n, const StageParams& p, cudaStream_t s);
+cudaError_t launch_advect2(int n, const StageParams& p, cudaStream_t s);   // 3D, two cells per thread (f4_advect2.cu)
 
 
 }  // namespace f4
