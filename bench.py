@@ -466,7 +466,7 @@ def main():
                    "flux_fix": bool(args.flux_fix)},
         "roofline": {"bound": "hbm", "achieved": stage_gbs, "peak": peak, "unit": "GB/s",
                      "frac": (stage_gbs / peak) if stage_gbs else None, "traffic": traffic,
-                     "kernel": "advect_kernel" if cfg.get("physics") == "advection" else "stage_kernel",
+                     "kernel": ("advect2_kernel" if d == 3 else "advect_kernel") if cfg.get("physics") == "advection" else "stage_kernel",
                      "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": stage_bytes, "avg_launch_ms": st_ms / max(st_n, 1)},
         "ghost_fill": {"GBps": ghost_gbs, "frac_of_hbm_peak": (ghost_gbs / peak) if ghost_gbs else None,

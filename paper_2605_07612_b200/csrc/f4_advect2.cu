@@ -217,6 +217,8 @@ __global__ void __launch_bounds__(CfgA2<N, TY, G>::NT, 512 / CfgA2<N, TY, G>::NT
     constexpr int sk = (sc + NS - 1) & (NS - 1);          // slot of plane c-1
     double2 a_new = zero2, b_new = zero2;
     if (c >= 0 && c < N) { a_new = ld2(pa + c * PP); if (pb) b_new = ld2(pb + c * PP); }
+    // stage 2: u_t comes from DRAM; pull the plane four iterations ahead into L2 (one 32-byte sector per two threads)
+    if (pb && (pi & 1) == 0 && c + 4 >= 0 && c + 4 < N) asm volatile("prefetch.global.L2 [%0];" ::"l"(pa + (c + 4) * PP));
     mbar_wait(bars_u32 + 8u * sc, (ph >> sc) & 1u);
     ph ^= 1u << sc;
     const double2 wB2 = ld2(ring + sc * PLANE + own);
