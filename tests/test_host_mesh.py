@@ -155,3 +155,43 @@ def test_full_size_config_patterns():
         rec, n1, n2 = m.pattern()
         assert n1 == 6 * nb and n2 == 0 and (rec[:, 0] == f4.OP_SRL).all()
         m.close()
+
+
+def test_asynchronous_adapt_builds_the_same_mesh_and_pattern():
+    # f4_adapt_begin / f4_adapt_end (host part on a worker thread, on a copy of the mesh) against the blocking f4_adapt:
+    # same leaves, same pattern records, over refine / coarsen / no-change rounds; the mesh in use stays valid meanwhile
+    rng = np.random.default_rng(11)
+    for dim, N in ((2, 8), (3, 8)):
+        bc = [PER, PER, OUT, OUT, PER, PER][: 2 * dim]
+        a = f4.Mesh(dim, N, 2, (2, 2, 2)[:dim], 0, 3, bc, max_blocks=4000)
+        b = f4.Mesh(dim, N, 2, (2, 2, 2)[:dim], 0, 3, bc, max_blocks=4000)
+        for rnd in range(6):
+            nb = a.num_blocks
+            flags = rng.integers(-1, 2, size=nb).astype(np.int32) if rnd != 3 else np.zeros(nb, dtype=np.int32)
+            b.adapt_begin(flags)
+            lev_before, co_before = b.get_blocks()            # still the old mesh
+            assert len(lev_before) == nb
+            with pytest.raises(f4.F4Error):
+                b.adapt_begin(flags)                          # one regrid at a time
+            ch_a, ch_b = a.adapt(flags), b.adapt_end()
+            assert ch_a == ch_b and (rnd != 3 or not ch_a)
+            la, ca = a.get_blocks()
+            lb, cb = b.get_blocks()
+            assert np.array_equal(la, lb) and np.array_equal(ca, cb)
+            ra, rb = a.pattern(), b.pattern()
+            assert ra[1:] == rb[1:] and np.array_equal(ra[0], rb[0])
+        with pytest.raises(f4.F4Error):
+            b.adapt_end()                                     # nothing pending
+        a.close()
+        b.close()
+
+
+def test_scalar_advection_mesh_has_one_variable():
+    cfg = W.config(8, scale=1)
+    m = f4.Mesh.from_config(cfg)
+    assert m.nvar == 1 and m._shape(False)[1] == 1
+    assert m.storage_bytes() == 2 * m.num_blocks * 20 ** 3 * 8          # two states, one variable, padded 20^3 blocks
+    # dt without a device: CFL dx / sum |v_i| (reading B6)
+    with pytest.raises(f4.F4Error):
+        m.compute_dt(0, 0.5)                                            # still needs bound storage (check_state)
+    m.close()
