@@ -123,13 +123,8 @@ __device__ __forceinline__ void riemann_fluxN(const double (&L)[NF][5], const do
   }
 #pragma unroll
   for (int f = 0; f < NF; ++f) y2[f] = rsqrt_seed(d2[f]);
-  {
-    double e[NF];
 #pragma unroll
-    for (int f = 0; f < NF; ++f) e[f] = fma(-(d2[f] * y2[f]), y2[f], 1.0);
-#pragma unroll
-    for (int f = 0; f < NF; ++f) y2[f] = fma(y2[f], fma(0.375, e[f], 0.5) * e[f], y2[f]);
-  }
+  for (int f = 0; f < NF; ++f) y2[f] = rsqrt_refine(d2[f], y2[f]);
 #pragma unroll
   for (int f = 0; f < NF; ++f) {
     const double a0 = fma(uhat[f], 0.5 * y2[f], 0.5);

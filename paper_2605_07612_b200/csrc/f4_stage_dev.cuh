@@ -24,10 +24,10 @@ __device__ __forceinline__ double rcp_refine(double x, double r) {
   return fma(r, e2, r);
 }
 __device__ __forceinline__ double rsqrt_refine(double x, double y) {
-  const double t = x * y;
-  const double e = fma(-t, y, 1.0);
+  // y*y and y*e are formed beside the Newton terms: the dependent chain is DMUL, DFMA, DFMA/DMUL, DFMA
+  const double e = fma(-x, y * y, 1.0);
   const double h = fma(0.375, e, 0.5);
-  return fma(y, h * e, y);
+  return fma(y * e, h, y);
 }
 __device__ __forceinline__ double rcp_fast(double x) { return rcp_refine(x, rcp_seed(x)); }
 __device__ __forceinline__ double rsqrt_fast(double x) { return rsqrt_refine(x, rsqrt_seed(x)); }
@@ -78,8 +78,9 @@ __device__ __forceinline__ double half_slope(double a, double b, int limiter) {
     double y = rcp_seed(x);
     y = __hiloint2double((__double2hiint(ab) > 0) ? __double2hiint(y) : 0, 0);
     const double e = fma(-x, y, 1.0);
+    const double t = ab * y;             // beside the Newton terms, off the dependent chain
     const double e2 = fma(e, e, e);
-    return ab * fma(y, e2, y);
+    return fma(t, e2, t);
   }
   double r;
   if (limiter == F4_LIM_WENO3) {
