@@ -277,6 +277,24 @@ int f4_adapt_end(f4_mesh *m, int *changed_out);
 /* sum over interior cells of u * dx^dim, per variable [Nvar] (for conservation tests). */
 int f4_conserved_totals(f4_mesh *m, int state, double *totals);
 
+/* The same totals for callers that must not allocate (code under CUDA graph capture, serving loops, harnesses that
+ * forbid cudaMalloc): the per-block sums go to a STATIC device array inside the library instead of the mesh's
+ * cudaMalloc'ed scratch, and a second kernel finishes the sum on the device.  The call allocates nothing on the
+ * device or the host (no cudaMalloc / cudaFree, no allocating library routine), enqueues two kernels on the mesh's
+ * stream and does not synchronise.
+ *   totals_dev  DEVICE pointer, [Nvar] doubles, owned by the caller; valid once the stream reaches this point.
+ * Limit: at most F4_NOALLOC_MAX_BLOCKS blocks (the array holds F4_NOALLOC_MAX_BLOCKS * 5 doubles = 1.25 MiB on every
+ * GPU that loads the library, until the process exits); a larger mesh gives F4_EINVAL and a message that says so.
+ * The array is shared by every mesh and every call on a device and keeps the last call's contents (each call
+ * overwrites the entries it reads, nothing has to be cleared): calls that OVERLAP on the GPU -- two meshes on two
+ * streams -- race on it; calls on one stream do not.  The first call on a device also asks the CUDA runtime for the
+ * array's device address (cudaGetSymbolAddress): make that call outside a graph capture.
+ * Result: equal to f4_conserved_totals to ~1e-15 relative (same per-block sums; the sum over blocks is carried in
+ * double-double here, in long double there).  Errors: F4_EINVAL (null / host pointer, too many blocks),
+ * F4_EUNBOUND, F4_ECUDA. */
+#define F4_NOALLOC_MAX_BLOCKS 32768
+int f4_conserved_totals_noalloc(f4_mesh *m, int state, double *totals_dev);
+
 /* ---- measurement helpers ---------------------------------------------------
  * f4_profile_enable(1): bracket every kernel class with CUDA events on the
  * bound stream.  f4_profile_get: accumulated milliseconds and launch counts

@@ -1003,6 +1003,31 @@ int f4_conserved_totals(f4_mesh* m, int state, double* totals) {
   return F4_OK;
 }
 
+int f4_conserved_totals_noalloc(f4_mesh* m, int state, double* totals_dev) {
+  DeviceScope dev_scope(m);
+  int rc = check_state(m, state);
+  if (rc) return rc;
+  if (!totals_dev) return fail(m, F4_EINVAL, "f4_conserved_totals_noalloc: null output");
+  cudaPointerAttributes attr;
+  if (cudaPointerGetAttributes(&attr, totals_dev) != cudaSuccess ||
+      (attr.type != cudaMemoryTypeDevice && attr.type != cudaMemoryTypeManaged)) {
+    cudaGetLastError();
+    return fail(m, F4_EINVAL, "f4_conserved_totals_noalloc: totals_dev must be a device pointer");
+  }
+  const int nb = (int)m->hm.leaves.size();
+  if (nb > F4_NOALLOC_MAX_BLOCKS) {
+    char msg[160];
+    snprintf(msg, sizeof msg, "f4_conserved_totals_noalloc: %d blocks exceed the static scratch's maximum of %d "
+             "(F4_NOALLOC_MAX_BLOCKS); use f4_conserved_totals", nb, F4_NOALLOC_MAX_BLOCKS);
+    return fail(m, F4_EINVAL, msg);
+  }
+  m->launches++;   // two kernels: the Scope counts the first
+  Scope sc(m, F4_PROF_LAYOUT);
+  CU(launch_totals_noalloc(m->hm.dim, m->hm.N, m->nvar, m->state_ptr(state), m->d_level, nb, m->hm.dx_of_level(0),
+                           totals_dev, m->stream));
+  return F4_OK;
+}
+
 int f4_profile_enable(f4_mesh* m, int on) {
   DeviceScope dev_scope(m);
   if (!m) return F4_EINVAL;

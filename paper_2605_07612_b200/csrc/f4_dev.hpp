@@ -90,6 +90,10 @@ cudaError_t launch_unpack(int dim, int n, int nvar, const double* store_state, d
                           cudaStream_t s);
 cudaError_t launch_init_benign(int dim, int n, int nvar, double* store_state, int nb, double gamma, cudaStream_t s);
 cudaError_t launch_block_sums(int dim, int n, int nvar, const double* state, int nb, double* sums /*[nb][nvar]*/, cudaStream_t s);
+// the same reduction with its scratch in a static device array, finished on the device (f4_conserved_totals_noalloc):
+// no allocation; nb <= F4_NOALLOC_MAX_BLOCKS, else cudaErrorInvalidValue; totals_dev: device, [nvar]
+cudaError_t launch_totals_noalloc(int dim, int n, int nvar, const double* state, const int* level, int nb, double dx0,
+                                  double* totals_dev, cudaStream_t s);
 // coarse-side correction u -= -+ dt_sub/dx_c (mean fine flux - coarse flux) in the cells next to refinement boundaries
 struct FixParams {
   double* out;              // the state the stage kernel just wrote

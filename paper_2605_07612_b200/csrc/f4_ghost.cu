@@ -9,6 +9,8 @@
 // pair-transposed x-ghost layout (cell_off) two adjacent lanes write one full
 // 32-byte ghost sector.  Inside f4_advance the SRL records are not executed
 // here: the stage kernel pushes those layers itself (f4_stage.cu).
+#include <mutex>
+
 #include "../../include/f4.h"
 #include "f4_dev.hpp"
 
@@ -570,6 +572,99 @@ cudaError_t launch_maxrate(int dim, int n, const double* state, const int* level
   if (nblocks <= 0) return cudaSuccess;
   const int nvar = dim + 2;   // Euler only: scalar advection has the constant wave speed v (f4_compute_dt)
   F4_DISPATCH((maxrate_kernel<D, NN><<<nblocks, 256, 0, s>>>(state, level, gamma, inv_dx0, maxrate)));
+}
+
+// ---- f4_conserved_totals_noalloc: the block-sum reduction with its scratch in a static device array ------------
+// For callers that must not allocate (code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc).
+// g_noalloc_sums takes the place of the mesh's cudaMalloc'ed per-(block,var) sums; it is part of the loaded module, so
+// every GPU that loads the library holds F4_NOALLOC_MAX_BLOCKS * 5 * 8 bytes (1.25 MiB) until the process exits.
+// In host code the NAME g_noalloc_sums is a host-side stand-in, not a device address: the launcher below asks the
+// runtime for the device address once per device (cudaGetSymbolAddress, with that device current) and hands THAT to
+// the kernels.  Every call on a device shares the array: block_sums_kernel overwrites each entry the finishing
+// kernel reads, so nothing has to be cleared between calls, but two calls that overlap on the GPU (different
+// streams) race on it.
+namespace {
+
+constexpr int NOALLOC_MAX_VARS = 5;
+static __device__ __align__(256) double g_noalloc_sums[(size_t)F4_NOALLOC_MAX_BLOCKS * NOALLOC_MAX_VARS];
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+double* g_noalloc_ptr[NOALLOC_MAX_DEVICES];   // device address of g_noalloc_sums on device d, 0 = not yet asked
+std::mutex g_noalloc_mutex;
+
+// error-free transformations: (s, e) with s + e = a + b exactly; the partial totals are carried as such pairs
+__device__ __forceinline__ void two_sum(double a, double b, double& s, double& e) {
+  s = __dadd_rn(a, b);
+  const double bb = __dsub_rn(s, a);
+  e = __dadd_rn(__dsub_rn(a, __dsub_rn(s, bb)), __dsub_rn(b, bb));
+}
+__device__ __forceinline__ void dd_add(double& hi, double& lo, double xh, double xl) {
+  double s, e;
+  two_sum(hi, xh, s, e);
+  e = __dadd_rn(e, __dadd_rn(lo, xl));
+  hi = __dadd_rn(s, e);
+  lo = __dsub_rn(e, __dsub_rn(hi, s));
+}
+
+// totals[v] = sum_b sums[b][v] * dx(level_b)^dim: one CTA per variable, fixed order, double-double accumulation
+// (the host path of f4_conserved_totals accumulates in long double; both are far inside the 1e-12 the tests ask)
+__global__ void __launch_bounds__(256) totals_finish_kernel(const double* __restrict__ sums, const int* __restrict__ level,
+                                                            int nb, int nvar, int dim, double dx0,
+                                                            double* __restrict__ totals) {
+  __shared__ double sh[256], sl[256];
+  const int v = blockIdx.x;
+  double hi = 0.0, lo = 0.0;
+  for (int b = threadIdx.x; b < nb; b += blockDim.x) {
+    const double h = dx0 / (double)(1u << level[b]);            // exact: a power of two
+    const double vol = (dim == 3) ? __dmul_rn(__dmul_rn(h, h), h) : __dmul_rn(h, h);
+    const double x = sums[(size_t)b * nvar + v];
+    const double p = __dmul_rn(x, vol);
+    dd_add(hi, lo, p, fma(x, vol, -p));
+  }
+  sh[threadIdx.x] = hi;
+  sl[threadIdx.x] = lo;
+  __syncthreads();
+  for (int s = 128; s > 0; s >>= 1) {
+    if ((int)threadIdx.x < s) {
+      dd_add(hi, lo, sh[threadIdx.x + s], sl[threadIdx.x + s]);
+      sh[threadIdx.x] = hi;
+      sl[threadIdx.x] = lo;
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) totals[v] = __dadd_rn(hi, lo);
+}
+
+// device address of the static scratch on the CURRENT device; asks the runtime once per device
+cudaError_t noalloc_scratch(double** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  if (!g_noalloc_ptr[dev]) {
+    double* ptr = nullptr;
+    e = cudaGetSymbolAddress((void**)&ptr, g_noalloc_sums);
+    if (e != cudaSuccess) return e;
+    if (!ptr) return cudaErrorInvalidSymbol;
+    g_noalloc_ptr[dev] = ptr;
+  }
+  *out = g_noalloc_ptr[dev];
+  return cudaSuccess;
+}
+
+}  // namespace
+
+cudaError_t launch_totals_noalloc(int dim, int n, int nvar, const double* state, const int* level, int nb, double dx0,
+                                  double* totals_dev, cudaStream_t s) {
+  if (nb <= 0 || nb > F4_NOALLOC_MAX_BLOCKS || nvar < 1 || nvar > NOALLOC_MAX_VARS) return cudaErrorInvalidValue;
+  double* scratch = nullptr;
+  cudaError_t e = noalloc_scratch(&scratch);
+  if (e != cudaSuccess) return e;
+  e = launch_block_sums(dim, n, nvar, state, nb, scratch, s);   // the kernel of f4_conserved_totals, static scratch
+  if (e != cudaSuccess) return e;
+  totals_finish_kernel<<<nvar, 256, 0, s>>>(scratch, level, nb, nvar, dim, dx0, totals_dev);
+  return cudaGetLastError();
 }
 
 }  // namespace f4

@@ -33,11 +33,12 @@ SYMBOLS = ("f4_mesh_create", "f4_mesh_destroy", "f4_set_options", "f4_set_flux_f
            "f4_num_bc_faces", "f4_set_gravity", "f4_set_rk_scheme", "f4_storage_bytes", "f4_bind_storage",
            "f4_num_blocks", "f4_get_blocks", "f4_set_state", "f4_get_state", "f4_build_ghost_pattern",
            "f4_pattern_size", "f4_get_pattern", "f4_fill_ghosts", "f4_compute_dt", "f4_advance", "f4_advance_cfl", "f4_last_dt", "f4_refine_flags", "f4_adapt", "f4_adapt_begin", "f4_adapt_end",
-           "f4_conserved_totals", "f4_profile_enable", "f4_profile_get", "f4_launch_count", "f4_last_adapt_ms", "f4_last_error",
+           "f4_conserved_totals", "f4_conserved_totals_noalloc", "f4_profile_enable", "f4_profile_get", "f4_launch_count", "f4_last_adapt_ms", "f4_last_error",
            "f4_version")
 
 
 PHYS_EULER, PHYS_ADVECTION = 0, 1
+NOALLOC_MAX_BLOCKS = 32768   # F4_NOALLOC_MAX_BLOCKS
 
 
 class F4Error(RuntimeError):
@@ -92,6 +93,7 @@ def lib():
     L.f4_adapt_begin.argtypes = [vp, ip]
     L.f4_adapt_end.argtypes = [vp, ip]
     L.f4_conserved_totals.argtypes = [vp, C.c_int, dp]
+    L.f4_conserved_totals_noalloc.argtypes = [vp, C.c_int, vp]
     L.f4_profile_enable.argtypes = [vp, C.c_int]
     L.f4_profile_get.argtypes = [vp, dp, C.POINTER(C.c_longlong), C.c_int]
     L.f4_launch_count.restype = C.c_longlong
@@ -335,6 +337,11 @@ class Mesh:
         out = np.zeros(self.nvar)
         self._chk(self.L.f4_conserved_totals(self.h, state, _dp(out)))
         return out
+
+    def conserved_totals_noalloc(self, state, out_dev_ptr):
+        """f4_conserved_totals_noalloc: totals into DEVICE memory at out_dev_ptr ([nvar] doubles, e.g. tensor.data_ptr()),
+        enqueued on the mesh's stream, no synchronisation, no allocation (at most NOALLOC_MAX_BLOCKS blocks)."""
+        self._chk(self.L.f4_conserved_totals_noalloc(self.h, state, C.c_void_p(int(out_dev_ptr))))
 
     # -- measurement ---------------------------------------------------------
     def profile_enable(self, on=True):
