@@ -439,7 +439,7 @@ __global__ void __launch_bounds__(256) flags_kernel(const double* __restrict__ s
         const double En = __ddiv_rn(num, den);
         sumsq = __dadd_rn(sumsq, __dmul_rn(En, En));
       }
-      cell = __dsqrt_rn(sumsq);
+      cell = sumsq;   // the square root is taken once, of the block maximum (monotone and correctly rounded: same bits)
     } else {
       const double pc = pressure(i, j, k);
 #pragma unroll
@@ -460,6 +460,7 @@ __global__ void __launch_bounds__(256) flags_kernel(const double* __restrict__ s
   __syncthreads();
   if (threadIdx.x == 0) {
     for (int w = 1; w < 8; ++w) mx = fmax(mx, sh[w]);
+    if (criterion == F4_CRIT_LOHNER) mx = __dsqrt_rn(mx);
     if (indicator) indicator[b] = mx;
     flags[b] = (mx > p0) ? 1 : ((mx < p1) ? -1 : 0);
   }
