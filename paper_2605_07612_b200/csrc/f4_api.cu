@@ -49,6 +49,8 @@ struct f4_mesh {
   DevRecord* d_r1c = nullptr;  // d_r1n plus the y- / z-face same-level copies into blocks that are C2F sources
   DevRecord* d_r1f = nullptr;  // d_r1c plus all x-face same-level copies (flux-fixing mode: the stage does not push x)
   int* d_nbr = nullptr;        // [max_blocks][6] same-level neighbour per face or -1
+  int nb_dev = 0;              // blocks of the mesh whose tables and records are on the device (during a regrid the
+                               // host mesh is already the new one while the device still holds the old pattern)
   // all of the above (and d_bfslot, d_fix) point into one device blob, uploaded from one pinned host buffer
   char* d_meta = nullptr;
   char* h_meta = nullptr;
@@ -302,6 +304,7 @@ int upload_meta(f4_mesh* m) {
   char* d = m->d_meta;
   m->d_level = (int*)(d + o_level);
   m->d_nbr = (int*)(d + o_nbr);
+  m->nb_dev = nb;
   m->d_bfslot = (int*)(d + o_bfs);
   m->d_r1 = (DevRecord*)(d + o_a);
   m->d_r2 = (DevRecord*)(d + o_b2);
@@ -332,6 +335,14 @@ int fill_ghosts_impl(f4_mesh* m, int state, int have, bool need_z, bool for_stag
   // nothing valid and the reader is a stage kernel: of the same-level copies it needs the x faces only (and the y / z
   // ones into C2F source blocks); its y / z halos come from the neighbours' interiors
   else if (for_stage) { r1 = m->d_r1f; n1 = m->n_r1f; after = no_push ? 0 : 1; }
+  if (r1 == m->d_r1 && n1 > m->n_r1n) {
+    // the whole pattern: the same-level copies go by SOURCE block (every interior row read once, f4_ghost.cu), the
+    // executor runs the rest of round 1 (physical boundaries, restrictions); the two write disjoint ghost regions
+    Scope sc(m, F4_PROF_R1);
+    CU(launch_srl_push(m->hm.dim, m->hm.N, m->nvar, st, m->d_nbr, m->nb_dev, m->stream));
+    r1 = m->d_r1n;
+    n1 = m->n_r1n;
+  }
   if (n1) {
     Scope sc(m, F4_PROF_R1);
     CU(launch_ghost(m->hm.dim, m->hm.N, m->nvar,

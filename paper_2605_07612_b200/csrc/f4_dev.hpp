@@ -74,6 +74,8 @@ struct GhostParams {
 };
 
 // every launcher returns the cudaError_t of the launch
+// all same-level copies of a whole fill, by source block (one CTA per block and variable); nbr: [nblocks][6]
+cudaError_t launch_srl_push(int dim, int n, int nvar, double* state, const int* nbr, int nblocks, cudaStream_t s);
 cudaError_t launch_ghost(int dim, int n, int nvar, const GhostParams& p, cudaStream_t s);
 cudaError_t launch_stage(int dim, int n, const StageParams& p, cudaStream_t s);
 // dt[0] = cfl / rate with rate = the CFL maximum as bits of a double (0 and dt[1] = 1 if the rate is not a positive finite

@@ -13,6 +13,7 @@
 
 #include "../../include/f4.h"
 #include "f4_dev.hpp"
+#include "f4_stage_dev.cuh"
 
 namespace f4 {
 namespace {
@@ -295,6 +296,81 @@ __global__ void __launch_bounds__(256, 4) ghost_exec_kernel(GhostParams p) {
       do_bc_values<DIM, N, NV>(p.state, rec.dst, face, o2 != 0 && o1 == 0, p.bcv,
                            p.dx0 * (1.0 / (double)(1u << p.level[rec.dst])),
                            (o1 & o2) ? p.bcdata + (size_t)rec.src * G::NVAR * ((DIM == 3) ? N * N : N) : nullptr);
+  }
+}
+
+// ---------------------------------------------------------------------------
+// Same-level copies of a WHOLE fill, by source block (the SRL part of round 1).
+// The record list is sorted by destination: a CTA of ghost_exec_kernel gathers the six faces of one block from six
+// neighbours, and the x-face sources -- the first / last 16 bytes of 160-byte rows -- cost a 64-byte DRAM atom each,
+// in rows that the y / z copies of OTHER destinations fetch again (DRAM reads 2.4 x the algorithmic bytes,
+// profiles/ghost_exec_r2.md).  Turned round, one CTA per (source block, variable) reads the block's interior rows
+// ONCE and stores every 16-byte unit into the ghost region of each same-level neighbour it belongs to (up to three:
+// an x, a y and a z face).
+// nbr[b][f] = same-level neighbour across face f or -1 (then a BC / F2C / C2F record fills that face); same-level
+// adjacency is symmetric, so b's cells next to its face f are the ghosts of nbr[b][f] at face f^1.
+// ---------------------------------------------------------------------------
+// The rows come in by the TMA engine: one bulk copy per z plane (its N interior rows with the ghost slots between
+// them are contiguous: N*P doubles) into shared memory, all planes of the CTA's z chunk requested at once by one
+// thread -- tens of KB in flight per CTA without a register -- then every thread stores the 16-byte units of the
+// chunk that belong to a face layer.
+template <int DIM, int N>
+struct PushCfg {
+  static constexpr int P = N + 2 * NG;
+  static constexpr int NZ = (DIM == 3) ? N : 1;
+  static constexpr int PLANE = N * P;                                   // doubles per bulk copy
+  static constexpr int ZC_MAX = (40 * 1024) / (PLANE * 8);              // planes per CTA: at most 40 KB
+  static constexpr int ZC = (NZ < ZC_MAX) ? NZ : (ZC_MAX >= 16 ? 16 : (ZC_MAX >= 8 ? 8 : (ZC_MAX >= 4 ? 4 : (ZC_MAX >= 2 ? 2 : 1))));
+  static constexpr int NCHUNK = NZ / ZC;
+  static constexpr size_t SMEM = (size_t)ZC * PLANE * 8 + 16;
+  static_assert(NZ % ZC == 0 && (PLANE * 8) % 16 == 0, "chunking");
+};
+
+template <int DIM, int N, int NV>
+__global__ void __launch_bounds__(256) srl_push_kernel(double* __restrict__ st, const int* __restrict__ nbr) {
+  using G = Geo<DIM, N, NV>;
+  using C = PushCfg<DIM, N>;
+  constexpr int H = G::H, P = G::P, PP = P * P, ZC = C::ZC, PLANE = C::PLANE;
+  constexpr int UNITS = H * N * ZC;                     // 16-byte units of the chunk's interior
+  extern __shared__ __align__(128) unsigned char push_smem[];
+  double* sm = reinterpret_cast<double*>(push_smem);
+  uint64_t* bar = reinterpret_cast<uint64_t*>(sm + ZC * PLANE);
+  __shared__ int nb[6];
+  const int b = blockIdx.x, v = blockIdx.y, k0 = blockIdx.z * ZC;
+  const size_t vo = (size_t)v * G::VS;
+  const double* sv = st + (size_t)b * G::BS + vo;
+  if (threadIdx.x == 0) {
+    mbar_init(bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    const uint32_t bar32 = smem_u32(bar);
+    mbar_expect_tx(bar32, (uint32_t)(ZC * PLANE * 8));
+#pragma unroll 1
+    for (int kk = 0; kk < ZC; ++kk)
+      bulk_g2s(smem_u32(sm + kk * PLANE), sv + (size_t)(k0 + kk) * PP, (uint32_t)(PLANE * 8), bar32);
+  }
+  if (threadIdx.x >= 32 && threadIdx.x < 38) {
+    const int f = threadIdx.x - 32;
+    nb[f] = (f < 2 * DIM) ? nbr[(size_t)b * 6 + f] : -1;
+  }
+  __syncthreads();                                      // the barrier is initialised, nb[] is there
+  mbar_wait(smem_u32(bar), 0);
+  const bool zlo = DIM == 3 && k0 < NG && nb[4] >= 0, zhi = DIM == 3 && k0 + ZC > N - NG && nb[5] >= 0;
+  for (int e = threadIdx.x; e < UNITS; e += 256) {
+    const int h = e % H, j = (e / H) % N, kk = e / (H * N), k = k0 + kk;
+    const bool x0 = h == 0 && nb[0] >= 0, x1 = h == H - 1 && nb[1] >= 0;
+    const bool y0 = j < NG && nb[2] >= 0, y1 = j >= N - NG && nb[3] >= 0;
+    const bool z0 = zlo && k < NG, z1 = zhi && k >= N - NG;
+    if (!(x0 | x1 | y0 | y1 | z0 | z1)) continue;       // a unit of the core: nobody's ghost
+    const double2 val = *reinterpret_cast<const double2*>(sm + kk * PLANE + j * P + 2 * h);
+    const int kp = (DIM == 3) ? k * PP : 0;
+    // x: pair-transposed ghost slots (cell_off): cells N, N+1 of row j in row j&~1, cells -2, -1 in row j|1
+    if (x0) st2(st + (size_t)nb[0] * G::BS + vo + kp + (j & ~1) * P + N + 2 * (j & 1), val);
+    if (x1) st2(st + (size_t)nb[1] * G::BS + vo + kp + (j | 1) * P + N + 2 * (j & 1), val);
+    // y: rows 0, 1 are the low neighbour's ghost rows N, N+1; rows N-2, N-1 the high neighbour's slots P-2, P-1
+    if (y0) st2(st + (size_t)nb[2] * G::BS + vo + kp + (N + j) * P + 2 * h, val);
+    if (y1) st2(st + (size_t)nb[3] * G::BS + vo + kp + (j - N + P) * P + 2 * h, val);
+    if (z0) st2(st + (size_t)nb[4] * G::BS + vo + (N + k) * PP + j * P + 2 * h, val);
+    if (z1) st2(st + (size_t)nb[5] * G::BS + vo + (k - N + P) * PP + j * P + 2 * h, val);
   }
 }
 
@@ -612,6 +688,16 @@ cudaError_t launch_ghost(int dim, int n, int nvar, const GhostParams& p, cudaStr
       ghost_exec_kernel<D, NN, NVV, 1><<<p.nrec, 256, 0, s>>>(p);
     else
       ghost_exec_kernel<D, NN, NVV, 2 * D><<<grouped, 256, 0, s>>>(p);
+  }));
+}
+cudaError_t launch_srl_push(int dim, int n, int nvar, double* state, const int* nbr, int nblocks, cudaStream_t s) {
+  if (nblocks <= 0) return cudaSuccess;
+  F4_DISPATCH(({
+    using C = PushCfg<D, NN>;
+    auto k = srl_push_kernel<D, NN, NVV>;
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+    if (e != cudaSuccess) return e;
+    k<<<dim3(nblocks, NVV, C::NCHUNK), 256, C::SMEM, s>>>(state, nbr);
   }));
 }
 cudaError_t launch_transfer(int dim, int n, int nvar, const double* old_state, double* new_state, const DevTransfer* plan,
