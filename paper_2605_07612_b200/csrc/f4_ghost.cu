@@ -314,54 +314,60 @@ __global__ void __launch_bounds__(256, 4) ghost_exec_kernel(GhostParams p) {
 // them are contiguous: N*P doubles) into shared memory, all planes of the CTA's z chunk requested at once by one
 // thread -- tens of KB in flight per CTA without a register -- then every thread stores the 16-byte units of the
 // chunk that belong to a face layer.
-template <int DIM, int N>
+template <int DIM, int N, int NV>
 struct PushCfg {
   static constexpr int P = N + 2 * NG;
   static constexpr int NZ = (DIM == 3) ? N : 1;
   static constexpr int PLANE = N * P;                                   // doubles per bulk copy
-  static constexpr int ZC_MAX = (40 * 1024) / (PLANE * 8);              // planes per CTA: at most 40 KB
-  static constexpr int ZC = (NZ < ZC_MAX) ? NZ : (ZC_MAX >= 16 ? 16 : (ZC_MAX >= 8 ? 8 : (ZC_MAX >= 4 ? 4 : (ZC_MAX >= 2 ? 2 : 1))));
+  static constexpr int BUDGET = 40 * 1024;                              // bytes of bulk copies per CTA
+  static constexpr int ZC_MAX = BUDGET / (PLANE * 8);
+  static constexpr int ZC = (NZ <= ZC_MAX) ? NZ : (ZC_MAX >= 16 ? 16 : (ZC_MAX >= 8 ? 8 : (ZC_MAX >= 4 ? 4 : (ZC_MAX >= 2 ? 2 : 1))));
   static constexpr int NCHUNK = NZ / ZC;
-  static constexpr size_t SMEM = (size_t)ZC * PLANE * 8 + 16;
-  static_assert(NZ % ZC == 0 && (PLANE * 8) % 16 == 0, "chunking");
+  static constexpr int VC = (NV * ZC * PLANE * 8 <= BUDGET) ? NV : 1;   // small blocks: all variables in one CTA
+  static constexpr size_t SMEM = (size_t)VC * ZC * PLANE * 8 + 16;
+  static_assert(NZ % ZC == 0 && (PLANE * 8) % 16 == 0 && NV % VC == 0, "chunking");
 };
 
 template <int DIM, int N, int NV>
 __global__ void __launch_bounds__(256) srl_push_kernel(double* __restrict__ st, const int* __restrict__ nbr) {
   using G = Geo<DIM, N, NV>;
-  using C = PushCfg<DIM, N>;
-  constexpr int H = G::H, P = G::P, PP = P * P, ZC = C::ZC, PLANE = C::PLANE;
-  constexpr int UNITS = H * N * ZC;                     // 16-byte units of the chunk's interior
+  using C = PushCfg<DIM, N, NV>;
+  constexpr int H = G::H, P = G::P, PP = P * P, ZC = C::ZC, PLANE = C::PLANE, VC = C::VC;
+  constexpr int UNITS = H * N * ZC;                     // 16-byte units of one variable's chunk interior
   extern __shared__ __align__(128) unsigned char push_smem[];
-  double* sm = reinterpret_cast<double*>(push_smem);
-  uint64_t* bar = reinterpret_cast<uint64_t*>(sm + ZC * PLANE);
+  double* sm = reinterpret_cast<double*>(push_smem);    // [VC][ZC][PLANE]
+  uint64_t* bar = reinterpret_cast<uint64_t*>(sm + VC * ZC * PLANE);
   __shared__ int nb[6];
-  const int b = blockIdx.x, v = blockIdx.y, k0 = blockIdx.z * ZC;
-  const size_t vo = (size_t)v * G::VS;
-  const double* sv = st + (size_t)b * G::BS + vo;
-  if (threadIdx.x == 0) {
-    mbar_init(bar, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  const int b = blockIdx.x, v0 = blockIdx.y * VC, k0 = blockIdx.z * ZC;
+  const double* sb = st + (size_t)b * G::BS;
+  if (threadIdx.x < 32) {                               // warp 0 requests the copies, a share per lane
     const uint32_t bar32 = smem_u32(bar);
-    mbar_expect_tx(bar32, (uint32_t)(ZC * PLANE * 8));
-#pragma unroll 1
-    for (int kk = 0; kk < ZC; ++kk)
-      bulk_g2s(smem_u32(sm + kk * PLANE), sv + (size_t)(k0 + kk) * PP, (uint32_t)(PLANE * 8), bar32);
-  }
-  if (threadIdx.x >= 32 && threadIdx.x < 38) {
+    if (threadIdx.x == 0) {
+      mbar_init(bar, 1);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+      mbar_expect_tx(bar32, (uint32_t)(VC * ZC * PLANE * 8));
+    }
+    __syncwarp();
+    for (int c = threadIdx.x; c < VC * ZC; c += 32) {
+      const int vv = c / ZC, kk = c % ZC;
+      bulk_g2s(smem_u32(sm + c * PLANE), sb + (size_t)(v0 + vv) * G::VS + (size_t)(k0 + kk) * PP, (uint32_t)(PLANE * 8), bar32);
+    }
+  } else if (threadIdx.x < 38) {
     const int f = threadIdx.x - 32;
     nb[f] = (f < 2 * DIM) ? nbr[(size_t)b * 6 + f] : -1;
   }
   __syncthreads();                                      // the barrier is initialised, nb[] is there
   mbar_wait(smem_u32(bar), 0);
   const bool zlo = DIM == 3 && k0 < NG && nb[4] >= 0, zhi = DIM == 3 && k0 + ZC > N - NG && nb[5] >= 0;
-  for (int e = threadIdx.x; e < UNITS; e += 256) {
-    const int h = e % H, j = (e / H) % N, kk = e / (H * N), k = k0 + kk;
+  for (int e = threadIdx.x; e < VC * UNITS; e += 256) {
+    const int vv = e / UNITS, r = e % UNITS;
+    const int h = r % H, j = (r / H) % N, kk = r / (H * N), k = k0 + kk;
     const bool x0 = h == 0 && nb[0] >= 0, x1 = h == H - 1 && nb[1] >= 0;
     const bool y0 = j < NG && nb[2] >= 0, y1 = j >= N - NG && nb[3] >= 0;
     const bool z0 = zlo && k < NG, z1 = zhi && k >= N - NG;
     if (!(x0 | x1 | y0 | y1 | z0 | z1)) continue;       // a unit of the core: nobody's ghost
-    const double2 val = *reinterpret_cast<const double2*>(sm + kk * PLANE + j * P + 2 * h);
+    const double2 val = *reinterpret_cast<const double2*>(sm + (vv * ZC + kk) * PLANE + j * P + 2 * h);
+    const size_t vo = (size_t)(v0 + vv) * G::VS;
     const int kp = (DIM == 3) ? k * PP : 0;
     // x: pair-transposed ghost slots (cell_off): cells N, N+1 of row j in row j&~1, cells -2, -1 in row j|1
     if (x0) st2(st + (size_t)nb[0] * G::BS + vo + kp + (j & ~1) * P + N + 2 * (j & 1), val);
@@ -693,11 +699,11 @@ cudaError_t launch_ghost(int dim, int n, int nvar, const GhostParams& p, cudaStr
 cudaError_t launch_srl_push(int dim, int n, int nvar, double* state, const int* nbr, int nblocks, cudaStream_t s) {
   if (nblocks <= 0) return cudaSuccess;
   F4_DISPATCH(({
-    using C = PushCfg<D, NN>;
+    using C = PushCfg<D, NN, NVV>;
     auto k = srl_push_kernel<D, NN, NVV>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
     if (e != cudaSuccess) return e;
-    k<<<dim3(nblocks, NVV, C::NCHUNK), 256, C::SMEM, s>>>(state, nbr);
+    k<<<dim3(nblocks, NVV / C::VC, C::NCHUNK), 256, C::SMEM, s>>>(state, nbr);
   }));
 }
 cudaError_t launch_transfer(int dim, int n, int nvar, const double* old_state, double* new_state, const DevTransfer* plan,
