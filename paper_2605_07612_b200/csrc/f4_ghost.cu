@@ -338,7 +338,9 @@ __global__ void __launch_bounds__(256) srl_push_kernel(double* __restrict__ st, 
   double* sm = reinterpret_cast<double*>(push_smem);    // [VC][ZC][PLANE]
   uint64_t* bar = reinterpret_cast<uint64_t*>(sm + VC * ZC * PLANE);
   __shared__ int nb[6];
-  const int b = blockIdx.x, v0 = blockIdx.y * VC, k0 = blockIdx.z * ZC;
+  // consecutive CTAs take the variables of one block: they read one contiguous stretch of the store
+  constexpr int NVQ = NV / VC;
+  const int b = blockIdx.x / NVQ, v0 = (blockIdx.x % NVQ) * VC, k0 = blockIdx.y * ZC;
   const double* sb = st + (size_t)b * G::BS;
   if (threadIdx.x < 32) {                               // warp 0 requests the copies, a share per lane
     const uint32_t bar32 = smem_u32(bar);
@@ -703,7 +705,7 @@ cudaError_t launch_srl_push(int dim, int n, int nvar, double* state, const int* 
     auto k = srl_push_kernel<D, NN, NVV>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
     if (e != cudaSuccess) return e;
-    k<<<dim3(nblocks, NVV / C::VC, C::NCHUNK), 256, C::SMEM, s>>>(state, nbr);
+    k<<<dim3((unsigned)nblocks * (NVV / C::VC), C::NCHUNK), 256, C::SMEM, s>>>(state, nbr);
   }));
 }
 cudaError_t launch_transfer(int dim, int n, int nvar, const double* old_state, double* new_state, const DevTransfer* plan,
