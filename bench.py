@@ -473,7 +473,8 @@ def main():
                        "ms_per_fill": fill_ms, "bytes_read": int(rd_b), "bytes_written": int(wr_b),
                        "records": rec_counts, "launches_per_fill": (gprof["ghost_r1"][1] + gprof["ghost_r2"][1]) // NFILL,
                        "in_step_executor_launches": int(g_n), "in_step_executor_ms_per_step": g_ms / args.steps,
-                       "note": "GBps: f4_fill_ghosts (whole pattern, SRL included) timed standalone after the step "
+                       "note": "GBps: f4_fill_ghosts (whole pattern: same-level copies by source block, then the "
+                               "BC/F2C/C2F records) timed standalone after the step "
                                "loop; inside advance the same-level copies are pushed by the stage kernel and the "
                                "executor runs only BC/F2C/C2F records (none on a uniform periodic mesh)"},
         "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()},
