@@ -171,9 +171,10 @@ int f4_pattern_size(const f4_mesh *m, int *n_r1, int *n_r2);
 int f4_get_pattern(const f4_mesh *m, int *records);
 
 /* ---- fill_ghosts -----------------------------------------------------------
- * Execute the whole pattern on one state: one batched kernel for R1, then one
- * for R2 iff the mesh has refinement boundaries.
- * Asynchronous.  (Inside f4_advance the same-level copies of the state a
+ * Execute the whole pattern on one state: R1 = one kernel for all same-level
+ * copies (by source block) and one batched kernel over the BC / F2C records,
+ * then one batched kernel for R2 iff the mesh has refinement boundaries
+ * (PAPER.md:202-212).  Asynchronous.  (Inside f4_advance the same-level copies of the state a
  * stage kernel produces are pushed by that kernel itself, and only the
  * BC / F2C / C2F records are executed by the batched kernel.) */
 int f4_fill_ghosts(f4_mesh *m, int state);
