@@ -311,8 +311,8 @@ __global__ void __launch_bounds__(256, 4) ghost_exec_kernel(GhostParams p) {
 // adjacency is symmetric, so b's cells next to its face f are the ghosts of nbr[b][f] at face f^1.
 // ---------------------------------------------------------------------------
 // The rows come in by the TMA engine: one bulk copy per z plane (its N interior rows with the ghost slots between
-// them are contiguous: N*P doubles) into shared memory, all planes of the CTA's z chunk requested at once by one
-// thread -- tens of KB in flight per CTA without a register -- then every thread stores the 16-byte units of the
+// them are contiguous: N*P doubles) into shared memory, all planes of the CTA's z chunk requested at once by the
+// lanes of one warp -- tens of KB in flight per CTA without a register -- then every thread stores the 16-byte units of the
 // chunk that belong to a face layer.
 template <int DIM, int N, int NV>
 struct PushCfg {
