@@ -506,7 +506,6 @@ __global__ void __launch_bounds__(Cfg<DIM, N, TY, G, EXBUF>::NT, (Cfg<DIM, N, TY
   auto phase3 = [&](int par, int kk, const double (&Fx)[5], const double (&Fy)[5], double (&acc)[5]) {
     double* eX = exX + (EXBUF == 2 ? par : 0) * C::EX;
     double* eY = exY + (EXBUF == 2 ? par : 0) * C::EX;
-    double* sRh = sRh0 + (EXBUF == 2 ? par : 0) * NV * NH;
     // ---- phase 3: difference with the next faces
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
